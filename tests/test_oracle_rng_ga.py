@@ -1,0 +1,343 @@
+"""Pins of the oracle's Philox stream, integer maps, Gaussian sampler and GA step.
+CPU only (-m "not gpu")."""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import stats
+
+import oracle
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _kat():
+    rows = []
+    for line in open(os.path.join(GOLD, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        v = [int(x, 16) for x in line.split()]
+        rows.append((v[0:4], v[4:6], v[6:10]))
+    return rows
+
+
+# ---------------------------------------------------------------- Philox
+def test_philox_random123_known_answers():
+    rows = _kat()
+    assert len(rows) == 3
+    for ctr, key, out in rows:
+        assert [int(x) for x in oracle.philox4x32_10(ctr, key)] == out
+
+
+def test_philox_is_a_bijection_in_the_counter_and_key_sensitive():
+    key = [123, 456]
+    seen = {tuple(oracle.philox4x32_10([i, 0, 0, 0], key)) for i in range(2000)}
+    assert len(seen) == 2000
+    a = oracle.philox4x32_10([1, 2, 3, 4], [5, 6])
+    for pos in range(4):
+        c = [1, 2, 3, 4]
+        c[pos] ^= 1
+        assert not np.array_equal(a, oracle.philox4x32_10(c, [5, 6]))
+    assert not np.array_equal(a, oracle.philox4x32_10([1, 2, 3, 4], [5, 7]))
+    words = np.concatenate([oracle.philox4x32_10([i, 7, 9, 1], key) for i in range(5000)])
+    # crude uniformity of the 32-bit words: mean of u = w/2^32 is 1/2 +- 5 sigma
+    u = words.astype(np.float64) / 2**32
+    assert abs(u.mean() - 0.5) < 5 * math.sqrt(1 / 12 / u.size)
+    bits = np.unpackbits(words.view(np.uint8)).mean()
+    assert abs(bits - 0.5) < 5 * 0.5 / math.sqrt(words.size * 32)
+
+
+# ---------------------------------------------------------------- integer maps (R4, R6)
+def test_index_map_exact_definition_and_range():
+    w0 = _kat()[0][2]                     # words of the all-zero block
+    # floor(w*n / 2^32) by exact integer arithmetic
+    for n in (1, 2, 13, 61, 64, 129, 321, 512, 1024, 4096, 16384, 2**31 + 5):
+        for w in list(w0) + [0, 1, 2**32 - 1, 2**31]:
+            assert oracle.index(w, n) == (w * n) // 2**32 < n
+    assert [oracle.index(w, 64) for w in w0] == [25, 56, 47, 38]
+    assert [oracle.index(w, 4096) for w in w0] == [1634, 3606, 3013, 2480]
+
+
+def test_bernoulli_thresholds():
+    assert oracle.bernoulli_threshold(0.0) == 0
+    assert oracle.bernoulli_threshold(-1.0) == 0
+    assert oracle.bernoulli_threshold(float("nan")) == 0
+    assert oracle.bernoulli_threshold(1.0) == 2**32
+    assert oracle.bernoulli_threshold(2.0) == 2**32
+    for p in (0.9, 0.05, 0.02, 0.2, 0.5, 1e-10, 1 - 1e-12):
+        T = oracle.bernoulli_threshold(p)
+        assert T == math.floor(p * 2**32) and T / 2**32 <= p < (T + 1) / 2**32
+    assert oracle.bernoulli_threshold(0.9) == 3865470566
+    assert oracle.bernoulli_threshold(0.05) == 214748364
+
+
+def test_init_population_range_layout_and_first_gene():
+    """genes random in [-1,+1].  R6: gene g <- word g&3 of call (g>>2, m, 0, INIT)."""
+    M, G, seed = 37, 61, 0x0123456789ABCDEF
+    W = oracle.init_population(M, G, seed)
+    assert W.dtype == np.float32 and W.shape == (M, G)
+    assert W.min() >= -1.0 and W.max() < 1.0
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for m, g in [(0, 0), (0, 3), (0, 4), (5, 17), (36, 60)]:
+        word = int(oracle.philox4x32_10([g >> 2, m, 0, 0], key)[g & 3])
+        assert W[m, g] == np.float32((word >> 8) * 2.0**-23 - 1.0)
+    # seed 0, chromosome 0, gene 0 is the first word of the all-zero known-answer block
+    W0 = oracle.init_population(1, 1, 0)
+    assert W0[0, 0] == np.float32((0x6627E8D5 >> 8) * 2.0**-23 - 1.0) == np.float32(-0.20190716)
+    # uniform on [-1,1): mean 0, var 1/3 (5 sigma), KS
+    Wb = oracle.init_population(512, 129, 7).ravel().astype(np.float64)
+    assert abs(Wb.mean()) < 5 * math.sqrt(1 / 3 / Wb.size)
+    assert abs(Wb.var() - 1 / 3) < 5 * math.sqrt(4 / 45 / Wb.size)
+    assert stats.kstest(Wb, stats.uniform(-1, 2).cdf).pvalue > 1e-4
+    assert np.array_equal(oracle.init_population(4, 9, 3), oracle.init_population(4, 9, 3))
+    assert not np.array_equal(oracle.init_population(4, 9, 3), oracle.init_population(4, 9, 4))
+
+
+# ---------------------------------------------------------------- Gaussian sampler (R5)
+def test_neg2ln_accuracy_against_libm():
+    rng = np.random.default_rng(1)
+    a = np.concatenate([rng.integers(0, 2**32, 400000, dtype=np.uint64).astype(np.uint32),
+                        np.arange(0, 2**32, 2**32 // 4096, dtype=np.uint64).astype(np.uint32),
+                        np.array([0, 1, 511, 512, 2**32 - 1, 2**32 - 512, 2**32 - 513, 2**31], dtype=np.uint32)])
+    t = oracle.neg2ln_u1_many(a).astype(np.float64)
+    u1 = ((a >> 9).astype(np.float64) + 1) * 2.0**-23
+    ref = -2 * np.log(u1)
+    nz = ref > 0
+    assert np.max(np.abs(t[nz] - ref[nz]) / ref[nz]) < 4e-7
+    assert np.max(np.abs(t - ref)) < 4e-6
+    assert np.all(t >= 0)
+    # edges: u1 = 1 -> -0 (sqrt gives -0, z = +-0); u1 = 2^-23 -> 23*2 ln 2
+    t1 = oracle.neg2ln_u1(0xFFFFFFFF)
+    assert t1 == 0 and np.signbit(t1)
+    assert abs(float(oracle.neg2ln_u1(0)) - 46 * math.log(2)) < 1e-5
+
+
+def test_cos_angle_accuracy_and_quadrants():
+    """c must be cos(2 pi u2), u2 = (b>>6)/2^26 -- this pins the quadrant table and both
+    polynomials (a swapped sin/cos or a wrong sign fails by O(1))."""
+    rng = np.random.default_rng(2)
+    b = np.concatenate([rng.integers(0, 2**32, 400000, dtype=np.uint64).astype(np.uint32),
+                        np.array([0, 63, 64, 2**30 - 1, 2**30, 2**31, 3 * 2**30, 2**32 - 1, 2**29], dtype=np.uint32)])
+    c = oracle.cos_angle_many(b).astype(np.float64)
+    u2 = (b >> 6).astype(np.float64) * 2.0**-26
+    assert np.max(np.abs(c - np.cos(2 * math.pi * u2))) < 4e-7
+    assert oracle.cos_angle(0) == 1.0 and oracle.cos_angle(2**31) == -1.0
+    assert oracle.cos_angle(2**30) == 0.0 and oracle.cos_angle(3 * 2**30) == 0.0
+
+
+def test_gauss_is_sqrt_times_cos_in_binary32():
+    rng = np.random.default_rng(3)
+    a = rng.integers(0, 2**32, 20000, dtype=np.uint64).astype(np.uint32)
+    b = rng.integers(0, 2**32, 20000, dtype=np.uint64).astype(np.uint32)
+    z = oracle.gauss_many(a, b)
+    r = np.sqrt(oracle.neg2ln_u1_many(a))                 # numpy float32 sqrt: correctly rounded
+    expect = (r * oracle.cos_angle_many(b)).astype(np.float32)
+    assert np.array_equal(z.view(np.uint32), expect.view(np.uint32))
+    assert abs(float(oracle.gauss(0xFFFFFFFF, 12345))) == 0.0
+    assert np.all(np.abs(z) <= math.sqrt(2 * 23 * math.log(2)) + 1e-5)
+
+
+def test_gauss_distribution():
+    n = 400000
+    words = np.stack([oracle.philox4x32_10([i, 0, 0, 9], [42, 0]) for i in range(n // 2)])
+    z = np.concatenate([oracle.gauss_many(words[:, 0], words[:, 1]),
+                        oracle.gauss_many(words[:, 2], words[:, 3])]).astype(np.float64)
+    assert abs(z.mean()) < 5 / math.sqrt(n)
+    assert abs(z.var() - 1) < 5 * math.sqrt(2 / n)
+    assert abs(stats.skew(z)) < 5 * math.sqrt(6 / n)
+    assert abs(stats.kurtosis(z)) < 5 * math.sqrt(24 / n)
+    assert stats.kstest(z, "norm").pvalue > 1e-4
+    assert 0.30 < np.mean(np.abs(z) > 1) < 0.335          # 0.3173
+
+
+# ---------------------------------------------------------------- GA step (R7)
+E, K, PC, PM, SIG = 4, 3, 0.9, 0.05, 0.1
+
+
+def _pop(M=64, G=13, seed=5):
+    rng = np.random.default_rng(seed)
+    W = rng.uniform(-1, 1, (M, G)).astype(np.float32)
+    F = rng.uniform(0.05, 0.5, M).astype(np.float32)
+    return W, F
+
+
+def _order(F):
+    key = np.where(np.isnan(F), np.inf, F).astype(np.float64)
+    return np.lexsort((np.arange(len(F)), key))
+
+
+def test_step_population_size_and_elites_preserved():
+    W, F = _pop()
+    Wn = oracle.step(W, F, E, K, PC, PM, SIG, seed=1, gen=0)
+    assert Wn.shape == W.shape and Wn.dtype == np.float32
+    order = _order(F)
+    for s in range(E):
+        assert np.array_equal(Wn[s].view(np.uint32), W[order[s]].view(np.uint32))
+
+
+def test_step_elite_order_ties_and_nan():
+    W, F = _pop(M=16)
+    F[:] = 0.3
+    F[[9, 3, 12]] = 0.1                     # three-way tie for best -> lower index first
+    F[5] = np.nan                           # NaN orders last
+    F[7] = -0.0
+    F[2] = 0.0                              # -0 == +0 -> tie -> index 2 before 7
+    Wn = oracle.step(W, F, 6, K, 0.0, 0.0, SIG, seed=1, gen=0)
+    for s, src in enumerate([2, 7, 3, 9, 12, 0]):
+        assert np.array_equal(Wn[s], W[src]), (s, src)
+    assert oracle.best_index(F) == 2
+    Fn = np.full(4, np.nan, dtype=np.float32)
+    assert oracle.best_index(Fn) == 0
+    # a NaN-fitness chromosome never wins a tournament against a finite one
+    W2, F2 = _pop(M=8)
+    F2[:7] = np.nan
+    Wn2 = oracle.step(W2, F2, 0, 8, 0.0, 0.0, SIG, seed=3, gen=0)
+    hits = sum(np.array_equal(Wn2[c], W2[7]) for c in range(8))
+    assert hits >= 5                        # P[7 among 8 entrants] = 1-(7/8)^8 = 0.66 each
+
+
+def test_step_children_without_operators_are_tournament_winners():
+    """p_c = p_m = 0 -> child c is a bit-copy of parent A = best of entrants 0..k-1,
+    entrants recomputed here from the Philox stream and the index map."""
+    W, F = _pop(M=64)
+    seed, gen = 0xDEADBEEFCAFE, 17
+    Wn = oracle.step(W, F, 2, 3, 0.0, 0.0, SIG, seed=seed, gen=gen)
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    rank = np.empty(64, dtype=int)
+    rank[_order(F)] = np.arange(64)
+    for c in range(2, 64):
+        words = np.concatenate([oracle.philox4x32_10([blk, c, gen, 1], key) for blk in range(2)])
+        entrants = [(int(w) * 64) >> 32 for w in words[:6]]
+        a = min(entrants[:3], key=lambda i: rank[i])
+        assert np.array_equal(Wn[c], W[a]), c
+
+
+def test_step_k1_is_uniform_choice_of_entrant_zero():
+    W, F = _pop(M=32)
+    seed, gen = 99, 3
+    Wn = oracle.step(W, F, 0, 1, 0.0, 0.0, SIG, seed=seed, gen=gen)
+    for c in range(32):
+        w0 = int(oracle.philox4x32_10([0, c, gen, 1], [seed, 0])[0])
+        assert np.array_equal(Wn[c], W[(w0 * 32) >> 32])
+
+
+def test_tournament_pressure_matches_closed_form():
+    """P[parent A = global best] = 1 - (1 - 1/M)^k."""
+    M, G = 16, 2
+    W = np.arange(M * G, dtype=np.float32).reshape(M, G)
+    F = np.linspace(1.0, 2.0, M).astype(np.float32)
+    F[11] = 0.5
+    for k in (1, 2, 5):
+        wins = total = 0
+        for gen in range(150):
+            Wn = oracle.step(W, F, 0, k, 0.0, 0.0, SIG, seed=7, gen=gen)
+            wins += int((Wn[:, 0] == W[11, 0]).sum())
+            total += M
+        p = 1 - (1 - 1 / M) ** k
+        assert abs(wins / total - p) < 5 * math.sqrt(p * (1 - p) / total)
+
+
+def test_crossover_structure_and_cut_range():
+    """Every child is A[0:q] ++ B[q:G] with q in [1,G-1], or a copy of A; the crossover rate is
+    p_c; q is uniform."""
+    M, G = 256, 13
+    W = (np.arange(M)[:, None] * 100 + np.arange(G)[None, :]).astype(np.float32)   # gene encodes (row, g)
+    F = np.random.default_rng(0).uniform(size=M).astype(np.float32)
+    cuts, crossed, total = [], 0, 0
+    for gen in range(20):
+        Wn = oracle.step(W, F, 2, 3, 0.9, 0.0, SIG, seed=5, gen=gen)
+        rows = (Wn // 100).astype(int)
+        assert np.array_equal(Wn - rows * 100, np.broadcast_to(np.arange(G, dtype=np.float32), (M, G)))
+        for c in range(2, M):
+            changes = np.nonzero(np.diff(rows[c]))[0]
+            assert len(changes) <= 1
+            # the crossover Bernoulli and the cut, recomputed from the stream
+            w = oracle.philox4x32_10([0, c, gen, 2], [5, 0])
+            hit = int(w[0]) < oracle.bernoulli_threshold(0.9)
+            q = 1 + ((int(w[1]) * (G - 1)) >> 32)
+            if len(changes) == 1:
+                assert hit and changes[0] + 1 == q and 1 <= q <= G - 1
+                cuts.append(q)
+            total += 1
+            crossed += hit
+    assert abs(crossed / total - 0.9) < 5 * math.sqrt(0.09 / total)
+    counts = np.bincount(cuts, minlength=G)[1:G]
+    assert counts.min() > 0 and stats.chisquare(counts).pvalue > 1e-4
+
+
+def test_crossover_degenerate_single_gene():
+    W = np.arange(8, dtype=np.float32).reshape(8, 1)
+    F = np.arange(8, dtype=np.float32)
+    Wn = oracle.step(W, F, 1, 2, 1.0, 0.0, SIG, seed=1, gen=0)
+    assert Wn[0, 0] == 0.0 and set(Wn.ravel()) <= set(W.ravel())
+
+
+def test_mutation_count_value_and_independence():
+    M, G = 128, 61
+    W = np.zeros((M, G), dtype=np.float32)
+    F = np.arange(M, dtype=np.float32)
+    seed, gen, sigma, pm = 11, 2, np.float32(0.1), 0.05
+    Wn = oracle.step(W, F, 4, 3, 0.0, pm, sigma, seed=seed, gen=gen)
+    assert np.all(Wn[:4] == 0)                                    # elites never mutated
+    mutated = Wn[4:] != 0
+    n = (M - 4) * G
+    assert abs(mutated.sum() - n * pm) < 5 * math.sqrt(n * pm * (1 - pm))
+    T = oracle.bernoulli_threshold(pm)
+    for c, g in [(4, 0), (4, 60), (77, 13), (127, 33)] + [tuple(x + np.array([4, 0])) for x in np.argwhere(mutated)[:20]]:
+        w = oracle.philox4x32_10([g, c, gen, 3], [seed, 0])
+        if int(w[0]) < T:
+            delta = np.float32(sigma * oracle.gauss(int(w[1]), int(w[2])))
+            assert Wn[c, g] == np.float32(0.0) + delta
+        else:
+            assert Wn[c, g] == 0
+    z = (Wn[4:][mutated] / sigma).astype(np.float64)
+    assert abs(z.mean()) < 5 / math.sqrt(z.size) and abs(z.std() - 1) < 5 / math.sqrt(2 * z.size)
+    # p_m = 1, sigma = 0 leaves the children unchanged; p_m = 1 mutates every gene
+    Wa, Fa = _pop()
+    base = oracle.step(Wa, Fa, E, K, PC, 0.0, SIG, seed=1, gen=0)
+    assert np.array_equal(oracle.step(Wa, Fa, E, K, PC, 1.0, 0.0, seed=1, gen=0), base)
+    allm = oracle.step(Wa, Fa, E, K, PC, 1.0, SIG, seed=1, gen=0)
+    assert np.all(allm[E:] != base[E:]) and np.array_equal(allm[:E], base[:E])
+
+
+def test_step_determinism_and_generation_dependence():
+    W, F = _pop()
+    a = oracle.step(W, F, E, K, PC, PM, SIG, seed=1, gen=0)
+    assert np.array_equal(a, oracle.step(W, F, E, K, PC, PM, SIG, seed=1, gen=0))
+    assert not np.array_equal(a, oracle.step(W, F, E, K, PC, PM, SIG, seed=1, gen=1))
+    assert not np.array_equal(a, oracle.step(W, F, E, K, PC, PM, SIG, seed=2, gen=0))
+    assert not np.array_equal(a, oracle.step(W, F, E, K, PC, PM, SIG, seed=1 + 2**32, gen=0))
+
+
+def test_step_rejects_bad_parameters():
+    W, F = _pop(M=8)
+    with pytest.raises(ValueError):
+        oracle.step(W, F, 8, K, PC, PM, SIG, seed=1, gen=0)       # E must be < M
+    with pytest.raises(ValueError):
+        oracle.step(W, F, 2, 0, PC, PM, SIG, seed=1, gen=0)       # k >= 1
+
+
+# ---------------------------------------------------------------- run (R8)
+def test_run_best_is_monotone_with_elitism_and_resumable():
+    import workloads as wl
+    cfg = wl.CONFIGS["c0"]
+    X, t, _ = wl.make_kb(cfg)
+    W0 = oracle.init_population(cfg.M, cfg.G, 0)
+    args = (cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+    Wf, Ff, best = oracle.run(cfg.d, cfg.family, X, t, W0, *args, seed=0, gen0=0, n_gens=10)
+    assert best.shape == (11,) and np.all(np.diff(best) <= 0) and best[-1] < best[0]
+    assert best[0] == np.float32(oracle.eval_fitness(cfg.d, cfg.family, X, t, W0).min())
+    # checkpoint / resume: 10 generations = 5 + restore + 5, bit-exact (state = population + gen)
+    W5, _, b5 = oracle.run(cfg.d, cfg.family, X, t, W0, *args, seed=0, gen0=0, n_gens=5)
+    W10, F10, b10 = oracle.run(cfg.d, cfg.family, X, t, W5, *args, seed=0, gen0=5, n_gens=5)
+    assert np.array_equal(W10, Wf) and np.array_equal(F10, Ff)
+    assert np.array_equal(np.concatenate([b5, b10[1:]]), best)
+    # run == manual loop of eval + step
+    W = W0.copy()
+    for g in range(3):
+        F = oracle.eval_fitness(cfg.d, cfg.family, X, t, W).astype(np.float32)
+        assert F.min() == best[g]
+        W = oracle.step(W, F, *args, seed=0, gen=g)
+    W3, _, _ = oracle.run(cfg.d, cfg.family, X, t, W0, *args, seed=0, gen0=0, n_gens=3)
+    assert np.array_equal(W, W3)
