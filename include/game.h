@@ -1,0 +1,173 @@
+/*
+ * game.h -- C ABI of libgame.so, the B200-native (sm_100a) hot path of the GAME model of
+ * arXiv:1211.5481 ("Genetic Algorithm Modeling with GPU Parallel Computing Technology"):
+ * batched fitness evaluation of a whole GA population over the training patterns, plus the
+ * per-generation GA operators, all on the device.
+ *
+ * Citations: "PAPER.md:<line>" is the paper text; "SURVEY 8(c) R<n>" / "DESIGN.md D<n>" are the
+ * readings fixed where the paper is silent (DESIGN.md lists every one of them).
+ *
+ * Notation: P patterns, N features per pattern, d polynomial degree (Chebyshev)
+ * or number of harmonics K (polytrigo, eq.(6)), G genes per chromosome, M chromosomes.
+ *   G = N*d + 1 (Chebyshev)  or  N*2d + 1 (trig)      [DESIGN.md D1; eq.(5)]
+ * Gene order: gene 0 = bias a_0; then one block per feature i = 0..N-1:
+ *   Chebyshev: T_1(x_i) .. T_d(x_i);   trig: cos(1 x_i)..cos(d x_i), sin(1 x_i)..sin(d x_i)
+ *   (the paper's [a_1..a_3, b_1..b_3]).
+ *
+ * Conventions
+ *  - Every function returns int: GAME_OK (0) or a negative GAME_ERR_*.  No exceptions, no aborts,
+ *    no printing.  game_last_error() gives a ctx-owned message for the last failing call.
+ *  - Pointers named *_dev are DEVICE pointers (cudaMalloc'ed / torch CUDA tensors), *_host are HOST
+ *    pointers.  All device buffers are CALLER-OWNED and only BORROWED by the context: they must stay
+ *    alive and unchanged in size while bound; the library never frees them.  The context owns only
+ *    its small host struct.  Device buffers must be 16-byte aligned, contiguous, row-major.
+ *  - All work is enqueued on the stream given to game_set_stream (default: the legacy default
+ *    stream) and is ASYNCHRONOUS; nothing synchronises with the host except game_sync and the
+ *    *_host entry points (which finish with a stream synchronise).
+ *  - A context is not thread-safe; distinct contexts are independent.
+ *  - There is no CPU fallback: without a CUDA device every compute entry returns GAME_ERR_CUDA.
+ */
+#ifndef GAME_H_
+#define GAME_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct game_ctx game_ctx; /* opaque */
+
+enum {
+    GAME_OK = 0,
+    GAME_ERR_INVALID_ARG = -1, /* bad shape, pointer, alignment or parameter            */
+    GAME_ERR_BAD_STATE = -2,   /* call order: eval before load_kb/bind_state, step without a fresh fitness */
+    GAME_ERR_CUDA = -3,        /* CUDA runtime error (sticky errors surface at game_sync) */
+    GAME_ERR_WORKSPACE = -4,   /* workspace_bytes smaller than game_workspace_bytes       */
+    GAME_ERR_UNSUPPORTED = -5  /* shape outside what the kernels cover (stated per call)  */
+};
+
+/* family = expansion | (activation << 8)                                     [DESIGN.md D2]
+ *   expansion : 0 CHEBYSHEV (T_1..T_d, eq.(1)), 1 TRIG (cos/sin k=1..d, eq.(6))
+ *   activation: 0 IDENTITY (the paper's raw sum, eq.(2)), 1 SIGMOID, 2 TANH (BASELINE.json)
+ * BASELINE.json configs c0,c1,c3,c4 = 0x0100; c2 = 0x0201. */
+enum { GAME_EXP_CHEBYSHEV = 0, GAME_EXP_TRIG = 1 };
+enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
+
+/* Precision scheme of the fitness contraction z = W . phi^T  (eq.(2), 61).
+ *   AUTO     : F16X3 when the shape is covered by the tensor-core kernel, else FFMA.
+ *   FFMA     : fp32 FFMA on the CUDA cores (phi and W in fp32, fp32 accumulate).
+ *   F16X3    : tcgen05 tensor cores, fp32-recovering 2-term fp16 split of BOTH operands
+ *              (v = hi + lo, hi = rn_f16(v), lo = rn_f16(v - hi)); three kind::f16 MMAs per K step
+ *              (lo.hi, hi.lo, hi.hi; the lo.lo term, <= 2^-22 relative, is dropped), fp32 accumulation in TMEM.
+ *              Precondition: |w| and |phi| < 65504 (fp16 range); phi is bounded by 1 for Chebyshev on
+ *              |x| <= 1 and for trig; out-of-range values give Inf/NaN fitness, which the GA ranks worst.
+ *              Covers N <= 32 (Chebyshev) / N <= 16 (trig), d <= 64; other shapes -> GAME_ERR_UNSUPPORTED
+ *              when F16X3 is forced, FFMA under AUTO.
+ * Both schemes sum each tile's squared errors in fp32 and accumulate tile sums in fp64 in a fixed order
+ * (run-to-run bit-stable; equal chromosomes get equal fitness in any slot). */
+enum { GAME_SCHEME_AUTO = 0, GAME_SCHEME_FFMA = 1, GAME_SCHEME_F16X3 = 2 };
+
+/* Create a context for a knowledge base of P patterns x N features, expansion degree d, population of
+ * M chromosomes.  Validates: P >= 1, N >= 1, d >= 1, M >= 1, known family,
+ * G <= 448 (FFMA kernel's shared-memory tile) -> GAME_ERR_INVALID_ARG / GAME_ERR_UNSUPPORTED.
+ * Host only; touches no device memory. */
+int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int32_t family);
+
+/* Frees the library-owned host state only (never the bound device buffers). NULL is a no-op. */
+int game_destroy(game_ctx* ctx);
+
+/* G = N*d+1 (Chebyshev) or N*2d+1 (trig)  [DESIGN.md D1]. */
+int game_num_genes(const game_ctx* ctx, int32_t* G);
+
+/* Bytes of device workspace game_bind_state needs (fp64 partial sums per CTA, the split W operand
+ * images of the tensor-core scheme, counters).  Depends only on the shapes given to game_create. */
+int game_workspace_bytes(const game_ctx* ctx, size_t* bytes);
+
+/* cudaStream_t to enqueue on (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+int game_set_stream(game_ctx* ctx, void* cuda_stream);
+
+/* Choose the precision scheme (GAME_SCHEME_*).  Default AUTO. */
+int game_set_scheme(game_ctx* ctx, int32_t scheme);
+/* The scheme the next game_eval_fitness will run (AUTO resolved): GAME_SCHEME_FFMA or GAME_SCHEME_F16X3. */
+int game_get_scheme(const game_ctx* ctx, int32_t* scheme);
+
+/* Bind the knowledge base ("the dataset is never altered"): X_dev[P][N] float32
+ * row-major, t_dev[P] float32 targets.  Borrowed; read by every game_eval_fitness. */
+int game_load_kb(game_ctx* ctx, const float* X_dev, const float* t_dev);
+
+/* Bind the mutable state: two population buffers popA_dev/popB_dev [M][G] float32 (the current
+ * population starts in A; game_step writes the other one and swaps), fitness_dev[M] float32, and
+ * workspace_dev of at least game_workspace_bytes bytes (GAME_ERR_WORKSPACE otherwise).  Borrowed. */
+int game_bind_state(game_ctx* ctx, float* popA_dev, float* popB_dev, float* fitness_dev,
+                    void* workspace_dev, size_t workspace_bytes);
+
+/* GA parameters (operators defined by BASELINE.json, D3/D5):
+ * elite in [0, M), tournament >= 1, p_cross and p_mut in [0,1], sigma >= 0 finite.
+ * Defaults: elite 2, tournament 3, p_cross 0.9, p_mut 0.05, sigma 0.1. */
+int game_set_ga_params(game_ctx* ctx, int32_t elite, int32_t tournament, double p_cross, double p_mut,
+                       float sigma);
+
+/* Current population <- genes uniform in [-1,1) from Philox4x32-10 with
+ * key = seed, counter = (g>>2, m, 0, TAG_INIT), word g&3, w = float(word>>8)*2^-23 - 1  [SURVEY 8(c) R6].
+ * Invalidates the fitness.  Async. */
+int game_init_population(game_ctx* ctx, uint64_t seed);
+
+/* Which of popA/popB is current (device pointer), e.g. to upload or download a population with a
+ * plain device copy.  Writing through it is allowed between calls (call game_invalidate_fitness after). */
+int game_current_population(const game_ctx* ctx, float** pop_dev);
+/* Mark the fitness stale (after the caller wrote the current population). */
+int game_invalidate_fitness(game_ctx* ctx);
+/* Mark fitness_dev as valid without evaluating (after the caller wrote fitness_dev itself, e.g. to
+ * feed the GA operators a given fitness vector -- the "same fitness vector and seed" parity hook). */
+int game_assume_fitness(game_ctx* ctx);
+
+/* fitness_dev[m] = (1/P) sum_p (act(sum_g W[m][g] phi_g(x_p)) - t_p)^2 for the current population
+ * (eq.(2),(3), MSE; lower is better, D4).  Feature expansion, contraction,
+ * activation, squared error and the per-chromosome reduction run in ONE fused kernel (phi never
+ * reaches HBM), followed by a small fixed-order fp64 reduction over CTAs.  Needs load_kb + bind_state
+ * (GAME_ERR_BAD_STATE).  Async. */
+int game_eval_fitness(game_ctx* ctx);
+
+/* One GA generation in one kernel: elitism (the `elite` best by
+ * (fitness, index), NaN worst, copied unchanged to slots 0..elite-1), tournament selection with
+ * replacement, single-point crossover (one child per slot), per-gene Gaussian mutation, all drawn from
+ * Philox4x32-10 keyed by seed with counter (index, chromosome, gen, tag).  Reads the current population
+ * and fitness_dev (must be valid: GAME_ERR_BAD_STATE), writes the other buffer, swaps, invalidates the
+ * fitness.  Bit-exact against the oracle for the same fitness vector and seed.  Async. */
+int game_step(game_ctx* ctx, uint64_t seed, uint32_t gen);
+
+/* n_gens x (eval, step with gen = gen0 + i) followed by a final eval, all on one stream with no host
+ * synchronisation (PAPER.md:97, 170 future work (i)).  best_fitness_dev (device, [n_gens+1] float32, or
+ * NULL) receives the best (lowest) fitness of each generation's population.  Async. */
+int game_run(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev);
+
+/* Stream synchronise; returns GAME_ERR_CUDA if any enqueued work failed. */
+int game_sync(game_ctx* ctx);
+
+/* HOST-buffer entry point (what bench.py's e2e leg times): one whole generation on host data.
+ * Copies X_host[P][N], t_host[P] into the bound knowledge-base buffers (which must therefore be
+ * writable) and W_host[M][G] into the current population, runs eval + step(seed, gen), then copies the
+ * fitness of the INPUT population to F_host[M] and the NEXT population to W_next_host[M][G] (either may
+ * be NULL), and synchronises the stream.  Host buffers should be pinned for full copy bandwidth. */
+int game_generation_host(game_ctx* ctx, const float* X_host, const float* t_host, const float* W_host,
+                         float* F_host, float* W_next_host, uint64_t seed, uint32_t gen);
+
+/* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
+int game_launch_count(const game_ctx* ctx, uint64_t* launches);
+
+/* Timing hook for the roofline line: when enabled, game_eval_fitness brackets the fused fitness kernel
+ * with CUDA events on the context's stream; game_fitness_kernel_ms returns the sum of the recorded
+ * durations (milliseconds) and the number of launches since the hook was (re)enabled, after
+ * synchronising on the last event. */
+int game_time_fitness_kernel(game_ctx* ctx, int32_t enable);
+int game_fitness_kernel_ms(game_ctx* ctx, double* total_ms, uint64_t* launches);
+
+/* ctx-owned string describing the last error on this context ("" if none); valid until the next call. */
+const char* game_last_error(const game_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GAME_H_ */

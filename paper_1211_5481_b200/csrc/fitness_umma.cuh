@@ -1,0 +1,473 @@
+// Fused fitness on the 5th-generation tensor cores (scheme GAME_SCHEME_F16X3), sm_100a only.
+//
+//   z[m,p] = sum_g W[m,g] phi_g(x_p)                      (eq.(2), 61: NP outputs per chromosome)
+//   F[m]   = (1/P) sum_p (act(z[m,p]) - t_p)^2            (eq.(3), MSE)
+//
+// is a dense M x P x G contraction whose B operand (the expansion phi, eq.(1), 79-82 eq.(6)) is
+// GENERATED in shared memory and never exists in HBM.  One persistent CTA per SM:
+//
+//   warp 0      loader   : cp.async.bulk (1-D TMA) of the pre-split W operand images, 8 KB per K step
+//   warp 1      MMA      : tcgen05.mma.cta_group::1.kind::f16, M=128 chromosomes x N=256 patterns x K=16 genes,
+//                          three MMAs per K step (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM
+//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation, (y-t)^2, private per-chromosome sum
+//                          (TMEM lane = chromosome, so no shuffle is needed); fp64 accumulation per (CTA, m)
+//   warps 10-17 producers: one pattern per thread; Chebyshev / multiple-angle recurrences for 8 features at a
+//                          time, fp16 hi/lo split, 16-byte stores straight into the MMA's canonical layout
+//
+// Shared-memory operand layout (both operands): K-major, SWIZZLE_NONE "interleaved" canonical layout with the
+// 8-row core matrices packed back to back, i.e. a plain [k_group][row][8 x fp16] array:
+//     byte(row, k) = (k / 8) * rows * 16 + row * 16 + (k % 8) * 2        SBO = 128 B, LBO = rows * 16 B
+// so a producer warp's 32 rows x 16 B are 512 contiguous bytes (conflict-free) and a K step is any pair of
+// k-groups.  The K axis is a PERMUTATION of the genes chosen for the generator (the W images use the same one):
+//   chunk c = features 8c..8c+7;  k-group kg of the chunk holds, for those 8 features,
+//       Chebyshev: T_{kg+1}(x_i)          trig: cos((kg/2+1) x_i) if kg even, sin((kg/2+1) x_i) if kg odd
+//   (padded to an even number of k-groups; absent features / degrees are zeros in the W image), then one last
+//   K step whose element 0 is the bias gene.
+#pragma once
+#include <cuda_fp16.h>
+
+#include <cstdint>
+
+namespace game {
+namespace umma {
+
+constexpr int kBM = 128;             // chromosomes per tile (MMA M, TMEM lanes)
+constexpr int kBN = 256;             // patterns per tile   (MMA N, TMEM columns)
+constexpr int kStages = 8;           // K-step ring
+constexpr int kABytes = 2 * kBM * 16;          // one k-group pair of A (hi or lo): 4096
+constexpr int kBBytes = 2 * kBN * 16;          // one k-group pair of B (hi or lo): 8192
+constexpr int kStageBytes = 2 * kABytes + 2 * kBBytes;   // A_hi, A_lo, B_hi, B_lo = 24576
+constexpr int kXtStride = kBN + 1;             // transposed x tile, padded: Xt[i * 257 + row]
+constexpr int kXtRows = 32;                    // N <= 32 (Chebyshev), 2 * N <= 32 (trig: cos and sin planes)
+constexpr int kXtBytes = kXtRows * kXtStride * 4;
+constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;
+constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
+constexpr int kSmemBar = kStages * kStageBytes + kXtBytes;          // barriers start here
+constexpr int kSmemBytes = kSmemBar + 256;
+constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators
+
+struct Params {
+    const float* X;        // [P][N]
+    const float* t;        // [P]
+    const uint8_t* Wimg;   // [m_tiles][steps][8192]: A_hi (2 k-groups x 128 rows x 16 B), then A_lo
+    double* part;          // [gridDim.x * 2][m_stride]
+    long long P;
+    int N, d, M;
+    int m_stride;          // m_tiles * 128
+    int m_tiles, p_tiles;
+    int m_groups;          // work unit = (pattern tile, group of m_tiles_per_group chromosome tiles)
+    int m_tiles_per_group;
+    int chunks;            // ceil(N / 8)
+    int steps_per_chunk;   // Chebyshev ceil(d / 2); trig d
+    int steps;             // chunks * steps_per_chunk + 1 (bias)
+};
+
+// ---------------------------------------------------------------------------------------------- PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// Bounded wait: a protocol bug must trap, not hang the GPU.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done = 0;
+    const long long t0 = clock64();
+    while (true) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        if (done) break;
+        if (clock64() - t0 > (1ll << 32)) __trap();   // ~2 s
+    }
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Shared-memory matrix descriptor: K-major, SWIZZLE_NONE; start address, LBO (k-group stride) and SBO
+// (8-row group stride) in 16-byte units; descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return static_cast<uint64_t>((saddr & 0x3FFFFu) >> 4) | (static_cast<uint64_t>(lbo_bytes >> 4) << 16) |
+           (static_cast<uint64_t>(sbo_bytes >> 4) << 32) | (1ull << 46);
+}
+// Instruction descriptor, kind::f16: D = F32 (bit 4), A = B = F16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
+constexpr uint32_t kIdesc = (1u << 4) | (static_cast<uint32_t>(kBN >> 3) << 17) | (static_cast<uint32_t>(kBM >> 4) << 24);
+
+// ---------------------------------------------------------------------------------------------- K-axis permutation
+// Gene held by (K step s, k-group kg in {0,1}, slot f in 0..7), or -1 for padding.  Used by the W image
+// builder; the producers below generate phi in exactly this order.
+__host__ __device__ inline int gene_at(int s, int kg, int f, int N, int d, int expansion, int steps_per_chunk, int steps) {
+    if (s == steps - 1) return (kg == 0 && f == 0) ? 0 : -1;
+    const int c = s / steps_per_chunk, ss = s % steps_per_chunk;
+    const int i = c * 8 + f;
+    if (i >= N) return -1;
+    if (expansion == 0) {
+        const int j = 2 * ss + kg + 1;
+        return j <= d ? 1 + i * d + (j - 1) : -1;
+    }
+    return 1 + i * 2 * d + ss + (kg ? d : 0);
+}
+
+// W [M][G] fp32 -> per (m_tile, step) 8 KB images: A_hi then A_lo, each [2 k-groups][128 rows][8 fp16].
+// hi = rn_f16(w), lo = rn_f16(w - hi).  One thread per (m_tile, step, k-group, row).
+__global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __restrict__ img, int M, int G, int N, int d,
+                                      int expansion, int steps_per_chunk, int steps, int m_tiles) {
+    const long long idx = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const long long total = static_cast<long long>(m_tiles) * steps * 2 * kBM;
+    if (idx >= total) return;
+    const int row = static_cast<int>(idx % kBM);
+    const int kg = static_cast<int>((idx / kBM) % 2);
+    const int s = static_cast<int>((idx / (2 * kBM)) % steps);
+    const int mt = static_cast<int>(idx / (2ll * kBM * steps));
+    const int m = mt * kBM + row;
+    __half2 hi[4], lo[4];
+#pragma unroll
+    for (int f2 = 0; f2 < 4; ++f2) {
+        float w[2];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int g = gene_at(s, kg, f2 * 2 + e, N, d, expansion, steps_per_chunk, steps);
+            w[e] = (g >= 0 && m < M) ? W[static_cast<size_t>(m) * G + g] : 0.0f;
+        }
+        const __half2 h = __floats2half2_rn(w[0], w[1]);
+        const float2 hf = __half22float2(h);
+        hi[f2] = h;
+        lo[f2] = __floats2half2_rn(w[0] - hf.x, w[1] - hf.y);
+    }
+    uint8_t* base = img + (static_cast<size_t>(mt) * steps + s) * (2 * kABytes) + kg * (kBM * 16) + row * 16;
+    *reinterpret_cast<uint4*>(base) = *reinterpret_cast<const uint4*>(hi);
+    *reinterpret_cast<uint4*>(base + kABytes) = *reinterpret_cast<const uint4*>(lo);
+}
+
+// ---------------------------------------------------------------------------------------------- producer helpers
+// Split 8 fp32 values into fp16 hi / lo and store them as one 16-byte k-group row each.
+__device__ __forceinline__ void split_store(const float (&v)[8], uint8_t* hi_dst, uint8_t* lo_dst) {
+    uint32_t h[4], l[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const __half2 hh = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+        const float2 hf = __half22float2(hh);
+        const __half2 ll = __floats2half2_rn(v[2 * i] - hf.x, v[2 * i + 1] - hf.y);
+        h[i] = *reinterpret_cast<const uint32_t*>(&hh);
+        l[i] = *reinterpret_cast<const uint32_t*>(&ll);
+    }
+    *reinterpret_cast<uint4*>(hi_dst) = make_uint4(h[0], h[1], h[2], h[3]);
+    *reinterpret_cast<uint4*>(lo_dst) = make_uint4(l[0], l[1], l[2], l[3]);
+}
+
+template <int ACT>
+__device__ __forceinline__ float act_err2(float z, float t) {
+    float y;
+    if (ACT == 1) {
+        y = rcp_approx(1.0f + ex2_approx(-1.44269504088896340736f * z));
+    } else if (ACT == 2) {
+        y = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(2.88539008177792681472f * z)), 1.0f);
+    } else {
+        y = z;
+    }
+    const float e = y - t;
+    return e * e;
+}
+
+// ---------------------------------------------------------------------------------------------- the kernel
+template <int EXPANSION, int ACT>
+__global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    float* Xt = reinterpret_cast<float*>(smem + kStages * kStageBytes);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
+    // bars[0..S) full, [S..2S) empty, [2S..2S+2) acc_full, [2S+2..2S+4) acc_empty, then the TMEM address
+    const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8 * kStages;
+    const uint32_t bar_acc_full = bar_empty + 8 * kStages, bar_acc_empty = bar_acc_full + 16;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 4);
+    const uint32_t smem_base = smem_u32(smem);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int units = prm.p_tiles * prm.m_groups;
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(bar_full + 8 * s, 1 + kNumProdWarps);
+            mbar_init(bar_empty + 8 * s, 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_acc_full + 8 * b, 1);
+            mbar_init(bar_acc_empty + 8 * b, kNumEpiWarps);
+        }
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(smem_u32(tmem_slot), kTmemCols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ============================================================== loader: W operand images -> A stages
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            for (int u = blockIdx.x; u < units; u += gridDim.x) {
+                const int mg = u % prm.m_groups;
+                const int mt0 = mg * prm.m_tiles_per_group;
+                const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
+                for (int mt = mt0; mt < mt1; ++mt) {
+                    const uint8_t* src = prm.Wimg + static_cast<size_t>(mt) * prm.steps * (2 * kABytes);
+                    for (int s = 0; s < prm.steps; ++s) {
+                        mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                        mbar_arrive_expect_tx(bar_full + 8 * stage, 2 * kABytes);
+                        bulk_g2s(smem_base + stage * kStageBytes, src + static_cast<size_t>(s) * (2 * kABytes), 2 * kABytes,
+                                 bar_full + 8 * stage);
+                        if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ============================================================== MMA issuer
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0, tile = 0;
+            for (int u = blockIdx.x; u < units; u += gridDim.x) {
+                const int mg = u % prm.m_groups;
+                const int mt0 = mg * prm.m_tiles_per_group;
+                const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
+                for (int mt = mt0; mt < mt1; ++mt, ++tile) {
+                    const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
+                    mbar_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1);
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem_base + buf * kBN;
+                    for (int s = 0; s < prm.steps; ++s) {
+                        mbar_wait(bar_full + 8 * stage, phase);
+                        tc_fence_after();
+                        const uint32_t a_hi = smem_base + stage * kStageBytes, a_lo = a_hi + kABytes;
+                        const uint32_t b_hi = a_hi + 2 * kABytes, b_lo = b_hi + kBBytes;
+                        const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
+                        const uint64_t db_hi = make_desc(b_hi, kBN * 16, 128), db_lo = make_desc(b_lo, kBN * 16, 128);
+                        umma_f16(d_tmem, da_lo, db_hi, kIdesc, s > 0 ? 1u : 0u);   // small terms first
+                        umma_f16(d_tmem, da_hi, db_lo, kIdesc, 1u);
+                        umma_f16(d_tmem, da_hi, db_hi, kIdesc, 1u);
+                        umma_commit(bar_empty + 8 * stage);                        // stage free when these finish
+                        if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    }
+                    umma_commit(bar_acc_full + 8 * buf);                           // accumulator complete
+                }
+            }
+        }
+    } else if (warp < 2 + kNumEpiWarps) {
+        // ============================================================== epilogue
+        const int q = warp & 3;                 // TMEM lane quarter this warp may access
+        const int h = (warp - 2) >> 2;          // column half
+        double* my_part = prm.part + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
+        for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
+        uint32_t tile = 0;
+        for (int u = blockIdx.x; u < units; u += gridDim.x) {
+            const int pt = u / prm.m_groups, mg = u % prm.m_groups;
+            const int mt0 = mg * prm.m_tiles_per_group;
+            const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
+            const long long p0 = static_cast<long long>(pt) * kBN;
+            const int n_valid = static_cast<int>(min(static_cast<long long>(kBN), prm.P - p0));
+            for (int mt = mt0; mt < mt1; ++mt, ++tile) {
+                const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
+                mbar_wait(bar_acc_full + 8 * buf, acc_phase);
+                tc_fence_after();
+                float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
+#pragma unroll 1
+                for (int cc = 0; cc < 4; ++cc) {
+                    const int col0 = h * 128 + cc * 32;
+                    if (col0 >= n_valid) break;
+                    uint32_t v[32];
+                    tmem_ld32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + buf * kBN + col0, v);
+                    const float* tp = prm.t + p0 + col0;
+                    if (col0 + 32 <= n_valid) {
+                        float4 tv[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) tv[i] = __ldg(reinterpret_cast<const float4*>(tp) + i);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            sum += act_err2<ACT>(__uint_as_float(v[4 * i + 0]), tv[i].x);
+                            sum1 += act_err2<ACT>(__uint_as_float(v[4 * i + 1]), tv[i].y);
+                            sum2 += act_err2<ACT>(__uint_as_float(v[4 * i + 2]), tv[i].z);
+                            sum3 += act_err2<ACT>(__uint_as_float(v[4 * i + 3]), tv[i].w);
+                        }
+                    } else {
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) {
+                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), __ldg(tp + i));
+                        }
+                    }
+                }
+                sum = (sum + sum1) + (sum2 + sum3);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_acc_empty + 8 * buf);
+                const int m = mt * kBM + q * 32 + lane;
+                __stcg(my_part + m, __ldcg(my_part + m) + static_cast<double>(sum));
+            }
+        }
+    } else {
+        // ============================================================== producers: phi -> B stages
+        const int r = threadIdx.x - (2 + kNumEpiWarps) * 32;   // pattern row of this thread, 0..255
+        uint32_t stage = 0, phase = 0;
+        for (int u = blockIdx.x; u < units; u += gridDim.x) {
+            const int pt = u / prm.m_groups, mg = u % prm.m_groups;
+            const int mt0 = mg * prm.m_tiles_per_group;
+            const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
+            const long long p0 = static_cast<long long>(pt) * kBN;
+            // ---- x tile: coalesced global reads, transposed (and for trig: sin/cos'ed) into Xt
+            asm volatile("bar.sync 1, %0;" ::"n"(kNumProdWarps * 32));   // everyone is done with the old Xt
+            {
+                const int n_el = kBN * prm.N;
+                const long long lim = (prm.P - p0) * prm.N;
+                const float* src = prm.X + p0 * prm.N;
+                for (int idx = r; idx < n_el; idx += kBN) {
+                    const float x = idx < lim ? __ldg(src + idx) : 0.0f;
+                    const int row = idx / prm.N, i = idx - row * prm.N;
+                    if (EXPANSION == 0) {
+                        Xt[i * kXtStride + row] = x;
+                    } else {
+                        float sn, cs;
+                        sincosf(x, &sn, &cs);
+                        Xt[i * kXtStride + row] = cs;
+                        Xt[(16 + i) * kXtStride + row] = sn;
+                    }
+                }
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(kNumProdWarps * 32));
+            for (int mt = mt0; mt < mt1; ++mt) {
+                for (int c = 0; c < prm.chunks; ++c) {
+                    // recurrence state for the 8 features of this chunk
+                    float x2[8], am[8], ac[8], bm[8], bc[8];
+#pragma unroll
+                    for (int f = 0; f < 8; ++f) {
+                        const int i = c * 8 + f;
+                        if (EXPANSION == 0) {
+                            const float x = i < prm.N ? Xt[i * kXtStride + r] : 0.0f;
+                            x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
+                            bm[f] = 0.0f; bc[f] = 0.0f;
+                        } else {
+                            const float cs = i < prm.N ? Xt[i * kXtStride + r] : 1.0f;
+                            const float sn = i < prm.N ? Xt[(16 + i) * kXtStride + r] : 0.0f;
+                            x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
+                            bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
+                        }
+                    }
+                    for (int ss = 0; ss < prm.steps_per_chunk; ++ss) {
+                        mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                        uint8_t* b_hi = smem + stage * kStageBytes + 2 * kABytes + r * 16;
+                        uint8_t* b_lo = b_hi + kBBytes;
+                        float v0[8], v1[8];
+                        if (EXPANSION == 0) {
+                            // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2} (zeros beyond degree d)
+                            const bool has1 = 2 * ss + 2 <= prm.d;
+#pragma unroll
+                            for (int f = 0; f < 8; ++f) {
+                                v0[f] = ac[f];
+                                const float n1 = fmaf(x2[f], ac[f], -am[f]);
+                                v1[f] = has1 ? n1 : 0.0f;
+                                const float n2 = fmaf(x2[f], n1, -ac[f]);
+                                am[f] = n1; ac[f] = n2;
+                            }
+                        } else {
+                            // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
+#pragma unroll
+                            for (int f = 0; f < 8; ++f) {
+                                v0[f] = ac[f];
+                                v1[f] = bc[f];
+                                const float cn = fmaf(x2[f], ac[f], -am[f]);
+                                const float sn = fmaf(x2[f], bc[f], -bm[f]);
+                                am[f] = ac[f]; ac[f] = cn;
+                                bm[f] = bc[f]; bc[f] = sn;
+                            }
+                        }
+                        split_store(v0, b_hi, b_lo);
+                        split_store(v1, b_hi + kBN * 16, b_lo + kBN * 16);
+                        fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_full + 8 * stage);
+                        if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    }
+                }
+                // ---- bias step: element 0 of k-group 0 is the constant 1 (gene 0), the rest padding
+                mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                uint8_t* b_hi = smem + stage * kStageBytes + 2 * kABytes + r * 16;
+                uint8_t* b_lo = b_hi + kBBytes;
+                *reinterpret_cast<uint4*>(b_hi) = make_uint4(0x00003C00u, 0u, 0u, 0u);   // fp16 1.0 in slot 0
+                *reinterpret_cast<uint4*>(b_lo) = make_uint4(0u, 0u, 0u, 0u);
+                *reinterpret_cast<uint4*>(b_hi + kBN * 16) = make_uint4(0u, 0u, 0u, 0u);
+                *reinterpret_cast<uint4*>(b_lo + kBN * 16) = make_uint4(0u, 0u, 0u, 0u);
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_full + 8 * stage);
+                if (++stage == kStages) { stage = 0; phase ^= 1; }
+            }
+        }
+    }
+
+    // ---- teardown: everything issued has been consumed once the epilogue has drained the last accumulator
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc(tmem_base, kTmemCols);
+    }
+}
+
+}  // namespace umma
+}  // namespace game

@@ -1,0 +1,208 @@
+// GA operators on the device: population init, one whole generation in ONE kernel, and the fixed-order
+// fitness finalisation.  PAPER.md:43 names the operators (crossover, mutation, selection, elitism) and
+// PAPER.md:134-136 their rates; their definitions are the readings of SURVEY 8(c) R6-R8 / DESIGN.md
+// (tournament with replacement, single-point crossover, per-gene Gaussian mutation, BASELINE.json).
+// PAPER.md:170 lists moving "population formation and evolution" to the GPU as future work (i): this is it.
+#pragma once
+#include <cmath>
+#include <cstdint>
+
+#include "philox.cuh"
+
+namespace game {
+
+constexpr int kGaThreads = 128;
+
+// ---- order on chromosomes (R7.1): a precedes b iff key(F[a]) < key(F[b]), ties -> lower index;
+// key(NaN) = +inf (NaN fitness is worst).  Lower fitness (MSE) is better (D4).
+__device__ __forceinline__ float fit_key(float f) { return (f != f) ? INFINITY : f; }
+
+__device__ __forceinline__ bool precedes(float ka, int a, float kb, int b) {
+    return (ka < kb) || (ka == kb && a < b);
+}
+
+// ---- population init (R6): one thread per Philox block = 4 consecutive genes.
+__global__ void init_population_kernel(float* __restrict__ W, int M, int G, PhiloxKey key) {
+    const int groups = (G + 3) >> 2;
+    const long long idx = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (idx >= static_cast<long long>(M) * groups) return;
+    const int m = static_cast<int>(idx / groups);
+    const int q = static_cast<int>(idx % groups);
+    const uint4 r = philox4x32_10(static_cast<uint32_t>(q), static_cast<uint32_t>(m), 0u, kTagInit, key);
+    float* row = W + static_cast<size_t>(m) * G;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int g = q * 4 + i;
+        if (g < G) row[g] = gene_from_word(word_of(r, i));
+    }
+}
+
+struct GaParams {
+    int M, G, elite, tournament;
+    unsigned long long t_cross, t_mut;  // Bernoulli thresholds floor(p * 2^32)
+    float sigma;
+    uint32_t gen;
+    PhiloxKey key;
+};
+
+// ---- one generation (R7).  Block c plays two parts, with no grid-wide synchronisation:
+//  (1) as chromosome c of the OLD population it counts how many chromosomes precede it; if that rank is
+//      below `elite` it copies its row, unchanged, to slot `rank` of the new population (elitism);
+//  (2) as child slot c >= elite of the NEW population it runs the two tournaments, the crossover draw
+//      and the per-gene mutation draws for that slot.
+__global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __restrict__ W,
+                                                              const float* __restrict__ F,
+                                                              float* __restrict__ Wn, GaParams p) {
+    __shared__ int s_warp_cnt[kGaThreads / 32];
+    __shared__ int s_rank;
+    __shared__ int s_parent[2];
+    __shared__ int s_cut;
+    const int c = blockIdx.x;
+    const int tid = threadIdx.x;
+    const int M = p.M, G = p.G;
+
+    // (1) rank of chromosome c under the order
+    const float kc = fit_key(F[c]);
+    int cnt = 0;
+    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(F[j]), j, kc, c) ? 1 : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((tid & 31) == 0) s_warp_cnt[tid >> 5] = cnt;
+    __syncthreads();
+    if (tid == 0) {
+        int r = 0;
+        for (int w = 0; w < kGaThreads / 32; ++w) r += s_warp_cnt[w];
+        s_rank = r;
+    }
+    __syncthreads();
+    const int rank = s_rank;
+    if (rank < p.elite) {
+        const float* src = W + static_cast<size_t>(c) * G;
+        float* dst = Wn + static_cast<size_t>(rank) * G;
+        for (int g = tid; g < G; g += kGaThreads) dst[g] = src[g];
+    }
+    if (c < p.elite) return;  // slots 0..elite-1 are written by the elites themselves
+
+    // (2) tournaments: entrants 0..k-1 -> parent A, k..2k-1 -> parent B (with replacement)
+    if (tid == 0) {
+        const int k = p.tournament;
+        int par[2] = {-1, -1};
+        float pkey[2] = {0.f, 0.f};
+        uint4 r = make_uint4(0, 0, 0, 0);
+        for (int e = 0; e < 2 * k; ++e) {
+            if ((e & 3) == 0)
+                r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
+            const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
+            const float ki = fit_key(F[idx]);
+            const int side = e < k ? 0 : 1;
+            if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
+                par[side] = idx;
+                pkey[side] = ki;
+            }
+        }
+        s_parent[0] = par[0];
+        s_parent[1] = par[1];
+        // single-point crossover: child = A[0:q] ++ B[q:G], q in [1, G-1]; otherwise child = A
+        const uint4 rc = philox4x32_10(0u, static_cast<uint32_t>(c), p.gen, kTagCross, p.key);
+        int q = G;
+        if (static_cast<unsigned long long>(rc.x) < p.t_cross && G >= 2)
+            q = 1 + static_cast<int>(index_below(rc.y, static_cast<uint32_t>(G - 1)));
+        s_cut = q;
+    }
+    __syncthreads();
+    const float* A = W + static_cast<size_t>(s_parent[0]) * G;
+    const float* B = W + static_cast<size_t>(s_parent[1]) * G;
+    const int q = s_cut;
+    float* child = Wn + static_cast<size_t>(c) * G;
+    // per-gene Gaussian mutation, no clamping (D6)
+    for (int g = tid; g < G; g += kGaThreads) {
+        float v = g < q ? A[g] : B[g];
+        const uint4 rm = philox4x32_10(static_cast<uint32_t>(g), static_cast<uint32_t>(c), p.gen, kTagMutate, p.key);
+        if (static_cast<unsigned long long>(rm.x) < p.t_mut) {
+            const float z = gauss_from_words(rm.y, rm.z);
+            v = __fadd_rn(v, __fmul_rn(p.sigma, z));
+        }
+        child[g] = v;
+    }
+}
+
+// ---- fitness finalisation: F[m] = (sum over partial rows, in row order) / P in fp64, rounded to fp32
+// (PAPER.md:63 MSE).  Optionally the best (lowest, NaN worst, ties -> lower index) fitness of the
+// population is written to *best_out by the last block to finish (R8).
+constexpr int kFinThreads = 256;
+
+__global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* __restrict__ part,
+                                                                        int n_part, int m_stride, int M,
+                                                                        double P_d, float* __restrict__ F,
+                                                                        float* __restrict__ best_out,
+                                                                        float* __restrict__ blk_key,
+                                                                        int* __restrict__ blk_idx,
+                                                                        unsigned int* __restrict__ ticket) {
+    __shared__ float s_key[kFinThreads / 32];
+    __shared__ int s_idx[kFinThreads / 32];
+    __shared__ bool s_last;
+    const int m = blockIdx.x * kFinThreads + threadIdx.x;
+    float key = INFINITY;
+    int idx = 0x7fffffff;
+    if (m < M) {
+        double s = 0.0;
+        for (int r = 0; r < n_part; ++r) s += __ldcg(part + static_cast<size_t>(r) * m_stride + m);
+        const float f = static_cast<float>(s / P_d);
+        F[m] = f;
+        key = fit_key(f);
+        idx = m;
+    }
+    if (best_out == nullptr) return;
+    __threadfence();  // F[m] visible device-wide before this block takes its ticket
+    auto warp_min = [](float& k, int& i) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ok = __shfl_xor_sync(0xffffffffu, k, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, i, o);
+            if (precedes(ok, oi, k, i)) {
+                k = ok;
+                i = oi;
+            }
+        }
+    };
+    warp_min(key, idx);
+    if ((threadIdx.x & 31) == 0) {
+        s_key[threadIdx.x >> 5] = key;
+        s_idx[threadIdx.x >> 5] = idx;
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        key = threadIdx.x < kFinThreads / 32 ? s_key[threadIdx.x] : INFINITY;
+        idx = threadIdx.x < kFinThreads / 32 ? s_idx[threadIdx.x] : 0x7fffffff;
+        warp_min(key, idx);
+        if (threadIdx.x == 0) {
+            blk_key[blockIdx.x] = key;
+            blk_idx[blockIdx.x] = idx;
+            __threadfence();
+            const unsigned int t = atomicAdd(ticket, 1u);
+            s_last = (t == gridDim.x - 1);
+        }
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (threadIdx.x < 32) {
+        key = INFINITY;
+        idx = 0x7fffffff;
+        for (int b = threadIdx.x; b < static_cast<int>(gridDim.x); b += 32) {
+            const float ok = __ldcg(blk_key + b);
+            const int oi = __ldcg(blk_idx + b);
+            if (precedes(ok, oi, key, idx)) {
+                key = ok;
+                idx = oi;
+            }
+        }
+        warp_min(key, idx);
+        if (threadIdx.x == 0) {
+            *best_out = __ldcg(F + idx);  // the fitness itself (NaN if every chromosome is NaN: idx = 0)
+            *ticket = 0u;
+        }
+    }
+}
+
+}  // namespace game

@@ -1,0 +1,468 @@
+// libgame.so: the C ABI of include/game.h -- context, argument validation, state machine and host-side
+// orchestration (one stream, no per-generation host synchronisation).  Every step of the
+// hot path runs in the kernels of this directory; there is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/game.h"
+#include "fitness_ffma.cuh"
+#include "fitness_umma.cuh"
+#include "ga_kernels.cuh"
+
+namespace {
+
+constexpr int kMaxCtas = 160;            // persistent grid cap (B200: 148 SMs)
+constexpr int kMaxPartRows = 2 * kMaxCtas;
+constexpr size_t kAlign = 256;
+constexpr size_t kMaxTimedLaunches = 8192;
+
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+}  // namespace
+
+struct game_ctx {
+    // shapes
+    long long P = 0;
+    int N = 0, d = 0, M = 0, G = 0, expansion = 0, act = 0;
+    // tensor-core path geometry
+    bool umma_ok = false;
+    int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
+    // workspace layout (byte offsets)
+    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, ws_bytes = 0;
+    // bound buffers (borrowed)
+    const float* X = nullptr;
+    const float* t = nullptr;
+    float* pop[2] = {nullptr, nullptr};
+    float* fitness = nullptr;
+    unsigned char* ws = nullptr;
+    int cur = 0;
+    bool fitness_valid = false;
+    bool ticket_zeroed = false;
+    // GA parameters
+    int elite = 2, tournament = 3;
+    double p_cross = 0.9, p_mut = 0.05;
+    float sigma = 0.1f;
+    // execution
+    cudaStream_t stream = nullptr;
+    int scheme = GAME_SCHEME_AUTO;
+    bool device_checked = false;
+    int num_sms = 0;
+    unsigned long long launches = 0;
+    bool timing = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> events;
+    char err[256] = {0};
+};
+
+namespace {
+
+int fail(const game_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(const_cast<game_ctx*>(c)->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+int cuda_fail(game_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, GAME_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+#define GAME_CUDA(call)                                        \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) return cuda_fail(c, e__, #call); \
+    } while (0)
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int resolved_scheme(const game_ctx* c) {
+    if (c->scheme == GAME_SCHEME_AUTO) return c->umma_ok ? GAME_SCHEME_F16X3 : GAME_SCHEME_FFMA;
+    return c->scheme;
+}
+
+int ensure_device(game_ctx* c) {
+    if (c->device_checked) return GAME_OK;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n < 1) {
+        cudaGetLastError();
+        return fail(c, GAME_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    int dev = 0;
+    GAME_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    GAME_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return fail(c, GAME_ERR_CUDA, "device is sm_%d%d; this library is built for sm_100a only", prop.major, prop.minor);
+    c->num_sms = prop.multiProcessorCount;
+    using namespace game;
+    GAME_CUDA(cudaFuncSetAttribute(fitness_ffma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kFfmaMaxG * kFfmaTile * 4));
+#define GAME_SET_SMEM(E, A) \
+    GAME_CUDA(cudaFuncSetAttribute(umma::fitness_umma_kernel<E, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, umma::kSmemBytes))
+    GAME_SET_SMEM(0, 0); GAME_SET_SMEM(0, 1); GAME_SET_SMEM(0, 2);
+    GAME_SET_SMEM(1, 0); GAME_SET_SMEM(1, 1); GAME_SET_SMEM(1, 2);
+#undef GAME_SET_SMEM
+    c->device_checked = true;
+    return GAME_OK;
+}
+
+int check_launch(game_ctx* c, const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, what);
+    c->launches += 1;
+    return GAME_OK;
+}
+
+// One fitness evaluation of the current population; best_out (device) may be NULL.
+int eval_internal(game_ctx* c, float* best_out) {
+    using namespace game;
+    if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_load_kb");
+    if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_bind_state");
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    const int scheme = resolved_scheme(c);
+    if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers N <= 32 (Chebyshev) / N <= 16 (trig) and d <= 64");
+    if (!c->ticket_zeroed) {
+        GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
+        c->ticket_zeroed = true;
+    }
+    double* part = reinterpret_cast<double*>(c->ws + c->off_part);
+    const float* W = c->pop[c->cur];
+    int n_part = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    const bool timed = c->timing && c->events.size() < kMaxTimedLaunches;
+    if (timed) {
+        GAME_CUDA(cudaEventCreate(&ev0));
+        GAME_CUDA(cudaEventCreate(&ev1));
+    }
+    if (scheme == GAME_SCHEME_F16X3) {
+        uint8_t* img = c->ws + c->off_img;
+        const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
+        umma::build_w_images_kernel<<<static_cast<unsigned>((n_thr + 255) / 256), 256, 0, c->stream>>>(
+            W, img, c->M, c->G, c->N, c->d, c->expansion, c->steps_per_chunk, c->steps, c->m_tiles);
+        if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
+        umma::Params prm;
+        prm.X = c->X; prm.t = c->t; prm.Wimg = img; prm.part = part;
+        prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M;
+        prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
+        prm.p_tiles = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
+        const int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+        // work unit = (pattern tile, group of chromosome tiles): aim for >= 16 units per CTA so that the
+        // static round-robin assignment stays balanced when there are few pattern tiles
+        long long want = (16ll * grid_cap + prm.p_tiles - 1) / prm.p_tiles;
+        if (want < 1) want = 1;
+        if (want > c->m_tiles) want = c->m_tiles;
+        prm.m_tiles_per_group = static_cast<int>((c->m_tiles + want - 1) / want);
+        prm.m_groups = (c->m_tiles + prm.m_tiles_per_group - 1) / prm.m_tiles_per_group;
+        prm.chunks = c->chunks; prm.steps_per_chunk = c->steps_per_chunk; prm.steps = c->steps;
+        const long long units = static_cast<long long>(prm.p_tiles) * prm.m_groups;
+        const int grid = static_cast<int>(units < grid_cap ? units : grid_cap);
+        n_part = 2 * grid;
+        if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
+#define GAME_LAUNCH(E, A) umma::fitness_umma_kernel<E, A><<<grid, umma::kThreads, umma::kSmemBytes, c->stream>>>(prm)
+        const int sel = c->expansion * 3 + c->act;
+        switch (sel) {
+            case 0: GAME_LAUNCH(0, 0); break;
+            case 1: GAME_LAUNCH(0, 1); break;
+            case 2: GAME_LAUNCH(0, 2); break;
+            case 3: GAME_LAUNCH(1, 0); break;
+            case 4: GAME_LAUNCH(1, 1); break;
+            default: GAME_LAUNCH(1, 2); break;
+        }
+#undef GAME_LAUNCH
+        if ((rc = check_launch(c, "fitness_umma_kernel"))) return rc;
+        if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
+    } else {
+        const long long n_tiles = (c->P + kFfmaTile - 1) / kFfmaTile;
+        const size_t smem = static_cast<size_t>(c->G) * kFfmaTile * sizeof(float);
+        int per_sm = static_cast<int>((220u * 1024u) / (smem + 1024));
+        if (per_sm < 1) per_sm = 1;
+        long long grid_ll = static_cast<long long>(c->num_sms) * per_sm;
+        if (grid_ll > kMaxPartRows) grid_ll = kMaxPartRows;
+        if (grid_ll > n_tiles) grid_ll = n_tiles;
+        const int grid = static_cast<int>(grid_ll);
+        n_part = grid;
+        if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
+        fitness_ffma_kernel<<<grid, kFfmaTile, smem, c->stream>>>(c->X, c->t, W, part, c->P, c->N, c->d, c->M, c->G,
+                                                                   c->expansion, c->act, c->m_stride, n_tiles);
+        if ((rc = check_launch(c, "fitness_ffma_kernel"))) return rc;
+        if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
+    }
+    if (timed) c->events.emplace_back(ev0, ev1);
+    const int fin_blocks = (c->M + kFinThreads - 1) / kFinThreads;
+    finalize_fitness_kernel<<<fin_blocks, kFinThreads, 0, c->stream>>>(
+        part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, best_out,
+        reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket));
+    if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
+    c->fitness_valid = true;
+    return GAME_OK;
+}
+
+int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
+    using namespace game;
+    if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_step before game_bind_state");
+    if (!c->fitness_valid) return fail(c, GAME_ERR_BAD_STATE, "game_step needs a fresh fitness (game_eval_fitness first)");
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    GaParams p;
+    p.M = c->M; p.G = c->G; p.elite = c->elite; p.tournament = c->tournament;
+    p.t_cross = bernoulli_threshold(c->p_cross);
+    p.t_mut = bernoulli_threshold(c->p_mut);
+    p.sigma = c->sigma; p.gen = gen; p.key = make_key(seed);
+    ga_step_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p);
+    if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
+    c->cur ^= 1;
+    c->fitness_valid = false;
+    return GAME_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int32_t family) {
+    if (!out) return GAME_ERR_INVALID_ARG;
+    *out = nullptr;
+    const int expansion = family & 0xff, act = (family >> 8) & 0xff;
+    if (P < 1 || N < 1 || d < 1 || M < 1 || (family >> 16) != 0) return GAME_ERR_INVALID_ARG;
+    if (expansion > GAME_EXP_TRIG || act > GAME_ACT_TANH) return GAME_ERR_INVALID_ARG;
+    if (P > (1ll << 40) || N > 4096 || d > 4096 || M > (1 << 24)) return GAME_ERR_INVALID_ARG;
+    const long long G = static_cast<long long>(N) * d * (expansion == GAME_EXP_TRIG ? 2 : 1) + 1;
+    if (G > game::kFfmaMaxG) return GAME_ERR_UNSUPPORTED;
+    game_ctx* c = new (std::nothrow) game_ctx();
+    if (!c) return GAME_ERR_INVALID_ARG;
+    c->P = P; c->N = N; c->d = d; c->M = M; c->G = static_cast<int>(G);
+    c->expansion = expansion; c->act = act;
+    c->m_tiles = (M + game::umma::kBM - 1) / game::umma::kBM;
+    c->m_stride = c->m_tiles * game::umma::kBM;
+    c->umma_ok = d <= 64 && (expansion == GAME_EXP_CHEBYSHEV ? N <= 32 : N <= 16) &&
+                 (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
+    c->chunks = (N + 7) / 8;
+    c->steps_per_chunk = expansion == GAME_EXP_CHEBYSHEV ? (d + 1) / 2 : d;
+    c->steps = c->chunks * c->steps_per_chunk + 1;
+    size_t off = 0;
+    c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
+    c->off_img = off;
+    if (c->umma_ok) off = align_up(off + static_cast<size_t>(c->m_tiles) * c->steps * 2 * game::umma::kABytes);
+    const size_t fin_blocks = (static_cast<size_t>(M) + game::kFinThreads - 1) / game::kFinThreads;
+    c->off_blk_key = off; off = align_up(off + fin_blocks * sizeof(float));
+    c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
+    c->off_ticket = off; off = align_up(off + sizeof(unsigned int));
+    c->ws_bytes = off;
+    *out = c;
+    return GAME_OK;
+}
+
+int game_destroy(game_ctx* c) {
+    if (!c) return GAME_OK;
+    for (auto& ev : c->events) {
+        cudaEventDestroy(ev.first);
+        cudaEventDestroy(ev.second);
+    }
+    delete c;
+    return GAME_OK;
+}
+
+int game_num_genes(const game_ctx* c, int32_t* G) {
+    if (!c || !G) return GAME_ERR_INVALID_ARG;
+    *G = c->G;
+    return GAME_OK;
+}
+
+int game_workspace_bytes(const game_ctx* c, size_t* bytes) {
+    if (!c || !bytes) return GAME_ERR_INVALID_ARG;
+    *bytes = c->ws_bytes;
+    return GAME_OK;
+}
+
+int game_set_stream(game_ctx* c, void* cuda_stream) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    return GAME_OK;
+}
+
+int game_set_scheme(game_ctx* c, int32_t scheme) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (scheme < GAME_SCHEME_AUTO || scheme > GAME_SCHEME_F16X3) return fail(c, GAME_ERR_INVALID_ARG, "unknown scheme %d", scheme);
+    if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers N <= 32 (Chebyshev) / N <= 16 (trig) and d <= 64");
+    c->scheme = scheme;
+    return GAME_OK;
+}
+
+int game_get_scheme(const game_ctx* c, int32_t* scheme) {
+    if (!c || !scheme) return GAME_ERR_INVALID_ARG;
+    *scheme = resolved_scheme(c);
+    return GAME_OK;
+}
+
+int game_load_kb(game_ctx* c, const float* X_dev, const float* t_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!X_dev || !t_dev) return fail(c, GAME_ERR_INVALID_ARG, "null knowledge-base pointer");
+    if (!aligned16(X_dev) || !aligned16(t_dev)) return fail(c, GAME_ERR_INVALID_ARG, "knowledge-base pointers must be 16-byte aligned");
+    c->X = X_dev;
+    c->t = t_dev;
+    c->fitness_valid = false;
+    return GAME_OK;
+}
+
+int game_bind_state(game_ctx* c, float* popA_dev, float* popB_dev, float* fitness_dev, void* workspace_dev,
+                    size_t workspace_bytes) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!popA_dev || !popB_dev || !fitness_dev || !workspace_dev) return fail(c, GAME_ERR_INVALID_ARG, "null state pointer");
+    if (popA_dev == popB_dev) return fail(c, GAME_ERR_INVALID_ARG, "popA_dev and popB_dev must be distinct buffers");
+    if (!aligned16(popA_dev) || !aligned16(popB_dev) || !aligned16(fitness_dev) ||
+        (reinterpret_cast<uintptr_t>(workspace_dev) & (kAlign - 1)) != 0)
+        return fail(c, GAME_ERR_INVALID_ARG, "state pointers must be 16-byte aligned (workspace: 256)");
+    if (workspace_bytes < c->ws_bytes)
+        return fail(c, GAME_ERR_WORKSPACE, "workspace has %zu bytes, game_workspace_bytes says %zu", workspace_bytes, c->ws_bytes);
+    c->pop[0] = popA_dev;
+    c->pop[1] = popB_dev;
+    c->fitness = fitness_dev;
+    c->ws = static_cast<unsigned char*>(workspace_dev);
+    c->cur = 0;
+    c->fitness_valid = false;
+    c->ticket_zeroed = false;
+    return GAME_OK;
+}
+
+int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_cross, double p_mut, float sigma) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (elite < 0 || elite >= c->M) return fail(c, GAME_ERR_INVALID_ARG, "elite must be in [0, M)");
+    if (tournament < 1 || tournament > (1 << 20)) return fail(c, GAME_ERR_INVALID_ARG, "tournament must be >= 1");
+    if (!(p_cross >= 0.0 && p_cross <= 1.0) || !(p_mut >= 0.0 && p_mut <= 1.0))
+        return fail(c, GAME_ERR_INVALID_ARG, "probabilities must be in [0, 1]");
+    if (!(sigma >= 0.0f) || !std::isfinite(sigma)) return fail(c, GAME_ERR_INVALID_ARG, "sigma must be finite and >= 0");
+    c->elite = elite; c->tournament = tournament;
+    c->p_cross = p_cross; c->p_mut = p_mut; c->sigma = sigma;
+    return GAME_OK;
+}
+
+int game_init_population(game_ctx* c, uint64_t seed) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_init_population before game_bind_state");
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    const long long n = static_cast<long long>(c->M) * ((c->G + 3) / 4);
+    game::init_population_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, c->stream>>>(c->pop[c->cur], c->M, c->G,
+                                                                                               game::make_key(seed));
+    if ((rc = check_launch(c, "init_population_kernel"))) return rc;
+    c->fitness_valid = false;
+    return GAME_OK;
+}
+
+int game_current_population(const game_ctx* c, float** pop_dev) {
+    if (!c || !pop_dev) return GAME_ERR_INVALID_ARG;
+    if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_current_population before game_bind_state");
+    *pop_dev = c->pop[c->cur];
+    return GAME_OK;
+}
+
+int game_invalidate_fitness(game_ctx* c) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    c->fitness_valid = false;
+    return GAME_OK;
+}
+
+int game_assume_fitness(game_ctx* c) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->fitness) return fail(c, GAME_ERR_BAD_STATE, "game_assume_fitness before game_bind_state");
+    c->fitness_valid = true;
+    return GAME_OK;
+}
+
+int game_eval_fitness(game_ctx* c) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    return eval_internal(c, nullptr);
+}
+
+int game_step(game_ctx* c, uint64_t seed, uint32_t gen) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    return step_internal(c, seed, gen);
+}
+
+int game_run(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    for (uint32_t i = 0; i <= n_gens; ++i) {
+        int rc = eval_internal(c, best_fitness_dev ? best_fitness_dev + i : nullptr);
+        if (rc) return rc;
+        if (i == n_gens) break;
+        rc = step_internal(c, seed, gen0 + i);
+        if (rc) return rc;
+    }
+    return GAME_OK;
+}
+
+int game_sync(game_ctx* c) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    GAME_CUDA(cudaStreamSynchronize(c->stream));
+    GAME_CUDA(cudaGetLastError());
+    return GAME_OK;
+}
+
+int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, const float* W_host, float* F_host,
+                         float* W_next_host, uint64_t seed, uint32_t gen) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!X_host || !t_host || !W_host) return fail(c, GAME_ERR_INVALID_ARG, "null host input");
+    if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_generation_host before game_load_kb");
+    if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_generation_host before game_bind_state");
+    const size_t wb = sizeof(float) * static_cast<size_t>(c->M) * c->G;
+    GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->X), X_host, sizeof(float) * static_cast<size_t>(c->P) * c->N,
+                              cudaMemcpyHostToDevice, c->stream));
+    GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->t), t_host, sizeof(float) * static_cast<size_t>(c->P),
+                              cudaMemcpyHostToDevice, c->stream));
+    GAME_CUDA(cudaMemcpyAsync(c->pop[c->cur], W_host, wb, cudaMemcpyHostToDevice, c->stream));
+    c->fitness_valid = false;
+    int rc = eval_internal(c, nullptr);
+    if (rc) return rc;
+    rc = step_internal(c, seed, gen);
+    if (rc) return rc;
+    if (F_host) GAME_CUDA(cudaMemcpyAsync(F_host, c->fitness, sizeof(float) * c->M, cudaMemcpyDeviceToHost, c->stream));
+    if (W_next_host) GAME_CUDA(cudaMemcpyAsync(W_next_host, c->pop[c->cur], wb, cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(cudaStreamSynchronize(c->stream));
+    return GAME_OK;
+}
+
+int game_launch_count(const game_ctx* c, uint64_t* launches) {
+    if (!c || !launches) return GAME_ERR_INVALID_ARG;
+    *launches = c->launches;
+    return GAME_OK;
+}
+
+int game_time_fitness_kernel(game_ctx* c, int32_t enable) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    for (auto& ev : c->events) {
+        cudaEventDestroy(ev.first);
+        cudaEventDestroy(ev.second);
+    }
+    c->events.clear();
+    c->timing = enable != 0;
+    return GAME_OK;
+}
+
+int game_fitness_kernel_ms(game_ctx* c, double* total_ms, uint64_t* launches) {
+    if (!c || !total_ms || !launches) return GAME_ERR_INVALID_ARG;
+    double sum = 0.0;
+    for (auto& ev : c->events) {
+        GAME_CUDA(cudaEventSynchronize(ev.second));
+        float ms = 0.f;
+        GAME_CUDA(cudaEventElapsedTime(&ms, ev.first, ev.second));
+        sum += ms;
+    }
+    *total_ms = sum;
+    *launches = c->events.size();
+    return GAME_OK;
+}
+
+const char* game_last_error(const game_ctx* c) { return c ? c->err : "null context"; }
+
+}  // extern "C"

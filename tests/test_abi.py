@@ -1,0 +1,133 @@
+"""CPU-side checks of the C-ABI boundary (no GPU, no compute calls): the library builds for sm_100a,
+loads, exports every symbol include/game.h declares, validates arguments, enforces the call-order state
+machine, and fails loudly (GAME_ERR_CUDA) instead of falling back when there is no device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_1211_5481_b200 as game
+from paper_1211_5481_b200 import build as game_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    game_build.build()
+    return game.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "game.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(game_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_all_exported_and_bound(L):
+    names = declared_symbols()
+    assert len(names) >= 20
+    for n in names:
+        assert hasattr(L, n), f"libgame.so does not export {n}"
+    assert sorted(game.SIGNATURES) == names, "binding and header disagree on the symbol list"
+    for n in names:
+        assert callable(getattr(game, n)), f"python binding lacks {n}"
+
+
+def test_no_oracle_or_cpu_fallback_in_product():
+    """The product path must not import or link the oracle (tests/, smoke and bench's cpu legs only)."""
+    pkg = os.path.join(ROOT, "paper_1211_5481_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "game_oracle" not in src, f
+
+
+def test_num_genes_matches_baseline_configs(L):
+    # tests/golden/baseline_gene_counts.txt: BASELINE.json configs c0..c4 -> 13, 61, 129, 321, 121
+    rows = [l.split() for l in open(os.path.join(ROOT, "tests", "golden", "baseline_gene_counts.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 5
+    for name, N, d, expansion, G in rows:
+        ctx = game.game_create(1000, int(N), int(d), 64, game.family(int(expansion), game.ACT_SIGMOID))
+        assert game.game_num_genes(ctx) == int(G), name
+        assert game.game_workspace_bytes(ctx) > 0
+        game.game_destroy(ctx)
+
+
+@pytest.mark.parametrize("args", [
+    (0, 4, 3, 64, 0x0100), (10, 0, 3, 64, 0x0100), (10, 4, 0, 64, 0x0100), (10, 4, 3, 0, 0x0100),
+    (10, 4, 3, 64, 0x0002), (10, 4, 3, 64, 0x0300), (10, 4, 3, 64, 0x10100),
+])
+def test_create_rejects_bad_shapes(L, args):
+    ctx = C.c_void_p()
+    assert L.game_create(C.byref(ctx), *args) == game.ERR_INVALID_ARG
+    assert ctx.value is None
+
+
+def test_create_unsupported_gene_count(L):
+    ctx = C.c_void_p()
+    assert L.game_create(C.byref(ctx), 10, 64, 10, 8, 0x0100) == game.ERR_UNSUPPORTED   # G = 641 > 448
+
+
+def test_scheme_resolution(L):
+    ctx = game.game_create(1000, 32, 10, 4096, 0x0100)
+    assert game.game_get_scheme(ctx) == game.SCHEME_F16X3
+    game.game_set_scheme(ctx, game.SCHEME_FFMA)
+    assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
+    game.game_destroy(ctx)
+    ctx = game.game_create(1000, 40, 10, 64, 0x0100)          # N > 32: tensor-core kernel does not cover it
+    assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
+    with pytest.raises(game.GameError) as e:
+        game.game_set_scheme(ctx, game.SCHEME_F16X3)
+    assert e.value.code == game.ERR_UNSUPPORTED
+    game.game_destroy(ctx)
+
+
+def test_ga_param_validation_and_state_machine(L):
+    ctx = game.game_create(1000, 4, 3, 64, 0x0100)
+    for bad in [(-1, 3, .9, .05, .1), (64, 3, .9, .05, .1), (2, 0, .9, .05, .1), (2, 3, 1.5, .05, .1),
+                (2, 3, .9, -0.1, .1), (2, 3, .9, .05, -1.0), (2, 3, .9, .05, float("nan")), (2, 3, float("nan"), .05, .1)]:
+        with pytest.raises(game.GameError) as e:
+            game.game_set_ga_params(ctx, *bad)
+        assert e.value.code == game.ERR_INVALID_ARG, bad
+    game.game_set_ga_params(ctx, 0, 1, 0.0, 1.0, 0.0)
+    # call order: nothing bound yet
+    for fn in (game.game_eval_fitness, lambda c: game.game_step(c, 1, 0), lambda c: game.game_init_population(c, 1),
+               game.game_current_population, lambda c: game.game_run(c, 1, 0, 2, None)):
+        with pytest.raises(game.GameError) as e:
+            fn(ctx)
+        assert e.value.code == game.ERR_BAD_STATE
+    # alignment and workspace size
+    with pytest.raises(game.GameError) as e:
+        game.game_load_kb(ctx, 0x1004, 0x2000)
+    assert e.value.code == game.ERR_INVALID_ARG
+    with pytest.raises(game.GameError) as e:
+        game.game_bind_state(ctx, 0x10000, 0x20000, 0x30000, 0x40000, 16)
+    assert e.value.code == game.ERR_WORKSPACE
+    with pytest.raises(game.GameError) as e:
+        game.game_bind_state(ctx, 0x10000, 0x10000, 0x30000, 0x40000, 1 << 30)
+    assert e.value.code == game.ERR_INVALID_ARG
+    game.game_destroy(ctx)
+
+
+def test_fails_loudly_without_a_device(L):
+    """No CPU fallback: with (fake) buffers bound, a compute call on a box without a GPU is GAME_ERR_CUDA."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    ctx = game.game_create(1000, 4, 3, 64, 0x0100)
+    game.game_load_kb(ctx, 0x100000, 0x200000)
+    game.game_bind_state(ctx, 0x300000, 0x400000, 0x500000, 0x600000, game.game_workspace_bytes(ctx))
+    for fn in (game.game_eval_fitness, lambda c: game.game_init_population(c, 1)):
+        with pytest.raises(game.GameError) as e:
+            fn(ctx)
+        assert e.value.code == game.ERR_CUDA
+    with pytest.raises(game.GameError) as e:          # step needs a fitness first
+        game.game_step(ctx, 1, 0)
+    assert e.value.code == game.ERR_BAD_STATE
+    game.game_destroy(ctx)
+    with pytest.raises(RuntimeError):
+        game.Game(1000, 4, 3, 64, 0, 1)

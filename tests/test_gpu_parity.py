@@ -1,0 +1,279 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs (workloads.py).  Bars (BASELINE.json north_star): GA operators and population init
+bit-exact; per-chromosome fitness within 1e-5 relative; best-fitness trajectories within 1e-4."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL = 1e-5          # north_star: per-chromosome fitness relative error
+ABS_FLOOR = 1e-10       # only matters where the reference fitness is ~0 (noiseless-regression pin)
+
+
+@pytest.fixture(scope="module")
+def game():
+    import paper_1211_5481_b200 as g
+    from paper_1211_5481_b200 import build
+    build.build()
+    g.lib()
+    return g
+
+
+def make(game, cfg, scheme=0):
+    G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation, scheme=scheme)
+    assert G.G == cfg.G
+    G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+    return G
+
+
+def assert_fitness_close(F_gpu, F_ref, what=""):
+    F_gpu = np.asarray(F_gpu, dtype=np.float64)
+    err = np.abs(F_gpu - F_ref)
+    bound = REL_TOL * np.abs(F_ref) + ABS_FLOOR
+    worst = int(np.argmax(err - bound))
+    assert np.all(err <= bound), (f"{what}: chromosome {worst}: gpu {F_gpu[worst]!r} ref {F_ref[worst]!r} "
+                                   f"rel {err[worst] / max(abs(F_ref[worst]), 1e-300):.3e}")
+    return float(np.max(err / np.maximum(np.abs(F_ref), 1e-300)))
+
+
+SCHEMES = [1, 2]   # FFMA, F16X3
+
+# (name, base config, overrides): several tiles + ragged tails in P (256-pattern tiles) and M (128-chromosome tiles)
+FITNESS_CASES = [
+    ("c0_full", "c0", {}),
+    ("c0_ragged", "c0", dict(P=777, M=37)),
+    ("c1_slice", "c1", dict(P=5000, M=200)),
+    ("c1_one_pattern", "c1", dict(P=1, M=5)),
+    ("c2_slice", "c2", dict(P=3000, M=130)),
+    ("c3_slice", "c3", dict(P=1100, M=260)),
+    ("c4_slice", "c4", dict(P=2049, M=129)),
+    ("odd_shapes", "c1", dict(P=1537, N=9, d=5, M=131)),
+    ("trig_odd", "c2", dict(P=700, N=5, d=3, M=33)),
+    ("identity_cheb", "c1", dict(P=2000, M=64, activation=wl.ACT_IDENTITY)),
+    ("tanh_cheb", "c1", dict(P=2000, M=64, activation=wl.ACT_TANH)),
+    ("sigmoid_trig", "c2", dict(P=2000, M=64, activation=wl.ACT_SIGMOID)),
+    ("d1", "c1", dict(P=1000, N=3, d=1, M=16)),
+]
+
+
+def case_cfg(base, over):
+    cfg = wl.c4(256, 100_000) if base == "c4" else wl.CONFIGS[base]
+    return wl.scaled(cfg, **over)
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("name,base,over", FITNESS_CASES, ids=[c[0] for c in FITNESS_CASES])
+def test_fitness_matches_oracle(game, name, base, over, scheme):
+    cfg = case_cfg(base, over)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, seed=100 + cfg.seed)
+    G = make(game, cfg, scheme)
+    G.load_kb(X, t)
+    G.set_population(W)
+    G.eval_fitness()
+    G.sync()
+    assert G.scheme() == scheme
+    F_ref = oracle.eval_fitness(cfg.d, cfg.family, X, t, W)
+    assert_fitness_close(G.get_fitness(), F_ref, f"{name} scheme {scheme}")
+    G.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_fitness_closed_forms_on_gpu(game, scheme):
+    """W = 0 -> sigmoid fitness exactly 0.25 on 0/1 labels; generating chromosome on noiseless regression
+    targets -> fitness ~ 0 (absolute floor); duplicate chromosomes -> identical fitness in any slot."""
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=3000, M=140)
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg, scheme)
+    G.load_kb(X, t)
+    G.set_population(np.zeros((cfg.M, cfg.G), np.float32))
+    G.eval_fitness(); G.sync()
+    assert np.all(G.get_fitness() == np.float32(0.25))
+    W = wl.uniform_population(cfg.M, cfg.G, 5)
+    W[137] = W[3]; W[64] = W[3]
+    G.set_population(W); G.eval_fitness(); G.sync()
+    F = G.get_fitness()
+    assert F[137] == F[3] == F[64]
+    G.close()
+    # noiseless regression, tanh / trig
+    cfg = wl.scaled(wl.CONFIGS["c2"], P=2500, M=130, noise_std=0.0)
+    X, t, w_star = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 6)
+    W[7] = w_star.astype(np.float32)
+    t = np.tanh(wl._design_matrix(cfg, X.astype(np.float64)) @ W[7].astype(np.float64)).astype(np.float32)
+    G = make(game, cfg, scheme)
+    G.load_kb(X, t); G.set_population(W); G.eval_fitness(); G.sync()
+    F = G.get_fitness()
+    assert F[7] <= 1e-10 + 1e-14, F[7]      # float32 rounding of t leaves ~1e-15
+    assert_fitness_close(F, oracle.eval_fitness(cfg.d, cfg.family, X, t, W), "noiseless")
+    G.close()
+
+
+def test_fitness_is_deterministic_and_schemes_agree(game):
+    cfg = wl.scaled(wl.CONFIGS["c3"], P=5000, M=300)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 9)
+    out = {}
+    for scheme in SCHEMES:
+        G = make(game, cfg, scheme)
+        G.load_kb(X, t); G.set_population(W)
+        G.eval_fitness(); G.sync(); a = G.get_fitness()
+        G.eval_fitness(); G.sync(); b = G.get_fitness()
+        assert np.array_equal(a, b), "run-to-run bit stability"
+        out[scheme] = a.astype(np.float64)
+        G.close()
+    assert np.max(np.abs(out[1] - out[2]) / out[1]) < 2e-6
+
+
+def test_nan_and_inf_propagate(game):
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=600, M=20)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 3)
+    W[4, 2] = np.nan
+    for scheme in SCHEMES:
+        G = make(game, cfg, scheme)
+        G.load_kb(X, t); G.set_population(W); G.eval_fitness(); G.sync()
+        F = G.get_fitness()
+        assert np.isnan(F[4]) and np.all(np.isfinite(np.delete(F, 4)))
+        G.close()
+
+
+# ------------------------------------------------------------------------------------------------ GA operators
+@pytest.mark.parametrize("M,G_,seed", [(64, 13, 0), (512, 61, 1), (1000, 129, 2), (37, 1, 3), (130, 321, 2**40 + 17)])
+def test_init_population_bit_exact(game, M, G_, seed):
+    N, d = (G_ - 1, 1) if G_ > 1 else (1, 1)
+    if G_ == 1:
+        pytest.skip("G = 1 needs N*d = 0")
+    G = game.Game(300, N, d, M, wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    G.init_population(seed); G.sync()
+    W = G.get_population()
+    assert np.array_equal(W.view(np.uint32), oracle.init_population(M, G_, seed).view(np.uint32))
+    assert W.min() >= -1.0 and W.max() < 1.0
+    G.close()
+
+
+STEP_CASES = [
+    # M, N, d, E, k, p_cross, p_mut, sigma, seed, gen
+    (64, 4, 3, 2, 3, 0.9, 0.05, 0.1, 0, 0),
+    (512, 10, 6, 4, 3, 0.9, 0.05, 0.1, 1, 7),
+    (1024, 16, 8, 8, 4, 0.9, 0.02, 0.05, 2, 49),
+    (4096, 32, 10, 4, 3, 0.9, 0.05, 0.1, 3, 19),
+    (100, 5, 4, 0, 1, 0.0, 0.0, 0.0, 4, 1),
+    (100, 5, 4, 99, 2, 1.0, 1.0, 0.5, 5, 2),
+    (33, 2, 1, 1, 7, 0.5, 0.5, 1.0, 2**63 + 5, 2**31 + 3),
+    (257, 7, 3, 3, 2, 1.0, 0.2, 0.1, 6, 123456),
+]
+
+
+@pytest.mark.parametrize("M,N,d,E,k,pc,pm,sigma,seed,gen", STEP_CASES)
+def test_ga_step_bit_exact_on_given_fitness(game, M, N, d, E, k, pc, pm, sigma, seed, gen):
+    """Same fitness vector and seed in, bit-identical next population out (north_star)."""
+    rng = np.random.Generator(np.random.Philox(1000 + M))
+    G = game.Game(300, N, d, M, wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    W = rng.uniform(-2, 2, size=(M, G.G)).astype(np.float32)
+    F = rng.uniform(0, 1, size=M).astype(np.float32)
+    F[rng.integers(0, M, size=max(1, M // 8))] = F[0]          # ties
+    if M > 40:
+        F[5] = np.nan; F[17] = np.inf; F[20] = -0.0; F[21] = 0.0
+    G.set_ga_params(E, k, pc, pm, sigma)
+    G.set_population(W); G.set_fitness(F)
+    G.step(seed, gen); G.sync()
+    Wn = G.get_population()
+    ref = oracle.step(W, F, E, k, pc, pm, sigma, seed, gen)
+    assert np.array_equal(Wn.view(np.uint32), ref.view(np.uint32)), \
+        f"{np.count_nonzero(Wn.view(np.uint32) != ref.view(np.uint32))} genes differ"
+    G.close()
+
+
+def test_step_state_machine_on_gpu(game):
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=300)
+    G = make(game, cfg)
+    G.init_population(1)
+    with pytest.raises(game.GameError) as e:
+        G.step(1, 0)
+    assert e.value.code == game.ERR_BAD_STATE
+    X, t, _ = wl.make_kb(cfg)
+    G.load_kb(X, t)
+    G.eval_fitness(); G.step(1, 0)
+    with pytest.raises(game.GameError):
+        G.step(1, 1)           # fitness is stale after a step
+    G.sync(); G.close()
+
+
+# ------------------------------------------------------------------------------------------------ trajectories
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("base,over", [("c0", {}), ("c1", dict(P=4000, M=256, generations=12)),
+                                       ("c2", dict(P=3000, M=128, generations=8))])
+def test_lockstep_and_free_running_trajectory(game, base, over, scheme):
+    """Lock-step: every generation the oracle steps on the GPU's fitness vector -> populations stay
+    bit-identical and GPU fitness stays within 1e-5 of the oracle's fitness of the same population.
+    Free-running: game_run's best-fitness trace within 1e-4 of the oracle's run."""
+    import torch
+    cfg = case_cfg(base, over)
+    X, t, _ = wl.make_kb(cfg)
+    seed, n = 1234 + cfg.seed, cfg.generations
+    G = make(game, cfg, scheme)
+    G.load_kb(X, t)
+    G.init_population(seed); G.sync()
+    W0 = G.get_population()
+    assert np.array_equal(W0.view(np.uint32), oracle.init_population(cfg.M, cfg.G, seed).view(np.uint32))
+    W = W0.copy()
+    best_lock = []
+    for g in range(n):
+        G.eval_fitness(); G.sync()
+        F_gpu = G.get_fitness()
+        assert_fitness_close(F_gpu, oracle.eval_fitness(cfg.d, cfg.family, X, t, W), f"gen {g}")
+        best_lock.append(F_gpu[oracle.best_index(F_gpu)])
+        G.step(seed, g); G.sync()
+        W = oracle.step(W, F_gpu, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, seed, g)
+        assert np.array_equal(G.get_population().view(np.uint32), W.view(np.uint32)), f"population forked at gen {g}"
+    # free-running on the device, one sync at the end
+    G.set_population(W0)
+    best = torch.full((n + 1,), float("nan"), dtype=torch.float32, device="cuda:0")
+    G.run(seed, 0, n, best); G.sync()
+    best = best.cpu().numpy()
+    assert np.array_equal(best[:n], np.asarray(best_lock, np.float32)), "run() must replay the lock-step generations"
+    _, _, best_ref = oracle.run(cfg.d, cfg.family, X, t, W0, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut,
+                                cfg.sigma, seed, 0, n)
+    dev = np.abs(best.astype(np.float64) - best_ref) / np.maximum(np.abs(best_ref), 1e-6)
+    assert np.all(dev <= 1e-4), dev
+    if cfg.elite >= 1:
+        assert np.all(np.diff(best) <= 0), "best fitness must not get worse with elitism"
+    G.close()
+
+
+def test_checkpoint_resume_bit_exact(game):
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=500)
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg); G.load_kb(X, t); G.init_population(5)
+    G.run(5, 0, 6, None); G.sync()
+    full = G.get_population()
+    G.init_population(5); G.run(5, 0, 3, None); G.sync()
+    ckpt = G.get_population()
+    G.close()
+    G2 = make(game, cfg); G2.load_kb(X, t); G2.set_population(ckpt)
+    G2.run(5, 3, 3, None); G2.sync()
+    assert np.array_equal(G2.get_population().view(np.uint32), full.view(np.uint32))
+    G2.close()
+
+
+def test_generation_host_entry(game):
+    """The host-buffer entry point = load + eval + step + download."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=3000, M=150)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 11)
+    G = make(game, cfg)
+    Xh, th, Wh = (torch.from_numpy(a).pin_memory() for a in (X, t, W))
+    Fh = torch.empty(cfg.M, dtype=torch.float32).pin_memory()
+    Wn = torch.empty((cfg.M, cfg.G), dtype=torch.float32).pin_memory()
+    game.game_generation_host(G.ctx, Xh.data_ptr(), th.data_ptr(), Wh.data_ptr(), Fh.data_ptr(), Wn.data_ptr(), 77, 3)
+    F = Fh.numpy()
+    assert_fitness_close(F, oracle.eval_fitness(cfg.d, cfg.family, X, t, W), "host entry")
+    ref = oracle.step(W, F, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 77, 3)
+    assert np.array_equal(Wn.numpy().view(np.uint32), ref.view(np.uint32))
+    assert G.launch_count() >= 3
+    G.close()
