@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the GAME hot path (arXiv:1211.5481) on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3] [--impl ours|reference]
+
+A *step* is one whole generation of the hot path over the synthetic knowledge base: fused fitness
+evaluation of the population + the GA generation kernel (a6-a10), enqueued on one
+stream with no host synchronisation between steps (a11).  Metric (BASELINE.json): chromosome-pattern
+fitness evaluations per second = P * M * K / t.  Workload: BASELINE.json configs[3] ("c3", the config the
+roofline headline is quoted on; it fits one GPU); --workload c0|c1|c2|c3 selects another.
+
+Legs of one run (N = 1): value (inputs resident in HBM), e2e (game_generation_host: pinned host buffers,
+H2D of the knowledge base + population and D2H of fitness + next population inside the timed region),
+roofline (the fused fitness kernel's executed tensor flops / its CUDA-event duration, against the measured
+fp16/bf16 peak of MEASURED_PEAKS.json), cpu_baseline (the oracle, as it stands, one host thread, on a bounded
+sample).  N > 1: replicas only (the path is single-GPU by BASELINE.json north_star):
+every rank runs the same workload on its own GPU, timing is the max over ranks, value the sum of units.
+--impl reference times the CPU oracle on bounded samples of the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import workloads as wl
+
+METRIC = "chromosome_pattern_fitness_evals_per_s"
+UNIT = "evals/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists).
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scheme", default="auto", choices=["auto", "ffma", "f16x3"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled every 100 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thread, self.index = [], None, None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        busy = [v for v in sm if mx and v > 0.3 * mx] or sm
+        return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(cfg, X, t, W, p_sample: int, seed: int, gen: int):
+    """One generation of the oracle (as it stands, one thread) on the first p_sample patterns."""
+    import oracle
+    t0 = time.perf_counter()
+    F = oracle.eval_fitness(cfg.d, cfg.family, X[:p_sample], t[:p_sample], W)
+    Wn = oracle.step(W, F.astype(np.float32), cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, seed, gen)
+    return time.perf_counter() - t0, Wn
+
+
+def run_reference(args, cfg, rank, world):
+    """--impl reference: the CPU oracle on bounded samples of the workload; rank 0 only."""
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    p_sample = min(cfg.P, 1024 if cfg.G > 100 else 8192)
+    small = wl.scaled(cfg, P=max(p_sample, 1))
+    X, t, _ = wl.make_kb(small)
+    W = oracle.init_population(cfg.M, cfg.G, cfg.seed)
+    total = 0.0
+    for i in range(args.warmup + args.steps):
+        dt, W = oracle_sample(cfg, X, t, W, p_sample, cfg.seed, i)
+        if i >= args.warmup:
+            total += dt
+    value = p_sample * cfg.M * args.steps / total
+    sample = f"each step: first {p_sample} patterns x all {cfg.M} chromosomes of {cfg.name}, oracle eval + GA step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(cfg, "oracle (CPU, fp64, 1 thread)", args.gpus),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Multi-GPU timing rule: the job takes as long as its slowest rank."""
+    if dist is None:
+        return ms
+    import torch
+    tt = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def job_value(P: int, M: int, steps: int, world: int, ms: float) -> float:
+    """Whole-job throughput: units all ranks processed / max-over-ranks time (replicas: weak scaling)."""
+    return P * M * steps * world / (ms * 1e-3)
+
+
+def config_dict(cfg, scheme_name, n_gpus):
+    return {"workload": f"{cfg.name}: BASELINE.json configs[{cfg.name[1:]}]", "P": cfg.P, "N": cfg.N, "d": cfg.d,
+            "G": cfg.G, "M": cfg.M, "expansion": "chebyshev" if cfg.expansion == 0 else "trig",
+            "activation": ["identity", "sigmoid", "tanh"][cfg.activation], "elite": cfg.elite,
+            "tournament": cfg.tournament, "p_cross": cfg.p_cross, "p_mut": cfg.p_mut, "sigma": cfg.sigma,
+            "scheme": scheme_name, "step": "one generation = fused fitness eval + GA step kernel",
+            "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas (replicas only)",
+            "l2": "inputs larger than L2 (X = %.0f MB)" % (cfg.P * cfg.N * 4 / 1e6) if cfg.P * cfg.N * 4 > 126e6
+                  else "L2 flushed between timed steps is not possible inside a no-sync generation loop; inputs fit L2"}
+
+
+def run_ours(args, cfg, rank, world, local_rank):
+    import torch
+    import paper_1211_5481_b200 as game
+    from paper_1211_5481_b200 import build as game_build
+
+    if rank == 0:
+        game_build.build()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    dev = f"cuda:{local_rank}"
+    torch.cuda.set_device(local_rank)
+    scheme = {"auto": game.SCHEME_AUTO, "ffma": game.SCHEME_FFMA, "f16x3": game.SCHEME_F16X3}[args.scheme]
+    X, t, _ = wl.make_kb(cfg, seed=cfg.seed + 1000 * rank)           # every replica its own knowledge base
+    G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation, device=dev, scheme=scheme)
+    G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+    scheme_name = {game.SCHEME_FFMA: "FFMA fp32", game.SCHEME_F16X3: "F16X3 (3 x tcgen05 kind::f16, 2-term fp16 split, fp32 accumulate)"}[G.scheme()]
+    G.load_kb(X, t)
+    seed = cfg.seed
+    G.init_population(seed)
+    G.sync()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def generations(first_gen, n):
+        for i in range(n):
+            game.game_eval_fitness(G.ctx)
+            game.game_step(G.ctx, seed, first_gen + i)
+
+    # ---------------- device-resident leg
+    generations(0, args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = G.launch_count()
+    game.game_time_fitness_kernel(G.ctx, True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    generations(args.warmup, args.steps)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    kernel_ms, kernel_n = game.game_fitness_kernel_ms(G.ctx)
+    game.game_time_fitness_kernel(G.ctx, False)
+    launches = G.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    ms = max_over_ranks(ms, dist, dev)
+    units = cfg.P * cfg.M * args.steps * world
+    value = job_value(cfg.P, cfg.M, args.steps, world, ms)
+
+    # ---------------- end-to-end leg: host buffers through game_generation_host
+    e2e = None
+    if not args.no_e2e:
+        Xh, th = torch.from_numpy(X).pin_memory(), torch.from_numpy(t).pin_memory()
+        Wh = [torch.empty((cfg.M, cfg.G), dtype=torch.float32).pin_memory() for _ in range(2)]
+        Fh = torch.empty(cfg.M, dtype=torch.float32).pin_memory()
+        Wh[0].copy_(G.current().cpu())
+
+        def host_generations(first_gen, n, k0):
+            for i in range(n):
+                a, b = Wh[(k0 + i) & 1], Wh[(k0 + i + 1) & 1]
+                game.game_generation_host(G.ctx, Xh.data_ptr(), th.data_ptr(), a.data_ptr(), Fh.data_ptr(), b.data_ptr(),
+                                          seed, first_gen + i)
+        w = max(1, min(args.warmup, 3))
+        host_generations(10_000, w, 0)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        host_generations(10_000 + w, args.steps, w)
+        e1.record()
+        barrier()
+        ms_e2e = max(e0.elapsed_time(e1), 0.0)
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        ms_e2e = max(ms_e2e, 0.0) if ms_e2e > 0 else wall_ms
+        ms_e2e = max_over_ranks(ms_e2e, dist, dev)
+        e2e = {"value": units / (ms_e2e * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": 4 * (cfg.P * cfg.N + cfg.P + cfg.M * cfg.G) * world,
+               "d2h_bytes_per_step": 4 * (cfg.M + cfg.M * cfg.G) * world, "ms_per_step": ms_e2e / args.steps,
+               "api": "game_generation_host (pinned host buffers; H2D X,t,W + eval + step + D2H F,W' per step)"}
+
+    if rank != 0:
+        G.close()
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    # ---------------- roofline of the dominant kernel (fused fitness)
+    peaks, peaks_src = load_peaks()
+    flops_per_launch = 2.0 * cfg.P * cfg.M * cfg.G * (3 if G.scheme() == game.SCHEME_F16X3 else 1)
+    avg_s = kernel_ms * 1e-3 / max(kernel_n, 1)
+    achieved = flops_per_launch / avg_s / 1e12
+    if G.scheme() == game.SCHEME_F16X3:
+        peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+        peak_note = (f"{peaks_src} bf16_tflops_sustained (fp16 and bf16 share the kind::f16 rate; the kernel is timed "
+                     f"inside a {ms / 1e3:.2f} s step loop); burst figure {peaks['bf16_tflops']}")
+        bound = "tensor"
+    else:
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        peak_note = "derived fp32 FFMA peak: 148 SM x 128 lanes x 2 flop x 1.965 GHz"
+        bound = "alu"
+    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel": "fitness_umma_kernel" if bound == "tensor" else "fitness_ffma_kernel",
+                "kernel_ms_avg": avg_s * 1e3, "kernel_launches_timed": kernel_n, "kernel_share_of_step": kernel_ms / ms,
+                "flops_per_launch": flops_per_launch, "peak_source": peak_note,
+                "hbm_algorithmic_bytes_per_launch": 4 * (cfg.P * (cfg.N + 1)),
+                "hbm_frac_of_measured": 4 * (cfg.P * (cfg.N + 1)) / avg_s / 1e9 / float(peaks["hbm_gbs"])}
+
+    # ---------------- CPU baseline: the oracle as it stands, one thread, bounded sample
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        p_sample = int(min(cfg.P, max(256, 2.5e7 * 321 / cfg.G / cfg.M)))      # ~10-20 s of CPU work
+        W0 = oracle.init_population(cfg.M, cfg.G, seed)
+        dt, _ = oracle_sample(cfg, X, t, W0, p_sample, seed, 0)
+        cpu = {"value": p_sample * cfg.M / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "host_cores_available": os.cpu_count(),
+               "sample": f"one generation (oracle eval + GA step) on the first {p_sample} patterns x all {cfg.M} chromosomes of {cfg.name}"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f16x3->f32" if bound == "tensor" else "f32", "data": "synthetic",
+            "config": config_dict(cfg, scheme_name, world), "generations_per_s": args.steps / (ms * 1e-3),
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    G.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus > 1 and world == 1 and args.impl == "ours":
+        import socket
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    cfg = wl.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+    else:
+        run_ours(args, cfg, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

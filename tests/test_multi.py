@@ -1,0 +1,65 @@
+"""N > 1 host logic on CPU (gloo, world_size 2): max-over-ranks timing, whole-job value, the replica
+knowledge-base seeds, the pattern-shard helper, and the reference arm under torchrun (rank 0 prints, the
+other ranks exit 0 without work)."""
+import json
+import os
+import subprocess
+import sys
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _worker(rank, world, port, out):
+    import bench
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = bench.max_over_ranks(10.0 + 5.0 * rank, dist, "cpu")
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=64)
+    X, _, _ = wl.make_kb(cfg, seed=cfg.seed + 1000 * rank)
+    sums = torch.tensor([float(X.sum())], dtype=torch.float64)
+    gathered = [torch.zeros_like(sums) for _ in range(world)]
+    dist.all_gather(gathered, sums)
+    if rank == 0:
+        json.dump({"ms": ms, "value": bench.job_value(1000, 64, 4, world, ms), "sums": [float(g) for g in gathered]},
+                  open(out, "w"))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_max_over_ranks_and_job_value_gloo(tmp_path):
+    out = str(tmp_path / "r.json")
+    mp.spawn(_worker, args=(2, 29533, out), nprocs=2, join=True)
+    r = json.load(open(out))
+    assert r["ms"] == 15.0                                   # slowest rank
+    assert r["value"] == 1000 * 64 * 4 * 2 / 15e-3           # units of ALL ranks / max time
+    assert r["sums"][0] != r["sums"][1]                      # every replica has its own knowledge base
+
+
+def test_shard_patterns_partition():
+    for P, w in [(10, 3), (1000, 2), (7, 8), (4_000_000, 8)]:
+        edges = [wl.shard_patterns(P, w, r) for r in range(w)]
+        assert edges[0][0] == 0 and edges[-1][1] == P
+        assert all(a[1] == b[0] for a, b in zip(edges, edges[1:]))
+        sizes = [b - a for a, b in edges]
+        assert max(sizes) - min(sizes) <= 1
+
+
+def test_reference_arm_under_torchrun_rank0_only():
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr",
+           "127.0.0.1", "--master-port", "29534", os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+           "--workload", "c0", "--steps", "2", "--warmup", "1"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["impl"] == "reference" and j["n_gpus"] == 2 and j["value"] > 0 and j["cpu_baseline"]["kind"] == "oracle"
+    assert j["e2e"]["h2d_bytes_per_step"] == 0 and j["gpu_launches"] == 0
