@@ -292,7 +292,7 @@ def run_ours(args, cfg, rank, world, local_rank):
     if world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()
-        p_sample = int(min(cfg.P, max(256, 2.5e7 * 321 / cfg.G / cfg.M)))      # ~10-20 s of CPU work
+        p_sample = int(min(cfg.P, max(256, 8e7 * 321 / cfg.G / cfg.M)))        # ~10-30 s of CPU work
         W0 = oracle.init_population(cfg.M, cfg.G, seed)
         dt, _ = oracle_sample(cfg, X, t, W0, p_sample, seed, 0)
         cpu = {"value": p_sample * cfg.M / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,

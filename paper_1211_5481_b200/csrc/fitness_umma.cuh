@@ -74,21 +74,36 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// Bounded wait: a protocol bug must trap, not hang the GPU.
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t done = 0;
-    const long long t0 = clock64();
-    while (true) {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(done)
-            : "r"(bar), "r"(parity)
-            : "memory");
-        if (done) break;
-        if (clock64() - t0 > (1ll << 32)) __trap();   // ~2 s
+// Bounded waits: a protocol bug must trap, not hang the GPU.
+__device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return done;
+}
+// Critical-path waits (MMA issuer, loader): tight poll, three instructions per iteration.
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
+    uint32_t n = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if (++n > (1u << 26)) __trap();
     }
+}
+// Waits of warps that are ahead of the pipeline (producers on a full ring, epilogue on an accumulator still
+// being computed): back off with nanosleep so that polling does not steal issue slots from the working warps
+// (ncu, profiles/r01: the clock-checked polling loop was 26 % of all issued warp instructions).
+template <int NS>
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+    uint32_t n = 0;
+    do {
+        __nanosleep(NS);
+        if (++n > (1u << 24)) __trap();
+    } while (!mbar_try_wait(bar, parity));
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -196,19 +211,32 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
 }
 
 // ---------------------------------------------------------------------------------------------- producer helpers
+// lo = v - hi in ONE instruction: the sm_100 mixed-precision FMA (SASS FHFMA) takes the fp16 hi straight from
+// the packed register: fma.rn.f32.f16 d = hi * (-1) + v (exact: v - hi is representable).
+__device__ __forceinline__ float sub_f16_from_f32(float v, unsigned short hi) {
+    float d;
+    const unsigned short minus_one = 0xBC00;
+    asm("fma.rn.f32.f16 %0, %1, %2, %3;" : "=f"(d) : "h"(hi), "h"(minus_one), "f"(v));
+    return d;
+}
 // Split 8 fp32 values into fp16 hi / lo and store them as one 16-byte k-group row each.
 __device__ __forceinline__ void split_store(const float (&v)[8], uint8_t* hi_dst, uint8_t* lo_dst) {
     uint32_t h[4], l[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const __half2 hh = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
-        const float2 hf = __half22float2(hh);
-        const __half2 ll = __floats2half2_rn(v[2 * i] - hf.x, v[2 * i + 1] - hf.y);
         h[i] = *reinterpret_cast<const uint32_t*>(&hh);
+        const float l0 = sub_f16_from_f32(v[2 * i], static_cast<unsigned short>(h[i] & 0xffffu));
+        const float l1 = sub_f16_from_f32(v[2 * i + 1], static_cast<unsigned short>(h[i] >> 16));
+        const __half2 ll = __floats2half2_rn(l0, l1);
         l[i] = *reinterpret_cast<const uint32_t*>(&ll);
     }
     *reinterpret_cast<uint4*>(hi_dst) = make_uint4(h[0], h[1], h[2], h[3]);
     *reinterpret_cast<uint4*>(lo_dst) = make_uint4(l[0], l[1], l[2], l[3]);
+}
+__device__ __forceinline__ void zero_store(uint8_t* hi_dst, uint8_t* lo_dst) {
+    *reinterpret_cast<uint4*>(hi_dst) = make_uint4(0u, 0u, 0u, 0u);
+    *reinterpret_cast<uint4*>(lo_dst) = make_uint4(0u, 0u, 0u, 0u);
 }
 
 template <int ACT>
@@ -268,7 +296,7 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                 for (int mt = mt0; mt < mt1; ++mt) {
                     const uint8_t* src = prm.Wimg + static_cast<size_t>(mt) * prm.steps * (2 * kABytes);
                     for (int s = 0; s < prm.steps; ++s) {
-                        mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                        mbar_wait_spin(bar_empty + 8 * stage, phase ^ 1);
                         mbar_arrive_expect_tx(bar_full + 8 * stage, 2 * kABytes);
                         bulk_g2s(smem_base + stage * kStageBytes, src + static_cast<size_t>(s) * (2 * kABytes), 2 * kABytes,
                                  bar_full + 8 * stage);
@@ -287,11 +315,11 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                 const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
                 for (int mt = mt0; mt < mt1; ++mt, ++tile) {
                     const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
-                    mbar_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1);
+                    mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + buf * kBN;
                     for (int s = 0; s < prm.steps; ++s) {
-                        mbar_wait(bar_full + 8 * stage, phase);
+                        mbar_wait_spin(bar_full + 8 * stage, phase);
                         tc_fence_after();
                         const uint32_t a_hi = smem_base + stage * kStageBytes, a_lo = a_hi + kABytes;
                         const uint32_t b_hi = a_hi + 2 * kABytes, b_lo = b_hi + kBBytes;
@@ -322,7 +350,7 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
             const int n_valid = static_cast<int>(min(static_cast<long long>(kBN), prm.P - p0));
             for (int mt = mt0; mt < mt1; ++mt, ++tile) {
                 const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
-                mbar_wait(bar_acc_full + 8 * buf, acc_phase);
+                mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
 #pragma unroll 1
@@ -408,20 +436,18 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                         }
                     }
                     for (int ss = 0; ss < prm.steps_per_chunk; ++ss) {
-                        mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                        mbar_wait_sleep<32>(bar_empty + 8 * stage, phase ^ 1);
                         uint8_t* b_hi = smem + stage * kStageBytes + 2 * kABytes + r * 16;
                         uint8_t* b_lo = b_hi + kBBytes;
                         float v0[8], v1[8];
                         if (EXPANSION == 0) {
                             // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2} (zeros beyond degree d)
-                            const bool has1 = 2 * ss + 2 <= prm.d;
 #pragma unroll
                             for (int f = 0; f < 8; ++f) {
                                 v0[f] = ac[f];
-                                const float n1 = fmaf(x2[f], ac[f], -am[f]);
-                                v1[f] = has1 ? n1 : 0.0f;
-                                const float n2 = fmaf(x2[f], n1, -ac[f]);
-                                am[f] = n1; ac[f] = n2;
+                                v1[f] = fmaf(x2[f], ac[f], -am[f]);
+                                ac[f] = fmaf(x2[f], v1[f], -ac[f]);
+                                am[f] = v1[f];
                             }
                         } else {
                             // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
@@ -436,7 +462,11 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                             }
                         }
                         split_store(v0, b_hi, b_lo);
-                        split_store(v1, b_hi + kBN * 16, b_lo + kBN * 16);
+                        if (EXPANSION == 0 && 2 * ss + 2 > prm.d) {
+                            zero_store(b_hi + kBN * 16, b_lo + kBN * 16);       // odd d: last k-group is padding
+                        } else {
+                            split_store(v1, b_hi + kBN * 16, b_lo + kBN * 16);
+                        }
                         fence_proxy_async_smem();
                         __syncwarp();
                         if (lane == 0) mbar_arrive(bar_full + 8 * stage);
@@ -444,7 +474,7 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                     }
                 }
                 // ---- bias step: element 0 of k-group 0 is the constant 1 (gene 0), the rest padding
-                mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                mbar_wait_sleep<32>(bar_empty + 8 * stage, phase ^ 1);
                 uint8_t* b_hi = smem + stage * kStageBytes + 2 * kABytes + r * 16;
                 uint8_t* b_lo = b_hi + kBBytes;
                 *reinterpret_cast<uint4*>(b_hi) = make_uint4(0x00003C00u, 0u, 0u, 0u);   // fp16 1.0 in slot 0
