@@ -4,15 +4,23 @@
 //   F[m]   = (1/P) sum_p (act(z[m,p]) - t_p)^2            (eq.(3), MSE)
 //
 // is a dense M x P x G contraction whose B operand (the expansion phi, eq.(1), 79-82 eq.(6)) is
-// GENERATED in shared memory and never exists in HBM.  One persistent CTA per SM:
+// GENERATED in shared memory and never exists in HBM.  Persistent kernel, one CTA PAIR (cluster of 2, the two
+// SMs of a TPC) per 256 chromosomes x 256 patterns tile, tcgen05 cta_group::2:
 //
-//   warp 0      loader   : cp.async.bulk (1-D TMA) of the pre-split W operand images, 8 KB per K step
-//   warp 1      MMA      : tcgen05.mma.cta_group::1.kind::f16, M=128 chromosomes x N=256 patterns x K=16 genes,
-//                          three MMAs per K step (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM
+//   warp 0      loader   : cp.async.bulk (1-D TMA) of this CTA's pre-split W operand images, 8 KB per K step
+//   warp 1      MMA      : leader CTA: tcgen05.mma.cta_group::2.kind::f16, M=256 (128 chromosomes per CTA) x
+//                          N=256 patterns (128 generated per CTA) x K=16 genes, three MMAs per K step
+//                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM;
+//                          peer CTA: relays "my stage is full" to the leader's barrier
 //   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation, (y-t)^2, private per-chromosome sum
 //                          (TMEM lane = chromosome, so no shuffle is needed); fp64 accumulation per (CTA, m)
-//   warps 10-17 producers: one pattern per thread; Chebyshev / multiple-angle recurrences for 8 features at a
+//   warps 10-17 producers: two sets of 4 warps alternating chunks; one pattern per thread; Chebyshev / multiple-angle recurrences for 8 features at a
 //                          time, fp16 hi/lo split, 16-byte stores straight into the MMA's canonical layout
+//
+// Why a pair: ncu on the single-CTA version (profiles/r01a) showed the shared-memory data pipe, not the tensor
+// pipe, saturating (tensor-core operand reads 46 % + producer stores 28 % + loads 4 % + bulk fills): with
+// cta_group::2 each SM reads only its half of B per MMA (8 KB instead of 12 KB) and generates only its 128
+// patterns (8 KB of stores per K step instead of 16 KB).
 //
 // Shared-memory operand layout (both operands): K-major, SWIZZLE_NONE "interleaved" canonical layout with the
 // 8-row core matrices packed back to back, i.e. a plain [k_group][row][8 x fp16] array:
@@ -31,20 +39,22 @@
 namespace game {
 namespace umma {
 
-constexpr int kBM = 128;             // chromosomes per tile (MMA M, TMEM lanes)
-constexpr int kBN = 256;             // patterns per tile   (MMA N, TMEM columns)
-constexpr int kStages = 8;           // K-step ring
+constexpr int kBM = 128;             // chromosomes per CTA tile (TMEM lanes); the pair's MMA M is 2 * kBM
+constexpr int kBN = 256;             // patterns per pair tile (MMA N, TMEM columns)
+constexpr int kRows = kBN / 2;       // pattern rows of the B operand generated and held by each CTA
+constexpr int kStages = 12;          // K-step ring
 constexpr int kABytes = 2 * kBM * 16;          // one k-group pair of A (hi or lo): 4096
-constexpr int kBBytes = 2 * kBN * 16;          // one k-group pair of B (hi or lo): 8192
-constexpr int kStageBytes = 2 * kABytes + 2 * kBBytes;   // A_hi, A_lo, B_hi, B_lo = 24576
-constexpr int kXtStride = kBN + 1;             // transposed x tile, padded: Xt[i * 257 + row]
+constexpr int kBBytes = 2 * kRows * 16;        // one k-group pair of this CTA's half of B (hi or lo): 4096
+constexpr int kStageBytes = 2 * kABytes + 2 * kBBytes;   // A_hi, A_lo, B_hi, B_lo = 16384
+constexpr int kXtStride = kRows + 1;           // transposed x tile, padded: Xt[i * 129 + row]
 constexpr int kXtRows = 32;                    // N <= 32 (Chebyshev), 2 * N <= 32 (trig: cos and sin planes)
 constexpr int kXtBytes = kXtRows * kXtStride * 4;
-constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;
+constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4 warps (128 rows each)
 constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
 constexpr int kSmemBar = kStages * kStageBytes + kXtBytes;          // barriers start here
 constexpr int kSmemBytes = kSmemBar + 256;
-constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators
+constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
+static_assert(kSmemBar % 8 == 0, "barrier alignment");
 
 struct Params {
     const float* X;        // [P][N]
@@ -54,9 +64,10 @@ struct Params {
     long long P;
     int N, d, M;
     int m_stride;          // m_tiles * 128
-    int m_tiles, p_tiles;
-    int m_groups;          // work unit = (pattern tile, group of m_tiles_per_group chromosome tiles)
-    int m_tiles_per_group;
+    int m_tiles;           // chromosome tiles, padded to an even number (one per CTA of a pair)
+    int p_tiles;           // pattern tiles of 256
+    int m_groups;          // work unit = (pattern tile, group of m_pairs_per_group chromosome-tile pairs)
+    int m_pairs_per_group;
     int chunks;            // ceil(N / 8)
     int steps_per_chunk;   // Chebyshev ceil(d / 2); trig d
     int steps;             // chunks * steps_per_chunk + 1 (bias)
@@ -64,17 +75,37 @@ struct Params {
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
-
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of the same smem offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t local_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+    return r;
+}
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// arrive on a barrier that may live in the other CTA of the pair (address from map_to_cta)
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// Bounded waits: a protocol bug must trap, not hang the GPU.
+// Bounded waits: a protocol bug must trap, not hang the GPU.  Default (CTA-scope) semantics on both the remote
+// arrive and the wait, as in CUTLASS's ClusterBarrier: cluster-scope acquire/release compile to CCTL.IVALL and
+// MEMBAR.ALL.GPU per call, which made the pair kernel 1.7x slower than the single-CTA one.  The data these
+// barriers guard is produced for / consumed by the async proxy and is fenced by its writers before they arrive.
 __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity) {
     uint32_t done;
     asm volatile(
@@ -86,7 +117,7 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return done;
 }
-// Critical-path waits (MMA issuer, loader): tight poll, three instructions per iteration.
+// Critical-path waits (MMA issuer, relay, loader): tight poll, three instructions per iteration.
 __device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
     uint32_t n = 0;
     while (!mbar_try_wait(bar, parity)) {
@@ -95,7 +126,7 @@ __device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
 }
 // Waits of warps that are ahead of the pipeline (producers on a full ring, epilogue on an accumulator still
 // being computed): back off with nanosleep so that polling does not steal issue slots from the working warps
-// (ncu, profiles/r01: the clock-checked polling loop was 26 % of all issued warp instructions).
+// (ncu, profiles/r01a: the clock-checked polling loop was 26 % of all issued warp instructions).
 template <int NS>
 __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
@@ -114,23 +145,28 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+// TMEM allocation for a CTA pair: issued by the same warp of BOTH CTAs.
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
 }
-__device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t addr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
 }
-__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+// D[tmem, both CTAs] (+)= A[smem of both CTAs] . B[smem of both CTAs]; issued by one thread of the leader CTA.
+__device__ __forceinline__ void umma_f16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
         "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+// When all MMAs issued so far have completed, arrive once on the barrier at this smem offset in BOTH CTAs.
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"(static_cast<unsigned short>(3))
+                 : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile(
@@ -161,9 +197,9 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
     return static_cast<uint64_t>((saddr & 0x3FFFFu) >> 4) | (static_cast<uint64_t>(lbo_bytes >> 4) << 16) |
            (static_cast<uint64_t>(sbo_bytes >> 4) << 32) | (1ull << 46);
 }
-// Instruction descriptor, kind::f16: D = F32 (bit 4), A = B = F16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
-constexpr uint32_t kIdesc = (1u << 4) | (static_cast<uint32_t>(kBN >> 3) << 17) | (static_cast<uint32_t>(kBM >> 4) << 24);
-
+// Instruction descriptor, kind::f16: D = F32 (bit 4), A = B = F16 (0), both K-major, N >> 3 at bit 17,
+// M >> 4 at bit 24 (M = 256: the pair's two 128-row halves).
+constexpr uint32_t kIdesc = (1u << 4) | (static_cast<uint32_t>(kBN >> 3) << 17) | (static_cast<uint32_t>((2 * kBM) >> 4) << 24);
 // ---------------------------------------------------------------------------------------------- K-axis permutation
 // Gene held by (K step s, k-group kg in {0,1}, slot f in 0..7), or -1 for padding.  Used by the W image
 // builder; the producers below generate phi in exactly this order.
@@ -254,34 +290,43 @@ __device__ __forceinline__ float act_err2(float z, float t) {
 }
 
 // ---------------------------------------------------------------------------------------------- the kernel
+// Barrier protocol (per CTA unless noted; "leader" = cluster rank 0):
+//   full[s]      leader: 1 (own loader, +tx) + 4 (own producer warps) + 1 (peer's relay)  -> MMA may consume stage s
+//                peer  : 1 (own loader, +tx) + 4 (own producer warps)                     -> relay forwards to leader
+//   empty[s]     1: tcgen05.commit of the MMAs that read stage s, multicast to both CTAs  -> loader / producers refill
+//   acc_full[b]  1: tcgen05.commit after a tile's last MMA, multicast to both CTAs        -> epilogue may read buffer b
+//   acc_empty[b] leader only, 16: the 8 epilogue warps of BOTH CTAs                       -> MMA may overwrite buffer b
 template <int EXPANSION, int ACT>
-__global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
     extern __shared__ __align__(1024) uint8_t smem[];
     float* Xt = reinterpret_cast<float*>(smem + kStages * kStageBytes);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
-    // bars[0..S) full, [S..2S) empty, [2S..2S+2) acc_full, [2S+2..2S+4) acc_empty, then the TMEM address
     const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8 * kStages;
     const uint32_t bar_acc_full = bar_empty + 8 * kStages, bar_acc_empty = bar_acc_full + 16;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 4);
     const uint32_t smem_base = smem_u32(smem);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t crank = cluster_ctarank();            // 0 = leader, 1 = peer
+    const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int units = prm.p_tiles * prm.m_groups;
+    const int m_pairs = prm.m_tiles >> 1;
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < kStages; ++s) {
-            mbar_init(bar_full + 8 * s, 1 + kNumProdWarps);
+            mbar_init(bar_full + 8 * s, 1 + kNumProdWarps / 2 + (crank == 0 ? 1 : 0));
             mbar_init(bar_empty + 8 * s, 1);
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar_acc_full + 8 * b, 1);
-            mbar_init(bar_acc_empty + 8 * b, kNumEpiWarps);
+            mbar_init(bar_acc_empty + 8 * b, 2 * kNumEpiWarps);
         }
         fence_barrier_init();
     }
-    if (warp == 1) tmem_alloc(smem_u32(tmem_slot), kTmemCols);
+    if (warp == 1) tmem_alloc_pair(smem_u32(tmem_slot), kTmemCols);
     tc_fence_before();
     __syncthreads();
+    cluster_sync_all();          // both CTAs' barriers are initialised before any remote arrive / multicast commit
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
@@ -289,11 +334,12 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
         // ============================================================== loader: W operand images -> A stages
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
-            for (int u = blockIdx.x; u < units; u += gridDim.x) {
+            for (int u = pair; u < units; u += n_pairs) {
                 const int mg = u % prm.m_groups;
-                const int mt0 = mg * prm.m_tiles_per_group;
-                const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
-                for (int mt = mt0; mt < mt1; ++mt) {
+                const int mp0 = mg * prm.m_pairs_per_group;
+                const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
+                for (int mp = mp0; mp < mp1; ++mp) {
+                    const int mt = 2 * mp + static_cast<int>(crank);
                     const uint8_t* src = prm.Wimg + static_cast<size_t>(mt) * prm.steps * (2 * kABytes);
                     for (int s = 0; s < prm.steps; ++s) {
                         mbar_wait_spin(bar_empty + 8 * stage, phase ^ 1);
@@ -306,14 +352,14 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
             }
         }
     } else if (warp == 1) {
-        // ============================================================== MMA issuer
-        if (lane == 0) {
+        if (lane == 0 && crank == 0) {
+            // ============================================================== MMA issuer (leader CTA)
             uint32_t stage = 0, phase = 0, tile = 0;
-            for (int u = blockIdx.x; u < units; u += gridDim.x) {
+            for (int u = pair; u < units; u += n_pairs) {
                 const int mg = u % prm.m_groups;
-                const int mt0 = mg * prm.m_tiles_per_group;
-                const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
-                for (int mt = mt0; mt < mt1; ++mt, ++tile) {
+                const int mp0 = mg * prm.m_pairs_per_group;
+                const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
+                for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                     const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
                     mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
                     tc_fence_after();
@@ -324,14 +370,28 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                         const uint32_t a_hi = smem_base + stage * kStageBytes, a_lo = a_hi + kABytes;
                         const uint32_t b_hi = a_hi + 2 * kABytes, b_lo = b_hi + kBBytes;
                         const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
-                        const uint64_t db_hi = make_desc(b_hi, kBN * 16, 128), db_lo = make_desc(b_lo, kBN * 16, 128);
-                        umma_f16(d_tmem, da_lo, db_hi, kIdesc, s > 0 ? 1u : 0u);   // small terms first
-                        umma_f16(d_tmem, da_hi, db_lo, kIdesc, 1u);
-                        umma_f16(d_tmem, da_hi, db_hi, kIdesc, 1u);
-                        umma_commit(bar_empty + 8 * stage);                        // stage free when these finish
+                        const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
+                        umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, s > 0 ? 1u : 0u);   // small terms first
+                        umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
+                        umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
+                        umma_commit_pair(bar_empty + 8 * stage);                        // stage free in both CTAs
                         if (++stage == kStages) { stage = 0; phase ^= 1; }
                     }
-                    umma_commit(bar_acc_full + 8 * buf);                           // accumulator complete
+                    umma_commit_pair(bar_acc_full + 8 * buf);                           // accumulators complete
+                }
+            }
+        } else if (lane == 0) {
+            // ============================================================== relay (peer CTA): my stage is full
+            uint32_t stage = 0, phase = 0;
+            const uint32_t leader_full = map_to_cta(bar_full, 0);
+            for (int u = pair; u < units; u += n_pairs) {
+                const int mg = u % prm.m_groups;
+                const int mp0 = mg * prm.m_pairs_per_group;
+                const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
+                for (int n = (mp1 - mp0) * prm.steps; n > 0; --n) {
+                    mbar_wait_spin(bar_full + 8 * stage, phase);
+                    mbar_arrive_cluster(leader_full + 8 * stage);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
         }
@@ -341,14 +401,15 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
         const int h = (warp - 2) >> 2;          // column half
         double* my_part = prm.part + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
         for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
+        const uint32_t leader_acc_empty = map_to_cta(bar_acc_empty, 0);
         uint32_t tile = 0;
-        for (int u = blockIdx.x; u < units; u += gridDim.x) {
+        for (int u = pair; u < units; u += n_pairs) {
             const int pt = u / prm.m_groups, mg = u % prm.m_groups;
-            const int mt0 = mg * prm.m_tiles_per_group;
-            const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
+            const int mp0 = mg * prm.m_pairs_per_group;
+            const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
             const long long p0 = static_cast<long long>(pt) * kBN;
             const int n_valid = static_cast<int>(min(static_cast<long long>(kBN), prm.P - p0));
-            for (int mt = mt0; mt < mt1; ++mt, ++tile) {
+            for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                 const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
                 mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
                 tc_fence_after();
@@ -383,27 +444,34 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                 sum = (sum + sum1) + (sum2 + sum3);
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_acc_empty + 8 * buf);
-                const int m = mt * kBM + q * 32 + lane;
+                if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8 * buf);
+                const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
                 __stcg(my_part + m, __ldcg(my_part + m) + static_cast<double>(sum));
             }
         }
     } else {
-        // ============================================================== producers: phi -> B stages
-        const int r = threadIdx.x - (2 + kNumEpiWarps) * 32;   // pattern row of this thread, 0..255
-        uint32_t stage = 0, phase = 0;
-        for (int u = blockIdx.x; u < units; u += gridDim.x) {
+        // ============================================================== producers: phi -> this CTA's half of B
+        // Two sets of 4 warps; a set owns whole chunks (8 features: the recurrences restart there), the sets
+        // alternate chunks, so two chunks are generated concurrently.  One fence + the arrivals per batch of
+        // up to kBatch K steps instead of per step (the fence waits for this warp's stores to land).
+        constexpr int kBatch = 6;
+        const int pidx = threadIdx.x - (2 + kNumEpiWarps) * 32;
+        const int set = pidx >> 7;              // which warp set
+        const int r = pidx & (kRows - 1);       // pattern row of this thread, 0..127
+        uint32_t stage = 0, phase = 0;          // ring position of the next K step in issue order (both sets track it)
+        uint32_t item = 0;                      // running chunk counter: chunk goes to set (item & 1)
+        for (int u = pair; u < units; u += n_pairs) {
             const int pt = u / prm.m_groups, mg = u % prm.m_groups;
-            const int mt0 = mg * prm.m_tiles_per_group;
-            const int mt1 = min(mt0 + prm.m_tiles_per_group, prm.m_tiles);
-            const long long p0 = static_cast<long long>(pt) * kBN;
+            const int mp0 = mg * prm.m_pairs_per_group;
+            const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
+            const long long p0 = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows;
             // ---- x tile: coalesced global reads, transposed (and for trig: sin/cos'ed) into Xt
             asm volatile("bar.sync 1, %0;" ::"n"(kNumProdWarps * 32));   // everyone is done with the old Xt
             {
-                const int n_el = kBN * prm.N;
-                const long long lim = (prm.P - p0) * prm.N;
+                const int n_el = kRows * prm.N;
+                const long long lim = (prm.P - p0) * prm.N;               // <= 0: no valid pattern in this half
                 const float* src = prm.X + p0 * prm.N;
-                for (int idx = r; idx < n_el; idx += kBN) {
+                for (int idx = pidx; idx < n_el; idx += kNumProdWarps * 32) {
                     const float x = idx < lim ? __ldg(src + idx) : 0.0f;
                     const int row = idx / prm.N, i = idx - row * prm.N;
                     if (EXPANSION == 0) {
@@ -417,85 +485,102 @@ __global__ void __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params 
                 }
             }
             asm volatile("bar.sync 1, %0;" ::"n"(kNumProdWarps * 32));
-            for (int mt = mt0; mt < mt1; ++mt) {
-                for (int c = 0; c < prm.chunks; ++c) {
-                    // recurrence state for the 8 features of this chunk
-                    float x2[8], am[8], ac[8], bm[8], bc[8];
+            for (int mp = mp0; mp < mp1; ++mp) {
+                for (int c = 0; c <= prm.chunks; ++c, ++item) {
+                    const int n_steps = c < prm.chunks ? prm.steps_per_chunk : 1;      // c == chunks: the bias step
+                    if ((item & 1u) == static_cast<uint32_t>(set)) {
+                        uint32_t st = stage, ph = phase;
+                        // recurrence state for the 8 features of this chunk
+                        float x2[8], am[8], ac[8], bm[8], bc[8];
 #pragma unroll
-                    for (int f = 0; f < 8; ++f) {
-                        const int i = c * 8 + f;
-                        if (EXPANSION == 0) {
-                            const float x = i < prm.N ? Xt[i * kXtStride + r] : 0.0f;
-                            x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
-                            bm[f] = 0.0f; bc[f] = 0.0f;
-                        } else {
-                            const float cs = i < prm.N ? Xt[i * kXtStride + r] : 1.0f;
-                            const float sn = i < prm.N ? Xt[(16 + i) * kXtStride + r] : 0.0f;
-                            x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
-                            bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
-                        }
-                    }
-                    for (int ss = 0; ss < prm.steps_per_chunk; ++ss) {
-                        mbar_wait_sleep<32>(bar_empty + 8 * stage, phase ^ 1);
-                        uint8_t* b_hi = smem + stage * kStageBytes + 2 * kABytes + r * 16;
-                        uint8_t* b_lo = b_hi + kBBytes;
-                        float v0[8], v1[8];
-                        if (EXPANSION == 0) {
-                            // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2} (zeros beyond degree d)
-#pragma unroll
-                            for (int f = 0; f < 8; ++f) {
-                                v0[f] = ac[f];
-                                v1[f] = fmaf(x2[f], ac[f], -am[f]);
-                                ac[f] = fmaf(x2[f], v1[f], -ac[f]);
-                                am[f] = v1[f];
-                            }
-                        } else {
-                            // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
-#pragma unroll
-                            for (int f = 0; f < 8; ++f) {
-                                v0[f] = ac[f];
-                                v1[f] = bc[f];
-                                const float cn = fmaf(x2[f], ac[f], -am[f]);
-                                const float sn = fmaf(x2[f], bc[f], -bm[f]);
-                                am[f] = ac[f]; ac[f] = cn;
-                                bm[f] = bc[f]; bc[f] = sn;
+                        for (int f = 0; f < 8; ++f) {
+                            const int i = c * 8 + f;
+                            const bool have = c < prm.chunks && i < prm.N;
+                            if (EXPANSION == 0) {
+                                const float x = have ? Xt[i * kXtStride + r] : 0.0f;
+                                x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
+                                bm[f] = 0.0f; bc[f] = 0.0f;
+                            } else {
+                                const float cs = have ? Xt[i * kXtStride + r] : 1.0f;
+                                const float sn = have ? Xt[(16 + i) * kXtStride + r] : 0.0f;
+                                x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
+                                bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
                             }
                         }
-                        split_store(v0, b_hi, b_lo);
-                        if (EXPANSION == 0 && 2 * ss + 2 > prm.d) {
-                            zero_store(b_hi + kBN * 16, b_lo + kBN * 16);       // odd d: last k-group is padding
-                        } else {
-                            split_store(v1, b_hi + kBN * 16, b_lo + kBN * 16);
+                        uint32_t ready = mbar_try_wait(bar_empty + 8 * st, ph ^ 1);
+                        for (int ss0 = 0; ss0 < n_steps; ss0 += kBatch) {
+                            const int nb = min(kBatch, n_steps - ss0);
+                            const uint32_t st0 = st;
+                            for (int j = 0; j < nb; ++j) {
+                                const int ss = ss0 + j;
+                                if (!ready) mbar_wait_sleep<32>(bar_empty + 8 * st, ph ^ 1);
+                                uint8_t* b_hi = smem + st * kStageBytes + 2 * kABytes + r * 16;
+                                uint8_t* b_lo = b_hi + kBBytes;
+                                if (++st == kStages) { st = 0; ph ^= 1; }
+                                ready = mbar_try_wait(bar_empty + 8 * st, ph ^ 1);     // poll the next stage early
+                                if (c == prm.chunks) {
+                                    // bias step: element 0 of k-group 0 is the constant 1 (gene 0), the rest padding
+                                    *reinterpret_cast<uint4*>(b_hi) = make_uint4(0x00003C00u, 0u, 0u, 0u);
+                                    *reinterpret_cast<uint4*>(b_lo) = make_uint4(0u, 0u, 0u, 0u);
+                                    zero_store(b_hi + kRows * 16, b_lo + kRows * 16);
+                                    continue;
+                                }
+                                float v0[8], v1[8];
+                                if (EXPANSION == 0) {
+                                    // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2}
+#pragma unroll
+                                    for (int f = 0; f < 8; ++f) {
+                                        v0[f] = ac[f];
+                                        v1[f] = fmaf(x2[f], ac[f], -am[f]);
+                                        ac[f] = fmaf(x2[f], v1[f], -ac[f]);
+                                        am[f] = v1[f];
+                                    }
+                                } else {
+                                    // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
+#pragma unroll
+                                    for (int f = 0; f < 8; ++f) {
+                                        v0[f] = ac[f];
+                                        v1[f] = bc[f];
+                                        const float cn = fmaf(x2[f], ac[f], -am[f]);
+                                        const float sn = fmaf(x2[f], bc[f], -bm[f]);
+                                        am[f] = ac[f]; ac[f] = cn;
+                                        bm[f] = bc[f]; bc[f] = sn;
+                                    }
+                                }
+                                split_store(v0, b_hi, b_lo);
+                                if (EXPANSION == 0 && 2 * ss + 2 > prm.d) {
+                                    zero_store(b_hi + kRows * 16, b_lo + kRows * 16);  // odd d: last k-group is padding
+                                } else {
+                                    split_store(v1, b_hi + kRows * 16, b_lo + kRows * 16);
+                                }
+                            }
+                            fence_proxy_async_smem();
+                            __syncwarp();
+                            if (lane == 0) {
+                                uint32_t sa = st0;
+                                for (int j = 0; j < nb; ++j) {
+                                    mbar_arrive(bar_full + 8 * sa);
+                                    if (++sa == kStages) sa = 0;
+                                }
+                            }
                         }
-                        fence_proxy_async_smem();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(bar_full + 8 * stage);
-                        if (++stage == kStages) { stage = 0; phase ^= 1; }
                     }
+                    stage += n_steps;
+                    while (stage >= kStages) { stage -= kStages; phase ^= 1; }
                 }
-                // ---- bias step: element 0 of k-group 0 is the constant 1 (gene 0), the rest padding
-                mbar_wait_sleep<32>(bar_empty + 8 * stage, phase ^ 1);
-                uint8_t* b_hi = smem + stage * kStageBytes + 2 * kABytes + r * 16;
-                uint8_t* b_lo = b_hi + kBBytes;
-                *reinterpret_cast<uint4*>(b_hi) = make_uint4(0x00003C00u, 0u, 0u, 0u);   // fp16 1.0 in slot 0
-                *reinterpret_cast<uint4*>(b_lo) = make_uint4(0u, 0u, 0u, 0u);
-                *reinterpret_cast<uint4*>(b_hi + kBN * 16) = make_uint4(0u, 0u, 0u, 0u);
-                *reinterpret_cast<uint4*>(b_lo + kBN * 16) = make_uint4(0u, 0u, 0u, 0u);
-                fence_proxy_async_smem();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_full + 8 * stage);
-                if (++stage == kStages) { stage = 0; phase ^= 1; }
             }
         }
     }
 
-    // ---- teardown: everything issued has been consumed once the epilogue has drained the last accumulator
+    // ---- teardown: everything issued has been consumed once both epilogues have drained the last accumulator;
+    // neither CTA may exit (or free TMEM) while the other can still signal its barriers or read its operands.
     tc_fence_before();
     __syncthreads();
+    cluster_sync_all();
     tc_fence_after();
     if (warp == 1) {
         __syncwarp();
-        tmem_dealloc(tmem_base, kTmemCols);
+        tmem_dealloc_pair(tmem_base, kTmemCols);
     }
 }
 

@@ -154,17 +154,19 @@ int eval_internal(game_ctx* c, float* best_out) {
         prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M;
         prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
         prm.p_tiles = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
-        const int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
-        // work unit = (pattern tile, group of chromosome tiles): aim for >= 16 units per CTA so that the
-        // static round-robin assignment stays balanced when there are few pattern tiles
-        long long want = (16ll * grid_cap + prm.p_tiles - 1) / prm.p_tiles;
+        int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+        grid_cap &= ~1;                                              // CTA pairs (clusters of 2)
+        const int pair_cap = grid_cap / 2, m_pairs = c->m_tiles / 2;
+        // work unit = (pattern tile, group of chromosome-tile pairs): aim for >= 16 units per CTA pair so that
+        // the static round-robin assignment stays balanced when there are few pattern tiles
+        long long want = (16ll * pair_cap + prm.p_tiles - 1) / prm.p_tiles;
         if (want < 1) want = 1;
-        if (want > c->m_tiles) want = c->m_tiles;
-        prm.m_tiles_per_group = static_cast<int>((c->m_tiles + want - 1) / want);
-        prm.m_groups = (c->m_tiles + prm.m_tiles_per_group - 1) / prm.m_tiles_per_group;
+        if (want > m_pairs) want = m_pairs;
+        prm.m_pairs_per_group = static_cast<int>((m_pairs + want - 1) / want);
+        prm.m_groups = (m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
         prm.chunks = c->chunks; prm.steps_per_chunk = c->steps_per_chunk; prm.steps = c->steps;
         const long long units = static_cast<long long>(prm.p_tiles) * prm.m_groups;
-        const int grid = static_cast<int>(units < grid_cap ? units : grid_cap);
+        const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);
         n_part = 2 * grid;
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
 #define GAME_LAUNCH(E, A) umma::fitness_umma_kernel<E, A><<<grid, umma::kThreads, umma::kSmemBytes, c->stream>>>(prm)
@@ -242,7 +244,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     if (!c) return GAME_ERR_INVALID_ARG;
     c->P = P; c->N = N; c->d = d; c->M = M; c->G = static_cast<int>(G);
     c->expansion = expansion; c->act = act;
-    c->m_tiles = (M + game::umma::kBM - 1) / game::umma::kBM;
+    c->m_tiles = 2 * ((M + 2 * game::umma::kBM - 1) / (2 * game::umma::kBM));   // one chromosome tile per CTA of a pair
     c->m_stride = c->m_tiles * game::umma::kBM;
     c->umma_ok = d <= 64 && (expansion == GAME_EXP_CHEBYSHEV ? N <= 32 : N <= 16) &&
                  (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
