@@ -42,19 +42,20 @@ namespace umma {
 constexpr int kBM = 128;             // chromosomes per CTA tile (TMEM lanes); the pair's MMA M is 2 * kBM
 constexpr int kBN = 256;             // patterns per pair tile (MMA N, TMEM columns)
 constexpr int kRows = kBN / 2;       // pattern rows of the B operand generated and held by each CTA
-constexpr int kStages = 12;          // K-step ring
-constexpr int kABytes = 2 * kBM * 16;          // one k-group pair of A (hi or lo): 4096
-constexpr int kBBytes = 2 * kRows * 16;        // one k-group pair of this CTA's half of B (hi or lo): 4096
-constexpr int kStageBytes = 2 * kABytes + 2 * kBBytes;   // A_hi, A_lo, B_hi, B_lo = 16384
-constexpr int kXtStride = kRows + 1;           // transposed x tile, padded: Xt[i * 129 + row]
-constexpr int kXtRows = 32;                    // N <= 32 (Chebyshev), 2 * N <= 32 (trig: cos and sin planes)
-constexpr int kXtBytes = kXtRows * kXtStride * 4;
+constexpr int kABytes = 2 * kBM * 16;          // one K step of A, hi or lo: 2 k-groups x 128 rows x 16 B = 4096
+constexpr int kBBytes = 2 * kRows * 16;        // one K step of this CTA's half of B, hi or lo: 4096
+constexpr int kSlotBytes = 2 * kABytes;        // one stage of either operand (hi + lo) = 8192
+static_assert(2 * kBBytes == kSlotBytes, "A and B stages share the slot size");
+constexpr int kSlots = 26;                     // 8 KB slots shared by the A ring and the B stages
+constexpr int kMinAStages = 4;
+constexpr int kMaxResidentSteps = kSlots - kMinAStages;   // phi of a whole pattern tile stays in smem up to here
+constexpr int kStreamBStages = 12;             // B ring when phi does not fit (regenerated per chromosome tile)
 constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4 warps (128 rows each)
 constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
-constexpr int kSmemBar = kStages * kStageBytes + kXtBytes;          // barriers start here
-constexpr int kSmemBytes = kSmemBar + 256;
+constexpr int kSmemBar = kSlots * kSlotBytes;  // barriers start here
+constexpr int kBarBytes = (5 * kSlots + 4) * 8 + 16;
+constexpr int kSmemBytes = kSmemBar + kBarBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
-static_assert(kSmemBar % 8 == 0, "barrier alignment");
 
 struct Params {
     const float* X;        // [P][N]
@@ -71,6 +72,8 @@ struct Params {
     int chunks;            // ceil(N / 8)
     int steps_per_chunk;   // Chebyshev ceil(d / 2); trig d
     int steps;             // chunks * steps_per_chunk + 1 (bias)
+    int resident;          // 1: n_b == steps, phi generated once per unit and reused by all its chromosome tiles
+    int n_a, n_b;          // A ring stages, B stages (n_a + n_b <= kSlots)
 };
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -289,21 +292,38 @@ __device__ __forceinline__ float act_err2(float z, float t) {
     return e * e;
 }
 
+
 // ---------------------------------------------------------------------------------------------- the kernel
-// Barrier protocol (per CTA unless noted; "leader" = cluster rank 0):
-//   full[s]      leader: 1 (own loader, +tx) + 4 (own producer warps) + 1 (peer's relay)  -> MMA may consume stage s
-//                peer  : 1 (own loader, +tx) + 4 (own producer warps)                     -> relay forwards to leader
-//   empty[s]     1: tcgen05.commit of the MMAs that read stage s, multicast to both CTAs  -> loader / producers refill
-//   acc_full[b]  1: tcgen05.commit after a tile's last MMA, multicast to both CTAs        -> epilogue may read buffer b
-//   acc_empty[b] leader only, 16: the 8 epilogue warps of BOTH CTAs                       -> MMA may overwrite buffer b
+// Shared memory: kSlots slots of 8 KB.  Slots [0, n_a) are the A ring (W operand images streamed from L2 by
+// the loader, one K step each); slots [n_a, n_a + n_b) hold this CTA's half of B (phi).  If the whole K extent
+// fits (steps <= kMaxResidentSteps: "resident", n_b == steps) phi of a pattern tile is generated ONCE per work
+// unit and reused by every chromosome-tile pair of the unit; the producers refill stage s for the next unit as
+// soon as the unit's last tile has consumed it.  Otherwise ("streaming") B is a ring refilled per tile.
+//
+// Barriers (per CTA unless noted; "leader" = cluster rank 0, "peer" = rank 1):
+//   a_full[i]    1 + tx : the loader's bulk copy of A stage i has landed; on the leader +1: the peer's relay thread
+//                         ("my A stage i, and the B stage it pairs with, are full")
+//   a_empty[i]   1      : tcgen05.commit of the MMAs that read A stage i, multicast to both CTAs
+//   b_full[i]    4      : the 4 producer warps of the owning set have written B stage i
+//   b_empty[i]   1      : tcgen05.commit (multicast) of the last MMAs that will read B stage i
+//   acc_full[b]  1      : tcgen05.commit after a tile's last MMA, multicast to both CTAs
+//   acc_empty[b] 16     : leader only; the 8 epilogue warps of BOTH CTAs have drained accumulator b
+struct Ring {
+    uint32_t i = 0, phase = 0;
+    __device__ __forceinline__ void advance(uint32_t n_stages) {
+        if (++i == n_stages) { i = 0; phase ^= 1; }
+    }
+};
+
 template <int EXPANSION, int ACT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    float* Xt = reinterpret_cast<float*>(smem + kStages * kStageBytes);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
-    const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8 * kStages;
-    const uint32_t bar_acc_full = bar_empty + 8 * kStages, bar_acc_empty = bar_acc_full + 16;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 4);
+    const uint32_t bar_a_full = smem_u32(bars), bar_a_empty = bar_a_full + 8 * kSlots;
+    const uint32_t bar_b_full = bar_a_empty + 8 * kSlots, bar_b_empty = bar_b_full + 8 * kSlots;
+    const uint32_t bar_peer = bar_b_empty + 8 * kSlots;
+    const uint32_t bar_acc_full = bar_peer + 8 * kSlots, bar_acc_empty = bar_acc_full + 16;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 5 * kSlots + 4);
     const uint32_t smem_base = smem_u32(smem);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -311,11 +331,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int units = prm.p_tiles * prm.m_groups;
     const int m_pairs = prm.m_tiles >> 1;
+    const uint32_t n_a = prm.n_a, n_b = prm.n_b;
+    const bool resident = prm.resident != 0;
+    const uint32_t b_base = smem_base + n_a * kSlotBytes;
 
     if (warp == 0 && lane == 0) {
-        for (int s = 0; s < kStages; ++s) {
-            mbar_init(bar_full + 8 * s, 1 + kNumProdWarps / 2 + (crank == 0 ? 1 : 0));
-            mbar_init(bar_empty + 8 * s, 1);
+        for (int s = 0; s < kSlots; ++s) {
+            mbar_init(bar_a_full + 8 * s, crank == 0 ? 2 : 1);   // leader: own loader + the peer's relay
+            mbar_init(bar_a_empty + 8 * s, 1);
+            mbar_init(bar_b_full + 8 * s, kNumProdWarps / 2);
+            mbar_init(bar_b_empty + 8 * s, 1);
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar_acc_full + 8 * b, 1);
@@ -331,67 +356,73 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp == 0) {
-        // ============================================================== loader: W operand images -> A stages
+        // ============================================================== loader: W operand images -> A ring
         if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
+            Ring ra;
+            uint32_t ready = mbar_try_wait(bar_a_empty + 8 * ra.i, ra.phase ^ 1);
             for (int u = pair; u < units; u += n_pairs) {
                 const int mg = u % prm.m_groups;
                 const int mp0 = mg * prm.m_pairs_per_group;
                 const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
                 for (int mp = mp0; mp < mp1; ++mp) {
                     const int mt = 2 * mp + static_cast<int>(crank);
-                    const uint8_t* src = prm.Wimg + static_cast<size_t>(mt) * prm.steps * (2 * kABytes);
+                    const uint8_t* src = prm.Wimg + static_cast<size_t>(mt) * prm.steps * kSlotBytes;
                     for (int s = 0; s < prm.steps; ++s) {
-                        mbar_wait_spin(bar_empty + 8 * stage, phase ^ 1);
-                        mbar_arrive_expect_tx(bar_full + 8 * stage, 2 * kABytes);
-                        bulk_g2s(smem_base + stage * kStageBytes, src + static_cast<size_t>(s) * (2 * kABytes), 2 * kABytes,
-                                 bar_full + 8 * stage);
-                        if (++stage == kStages) { stage = 0; phase ^= 1; }
+                        if (!ready) mbar_wait_spin(bar_a_empty + 8 * ra.i, ra.phase ^ 1);
+                        const uint32_t cur = ra.i;
+                        ra.advance(n_a);
+                        ready = mbar_try_wait(bar_a_empty + 8 * ra.i, ra.phase ^ 1);   // poll the next stage early
+                        mbar_arrive_expect_tx(bar_a_full + 8 * cur, kSlotBytes);
+                        bulk_g2s(smem_base + cur * kSlotBytes, src + static_cast<size_t>(s) * kSlotBytes, kSlotBytes,
+                                 bar_a_full + 8 * cur);
                     }
                 }
             }
         }
     } else if (warp == 1) {
-        if (lane == 0 && crank == 0) {
-            // ============================================================== MMA issuer (leader CTA)
-            uint32_t stage = 0, phase = 0, tile = 0;
-            for (int u = pair; u < units; u += n_pairs) {
+        if (lane == 0) {
+            // ====================================== MMA issuer (leader) / relay "my stages are full" (peer)
+            // The issuing thread does not run ahead of the tensor pipe (measured: every mbarrier poll on its path
+            // added ~110 cycles per K step), so it waits on ONE barrier per step -- the leader's a_full[i] counts its
+            // own loader and the peer's relay -- and polls the next step's barrier BEFORE issuing this step's MMAs.
+            Ring ra, rb;
+            uint32_t tile = 0, unit_parity = 0;
+            const uint32_t leader_a_full = map_to_cta(bar_a_full, 0);
+            uint32_t ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);
+            for (int u = pair; u < units; u += n_pairs, unit_parity ^= 1) {
                 const int mg = u % prm.m_groups;
                 const int mp0 = mg * prm.m_pairs_per_group;
                 const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
                 for (int mp = mp0; mp < mp1; ++mp, ++tile) {
+                    const bool need_b = !resident || mp == mp0;          // B stages must be (re)filled for this tile
+                    const bool release_b = !resident || mp == mp1 - 1;   // last reader of the B stages
                     const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
-                    mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
-                    tc_fence_after();
                     const uint32_t d_tmem = tmem_base + buf * kBN;
+                    if (crank == 0) mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
                     for (int s = 0; s < prm.steps; ++s) {
-                        mbar_wait_spin(bar_full + 8 * stage, phase);
-                        tc_fence_after();
-                        const uint32_t a_hi = smem_base + stage * kStageBytes, a_lo = a_hi + kABytes;
-                        const uint32_t b_hi = a_hi + 2 * kABytes, b_lo = b_hi + kBBytes;
-                        const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
-                        const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
-                        umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, s > 0 ? 1u : 0u);   // small terms first
-                        umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
-                        umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
-                        umma_commit_pair(bar_empty + 8 * stage);                        // stage free in both CTAs
-                        if (++stage == kStages) { stage = 0; phase ^= 1; }
+                        if (resident) { rb.i = s; rb.phase = unit_parity; }
+                        if (!ready) mbar_wait_spin(bar_a_full + 8 * ra.i, ra.phase);
+                        if (need_b) mbar_wait_spin(bar_b_full + 8 * rb.i, rb.phase);
+                        const uint32_t cur = ra.i;
+                        ra.advance(n_a);
+                        ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);            // next step's poll, early
+                        if (crank == 0) {
+                            tc_fence_after();
+                            const uint32_t a_hi = smem_base + cur * kSlotBytes, a_lo = a_hi + kABytes;
+                            const uint32_t b_hi = b_base + rb.i * kSlotBytes, b_lo = b_hi + kBBytes;
+                            const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
+                            const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
+                            umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, s > 0 ? 1u : 0u);   // small terms first
+                            umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
+                            umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
+                            umma_commit_pair(bar_a_empty + 8 * cur);                        // A stage free in both CTAs
+                            if (release_b) umma_commit_pair(bar_b_empty + 8 * rb.i);        // B stage free in both CTAs
+                        } else {
+                            mbar_arrive_cluster(leader_a_full + 8 * cur);                   // relay: my stages are full
+                        }
+                        if (!resident) rb.advance(n_b);
                     }
-                    umma_commit_pair(bar_acc_full + 8 * buf);                           // accumulators complete
-                }
-            }
-        } else if (lane == 0) {
-            // ============================================================== relay (peer CTA): my stage is full
-            uint32_t stage = 0, phase = 0;
-            const uint32_t leader_full = map_to_cta(bar_full, 0);
-            for (int u = pair; u < units; u += n_pairs) {
-                const int mg = u % prm.m_groups;
-                const int mp0 = mg * prm.m_pairs_per_group;
-                const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
-                for (int n = (mp1 - mp0) * prm.steps; n > 0; --n) {
-                    mbar_wait_spin(bar_full + 8 * stage, phase);
-                    mbar_arrive_cluster(leader_full + 8 * stage);
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    if (crank == 0) umma_commit_pair(bar_acc_full + 8 * buf);               // accumulators complete
                 }
             }
         }
@@ -418,7 +449,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 for (int cc = 0; cc < 4; ++cc) {
                     const int col0 = h * 128 + cc * 32;
                     if (col0 >= n_valid) break;
-                    uint32_t v[32];
+                                    uint32_t v[32];
                     tmem_ld32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + buf * kBN + col0, v);
                     const float* tp = prm.t + p0 + col0;
                     if (col0 + 32 <= n_valid) {
@@ -451,73 +482,55 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         }
     } else {
         // ============================================================== producers: phi -> this CTA's half of B
-        // Two sets of 4 warps; a set owns whole chunks (8 features: the recurrences restart there), the sets
-        // alternate chunks, so two chunks are generated concurrently.  One fence + the arrivals per batch of
-        // up to kBatch K steps instead of per step (the fence waits for this warp's stores to land).
+        // Two sets of 4 warps; a set owns whole chunks (8 features: the recurrences restart there) and the sets
+        // alternate chunks.  One proxy fence + the arrivals per batch of up to kBatch K steps (the fence waits for
+        // this warp's stores to land).  x is read straight from global memory (once per unit when resident).
         constexpr int kBatch = 6;
         const int pidx = threadIdx.x - (2 + kNumEpiWarps) * 32;
         const int set = pidx >> 7;              // which warp set
         const int r = pidx & (kRows - 1);       // pattern row of this thread, 0..127
-        uint32_t stage = 0, phase = 0;          // ring position of the next K step in issue order (both sets track it)
+        Ring rb;                                // position of the next K step in issue order (both sets track it)
         uint32_t item = 0;                      // running chunk counter: chunk goes to set (item & 1)
         for (int u = pair; u < units; u += n_pairs) {
             const int pt = u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
             const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
-            const long long p0 = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows;
-            // ---- x tile: coalesced global reads, transposed (and for trig: sin/cos'ed) into Xt
-            asm volatile("bar.sync 1, %0;" ::"n"(kNumProdWarps * 32));   // everyone is done with the old Xt
-            {
-                const int n_el = kRows * prm.N;
-                const long long lim = (prm.P - p0) * prm.N;               // <= 0: no valid pattern in this half
-                const float* src = prm.X + p0 * prm.N;
-                for (int idx = pidx; idx < n_el; idx += kNumProdWarps * 32) {
-                    const float x = idx < lim ? __ldg(src + idx) : 0.0f;
-                    const int row = idx / prm.N, i = idx - row * prm.N;
-                    if (EXPANSION == 0) {
-                        Xt[i * kXtStride + row] = x;
-                    } else {
-                        float sn, cs;
-                        sincosf(x, &sn, &cs);
-                        Xt[i * kXtStride + row] = cs;
-                        Xt[(16 + i) * kXtStride + row] = sn;
-                    }
-                }
-            }
-            asm volatile("bar.sync 1, %0;" ::"n"(kNumProdWarps * 32));
-            for (int mp = mp0; mp < mp1; ++mp) {
+            const long long p = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows + r;
+            const bool valid = p < prm.P;
+            const float* xrow = prm.X + (valid ? p : 0) * prm.N;
+            const int n_fill = resident ? 1 : mp1 - mp0;        // how many times the K extent is generated
+            for (int fill = 0; fill < n_fill; ++fill) {
                 for (int c = 0; c <= prm.chunks; ++c, ++item) {
                     const int n_steps = c < prm.chunks ? prm.steps_per_chunk : 1;      // c == chunks: the bias step
                     if ((item & 1u) == static_cast<uint32_t>(set)) {
-                        uint32_t st = stage, ph = phase;
+                        Ring rs = rb;
                         // recurrence state for the 8 features of this chunk
                         float x2[8], am[8], ac[8], bm[8], bc[8];
 #pragma unroll
                         for (int f = 0; f < 8; ++f) {
                             const int i = c * 8 + f;
-                            const bool have = c < prm.chunks && i < prm.N;
+                            const float x = (valid && c < prm.chunks && i < prm.N) ? __ldg(xrow + i) : 0.0f;
                             if (EXPANSION == 0) {
-                                const float x = have ? Xt[i * kXtStride + r] : 0.0f;
                                 x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
                                 bm[f] = 0.0f; bc[f] = 0.0f;
                             } else {
-                                const float cs = have ? Xt[i * kXtStride + r] : 1.0f;
-                                const float sn = have ? Xt[(16 + i) * kXtStride + r] : 0.0f;
+                                float sn, cs;
+                                sincosf(x, &sn, &cs);
                                 x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
                                 bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
                             }
                         }
-                        uint32_t ready = mbar_try_wait(bar_empty + 8 * st, ph ^ 1);
+                        uint32_t ready = mbar_try_wait(bar_b_empty + 8 * rs.i, rs.phase ^ 1);
                         for (int ss0 = 0; ss0 < n_steps; ss0 += kBatch) {
                             const int nb = min(kBatch, n_steps - ss0);
-                            const uint32_t st0 = st;
+                            const uint32_t first_stage = rs.i;
                             for (int j = 0; j < nb; ++j) {
                                 const int ss = ss0 + j;
-                                if (!ready) mbar_wait_sleep<32>(bar_empty + 8 * st, ph ^ 1);
-                                uint8_t* b_hi = smem + st * kStageBytes + 2 * kABytes + r * 16;
+                                if (!ready) mbar_wait_sleep<32>(bar_b_empty + 8 * rs.i, rs.phase ^ 1);
+                                uint8_t* b_hi = smem + (n_a + rs.i) * kSlotBytes + r * 16;
                                 uint8_t* b_lo = b_hi + kBBytes;
-                                if (++st == kStages) { st = 0; ph ^= 1; }
-                                ready = mbar_try_wait(bar_empty + 8 * st, ph ^ 1);     // poll the next stage early
+                                rs.advance(n_b);
+                                ready = mbar_try_wait(bar_b_empty + 8 * rs.i, rs.phase ^ 1);   // poll the next stage early
                                 if (c == prm.chunks) {
                                     // bias step: element 0 of k-group 0 is the constant 1 (gene 0), the rest padding
                                     *reinterpret_cast<uint4*>(b_hi) = make_uint4(0x00003C00u, 0u, 0u, 0u);
@@ -557,16 +570,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                             fence_proxy_async_smem();
                             __syncwarp();
                             if (lane == 0) {
-                                uint32_t sa = st0;
+                                uint32_t sa = first_stage;
                                 for (int j = 0; j < nb; ++j) {
-                                    mbar_arrive(bar_full + 8 * sa);
-                                    if (++sa == kStages) sa = 0;
+                                    mbar_arrive(bar_b_full + 8 * sa);
+                                    if (++sa == n_b) sa = 0;
                                 }
                             }
                         }
                     }
-                    stage += n_steps;
-                    while (stage >= kStages) { stage -= kStages; phase ^= 1; }
+                    for (int j = 0; j < n_steps; ++j) rb.advance(n_b);
                 }
             }
         }

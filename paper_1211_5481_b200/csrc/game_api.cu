@@ -165,6 +165,9 @@ int eval_internal(game_ctx* c, float* best_out) {
         prm.m_pairs_per_group = static_cast<int>((m_pairs + want - 1) / want);
         prm.m_groups = (m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
         prm.chunks = c->chunks; prm.steps_per_chunk = c->steps_per_chunk; prm.steps = c->steps;
+        prm.resident = c->steps <= umma::kMaxResidentSteps ? 1 : 0;
+        prm.n_b = prm.resident ? c->steps : umma::kStreamBStages;
+        prm.n_a = umma::kSlots - prm.n_b;
         const long long units = static_cast<long long>(prm.p_tiles) * prm.m_groups;
         const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);
         n_part = 2 * grid;

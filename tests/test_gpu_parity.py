@@ -56,6 +56,11 @@ FITNESS_CASES = [
     ("tanh_cheb", "c1", dict(P=2000, M=64, activation=wl.ACT_TANH)),
     ("sigmoid_trig", "c2", dict(P=2000, M=64, activation=wl.ACT_SIGMOID)),
     ("d1", "c1", dict(P=1000, N=3, d=1, M=16)),
+    # K extent too long for phi to stay resident in shared memory -> the kernel's streaming mode (25 K steps)
+    ("stream_cheb", "c3", dict(P=1300, N=32, d=12, M=300)),
+    ("stream_trig", "c2", dict(P=900, N=16, d=12, M=140)),
+    # many chromosome tiles per unit with resident phi (reuse across 5 tile pairs), ragged everything
+    ("resident_reuse", "c3", dict(P=2100, N=31, d=9, M=1111)),
 ]
 
 
