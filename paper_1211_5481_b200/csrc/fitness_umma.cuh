@@ -44,26 +44,32 @@ constexpr int kBN = 256;             // patterns per pair tile (MMA N, TMEM colu
 constexpr int kRows = kBN / 2;       // pattern rows of the B operand generated and held by each CTA
 constexpr int kABytes = 2 * kBM * 16;          // one K step of A, hi or lo: 2 k-groups x 128 rows x 16 B = 4096
 constexpr int kBBytes = 2 * kRows * 16;        // one K step of this CTA's half of B, hi or lo: 4096
-constexpr int kSlotBytes = 2 * kABytes;        // one stage of either operand (hi + lo) = 8192
-static_assert(2 * kBBytes == kSlotBytes, "A and B stages share the slot size");
-constexpr int kSlots = 26;                     // 8 KB slots shared by the A ring and the B stages
-constexpr int kMinAStages = 4;
-constexpr int kMaxResidentSteps = kSlots - kMinAStages;   // phi of a whole pattern tile stays in smem up to here
-constexpr int kStreamBStages = 12;             // B ring when phi does not fit (regenerated per chromosome tile)
+constexpr int kSlotBytes = 2 * kABytes;        // one K step of either operand (hi + lo) = 8192
+static_assert(2 * kBBytes == kSlotBytes, "A and B steps share the slot size");
+constexpr int kKS = 2;                         // K steps per pipeline stage: the issuing thread's fixed cost per
+                                               // stage (poll ~150, commit ~120, fence ~45 cycles, measured) is
+                                               // amortised over 3 * kKS MMAs of 128 cycles each
+constexpr int kStageBytes = kKS * kSlotBytes;  // 16384
+constexpr int kStagesTotal = 14;               // 16 KB stages shared by the A ring and the B stages (224 KB)
+constexpr int kMaxResidentStages = 11;         // phi of a whole pattern tile stays in smem up to 22 K steps
+constexpr int kStreamBStages = 6;              // B ring when phi does not fit (regenerated per chromosome tile)
 constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4 warps (128 rows each)
 constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
-constexpr int kSmemBar = kSlots * kSlotBytes;  // barriers start here
-constexpr int kBarBytes = (5 * kSlots + 4) * 8 + 16;
+constexpr int kSmemBar = kStagesTotal * kStageBytes;  // barriers start here
+constexpr int kBarBytes = (4 * kStagesTotal + 4) * 8 + 16;
 constexpr int kSmemBytes = kSmemBar + kBarBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
+static_assert(kSmemBytes <= 232448, "shared memory budget");
 
 struct Params {
     const float* X;        // [P][N]
     const float* t;        // [P]
+    const float* W;        // [M][G]: only gene 0 (the bias a_0) is read here, by the epilogue
     const uint8_t* Wimg;   // [m_tiles][steps][8192]: A_hi (2 k-groups x 128 rows x 16 B), then A_lo
     double* part;          // [gridDim.x * 2][m_stride]
+    long long* stall;      // optional [gridDim.x][4]: cycles the MMA/relay thread stalled on a_full, b_full, acc_empty; total
     long long P;
-    int N, d, M;
+    int N, d, M, G;
     int m_stride;          // m_tiles * 128
     int m_tiles;           // chromosome tiles, padded to an even number (one per CTA of a pair)
     int p_tiles;           // pattern tiles of 256
@@ -71,9 +77,10 @@ struct Params {
     int m_pairs_per_group;
     int chunks;            // ceil(N / 8)
     int steps_per_chunk;   // Chebyshev ceil(d / 2); trig d
-    int steps;             // chunks * steps_per_chunk + 1 (bias)
-    int resident;          // 1: n_b == steps, phi generated once per unit and reused by all its chromosome tiles
-    int n_a, n_b;          // A ring stages, B stages (n_a + n_b <= kSlots)
+    int steps;             // chunks * steps_per_chunk K steps (the bias gene is added by the epilogue)
+    int stages;            // ceil(steps / kKS) pipeline stages per tile
+    int resident;          // 1: n_b == stages, phi generated once per unit and reused by all its chromosome tiles
+    int n_a, n_b;          // A ring stages, B stages (n_a + n_b <= kStagesTotal)
 };
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -206,8 +213,7 @@ constexpr uint32_t kIdesc = (1u << 4) | (static_cast<uint32_t>(kBN >> 3) << 17) 
 // ---------------------------------------------------------------------------------------------- K-axis permutation
 // Gene held by (K step s, k-group kg in {0,1}, slot f in 0..7), or -1 for padding.  Used by the W image
 // builder; the producers below generate phi in exactly this order.
-__host__ __device__ inline int gene_at(int s, int kg, int f, int N, int d, int expansion, int steps_per_chunk, int steps) {
-    if (s == steps - 1) return (kg == 0 && f == 0) ? 0 : -1;
+__host__ __device__ inline int gene_at(int s, int kg, int f, int N, int d, int expansion, int steps_per_chunk) {
     const int c = s / steps_per_chunk, ss = s % steps_per_chunk;
     const int i = c * 8 + f;
     if (i >= N) return -1;
@@ -236,7 +242,7 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
         float w[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const int g = gene_at(s, kg, f2 * 2 + e, N, d, expansion, steps_per_chunk, steps);
+            const int g = gene_at(s, kg, f2 * 2 + e, N, d, expansion, steps_per_chunk);
             w[e] = (g >= 0 && m < M) ? W[static_cast<size_t>(m) * G + g] : 0.0f;
         }
         const __half2 h = __floats2half2_rn(w[0], w[1]);
@@ -278,33 +284,38 @@ __device__ __forceinline__ void zero_store(uint8_t* hi_dst, uint8_t* lo_dst) {
     *reinterpret_cast<uint4*>(lo_dst) = make_uint4(0u, 0u, 0u, 0u);
 }
 
+// (act(z + bias) - t)^2.  `bias_term` is the bias gene pre-multiplied so that it rides on the FFMA that scales z for
+// ex2: sigmoid -log2(e) * a_0, tanh 2 log2(e) * a_0, identity a_0 itself.
 template <int ACT>
-__device__ __forceinline__ float act_err2(float z, float t) {
+__device__ __forceinline__ float bias_term_of(float a0) {
+    return ACT == 1 ? -1.44269504088896340736f * a0 : (ACT == 2 ? 2.88539008177792681472f * a0 : a0);
+}
+template <int ACT>
+__device__ __forceinline__ float act_err2(float z, float bias_term, float t) {
     float y;
     if (ACT == 1) {
-        y = rcp_approx(1.0f + ex2_approx(-1.44269504088896340736f * z));
+        y = rcp_approx(1.0f + ex2_approx(fmaf(z, -1.44269504088896340736f, bias_term)));
     } else if (ACT == 2) {
-        y = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(2.88539008177792681472f * z)), 1.0f);
+        y = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(fmaf(z, 2.88539008177792681472f, bias_term))), 1.0f);
     } else {
-        y = z;
+        y = z + bias_term;
     }
     const float e = y - t;
     return e * e;
 }
 
-
 // ---------------------------------------------------------------------------------------------- the kernel
-// Shared memory: kSlots slots of 8 KB.  Slots [0, n_a) are the A ring (W operand images streamed from L2 by
-// the loader, one K step each); slots [n_a, n_a + n_b) hold this CTA's half of B (phi).  If the whole K extent
-// fits (steps <= kMaxResidentSteps: "resident", n_b == steps) phi of a pattern tile is generated ONCE per work
-// unit and reused by every chromosome-tile pair of the unit; the producers refill stage s for the next unit as
-// soon as the unit's last tile has consumed it.  Otherwise ("streaming") B is a ring refilled per tile.
+// Shared memory: kStagesTotal stages of 16 KB (kKS = 2 K steps each).  Stages [0, n_a) are the A ring (W operand
+// images streamed from L2 by the loader); stages [n_a, n_a + n_b) hold this CTA's half of B (phi).  If the whole
+// K extent fits (stages <= kMaxResidentStages: "resident", n_b == stages) phi of a pattern tile is generated ONCE
+// per work unit and reused by every chromosome-tile pair of the unit; the producers refill a stage for the next
+// unit as soon as the unit's last tile has consumed it.  Otherwise ("streaming") B is a ring refilled per tile.
 //
 // Barriers (per CTA unless noted; "leader" = cluster rank 0, "peer" = rank 1):
 //   a_full[i]    1 + tx : the loader's bulk copy of A stage i has landed; on the leader +1: the peer's relay thread
 //                         ("my A stage i, and the B stage it pairs with, are full")
 //   a_empty[i]   1      : tcgen05.commit of the MMAs that read A stage i, multicast to both CTAs
-//   b_full[i]    4      : the 4 producer warps of the owning set have written B stage i
+//   b_full[i]    4 * (K steps in the stage): the 4 producer warps that own each of its K steps have written it
 //   b_empty[i]   1      : tcgen05.commit (multicast) of the last MMAs that will read B stage i
 //   acc_full[b]  1      : tcgen05.commit after a tile's last MMA, multicast to both CTAs
 //   acc_empty[b] 16     : leader only; the 8 epilogue warps of BOTH CTAs have drained accumulator b
@@ -313,17 +324,22 @@ struct Ring {
     __device__ __forceinline__ void advance(uint32_t n_stages) {
         if (++i == n_stages) { i = 0; phase ^= 1; }
     }
+    __device__ __forceinline__ Ring at(uint32_t offset, uint32_t n_stages) const {
+        Ring r = *this;
+        r.i += offset;
+        while (r.i >= n_stages) { r.i -= n_stages; r.phase ^= 1; }
+        return r;
+    }
 };
 
 template <int EXPANSION, int ACT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
-    const uint32_t bar_a_full = smem_u32(bars), bar_a_empty = bar_a_full + 8 * kSlots;
-    const uint32_t bar_b_full = bar_a_empty + 8 * kSlots, bar_b_empty = bar_b_full + 8 * kSlots;
-    const uint32_t bar_peer = bar_b_empty + 8 * kSlots;
-    const uint32_t bar_acc_full = bar_peer + 8 * kSlots, bar_acc_empty = bar_acc_full + 16;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 5 * kSlots + 4);
+    const uint32_t bar_a_full = smem_u32(bars), bar_a_empty = bar_a_full + 8 * kStagesTotal;
+    const uint32_t bar_b_full = bar_a_empty + 8 * kStagesTotal, bar_b_empty = bar_b_full + 8 * kStagesTotal;
+    const uint32_t bar_acc_full = bar_b_empty + 8 * kStagesTotal, bar_acc_empty = bar_acc_full + 16;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4 * kStagesTotal + 4);
     const uint32_t smem_base = smem_u32(smem);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -332,14 +348,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     const int units = prm.p_tiles * prm.m_groups;
     const int m_pairs = prm.m_tiles >> 1;
     const uint32_t n_a = prm.n_a, n_b = prm.n_b;
+    const int stages = prm.stages;
     const bool resident = prm.resident != 0;
-    const uint32_t b_base = smem_base + n_a * kSlotBytes;
+    const uint32_t b_base = smem_base + n_a * kStageBytes;
 
     if (warp == 0 && lane == 0) {
-        for (int s = 0; s < kSlots; ++s) {
+        for (int s = 0; s < kStagesTotal; ++s) {
+            // K steps held by B stage s (resident: the tile's last stage may hold fewer than kKS)
+            const int ks = resident ? min(kKS, prm.steps - s * kKS) : kKS;
             mbar_init(bar_a_full + 8 * s, crank == 0 ? 2 : 1);   // leader: own loader + the peer's relay
             mbar_init(bar_a_empty + 8 * s, 1);
-            mbar_init(bar_b_full + 8 * s, kNumProdWarps / 2);
+            mbar_init(bar_b_full + 8 * s, (kNumProdWarps / 2) * max(ks, 1));
             mbar_init(bar_b_empty + 8 * s, 1);
         }
         for (int b = 0; b < 2; ++b) {
@@ -367,13 +386,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 for (int mp = mp0; mp < mp1; ++mp) {
                     const int mt = 2 * mp + static_cast<int>(crank);
                     const uint8_t* src = prm.Wimg + static_cast<size_t>(mt) * prm.steps * kSlotBytes;
-                    for (int s = 0; s < prm.steps; ++s) {
+                    for (int j = 0; j < stages; ++j) {
                         if (!ready) mbar_wait_spin(bar_a_empty + 8 * ra.i, ra.phase ^ 1);
                         const uint32_t cur = ra.i;
                         ra.advance(n_a);
                         ready = mbar_try_wait(bar_a_empty + 8 * ra.i, ra.phase ^ 1);   // poll the next stage early
-                        mbar_arrive_expect_tx(bar_a_full + 8 * cur, kSlotBytes);
-                        bulk_g2s(smem_base + cur * kSlotBytes, src + static_cast<size_t>(s) * kSlotBytes, kSlotBytes,
+                        const uint32_t bytes = static_cast<uint32_t>(min(kKS, prm.steps - j * kKS)) * kSlotBytes;
+                        mbar_arrive_expect_tx(bar_a_full + 8 * cur, bytes);
+                        bulk_g2s(smem_base + cur * kStageBytes, src + static_cast<size_t>(j) * kStageBytes, bytes,
                                  bar_a_full + 8 * cur);
                     }
                 }
@@ -382,12 +402,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     } else if (warp == 1) {
         if (lane == 0) {
             // ====================================== MMA issuer (leader) / relay "my stages are full" (peer)
-            // The issuing thread does not run ahead of the tensor pipe (measured: every mbarrier poll on its path
-            // added ~110 cycles per K step), so it waits on ONE barrier per step -- the leader's a_full[i] counts its
-            // own loader and the peer's relay -- and polls the next step's barrier BEFORE issuing this step's MMAs.
+            // The issuing thread is the serial resource of the whole kernel (measured per stage: barrier poll ~150
+            // cycles, commit ~120, fence + descriptors ~45, each MMA issue ~60), so a stage carries kKS K steps
+            // (3 * kKS MMAs), the leader waits on ONE barrier per stage -- its a_full[i] counts its own loader and
+            // the peer's relay -- and it polls the next stage's barrier BEFORE issuing this stage's MMAs.
             Ring ra, rb;
             uint32_t tile = 0, unit_parity = 0;
             const uint32_t leader_a_full = map_to_cta(bar_a_full, 0);
+            long long st_a = 0, st_b = 0, st_c = 0;
+            const long long t_begin = clock64();
             uint32_t ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);
             for (int u = pair; u < units; u += n_pairs, unit_parity ^= 1) {
                 const int mg = u % prm.m_groups;
@@ -398,23 +421,38 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     const bool release_b = !resident || mp == mp1 - 1;   // last reader of the B stages
                     const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
                     const uint32_t d_tmem = tmem_base + buf * kBN;
-                    if (crank == 0) mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
-                    for (int s = 0; s < prm.steps; ++s) {
-                        if (resident) { rb.i = s; rb.phase = unit_parity; }
-                        if (!ready) mbar_wait_spin(bar_a_full + 8 * ra.i, ra.phase);
-                        if (need_b) mbar_wait_spin(bar_b_full + 8 * rb.i, rb.phase);
+                    if (crank == 0 && !mbar_try_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1)) {
+                        const long long t0 = clock64();
+                        mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
+                        st_c += clock64() - t0;
+                    }
+                    for (int j = 0; j < stages; ++j) {
+                        if (resident) { rb.i = j; rb.phase = unit_parity; }
+                        if (!ready) {
+                            const long long t0 = clock64();
+                            mbar_wait_spin(bar_a_full + 8 * ra.i, ra.phase);
+                            st_a += clock64() - t0;
+                        }
+                        if (need_b && !mbar_try_wait(bar_b_full + 8 * rb.i, rb.phase)) {
+                            const long long t0 = clock64();
+                            mbar_wait_spin(bar_b_full + 8 * rb.i, rb.phase);
+                            st_b += clock64() - t0;
+                        }
                         const uint32_t cur = ra.i;
                         ra.advance(n_a);
-                        ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);            // next step's poll, early
+                        ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);            // next stage's poll, early
                         if (crank == 0) {
                             tc_fence_after();
-                            const uint32_t a_hi = smem_base + cur * kSlotBytes, a_lo = a_hi + kABytes;
-                            const uint32_t b_hi = b_base + rb.i * kSlotBytes, b_lo = b_hi + kBBytes;
-                            const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
-                            const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
-                            umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, s > 0 ? 1u : 0u);   // small terms first
-                            umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
-                            umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
+                            const int nk = min(kKS, prm.steps - j * kKS);
+                            for (int k = 0; k < nk; ++k) {
+                                const uint32_t a_hi = smem_base + cur * kStageBytes + k * kSlotBytes, a_lo = a_hi + kABytes;
+                                const uint32_t b_hi = b_base + rb.i * kStageBytes + k * kSlotBytes, b_lo = b_hi + kBBytes;
+                                const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
+                                const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
+                                umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, (j | k) != 0 ? 1u : 0u);   // small terms first
+                                umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
+                                umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
+                            }
                             umma_commit_pair(bar_a_empty + 8 * cur);                        // A stage free in both CTAs
                             if (release_b) umma_commit_pair(bar_b_empty + 8 * rb.i);        // B stage free in both CTAs
                         } else {
@@ -424,6 +462,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     }
                     if (crank == 0) umma_commit_pair(bar_acc_full + 8 * buf);               // accumulators complete
                 }
+            }
+            if (prm.stall != nullptr) {
+                long long* out = prm.stall + static_cast<size_t>(blockIdx.x) * 4;
+                out[0] = st_a; out[1] = st_b; out[2] = st_c; out[3] = clock64() - t_begin;
             }
         }
     } else if (warp < 2 + kNumEpiWarps) {
@@ -442,6 +484,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const int n_valid = static_cast<int>(min(static_cast<long long>(kBN), prm.P - p0));
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                 const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
+                const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
+                // the bias gene a_0 is not part of the contraction: it rides on the epilogue's FFMA
+                const float bias = bias_term_of<ACT>(m < prm.M ? __ldg(prm.W + static_cast<size_t>(m) * prm.G) : 0.0f);
                 mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
@@ -449,7 +494,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 for (int cc = 0; cc < 4; ++cc) {
                     const int col0 = h * 128 + cc * 32;
                     if (col0 >= n_valid) break;
-                                    uint32_t v[32];
+                    uint32_t v[32];
                     tmem_ld32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + buf * kBN + col0, v);
                     const float* tp = prm.t + p0 + col0;
                     if (col0 + 32 <= n_valid) {
@@ -459,16 +504,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                         tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 8; ++i) {
-                            sum += act_err2<ACT>(__uint_as_float(v[4 * i + 0]), tv[i].x);
-                            sum1 += act_err2<ACT>(__uint_as_float(v[4 * i + 1]), tv[i].y);
-                            sum2 += act_err2<ACT>(__uint_as_float(v[4 * i + 2]), tv[i].z);
-                            sum3 += act_err2<ACT>(__uint_as_float(v[4 * i + 3]), tv[i].w);
+                            sum += act_err2<ACT>(__uint_as_float(v[4 * i + 0]), bias, tv[i].x);
+                            sum1 += act_err2<ACT>(__uint_as_float(v[4 * i + 1]), bias, tv[i].y);
+                            sum2 += act_err2<ACT>(__uint_as_float(v[4 * i + 2]), bias, tv[i].z);
+                            sum3 += act_err2<ACT>(__uint_as_float(v[4 * i + 3]), bias, tv[i].w);
                         }
                     } else {
                         tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
-                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), __ldg(tp + i));
+                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), bias, __ldg(tp + i));
                         }
                     }
                 }
@@ -476,7 +521,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8 * buf);
-                const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
                 __stcg(my_part + m, __ldcg(my_part + m) + static_cast<double>(sum));
             }
         }
@@ -489,7 +533,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         const int pidx = threadIdx.x - (2 + kNumEpiWarps) * 32;
         const int set = pidx >> 7;              // which warp set
         const int r = pidx & (kRows - 1);       // pattern row of this thread, 0..127
-        Ring rb;                                // position of the next K step in issue order (both sets track it)
+        Ring rb;                                // ring position of the current fill's first stage
         uint32_t item = 0;                      // running chunk counter: chunk goes to set (item & 1)
         for (int u = pair; u < units; u += n_pairs) {
             const int pt = u / prm.m_groups, mg = u % prm.m_groups;
@@ -500,86 +544,78 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const float* xrow = prm.X + (valid ? p : 0) * prm.N;
             const int n_fill = resident ? 1 : mp1 - mp0;        // how many times the K extent is generated
             for (int fill = 0; fill < n_fill; ++fill) {
-                for (int c = 0; c <= prm.chunks; ++c, ++item) {
-                    const int n_steps = c < prm.chunks ? prm.steps_per_chunk : 1;      // c == chunks: the bias step
-                    if ((item & 1u) == static_cast<uint32_t>(set)) {
-                        Ring rs = rb;
-                        // recurrence state for the 8 features of this chunk
-                        float x2[8], am[8], ac[8], bm[8], bc[8];
+                for (int c = 0; c < prm.chunks; ++c, ++item) {
+                    if ((item & 1u) != static_cast<uint32_t>(set)) continue;
+                    // recurrence state for the 8 features of this chunk
+                    float x2[8], am[8], ac[8], bm[8], bc[8];
 #pragma unroll
-                        for (int f = 0; f < 8; ++f) {
-                            const int i = c * 8 + f;
-                            const float x = (valid && c < prm.chunks && i < prm.N) ? __ldg(xrow + i) : 0.0f;
+                    for (int f = 0; f < 8; ++f) {
+                        const int i = c * 8 + f;
+                        const float x = (valid && i < prm.N) ? __ldg(xrow + i) : 0.0f;
+                        if (EXPANSION == 0) {
+                            x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
+                            bm[f] = 0.0f; bc[f] = 0.0f;
+                        } else {
+                            float sn, cs;
+                            sincosf(x, &sn, &cs);
+                            x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
+                            bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
+                        }
+                    }
+                    const int s_chunk = c * prm.steps_per_chunk;           // first K step of this chunk in the tile
+                    for (int ss0 = 0; ss0 < prm.steps_per_chunk; ss0 += kBatch) {
+                        const int nb = min(kBatch, prm.steps_per_chunk - ss0);
+                        for (int jb = 0; jb < nb; ++jb) {
+                            const int ss = ss0 + jb, s = s_chunk + ss;
+                            const Ring pos = rb.at(s / kKS, n_b);
+                            if (!mbar_try_wait(bar_b_empty + 8 * pos.i, pos.phase ^ 1))
+                                mbar_wait_sleep<32>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
+                            uint8_t* b_hi = smem + (n_a + pos.i) * kStageBytes + (s % kKS) * kSlotBytes + r * 16;
+                            uint8_t* b_lo = b_hi + kBBytes;
+                            float v0[8], v1[8];
                             if (EXPANSION == 0) {
-                                x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
-                                bm[f] = 0.0f; bc[f] = 0.0f;
+                                // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2}
+#pragma unroll
+                                for (int f = 0; f < 8; ++f) {
+                                    v0[f] = ac[f];
+                                    v1[f] = fmaf(x2[f], ac[f], -am[f]);
+                                    ac[f] = fmaf(x2[f], v1[f], -ac[f]);
+                                    am[f] = v1[f];
+                                }
                             } else {
-                                float sn, cs;
-                                sincosf(x, &sn, &cs);
-                                x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
-                                bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
+                                // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
+#pragma unroll
+                                for (int f = 0; f < 8; ++f) {
+                                    v0[f] = ac[f];
+                                    v1[f] = bc[f];
+                                    const float cn = fmaf(x2[f], ac[f], -am[f]);
+                                    const float sn = fmaf(x2[f], bc[f], -bm[f]);
+                                    am[f] = ac[f]; ac[f] = cn;
+                                    bm[f] = bc[f]; bc[f] = sn;
+                                }
+                            }
+                            split_store(v0, b_hi, b_lo);
+                            if (EXPANSION == 0 && 2 * ss + 2 > prm.d) {
+                                zero_store(b_hi + kRows * 16, b_lo + kRows * 16);      // odd d: last k-group is padding
+                            } else {
+                                split_store(v1, b_hi + kRows * 16, b_lo + kRows * 16);
                             }
                         }
-                        uint32_t ready = mbar_try_wait(bar_b_empty + 8 * rs.i, rs.phase ^ 1);
-                        for (int ss0 = 0; ss0 < n_steps; ss0 += kBatch) {
-                            const int nb = min(kBatch, n_steps - ss0);
-                            const uint32_t first_stage = rs.i;
-                            for (int j = 0; j < nb; ++j) {
-                                const int ss = ss0 + j;
-                                if (!ready) mbar_wait_sleep<32>(bar_b_empty + 8 * rs.i, rs.phase ^ 1);
-                                uint8_t* b_hi = smem + (n_a + rs.i) * kSlotBytes + r * 16;
-                                uint8_t* b_lo = b_hi + kBBytes;
-                                rs.advance(n_b);
-                                ready = mbar_try_wait(bar_b_empty + 8 * rs.i, rs.phase ^ 1);   // poll the next stage early
-                                if (c == prm.chunks) {
-                                    // bias step: element 0 of k-group 0 is the constant 1 (gene 0), the rest padding
-                                    *reinterpret_cast<uint4*>(b_hi) = make_uint4(0x00003C00u, 0u, 0u, 0u);
-                                    *reinterpret_cast<uint4*>(b_lo) = make_uint4(0u, 0u, 0u, 0u);
-                                    zero_store(b_hi + kRows * 16, b_lo + kRows * 16);
-                                    continue;
-                                }
-                                float v0[8], v1[8];
-                                if (EXPANSION == 0) {
-                                    // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2}
-#pragma unroll
-                                    for (int f = 0; f < 8; ++f) {
-                                        v0[f] = ac[f];
-                                        v1[f] = fmaf(x2[f], ac[f], -am[f]);
-                                        ac[f] = fmaf(x2[f], v1[f], -ac[f]);
-                                        am[f] = v1[f];
-                                    }
-                                } else {
-                                    // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
-#pragma unroll
-                                    for (int f = 0; f < 8; ++f) {
-                                        v0[f] = ac[f];
-                                        v1[f] = bc[f];
-                                        const float cn = fmaf(x2[f], ac[f], -am[f]);
-                                        const float sn = fmaf(x2[f], bc[f], -bm[f]);
-                                        am[f] = ac[f]; ac[f] = cn;
-                                        bm[f] = bc[f]; bc[f] = sn;
-                                    }
-                                }
-                                split_store(v0, b_hi, b_lo);
-                                if (EXPANSION == 0 && 2 * ss + 2 > prm.d) {
-                                    zero_store(b_hi + kRows * 16, b_lo + kRows * 16);  // odd d: last k-group is padding
-                                } else {
-                                    split_store(v1, b_hi + kRows * 16, b_lo + kRows * 16);
-                                }
-                            }
-                            fence_proxy_async_smem();
-                            __syncwarp();
-                            if (lane == 0) {
-                                uint32_t sa = first_stage;
-                                for (int j = 0; j < nb; ++j) {
-                                    mbar_arrive(bar_b_full + 8 * sa);
-                                    if (++sa == n_b) sa = 0;
-                                }
+                        fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            for (int jb = 0; jb < nb; ++jb) {
+                                const int s = s_chunk + ss0 + jb;
+                                const Ring pos = rb.at(s / kKS, n_b);
+                                mbar_arrive(bar_b_full + 8 * pos.i);
+                                // streaming ring stages always expect kKS K steps: stand in for the missing ones
+                                if (!resident && s == prm.steps - 1)
+                                    for (int e = prm.steps % kKS; e != 0 && e < kKS; ++e) mbar_arrive(bar_b_full + 8 * pos.i);
                             }
                         }
                     }
-                    for (int j = 0; j < n_steps; ++j) rb.advance(n_b);
                 }
+                rb = rb.at(stages, n_b);
             }
         }
     }

@@ -34,7 +34,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -150,8 +150,8 @@ int eval_internal(game_ctx* c, float* best_out) {
             W, img, c->M, c->G, c->N, c->d, c->expansion, c->steps_per_chunk, c->steps, c->m_tiles);
         if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
         umma::Params prm;
-        prm.X = c->X; prm.t = c->t; prm.Wimg = img; prm.part = part;
-        prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M;
+        prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.part = part;
+        prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
         prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
         prm.p_tiles = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
         int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
@@ -165,9 +165,11 @@ int eval_internal(game_ctx* c, float* best_out) {
         prm.m_pairs_per_group = static_cast<int>((m_pairs + want - 1) / want);
         prm.m_groups = (m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
         prm.chunks = c->chunks; prm.steps_per_chunk = c->steps_per_chunk; prm.steps = c->steps;
-        prm.resident = c->steps <= umma::kMaxResidentSteps ? 1 : 0;
-        prm.n_b = prm.resident ? c->steps : umma::kStreamBStages;
-        prm.n_a = umma::kSlots - prm.n_b;
+        prm.stages = (c->steps + umma::kKS - 1) / umma::kKS;
+        prm.resident = prm.stages <= umma::kMaxResidentStages ? 1 : 0;
+        prm.n_b = prm.resident ? prm.stages : umma::kStreamBStages;
+        prm.n_a = umma::kStagesTotal - prm.n_b;
+        prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
         const long long units = static_cast<long long>(prm.p_tiles) * prm.m_groups;
         const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);
         n_part = 2 * grid;
@@ -253,7 +255,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
                  (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
     c->chunks = (N + 7) / 8;
     c->steps_per_chunk = expansion == GAME_EXP_CHEBYSHEV ? (d + 1) / 2 : d;
-    c->steps = c->chunks * c->steps_per_chunk + 1;
+    c->steps = c->chunks * c->steps_per_chunk;
     size_t off = 0;
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
     c->off_img = off;
@@ -262,6 +264,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_blk_key = off; off = align_up(off + fin_blocks * sizeof(float));
     c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
     c->off_ticket = off; off = align_up(off + sizeof(unsigned int));
+    c->off_stall = off; off = align_up(off + sizeof(long long) * 4 * kMaxCtas);
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
