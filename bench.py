@@ -40,7 +40,7 @@ UNIT = "evals/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists).
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"c3": 547028480}      # profiles/r01b_README.md: 537.8 MB read + 9.2 MB written
 
 
 def parse_args():
@@ -268,7 +268,8 @@ def run_ours(args, cfg, rank, world, local_rank):
 
     # ---------------- roofline of the dominant kernel (fused fitness)
     peaks, peaks_src = load_peaks()
-    flops_per_launch = 2.0 * cfg.P * cfg.M * cfg.G * (3 if G.scheme() == game.SCHEME_F16X3 else 1)
+    flops_per_launch = (6.0 * cfg.P * cfg.M * (cfg.G - 1) if G.scheme() == game.SCHEME_F16X3      # 3 MMAs per gene; the bias gene rides on the epilogue
+                        else 2.0 * cfg.P * cfg.M * cfg.G)
     avg_s = kernel_ms * 1e-3 / max(kernel_n, 1)
     achieved = flops_per_launch / avg_s / 1e12
     if G.scheme() == game.SCHEME_F16X3:

@@ -7,7 +7,7 @@
 // GENERATED in shared memory and never exists in HBM.  Persistent kernel, one CTA PAIR (cluster of 2, the two
 // SMs of a TPC) per 256 chromosomes x 256 patterns tile, tcgen05 cta_group::2:
 //
-//   warp 0      loader   : cp.async.bulk (1-D TMA) of this CTA's pre-split W operand images, 8 KB per K step
+//   warp 0      loader   : cp.async.bulk (1-D TMA) of this CTA's pre-split W operand images, 16 KB (2 K steps) per stage
 //   warp 1      MMA      : leader CTA: tcgen05.mma.cta_group::2.kind::f16, M=256 (128 chromosomes per CTA) x
 //                          N=256 patterns (128 generated per CTA) x K=16 genes, three MMAs per K step
 //                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM;
@@ -29,8 +29,8 @@
 // k-groups.  The K axis is a PERMUTATION of the genes chosen for the generator (the W images use the same one):
 //   chunk c = features 8c..8c+7;  k-group kg of the chunk holds, for those 8 features,
 //       Chebyshev: T_{kg+1}(x_i)          trig: cos((kg/2+1) x_i) if kg even, sin((kg/2+1) x_i) if kg odd
-//   (padded to an even number of k-groups; absent features / degrees are zeros in the W image), then one last
-//   K step whose element 0 is the bias gene.
+//   (padded to an even number of k-groups; absent features / degrees are zeros in the W image).  The bias gene
+//   a_0 is not on the K axis: the epilogue adds it on the FFMA that scales z for ex2.
 #pragma once
 #include <cuda_fp16.h>
 
