@@ -7,7 +7,7 @@
 // GENERATED in shared memory and never exists in HBM.  Persistent kernel, one CTA PAIR (cluster of 2, the two
 // SMs of a TPC) per 256 chromosomes x 256 patterns tile, tcgen05 cta_group::2:
 //
-//   warp 0      loader   : cp.async.bulk (1-D TMA) of this CTA's pre-split W operand images, 16 KB (2 K steps) per stage
+//   warp 0      loader   : cp.async.bulk (1-D TMA) of this CTA's pre-split W operand images, 32 KB (4 K steps) per stage
 //   warp 1      MMA      : leader CTA: tcgen05.mma.cta_group::2.kind::f16, M=256 (128 chromosomes per CTA) x
 //                          N=256 patterns (128 generated per CTA) x K=16 genes, three MMAs per K step
 //                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM;
@@ -46,13 +46,14 @@ constexpr int kABytes = 2 * kBM * 16;          // one K step of A, hi or lo: 2 k
 constexpr int kBBytes = 2 * kRows * 16;        // one K step of this CTA's half of B, hi or lo: 4096
 constexpr int kSlotBytes = 2 * kABytes;        // one K step of either operand (hi + lo) = 8192
 static_assert(2 * kBBytes == kSlotBytes, "A and B steps share the slot size");
-constexpr int kKS = 2;                         // K steps per pipeline stage: the issuing thread's fixed cost per
+constexpr int kKS = 4;                         // K steps per pipeline stage: the issuing thread's fixed cost per
                                                // stage (poll ~150, commit ~120, fence ~45 cycles, measured) is
-                                               // amortised over 3 * kKS MMAs of 128 cycles each
-constexpr int kStageBytes = kKS * kSlotBytes;  // 16384
-constexpr int kStagesTotal = 14;               // 16 KB stages shared by the A ring and the B stages (224 KB)
-constexpr int kMaxResidentStages = 11;         // phi of a whole pattern tile stays in smem up to 22 K steps
-constexpr int kStreamBStages = 6;              // B ring when phi does not fit (regenerated per chromosome tile)
+                                               // amortised over 3 * kKS MMAs of 128 cycles each (kKS = 1: 27.6 ms,
+                                               // 2: 22.4 ms, 4: 20.3 ms per c3 evaluation)
+constexpr int kStageBytes = kKS * kSlotBytes;  // 32768
+constexpr int kStagesTotal = 7;                // 32 KB stages shared by the A ring and the B stages (224 KB)
+constexpr int kMaxResidentStages = 5;          // phi of a whole pattern tile stays in smem up to 20 K steps
+constexpr int kStreamBStages = 3;              // B ring when phi does not fit (regenerated per chromosome tile)
 constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4 warps (128 rows each)
 constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
 constexpr int kSmemBar = kStagesTotal * kStageBytes;  // barriers start here
@@ -305,7 +306,7 @@ __device__ __forceinline__ float act_err2(float z, float bias_term, float t) {
 }
 
 // ---------------------------------------------------------------------------------------------- the kernel
-// Shared memory: kStagesTotal stages of 16 KB (kKS = 2 K steps each).  Stages [0, n_a) are the A ring (W operand
+// Shared memory: kStagesTotal stages of 32 KB (kKS = 4 K steps each).  Stages [0, n_a) are the A ring (W operand
 // images streamed from L2 by the loader); stages [n_a, n_a + n_b) hold this CTA's half of B (phi).  If the whole
 // K extent fits (stages <= kMaxResidentStages: "resident", n_b == stages) phi of a pattern tile is generated ONCE
 // per work unit and reused by every chromosome-tile pair of the unit; the producers refill a stage for the next
