@@ -40,7 +40,7 @@ UNIT = "evals/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists).
-NCU_TRAFFIC_BYTES = {"c3": 547028480}      # profiles/r01b_README.md: 537.8 MB read + 9.2 MB written
+NCU_TRAFFIC_BYTES = {"c3": 544669440}      # profiles/r01c_README.md: 535.2 MB read + 9.5 MB written
 
 
 def parse_args():
@@ -48,7 +48,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS) + ["c4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="auto", choices=["auto", "ffma", "f16x3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -312,6 +312,59 @@ def run_ours(args, cfg, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_c4_sweep(args):
+    """BASELINE.json configs[4]: fitness-kernel sweep (no GA step), M x P grid at N=20, d=6 (G=121).  One JSON line:
+    `value` is the largest point; `sweep` lists evals/s and the tensor / HBM roofline fractions of every point."""
+    import torch
+    import paper_1211_5481_b200 as game
+    from paper_1211_5481_b200 import build as game_build
+
+    game_build.build()
+    peaks, peaks_src = load_peaks()
+    big = wl.c4(max(wl.C4_M), max(wl.C4_P))
+    X, t, _ = wl.make_kb(big)
+    Xd, td = torch.from_numpy(X).cuda(), torch.from_numpy(t).cuda()
+    sweep, launches = [], 0
+    sampler = ClockSampler(0)
+    sampler.start()
+    for M in wl.C4_M:
+        W = torch.from_numpy(wl.uniform_population(M, big.G, seed=4)).cuda()
+        for P in wl.C4_P:
+            G = game.Game(P, big.N, big.d, M, big.expansion, big.activation)
+            G.X.copy_(Xd[:P]); G.t.copy_(td[:P]); G.set_population(W)
+            for _ in range(max(args.warmup, 3)):
+                game.game_eval_fitness(G.ctx)
+            torch.cuda.synchronize()
+            game.game_time_fitness_kernel(G.ctx, True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                game.game_eval_fitness(G.ctx)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            kms, kn = game.game_fitness_kernel_ms(G.ctx)
+            launches += 3 * args.steps
+            tf = 6.0 * P * M * (big.G - 1) / (kms / kn * 1e-3) / 1e12
+            sweep.append({"M": M, "P": P, "ms_per_eval": ms, "evals_per_s": P * M / (ms * 1e-3), "kernel_ms": kms / kn,
+                          "tensor_tflops": tf, "tensor_frac": tf / float(peaks["bf16_tflops"]),
+                          "hbm_frac": 4.0 * P * (big.N + 1) / (kms / kn * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
+                          "l2": "X larger than L2" if P * big.N * 4 > 126e6 else "X fits L2 (not flushed)"})
+            G.close()
+    clocks = sampler.stop()
+    last = sweep[-1]
+    line = {"metric": METRIC, "value": last["evals_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": last["ms_per_eval"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f16x3->f32", "data": "synthetic",
+            "config": {"workload": "c4: BASELINE.json configs[4] fitness-kernel sweep (no GA step); value = largest point",
+                       "N": big.N, "d": big.d, "G": big.G, "M": list(wl.C4_M), "P": list(wl.C4_P),
+                       "peak": f"{peaks_src} bf16_tflops (burst: every point is timed alone)"},
+            "e2e": None, "gpu_launches": launches, "clocks": clocks, "sweep": sweep,
+            "roofline": {"bound": "tensor", "achieved": last["tensor_tflops"], "peak": float(peaks["bf16_tflops"]), "unit": "TFLOP/s",
+                         "frac": last["tensor_frac"], "traffic": None}, "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -325,6 +378,10 @@ def main():
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
                "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
         sys.exit(subprocess.call(cmd))
+    if args.workload == "c4":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_c4_sweep(args)
+        return
     cfg = wl.CONFIGS[args.workload]
     if args.impl == "reference":
         run_reference(args, cfg, rank, world)
