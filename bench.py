@@ -203,9 +203,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         torch.cuda.synchronize()
 
     def generations(first_gen, n):
-        for i in range(n):
-            game.game_eval_fitness(G.ctx)
-            game.game_step(G.ctx, seed, first_gen + i)
+        game.game_evolve(G.ctx, seed, first_gen, n)          # n x (fused fitness eval, GA step): launches only
 
     # ---------------- device-resident leg
     generations(0, args.warmup)

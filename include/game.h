@@ -143,6 +143,11 @@ int game_step(game_ctx* ctx, uint64_t seed, uint32_t gen);
  * NULL) receives the best (lowest) fitness of each generation's population.  Async. */
 int game_run(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev);
 
+/* n_gens x (eval, step with gen = gen0 + i) with NO trailing evaluation (the population is left one step past its
+ * last fitness): the generation loop of PAPER.md:97 as one call, launches only, no host synchronisation.  This is
+ * what bench.py times as "K steps".  Async. */
+int game_evolve(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens);
+
 /* Stream synchronise; returns GAME_ERR_CUDA if any enqueued work failed. */
 int game_sync(game_ctx* ctx);
 

@@ -41,6 +41,7 @@ SIGNATURES = {
     "game_eval_fitness": (C.c_int, [_VP]),
     "game_step": (C.c_int, [_VP, C.c_uint64, C.c_uint32]),
     "game_run": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, _F32P]),
+    "game_evolve": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32]),
     "game_sync": (C.c_int, [_VP]),
     "game_generation_host": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, _F32P, C.c_uint64, C.c_uint32]),
     "game_launch_count": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
@@ -162,6 +163,10 @@ def game_step(ctx, seed: int, gen: int) -> None:
 
 def game_run(ctx, seed: int, gen0: int, n_gens: int, best_fitness_dev: int | None) -> None:
     _check(ctx, lib().game_run(ctx, seed, gen0, n_gens, best_fitness_dev))
+
+
+def game_evolve(ctx, seed: int, gen0: int, n_gens: int) -> None:
+    _check(ctx, lib().game_evolve(ctx, seed, gen0, n_gens))
 
 
 def game_sync(ctx) -> None:

@@ -410,6 +410,17 @@ int game_run(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* 
     return GAME_OK;
 }
 
+int game_evolve(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    for (uint32_t i = 0; i < n_gens; ++i) {
+        int rc = eval_internal(c, nullptr);
+        if (rc) return rc;
+        rc = step_internal(c, seed, gen0 + i);
+        if (rc) return rc;
+    }
+    return GAME_OK;
+}
+
 int game_sync(game_ctx* c) {
     if (!c) return GAME_ERR_INVALID_ARG;
     GAME_CUDA(cudaStreamSynchronize(c->stream));

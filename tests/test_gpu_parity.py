@@ -282,3 +282,51 @@ def test_generation_host_entry(game):
     assert np.array_equal(Wn.numpy().view(np.uint32), ref.view(np.uint32))
     assert G.launch_count() >= 3
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ full sizes
+def test_full_size_c1_all_chromosomes(game):
+    """BASELINE.json configs[1] at full size, in the launch configuration bench.py times (AUTO scheme, persistent
+    grid of CTA pairs): every chromosome against the oracle."""
+    cfg = wl.CONFIGS["c1"]
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg)
+    G.load_kb(X, t); G.init_population(cfg.seed); G.eval_fitness(); G.sync()
+    assert G.scheme() == game.SCHEME_F16X3
+    W = G.get_population()
+    assert_fitness_close(G.get_fitness(), oracle.eval_fitness(cfg.d, cfg.family, X, t, W), "c1 full size")
+    G.close()
+
+
+def test_full_size_c3_sampled_chromosomes(game):
+    """BASELINE.json configs[3] (the headline workload) at full size P = 4e6, M = 4096: the oracle cannot finish the
+    whole population, so sampled chromosomes (best, worst, first, last, two tile edges) are computed one by one."""
+    cfg = wl.CONFIGS["c3"]
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg)
+    G.load_kb(X, t); G.init_population(cfg.seed); G.eval_fitness(); G.sync()
+    assert G.scheme() == game.SCHEME_F16X3
+    W, F = G.get_population(), G.get_fitness()
+    assert np.all(np.isfinite(F)) and F.min() > 0
+    rows = sorted({int(np.argmin(F)), int(np.argmax(F)), 0, cfg.M - 1, 127, 128})
+    F_ref = oracle.eval_fitness(cfg.d, cfg.family, X, t, W[rows])
+    assert_fitness_close(F[rows], F_ref, "c3 full size, sampled rows")
+    # property that holds at any size: duplicated chromosomes get bit-identical fitness in any slot
+    W[4000] = W[rows[0]]; W[77] = W[rows[0]]
+    G.set_population(W); G.eval_fitness(); G.sync()
+    F2 = G.get_fitness()
+    assert F2[4000] == F2[77] == F2[rows[0]] == F[rows[0]]
+    G.close()
+
+
+def test_evolve_equals_eval_step_loop(game):
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=3000, M=300)
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg); G.load_kb(X, t); G.init_population(9)
+    for g in range(4):
+        G.eval_fitness(); G.step(9, g)
+    G.sync(); a = G.get_population()
+    G.init_population(9)
+    game.game_evolve(G.ctx, 9, 0, 4); G.sync()
+    assert np.array_equal(G.get_population().view(np.uint32), a.view(np.uint32))
+    G.close()
