@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
 // ---- fitness finalisation: F[m] = (sum over partial rows, in row order) / P in fp64, rounded to fp32
 // (PAPER.md:63 MSE).  Optionally the best (lowest, NaN worst, ties -> lower index) fitness of the
 // population is written to *best_out by the last block to finish (R8).
-constexpr int kFinThreads = 256;
+constexpr int kFinThreads = 256, kFinCols = 32, kFinGroups = kFinThreads / kFinCols;
 
 __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* __restrict__ part,
                                                                         int n_part, int m_stride, int M,
@@ -141,12 +141,29 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
     __shared__ bool s_last;
-    const int m = blockIdx.x * kFinThreads + threadIdx.x;
+    // 32 chromosomes per block x 8 row groups: row group g sums partial rows g, g+8, g+16, ... with four independent
+    // accumulators (the loads are L2 latency-bound: one thread walking all ~300 rows took 108 us at M = 4096), then the
+    // eight group sums are added in group order -- a fixed order, so the result is bit-stable.
+    __shared__ double s_grp[kFinGroups][kFinCols];
+    const int col = threadIdx.x % kFinCols, grp = threadIdx.x / kFinCols;
+    const int m = blockIdx.x * kFinCols + col;
     float key = INFINITY;
     int idx = 0x7fffffff;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
     if (m < M) {
+        int r = grp;
+        for (; r + 3 * kFinGroups < n_part; r += 4 * kFinGroups) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
+        }
+        for (int i = 0; r < n_part; r += kFinGroups, ++i) acc[i] += __ldcg(part + static_cast<size_t>(r) * m_stride + m);
+    }
+    s_grp[grp][col] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+    __syncthreads();
+    if (m < M && grp == 0) {
         double s = 0.0;
-        for (int r = 0; r < n_part; ++r) s += __ldcg(part + static_cast<size_t>(r) * m_stride + m);
+#pragma unroll
+        for (int g = 0; g < kFinGroups; ++g) s += s_grp[g][col];
         const float f = static_cast<float>(s / P_d);
         F[m] = f;
         key = fit_key(f);

@@ -204,7 +204,7 @@ int eval_internal(game_ctx* c, float* best_out) {
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     }
     if (timed) c->events.emplace_back(ev0, ev1);
-    const int fin_blocks = (c->M + kFinThreads - 1) / kFinThreads;
+    const int fin_blocks = (c->M + kFinCols - 1) / kFinCols;
     finalize_fitness_kernel<<<fin_blocks, kFinThreads, 0, c->stream>>>(
         part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, best_out,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
@@ -260,7 +260,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
     c->off_img = off;
     if (c->umma_ok) off = align_up(off + static_cast<size_t>(c->m_tiles) * c->steps * 2 * game::umma::kABytes);
-    const size_t fin_blocks = (static_cast<size_t>(M) + game::kFinThreads - 1) / game::kFinThreads;
+    const size_t fin_blocks = (static_cast<size_t>(M) + game::kFinCols - 1) / game::kFinCols;
     c->off_blk_key = off; off = align_up(off + fin_blocks * sizeof(float));
     c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
     c->off_ticket = off; off = align_up(off + sizeof(unsigned int));
