@@ -58,7 +58,8 @@ constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4
 constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
 constexpr int kSmemBar = kStagesTotal * kStageBytes;  // barriers start here
 constexpr int kBarBytes = (4 * kStagesTotal + 4) * 8 + 16;
-constexpr int kSmemBytes = kSmemBar + kBarBytes;
+constexpr int kTsBytes = kBN * 4;                 // targets of the current pattern tile, staged once per unit
+constexpr int kSmemBytes = kSmemBar + kBarBytes + kTsBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
 static_assert(kSmemBytes <= 232448, "shared memory budget");
 
@@ -341,6 +342,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     const uint32_t bar_b_full = bar_a_empty + 8 * kStagesTotal, bar_b_empty = bar_b_full + 8 * kStagesTotal;
     const uint32_t bar_acc_full = bar_b_empty + 8 * kStagesTotal, bar_acc_empty = bar_acc_full + 16;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4 * kStagesTotal + 4);
+    float* ts_all = reinterpret_cast<float*>(smem + kSmemBar + kBarBytes);
     const uint32_t smem_base = smem_u32(smem);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -483,6 +485,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
             const long long p0 = static_cast<long long>(pt) * kBN;
             const int n_valid = static_cast<int>(min(static_cast<long long>(kBN), prm.P - p0));
+            // the 4 warps that share a column half stage its 128 targets in shared memory once per unit (they are the
+            // same for every chromosome tile of the unit); named barrier per half, 128 threads
+            float* ts = ts_all + h * 128;
+            asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");      // everyone is done with the previous tile's t
+            {
+                const int gi = q * 32 + lane;
+                ts[gi] = (h * 128 + gi < n_valid) ? __ldg(prm.t + p0 + h * 128 + gi) : 0.0f;
+            }
+            asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                 const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
                 const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
@@ -497,24 +508,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     if (col0 >= n_valid) break;
                     uint32_t v[32];
                     tmem_ld32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + buf * kBN + col0, v);
-                    const float* tp = prm.t + p0 + col0;
+                    const float4* tp = reinterpret_cast<const float4*>(ts + cc * 32);
+                    tmem_ld_wait();
                     if (col0 + 32 <= n_valid) {
-                        float4 tv[8];
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) tv[i] = __ldg(reinterpret_cast<const float4*>(tp) + i);
-                        tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 8; ++i) {
-                            sum += act_err2<ACT>(__uint_as_float(v[4 * i + 0]), bias, tv[i].x);
-                            sum1 += act_err2<ACT>(__uint_as_float(v[4 * i + 1]), bias, tv[i].y);
-                            sum2 += act_err2<ACT>(__uint_as_float(v[4 * i + 2]), bias, tv[i].z);
-                            sum3 += act_err2<ACT>(__uint_as_float(v[4 * i + 3]), bias, tv[i].w);
+                            const float4 tv = tp[i];
+                            sum += act_err2<ACT>(__uint_as_float(v[4 * i + 0]), bias, tv.x);
+                            sum1 += act_err2<ACT>(__uint_as_float(v[4 * i + 1]), bias, tv.y);
+                            sum2 += act_err2<ACT>(__uint_as_float(v[4 * i + 2]), bias, tv.z);
+                            sum3 += act_err2<ACT>(__uint_as_float(v[4 * i + 3]), bias, tv.w);
                         }
                     } else {
-                        tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
-                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), bias, __ldg(tp + i));
+                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), bias, ts[cc * 32 + i]);
                         }
                     }
                 }
