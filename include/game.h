@@ -155,7 +155,9 @@ int game_sync(game_ctx* ctx);
  * Copies X_host[P][N], t_host[P] into the bound knowledge-base buffers (which must therefore be
  * writable) and W_host[M][G] into the current population, runs eval + step(seed, gen), then copies the
  * fitness of the INPUT population to F_host[M] and the NEXT population to W_next_host[M][G] (either may
- * be NULL), and synchronises the stream.  Host buffers should be pinned for full copy bandwidth. */
+ * be NULL), and synchronises the stream.  Host buffers should be pinned for full copy bandwidth.  A knowledge base of
+ * 64 MB or more is uploaded in 8 pattern ranges on a library-owned copy stream and each range is evaluated as soon as it
+ * has landed (partial sums carried across the launches), so the PCIe transfer hides behind the fitness kernel. */
 int game_generation_host(game_ctx* ctx, const float* X_host, const float* t_host, const float* W_host,
                          float* F_host, float* W_next_host, uint64_t seed, uint32_t gen);
 

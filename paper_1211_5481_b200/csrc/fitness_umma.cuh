@@ -74,7 +74,9 @@ struct Params {
     int N, d, M, G;
     int m_stride;          // m_tiles * 128
     int m_tiles;           // chromosome tiles, padded to an even number (one per CTA of a pair)
-    int p_tiles;           // pattern tiles of 256
+    int p_tiles;           // pattern tiles of 256 covered by THIS launch ...
+    int p_tile0;           // ... starting at this tile (a generation may be evaluated in several pattern ranges)
+    int zero_part;         // 1: this launch starts the generation (clear this CTA's partial sums first)
     int m_groups;          // work unit = (pattern tile, group of m_pairs_per_group chromosome-tile pairs)
     int m_pairs_per_group;
     int chunks;            // ceil(N / 8)
@@ -476,11 +478,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         const int q = warp & 3;                 // TMEM lane quarter this warp may access
         const int h = (warp - 2) >> 2;          // column half
         double* my_part = prm.part + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
-        for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
+        if (prm.zero_part)
+            for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
         const uint32_t leader_acc_empty = map_to_cta(bar_acc_empty, 0);
         uint32_t tile = 0;
         for (int u = pair; u < units; u += n_pairs) {
-            const int pt = u / prm.m_groups, mg = u % prm.m_groups;
+            const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
             const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
             const long long p0 = static_cast<long long>(pt) * kBN;
@@ -545,7 +548,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         Ring rb;                                // ring position of the current fill's first stage
         uint32_t item = 0;                      // running chunk counter: chunk goes to set (item & 1)
         for (int u = pair; u < units; u += n_pairs) {
-            const int pt = u / prm.m_groups, mg = u % prm.m_groups;
+            const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
             const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
             const long long p = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows + r;

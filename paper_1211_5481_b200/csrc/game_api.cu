@@ -56,6 +56,8 @@ struct game_ctx {
     unsigned long long launches = 0;
     bool timing = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> events;
+    cudaStream_t copy_stream = nullptr;              // game_generation_host: H2D of pattern ranges overlapped with compute
+    std::vector<cudaEvent_t> copy_events;
     char err[256] = {0};
 };
 
@@ -120,8 +122,15 @@ int check_launch(game_ctx* c, const char* what) {
     return GAME_OK;
 }
 
-// One fitness evaluation of the current population; best_out (device) may be NULL.
-int eval_internal(game_ctx* c, float* best_out) {
+// Host knowledge base to be uploaded range by range while earlier ranges are being evaluated (game_generation_host).
+struct HostKb {
+    const float* X;
+    const float* t;
+};
+
+// One fitness evaluation of the current population; best_out (device) may be NULL.  With `hk` the knowledge base is
+// copied from host memory in pattern ranges on a second stream, each range evaluated as soon as it has landed.
+int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr) {
     using namespace game;
     if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_load_kb");
     if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_bind_state");
@@ -153,13 +162,13 @@ int eval_internal(game_ctx* c, float* best_out) {
         prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.part = part;
         prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
         prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
-        prm.p_tiles = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
+        const int p_tiles_all = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
         int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
         grid_cap &= ~1;                                              // CTA pairs (clusters of 2)
         const int pair_cap = grid_cap / 2, m_pairs = c->m_tiles / 2;
         // work unit = (pattern tile, group of chromosome-tile pairs): aim for >= 16 units per CTA pair so that
         // the static round-robin assignment stays balanced when there are few pattern tiles
-        long long want = (16ll * pair_cap + prm.p_tiles - 1) / prm.p_tiles;
+        long long want = (16ll * pair_cap + p_tiles_all - 1) / p_tiles_all;
         if (want < 1) want = 1;
         if (want > m_pairs) want = m_pairs;
         prm.m_pairs_per_group = static_cast<int>((m_pairs + want - 1) / want);
@@ -170,24 +179,61 @@ int eval_internal(game_ctx* c, float* best_out) {
         prm.n_b = prm.resident ? prm.stages : umma::kStreamBStages;
         prm.n_a = umma::kStagesTotal - prm.n_b;
         prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
-        const long long units = static_cast<long long>(prm.p_tiles) * prm.m_groups;
-        const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);
+        const long long units = static_cast<long long>(p_tiles_all) * prm.m_groups;
+        const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);   // the same grid for every range
         n_part = 2 * grid;
-        if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
-#define GAME_LAUNCH(E, A) umma::fitness_umma_kernel<E, A><<<grid, umma::kThreads, umma::kSmemBytes, c->stream>>>(prm)
-        const int sel = c->expansion * 3 + c->act;
-        switch (sel) {
-            case 0: GAME_LAUNCH(0, 0); break;
-            case 1: GAME_LAUNCH(0, 1); break;
-            case 2: GAME_LAUNCH(0, 2); break;
-            case 3: GAME_LAUNCH(1, 0); break;
-            case 4: GAME_LAUNCH(1, 1); break;
-            default: GAME_LAUNCH(1, 2); break;
+        // pattern ranges: one launch, or (host knowledge base >= 64 MB) 8 ranges pipelined against their H2D copies
+        const size_t kb_bytes = sizeof(float) * static_cast<size_t>(c->P) * (c->N + 1);
+        const int n_ranges = (hk != nullptr && kb_bytes >= (64u << 20) && p_tiles_all >= 64) ? 8 : 1;
+        if (hk != nullptr) {
+            if (!c->copy_stream) GAME_CUDA(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+            while (static_cast<int>(c->copy_events.size()) < n_ranges + 1) {
+                cudaEvent_t e;
+                GAME_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                c->copy_events.push_back(e);
+            }
+            // the copies overwrite X / t: they must follow everything already enqueued on the compute stream
+            GAME_CUDA(cudaEventRecord(c->copy_events[n_ranges], c->stream));
+            GAME_CUDA(cudaStreamWaitEvent(c->copy_stream, c->copy_events[n_ranges], 0));
         }
+        if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
+        for (int k = 0; k < n_ranges; ++k) {
+            const int tile0 = static_cast<int>(static_cast<long long>(p_tiles_all) * k / n_ranges);
+            const int tile1 = static_cast<int>(static_cast<long long>(p_tiles_all) * (k + 1) / n_ranges);
+            if (hk != nullptr) {
+                const long long p0 = static_cast<long long>(tile0) * umma::kBN;
+                long long p1 = static_cast<long long>(tile1) * umma::kBN;
+                if (p1 > c->P) p1 = c->P;
+                GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->X) + p0 * c->N, hk->X + p0 * c->N,
+                                          sizeof(float) * static_cast<size_t>(p1 - p0) * c->N, cudaMemcpyHostToDevice, c->copy_stream));
+                GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->t) + p0, hk->t + p0, sizeof(float) * static_cast<size_t>(p1 - p0),
+                                          cudaMemcpyHostToDevice, c->copy_stream));
+                GAME_CUDA(cudaEventRecord(c->copy_events[k], c->copy_stream));
+                GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[k], 0));
+            }
+            prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = k == 0 ? 1 : 0;
+#define GAME_LAUNCH(E, A) umma::fitness_umma_kernel<E, A><<<grid, umma::kThreads, umma::kSmemBytes, c->stream>>>(prm)
+            const int sel = c->expansion * 3 + c->act;
+            switch (sel) {
+                case 0: GAME_LAUNCH(0, 0); break;
+                case 1: GAME_LAUNCH(0, 1); break;
+                case 2: GAME_LAUNCH(0, 2); break;
+                case 3: GAME_LAUNCH(1, 0); break;
+                case 4: GAME_LAUNCH(1, 1); break;
+                default: GAME_LAUNCH(1, 2); break;
+            }
 #undef GAME_LAUNCH
+            if (k + 1 < n_ranges && (rc = check_launch(c, "fitness_umma_kernel"))) return rc;
+        }
         if ((rc = check_launch(c, "fitness_umma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     } else {
+        if (hk != nullptr) {
+            GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->X), hk->X, sizeof(float) * static_cast<size_t>(c->P) * c->N,
+                                      cudaMemcpyHostToDevice, c->stream));
+            GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->t), hk->t, sizeof(float) * static_cast<size_t>(c->P),
+                                      cudaMemcpyHostToDevice, c->stream));
+        }
         const long long n_tiles = (c->P + kFfmaTile - 1) / kFfmaTile;
         const size_t smem = static_cast<size_t>(c->G) * kFfmaTile * sizeof(float);
         int per_sm = static_cast<int>((220u * 1024u) / (smem + 1024));
@@ -276,6 +322,8 @@ int game_destroy(game_ctx* c) {
         cudaEventDestroy(ev.first);
         cudaEventDestroy(ev.second);
     }
+    for (auto& e : c->copy_events) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
     return GAME_OK;
 }
@@ -435,13 +483,12 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_generation_host before game_load_kb");
     if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_generation_host before game_bind_state");
     const size_t wb = sizeof(float) * static_cast<size_t>(c->M) * c->G;
-    GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->X), X_host, sizeof(float) * static_cast<size_t>(c->P) * c->N,
-                              cudaMemcpyHostToDevice, c->stream));
-    GAME_CUDA(cudaMemcpyAsync(const_cast<float*>(c->t), t_host, sizeof(float) * static_cast<size_t>(c->P),
-                              cudaMemcpyHostToDevice, c->stream));
     GAME_CUDA(cudaMemcpyAsync(c->pop[c->cur], W_host, wb, cudaMemcpyHostToDevice, c->stream));
     c->fitness_valid = false;
-    int rc = eval_internal(c, nullptr);
+    const HostKb hk{X_host, t_host};
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    rc = eval_internal(c, nullptr, &hk);
     if (rc) return rc;
     rc = step_internal(c, seed, gen);
     if (rc) return rc;

@@ -330,3 +330,26 @@ def test_evolve_equals_eval_step_loop(game):
     game.game_evolve(G.ctx, 9, 0, 4); G.sync()
     assert np.array_equal(G.get_population().view(np.uint32), a.view(np.uint32))
     G.close()
+
+
+def test_generation_host_entry_pipelined_ranges(game):
+    """A knowledge base >= 64 MB makes game_generation_host upload it in 8 pattern ranges on a copy stream, each
+    evaluated as soon as it has landed (partial sums carried across the launches): same bars as everywhere else."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS["c3"], P=560_123, M=300)          # 72 MB of X, ragged last tile
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 12)
+    G = make(game, cfg)
+    G.X.zero_(); G.t.zero_()                                     # the device copy must come from the host buffers
+    Xh, th, Wh = (torch.from_numpy(a).pin_memory() for a in (X, t, W))
+    Fh = torch.empty(cfg.M, dtype=torch.float32).pin_memory()
+    Wn = torch.empty((cfg.M, cfg.G), dtype=torch.float32).pin_memory()
+    for rep in range(2):                                         # twice: the copy stream must wait for the previous eval
+        game.game_generation_host(G.ctx, Xh.data_ptr(), th.data_ptr(), Wh.data_ptr(), Fh.data_ptr(), Wn.data_ptr(), 5, rep)
+    F = Fh.numpy().copy()
+    rows = [0, 1, 127, 128, 255, 256, 299]
+    assert_fitness_close(F[rows], oracle.eval_fitness(cfg.d, cfg.family, X, t, W[rows]), "pipelined host entry")
+    ref = oracle.step(W, F, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 5, 1)
+    assert np.array_equal(Wn.numpy().view(np.uint32), ref.view(np.uint32))
+    assert torch.equal(G.X.cpu(), torch.from_numpy(X))
+    G.close()
