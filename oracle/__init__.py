@@ -78,6 +78,10 @@ def lib() -> C.CDLL:
         L.oracle_step.restype = C.c_int
         L.oracle_step.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
                                   C.c_uint64, C.c_uint32, f32p, f32p, f32p]
+        L.oracle_predict.restype = None
+        L.oracle_predict.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, f32p, f32p, f64p]
+        L.oracle_confusion.restype = None
+        L.oracle_confusion.argtypes = [C.c_int64, f64p, f32p, C.c_double, C.POINTER(C.c_int64)]
         L.oracle_run.restype = C.c_int
         L.oracle_run.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, f32p, f32p,
                                  C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
@@ -225,3 +229,23 @@ def run(d: int, fam: int, X, t, W, E: int, k: int, p_cross: float, p_mut: float,
     if rc:
         raise ValueError(f"oracle_run failed: {rc}")
     return W, F, best
+
+
+def predict(d: int, fam: int, X, w) -> np.ndarray:
+    """y[q] = act(w . phi(x_q)) in float64 for one chromosome (test / validation use case)."""
+    X, w = _f32(X), _f32(w)
+    Q, N = X.shape
+    assert w.shape == (num_genes(N, d, fam),)
+    y = np.empty(Q, dtype=np.float64)
+    lib().oracle_predict(Q, N, d, fam, _p(X, C.c_float), _p(w, C.c_float), _p(y, C.c_double))
+    return y
+
+
+def confusion(y, t, threshold: float = 0.5):
+    """(TP, FP, TN, FN) of the thresholded outputs against 0/1 targets."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    t = _f32(t)
+    assert y.shape == t.shape
+    counts = (C.c_int64 * 4)()
+    lib().oracle_confusion(y.size, _p(y, C.c_double), _p(t, C.c_float), threshold, counts)
+    return tuple(int(c) for c in counts)

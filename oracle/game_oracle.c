@@ -397,3 +397,24 @@ void oracle_gauss_many(int64_t n, const uint32_t *a, const uint32_t *b, float *o
 {
     for (int64_t i = 0; i < n; ++i) out[i] = oracle_gauss(a[i], b[i]);
 }
+
+/* ---- test / validation use case  ("test" and "run" apply a trained chromosome to patterns;
+ * PAPER.md:91 "crispy" classification).  y[q] = act(sum_g w[g] phi_g(x_q)) -- eq.(2) with D1/D2 -- for one
+ * chromosome over Q patterns, and the confusion counts of the thresholded outputs against 0/1 targets:
+ * counts = {TP, FP, TN, FN} with predicted class = (y > threshold), true class = (t > 0.5). */
+void oracle_predict(int64_t Q, int N, int d, int family, const float *X, const float *w, double *y)
+{
+    for (int64_t q = 0; q < Q; ++q) y[q] = oracle_output(N, d, family, X + q * N, w);
+}
+
+void oracle_confusion(int64_t Q, const double *y, const float *t, double threshold, int64_t counts[4])
+{
+    counts[0] = counts[1] = counts[2] = counts[3] = 0;
+    for (int64_t q = 0; q < Q; ++q) {
+        int pred = y[q] > threshold, truth = t[q] > 0.5f;
+        if (pred && truth) counts[0]++;
+        else if (pred && !truth) counts[1]++;
+        else if (!pred && !truth) counts[2]++;
+        else counts[3]++;
+    }
+}

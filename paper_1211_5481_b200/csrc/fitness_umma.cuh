@@ -14,8 +14,10 @@
 //                          peer CTA: relays "my stage is full" to the leader's barrier
 //   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation, (y-t)^2, private per-chromosome sum
 //                          (TMEM lane = chromosome, so no shuffle is needed); fp64 accumulation per (CTA, m)
-//   warps 10-17 producers: two sets of 4 warps alternating chunks; one pattern per thread; Chebyshev / multiple-angle recurrences for 8 features at a
-//                          time, fp16 hi/lo split, 16-byte stores straight into the MMA's canonical layout
+//   warps 10-17 producers: two sets of 4 warps alternating chunks; one pattern per thread; Chebyshev / multiple-angle
+//                          recurrences for 8 features at a time, fp16 hi/lo split, 16-byte stores straight into the
+//                          MMA's canonical layout; phi of a pattern tile stays resident in shared memory and is
+//                          reused by every chromosome-tile pair of the work unit (see "the kernel" below)
 //
 // Why a pair: ncu on the single-CTA version (profiles/r01a) showed the shared-memory data pipe, not the tensor
 // pipe, saturating (tensor-core operand reads 46 % + producer stores 28 % + loads 4 % + bulk fills): with

@@ -364,3 +364,33 @@ def test_workload_recipe_shapes_and_balance():
     X, t, _ = wl.make_kb(c2)
     assert abs(X).max() <= np.float32(math.pi) and abs(t).max() < 1.1
     assert wl.shard_patterns(10, 3, 0) == (0, 4) and wl.shard_patterns(10, 3, 2) == (7, 10)
+
+
+# ------------------------------------------------------------------------------------------------ predict / confusion
+def test_predict_is_the_model_behind_the_fitness():
+    """mean((predict - t)^2) must be the (already pinned) fitness of that chromosome: ties the test / validation use
+    case to eq.(2)-(3); and a numpy chebvander evaluation of the same outputs (library routine)."""
+    import workloads as wl
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=400, M=6)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 21)
+    F = oracle.eval_fitness(cfg.d, cfg.family, X, t, W)
+    for m in range(cfg.M):
+        y = oracle.predict(cfg.d, cfg.family, X, W[m])
+        assert abs(np.mean((y - t.astype(np.float64)) ** 2) - F[m]) <= 1e-15
+        z = wl._design_matrix(cfg, X.astype(np.float64)) @ W[m].astype(np.float64)
+        assert np.max(np.abs(y - 1.0 / (1.0 + np.exp(-z)))) <= 1e-14
+
+
+def test_confusion_counts_brute_force_and_identities():
+    y = np.array([0.9, 0.2, 0.5, 0.51, 0.49, 1.0, 0.0, np.nan])
+    t = np.array([1, 1, 1, 0, 0, 0, 0, 1], dtype=np.float32)
+    # by hand at threshold 0.5: pred = [1,0,0,1,0,1,0,0] (y > thr; 0.5 and NaN are not above it)
+    assert oracle.confusion(y, t, 0.5) == (1, 2, 2, 3)
+    rng = np.random.default_rng(3)
+    y = rng.uniform(size=1000); t = (rng.uniform(size=1000) > 0.4).astype(np.float32)
+    tp, fp, tn, fn = oracle.confusion(y, t, 0.3)
+    pred = y > 0.3
+    assert (tp, fp, tn, fn) == (int(np.sum(pred & (t > 0.5))), int(np.sum(pred & (t <= 0.5))),
+                                int(np.sum(~pred & (t <= 0.5))), int(np.sum(~pred & (t > 0.5))))
+    assert tp + fp + tn + fn == 1000 and oracle.confusion(t.astype(np.float64), t, 0.5) == (int(t.sum()), 0, int(1000 - t.sum()), 0)
