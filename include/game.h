@@ -161,6 +161,17 @@ int game_sync(game_ctx* ctx);
 int game_generation_host(game_ctx* ctx, const float* X_host, const float* t_host, const float* W_host,
                          float* F_host, float* W_next_host, uint64_t seed, uint32_t gen);
 
+/* Test / validation use case: outputs of ONE chromosome w_dev[G] (device; e.g. a row of the current
+ * population) on Q patterns X_dev[Q][N] (device, any Q >= 1, independent of the bound knowledge base):
+ * y_dev[q] = act(sum_g w[g] phi_g(x_q)), fp32.  Async. */
+int game_predict(game_ctx* ctx, const float* w_dev, const float* X_dev, int64_t Q, float* y_dev);
+
+/* Confusion counts of thresholded outputs against 0/1 targets (PAPER.md:91, 140-146 classification quality):
+ * counts_dev[4] (device, 64-bit) = {TP, FP, TN, FN}, predicted class = (y > threshold), true class = (t > 0.5).
+ * The counters are cleared first.  Async. */
+int game_confusion(game_ctx* ctx, const float* y_dev, const float* t_dev, int64_t Q, float threshold,
+                   uint64_t* counts_dev);
+
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 int game_launch_count(const game_ctx* ctx, uint64_t* launches);
 

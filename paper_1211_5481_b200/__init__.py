@@ -44,6 +44,8 @@ SIGNATURES = {
     "game_evolve": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32]),
     "game_sync": (C.c_int, [_VP]),
     "game_generation_host": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, _F32P, C.c_uint64, C.c_uint32]),
+    "game_predict": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, _F32P]),
+    "game_confusion": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, C.c_float, _VP]),
     "game_launch_count": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
     "game_time_fitness_kernel": (C.c_int, [_VP, C.c_int32]),
     "game_fitness_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
@@ -176,6 +178,14 @@ def game_sync(ctx) -> None:
 def game_generation_host(ctx, X_host: int, t_host: int, W_host: int, F_host: int | None, W_next_host: int | None,
                          seed: int, gen: int) -> None:
     _check(ctx, lib().game_generation_host(ctx, X_host, t_host, W_host, F_host, W_next_host, seed, gen))
+
+
+def game_predict(ctx, w_dev: int, X_dev: int, Q: int, y_dev: int) -> None:
+    _check(ctx, lib().game_predict(ctx, w_dev, X_dev, Q, y_dev))
+
+
+def game_confusion(ctx, y_dev: int, t_dev: int, Q: int, threshold: float, counts_dev: int) -> None:
+    _check(ctx, lib().game_confusion(ctx, y_dev, t_dev, Q, threshold, counts_dev))
 
 
 def game_launch_count(ctx) -> int:

@@ -14,6 +14,7 @@
 #include "fitness_ffma.cuh"
 #include "fitness_umma.cuh"
 #include "ga_kernels.cuh"
+#include "predict.cuh"
 
 namespace {
 
@@ -496,6 +497,31 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     if (W_next_host) GAME_CUDA(cudaMemcpyAsync(W_next_host, c->pop[c->cur], wb, cudaMemcpyDeviceToHost, c->stream));
     GAME_CUDA(cudaStreamSynchronize(c->stream));
     return GAME_OK;
+}
+
+int game_predict(game_ctx* c, const float* w_dev, const float* X_dev, int64_t Q, float* y_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!w_dev || !X_dev || !y_dev || Q < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_predict: null pointer or Q < 1");
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    long long blocks = (Q + game::kPredictThreads - 1) / game::kPredictThreads;
+    if (blocks > 8ll * c->num_sms) blocks = 8ll * c->num_sms;
+    game::predict_kernel<<<static_cast<unsigned>(blocks), game::kPredictThreads, sizeof(float) * c->G, c->stream>>>(
+        X_dev, w_dev, y_dev, Q, c->N, c->d, c->G, c->expansion, c->act);
+    return check_launch(c, "predict_kernel");
+}
+
+int game_confusion(game_ctx* c, const float* y_dev, const float* t_dev, int64_t Q, float threshold, uint64_t* counts_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!y_dev || !t_dev || !counts_dev || Q < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_confusion: null pointer or Q < 1");
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    GAME_CUDA(cudaMemsetAsync(counts_dev, 0, 4 * sizeof(uint64_t), c->stream));
+    long long blocks = (Q + game::kPredictThreads - 1) / game::kPredictThreads;
+    if (blocks > 8ll * c->num_sms) blocks = 8ll * c->num_sms;
+    game::confusion_kernel<<<static_cast<unsigned>(blocks), game::kPredictThreads, 0, c->stream>>>(
+        y_dev, t_dev, Q, threshold, reinterpret_cast<unsigned long long*>(counts_dev));
+    return check_launch(c, "confusion_kernel");
 }
 
 int game_launch_count(const game_ctx* c, uint64_t* launches) {

@@ -353,3 +353,35 @@ def test_generation_host_entry_pipelined_ranges(game):
     assert np.array_equal(Wn.numpy().view(np.uint32), ref.view(np.uint32))
     assert torch.equal(G.X.cpu(), torch.from_numpy(X))
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ test / validation use case
+@pytest.mark.parametrize("base,over", [("c0", dict(P=777, M=16)), ("c1", dict(P=5001, M=16)), ("c2", dict(P=3000, M=16)),
+                                       ("c3", dict(P=2047, M=16)), ("c1", dict(P=1000, M=16, activation=wl.ACT_IDENTITY))])
+def test_predict_and_confusion_match_oracle(game, base, over):
+    """game_predict / game_confusion: outputs of one chromosome on held-out patterns within 1e-5
+    (relative to max(1, |y|): fp32 recurrences and a G-term fp32 dot product, |z| up to ~10) of the fp64 oracle; confusion counts bit-exact when both sides threshold the SAME fp32 outputs, and equal to
+    the oracle's own counts wherever no output lies within the tolerance of the threshold."""
+    import torch
+    cfg = case_cfg(base, over)
+    X, t, _ = wl.make_kb(cfg, seed=77)
+    W = wl.uniform_population(cfg.M, cfg.G, 31)
+    G = make(game, cfg)
+    Xd, td = torch.from_numpy(X).cuda(), torch.from_numpy(t).cuda()
+    Wd = torch.from_numpy(W).cuda()
+    y = torch.empty(cfg.P, dtype=torch.float32, device="cuda")
+    counts = torch.zeros(4, dtype=torch.int64, device="cuda")
+    for m in (0, cfg.M - 1):
+        game.game_predict(G.ctx, Wd[m].data_ptr(), Xd.data_ptr(), cfg.P, y.data_ptr())
+        game.game_confusion(G.ctx, y.data_ptr(), td.data_ptr(), cfg.P, 0.5, counts.data_ptr())
+        G.sync()
+        y_gpu = y.cpu().numpy()
+        y_ref = oracle.predict(cfg.d, cfg.family, X, W[m])
+        scale = np.maximum(1.0, np.abs(y_ref))
+        assert np.max(np.abs(y_gpu - y_ref) / scale) <= 1e-5
+        got = tuple(int(c) for c in counts.cpu().numpy())
+        assert got == oracle.confusion(y_gpu.astype(np.float64), t, 0.5)          # same fp32 outputs in -> bit-exact
+        if np.min(np.abs(y_ref - 0.5)) > 2e-5:
+            assert got == oracle.confusion(y_ref, t, 0.5)
+        assert sum(got) == cfg.P
+    G.close()
