@@ -51,6 +51,8 @@ def parse_args():
     ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS) + ["c4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="auto", choices=["auto", "ffma", "f16x3"])
+    ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
+                    help="N > 1: independent replicas (default), or ONE population over pattern shards with an all-reduce of M sums per generation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -167,7 +169,7 @@ def config_dict(cfg, scheme_name, n_gpus):
             "activation": ["identity", "sigmoid", "tanh"][cfg.activation], "elite": cfg.elite,
             "tournament": cfg.tournament, "p_cross": cfg.p_cross, "p_mut": cfg.p_mut, "sigma": cfg.sigma,
             "scheme": scheme_name, "step": "one generation = fused fitness eval + GA step kernel",
-            "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas (replicas only)",
+            "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} ranks: independent replicas by default; --multi shard = one population, patterns sharded, all-reduce of M sums per generation",
             "l2": "inputs larger than L2 (X = %.0f MB)" % (cfg.P * cfg.N * 4 / 1e6) if cfg.P * cfg.N * 4 > 126e6
                   else "L2 flushed between timed steps is not possible inside a no-sync generation loop; inputs fit L2"}
 
@@ -202,8 +204,18 @@ def run_ours(args, cfg, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
+    shard = dist is not None and args.multi == "shard"
+    sse = torch.zeros(cfg.M, dtype=torch.float64, device=dev) if shard else None
+
     def generations(first_gen, n):
-        game.game_evolve(G.ctx, seed, first_gen, n)          # n x (fused fitness eval, GA step): launches only
+        if not shard:
+            game.game_evolve(G.ctx, seed, first_gen, n)      # n x (fused fitness eval, GA step): launches only
+            return
+        for i in range(n):                                   # one population, patterns sharded over the ranks
+            game.game_eval_sse(G.ctx, sse.data_ptr())
+            dist.all_reduce(sse, op=dist.ReduceOp.SUM)       # M doubles per generation over NVLink
+            game.game_set_fitness_from_sse(G.ctx, sse.data_ptr(), cfg.P * world, None)
+            game.game_step(G.ctx, seed, first_gen + i)
 
     # ---------------- device-resident leg
     generations(0, args.warmup)

@@ -161,6 +161,16 @@ int game_sync(game_ctx* ctx);
 int game_generation_host(game_ctx* ctx, const float* X_host, const float* t_host, const float* W_host,
                          float* F_host, float* W_next_host, uint64_t seed, uint32_t gen);
 
+/* Pattern-sharded evaluation (PAPER.md:172 future work (iii) multi-GPU; "massive data sets"): each
+ * rank binds ITS shard of the knowledge base (P = shard size) and the same population.  game_eval_sse writes the
+ * un-normalised sums sse_dev[m] = sum over this shard of (act(z) - t)^2 (device, fp64 [M]) instead of a fitness; the caller
+ * adds them across ranks (one all-reduce of M doubles per generation, e.g. ncclAllReduce / torch.distributed) and calls
+ * game_set_fitness_from_sse(sum, P_total): fitness_dev[m] = float(sse[m] / P_total), marked valid; best_fitness_dev may be
+ * NULL.  Every rank then calls game_step with the same seed: the counter-based RNG and the identical all-reduced fitness
+ * give identical populations on all ranks, no broadcast.  Async. */
+int game_eval_sse(game_ctx* ctx, double* sse_dev);
+int game_set_fitness_from_sse(game_ctx* ctx, const double* sse_dev, int64_t P_total, float* best_fitness_dev);
+
 /* Test / validation use case: outputs of ONE chromosome w_dev[G] (device; e.g. a row of the current
  * population) on Q patterns X_dev[Q][N] (device, any Q >= 1, independent of the bound knowledge base):
  * y_dev[q] = act(sum_g w[g] phi_g(x_q)), fp32.  Async. */

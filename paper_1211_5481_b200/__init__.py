@@ -44,6 +44,8 @@ SIGNATURES = {
     "game_evolve": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32]),
     "game_sync": (C.c_int, [_VP]),
     "game_generation_host": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, _F32P, C.c_uint64, C.c_uint32]),
+    "game_eval_sse": (C.c_int, [_VP, _VP]),
+    "game_set_fitness_from_sse": (C.c_int, [_VP, _VP, C.c_int64, _F32P]),
     "game_predict": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, _F32P]),
     "game_confusion": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, C.c_float, _VP]),
     "game_launch_count": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
@@ -178,6 +180,14 @@ def game_sync(ctx) -> None:
 def game_generation_host(ctx, X_host: int, t_host: int, W_host: int, F_host: int | None, W_next_host: int | None,
                          seed: int, gen: int) -> None:
     _check(ctx, lib().game_generation_host(ctx, X_host, t_host, W_host, F_host, W_next_host, seed, gen))
+
+
+def game_eval_sse(ctx, sse_dev: int) -> None:
+    _check(ctx, lib().game_eval_sse(ctx, sse_dev))
+
+
+def game_set_fitness_from_sse(ctx, sse_dev: int, P_total: int, best_fitness_dev: int | None = None) -> None:
+    _check(ctx, lib().game_set_fitness_from_sse(ctx, sse_dev, P_total, best_fitness_dev))
 
 
 def game_predict(ctx, w_dev: int, X_dev: int, Q: int, y_dev: int) -> None:

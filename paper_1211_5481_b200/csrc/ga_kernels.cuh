@@ -134,6 +134,7 @@ constexpr int kFinThreads = 256, kFinCols = 32, kFinGroups = kFinThreads / kFinC
 __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* __restrict__ part,
                                                                         int n_part, int m_stride, int M,
                                                                         double P_d, float* __restrict__ F,
+                                                                        double* __restrict__ sse_out,
                                                                         float* __restrict__ best_out,
                                                                         float* __restrict__ blk_key,
                                                                         int* __restrict__ blk_idx,
@@ -164,11 +165,16 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         double s = 0.0;
 #pragma unroll
         for (int g = 0; g < kFinGroups; ++g) s += s_grp[g][col];
-        const float f = static_cast<float>(s / P_d);
-        F[m] = f;
-        key = fit_key(f);
-        idx = m;
+        if (sse_out != nullptr) {            // pattern-sharded evaluation: hand out the un-normalised sum instead
+            sse_out[m] = s;
+        } else {
+            const float f = static_cast<float>(s / P_d);
+            F[m] = f;
+            key = fit_key(f);
+            idx = m;
+        }
     }
+    if (sse_out != nullptr) return;
     if (best_out == nullptr) return;
     __threadfence();  // F[m] visible device-wide before this block takes its ticket
     auto warp_min = [](float& k, int& i) {

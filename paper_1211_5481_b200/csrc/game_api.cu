@@ -131,7 +131,7 @@ struct HostKb {
 
 // One fitness evaluation of the current population; best_out (device) may be NULL.  With `hk` the knowledge base is
 // copied from host memory in pattern ranges on a second stream, each range evaluated as soon as it has landed.
-int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr) {
+int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, double* sse_out = nullptr) {
     using namespace game;
     if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_load_kb");
     if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_bind_state");
@@ -253,11 +253,11 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr) {
     if (timed) c->events.emplace_back(ev0, ev1);
     const int fin_blocks = (c->M + kFinCols - 1) / kFinCols;
     finalize_fitness_kernel<<<fin_blocks, kFinThreads, 0, c->stream>>>(
-        part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, best_out,
+        part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
         reinterpret_cast<unsigned int*>(c->ws + c->off_ticket));
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
-    c->fitness_valid = true;
+    c->fitness_valid = sse_out == nullptr;
     return GAME_OK;
 }
 
@@ -496,6 +496,32 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     if (F_host) GAME_CUDA(cudaMemcpyAsync(F_host, c->fitness, sizeof(float) * c->M, cudaMemcpyDeviceToHost, c->stream));
     if (W_next_host) GAME_CUDA(cudaMemcpyAsync(W_next_host, c->pop[c->cur], wb, cudaMemcpyDeviceToHost, c->stream));
     GAME_CUDA(cudaStreamSynchronize(c->stream));
+    return GAME_OK;
+}
+
+int game_eval_sse(game_ctx* c, double* sse_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!sse_dev) return fail(c, GAME_ERR_INVALID_ARG, "game_eval_sse: null sse_dev");
+    return eval_internal(c, nullptr, nullptr, sse_dev);
+}
+
+int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_total, float* best_fitness_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!sse_dev || P_total < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_set_fitness_from_sse: null sse_dev or P_total < 1");
+    if (!c->fitness || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_set_fitness_from_sse before game_bind_state");
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    if (!c->ticket_zeroed) {
+        GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
+        c->ticket_zeroed = true;
+    }
+    const int fin_blocks = (c->M + game::kFinCols - 1) / game::kFinCols;
+    game::finalize_fitness_kernel<<<fin_blocks, game::kFinThreads, 0, c->stream>>>(
+        sse_dev, 1, c->M, c->M, static_cast<double>(P_total), c->fitness, nullptr, best_fitness_dev,
+        reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket));
+    if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
+    c->fitness_valid = true;
     return GAME_OK;
 }
 

@@ -385,3 +385,40 @@ def test_predict_and_confusion_match_oracle(game, base, over):
             assert got == oracle.confusion(y_ref, t, 0.5)
         assert sum(got) == cfg.P
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ pattern sharding (N3)
+@pytest.mark.parametrize("world", [2, 3])
+def test_pattern_sharded_evaluation_single_device(game, world):
+    """The multi-GPU path emulated on ONE device (ranks run one after the other, nothing waits on anything): each
+    'rank' binds its contiguous shard of the patterns, game_eval_sse gives its partial sums, their sum goes through
+    game_set_fitness_from_sse on every rank; fitness within 1e-5 of the oracle on the WHOLE knowledge base, and the
+    GA step from it bit-identical on all ranks and to the oracle's."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS["c3"], P=3001, M=200)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 41)
+    ranks, sse = [], torch.zeros(cfg.M, dtype=torch.float64, device="cuda")
+    for r in range(world):
+        p0, p1 = wl.shard_patterns(cfg.P, world, r)
+        G = make(game, wl.scaled(cfg, P=p1 - p0))
+        G.load_kb(X[p0:p1], t[p0:p1]); G.set_population(W)
+        part = torch.empty(cfg.M, dtype=torch.float64, device="cuda")
+        game.game_eval_sse(G.ctx, part.data_ptr()); G.sync()
+        with pytest.raises(game.GameError):
+            G.step(1, 0)                      # partial sums are not a fitness
+        sse += part                           # the all-reduce
+        ranks.append(G)
+    F_ref, S_ref = oracle.eval_fitness(cfg.d, cfg.family, X, t, W, return_sse=True)
+    assert np.max(np.abs(sse.cpu().numpy() - S_ref) / S_ref) <= 1e-5
+    pops = []
+    for G in ranks:
+        game.game_set_fitness_from_sse(G.ctx, sse.data_ptr(), cfg.P, None)
+        G.step(11, 4); G.sync()
+        assert_fitness_close(G.get_fitness(), F_ref, "sharded fitness")
+        pops.append(G.get_population())
+    ref = oracle.step(W, ranks[0].get_fitness(), cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 11, 4)
+    for P_ in pops:
+        assert np.array_equal(P_.view(np.uint32), ref.view(np.uint32))
+    for G in ranks:
+        G.close()

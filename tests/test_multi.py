@@ -63,3 +63,35 @@ def test_reference_arm_under_torchrun_rank0_only():
     j = json.loads(lines[0])
     assert j["impl"] == "reference" and j["n_gpus"] == 2 and j["value"] > 0 and j["cpu_baseline"]["kind"] == "oracle"
     assert j["e2e"]["h2d_bytes_per_step"] == 0 and j["gpu_launches"] == 0
+
+
+def _shard_worker(rank, world, port, out):
+    """Pattern-sharded generation on CPU: every rank evaluates the oracle's SSE on its shard, one all-reduce (gloo) of M
+    doubles, every rank steps the GA on the same all-reduced fitness."""
+    import oracle
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=1001, M=40)
+    X, t, _ = wl.make_kb(cfg)                                     # same seed on every rank = one global knowledge base
+    W = oracle.init_population(cfg.M, cfg.G, 5)
+    p0, p1 = wl.shard_patterns(cfg.P, world, rank)
+    _, sse = oracle.eval_fitness(cfg.d, cfg.family, X[p0:p1], t[p0:p1], W, return_sse=True)
+    tot = torch.from_numpy(sse.copy())
+    dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    F = (tot.numpy() / cfg.P).astype(np.float32)
+    Wn = oracle.step(W, F, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 5, 0)
+    gathered = [torch.zeros(Wn.shape, dtype=torch.float32) for _ in range(world)]
+    dist.all_gather(gathered, torch.from_numpy(Wn.copy()))
+    if rank == 0:
+        F_full = oracle.eval_fitness(cfg.d, cfg.family, X, t, W)
+        json.dump({"same_pop": all(torch.equal(g, gathered[0]) for g in gathered),
+                   "max_rel": float(np.max(np.abs(tot.numpy() / cfg.P - F_full) / F_full))}, open(out, "w"))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_pattern_sharded_generation_gloo(tmp_path):
+    out = str(tmp_path / "s.json")
+    mp.spawn(_shard_worker, args=(2, 29535, out), nprocs=2, join=True)
+    r = json.load(open(out))
+    assert r["same_pop"] and r["max_rel"] <= 1e-13
