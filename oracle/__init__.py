@@ -78,6 +78,10 @@ def lib() -> C.CDLL:
         L.oracle_step.restype = C.c_int
         L.oracle_step.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
                                   C.c_uint64, C.c_uint32, f32p, f32p, f32p]
+        L.oracle_run_until.restype = C.c_int
+        L.oracle_run_until.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, f32p, f32p,
+                                       C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
+                                       C.c_uint64, C.c_uint32, C.c_uint32, C.c_float, f32p, f32p, f32p, u32p]
         L.oracle_predict.restype = None
         L.oracle_predict.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, f32p, f32p, f64p]
         L.oracle_confusion.restype = None
@@ -249,3 +253,21 @@ def confusion(y, t, threshold: float = 0.5):
     counts = (C.c_int64 * 4)()
     lib().oracle_confusion(y.size, _p(y, C.c_double), _p(t, C.c_float), threshold, counts)
     return tuple(int(c) for c in counts)
+
+
+def run_until(d: int, fam: int, X, t, W, E: int, k: int, p_cross: float, p_mut: float, sigma: float,
+              seed: int, gen0: int, max_gens: int, threshold: float):
+    """Run with the stop rule. Returns (final population, final fitness f32, best[0..done], done)."""
+    X, t = _f32(X), _f32(t)
+    W = _f32(W).copy()
+    P, N = X.shape
+    M, G = W.shape
+    F = np.empty(M, dtype=np.float32)
+    best = np.full(max_gens + 1, np.nan, dtype=np.float32)
+    done = C.c_uint32()
+    rc = lib().oracle_run_until(P, N, d, M, fam, _p(X, C.c_float), _p(t, C.c_float), E, k, p_cross, p_mut, sigma,
+                                seed, gen0, max_gens, threshold, _p(W, C.c_float), _p(F, C.c_float),
+                                _p(best, C.c_float), C.byref(done))
+    if rc:
+        raise ValueError(f"oracle_run_until failed: {rc}")
+    return W, F, best[:done.value + 1], done.value

@@ -418,3 +418,36 @@ void oracle_confusion(int64_t Q, const double *y, const float *t, double thresho
         else counts[3]++;
     }
 }
+
+/* ---- run with the paper's stop rule  ("until the maximum number of iterations or the learning error
+ * threshold", "MSE error threshold 0.001").  As oracle_run, but generation g's population is final as
+ * soon as its best fitness <= threshold (a NaN best never stops).  Returns the number of GA steps performed in
+ * *gens_done (0..max_gens); best[0..*gens_done] are written, W/F32 hold the final population and its fitness. */
+int oracle_run_until(int64_t P, int N, int d, int M, int family, const float *X, const float *t,
+                     int E, int k, double p_cross, double p_mut, float sigma,
+                     uint64_t seed, uint32_t gen0, uint32_t max_gens, float threshold,
+                     float *W, float *F32, float *best, uint32_t *gens_done)
+{
+    int G = oracle_num_genes(N, d, family);
+    if (G < 0) return -1;
+    double *F = (double *)malloc(sizeof(double) * (size_t)M);
+    float *Wn = (float *)malloc(sizeof(float) * (size_t)M * G);
+    if (!F || !Wn) { free(F); free(Wn); return -2; }
+    int rc = 0;
+    uint32_t g = 0;
+    for (;; ++g) {
+        rc = oracle_eval_fitness(P, N, d, M, family, X, t, W, F, NULL);
+        if (rc) break;
+        for (int m = 0; m < M; ++m) F32[m] = (float)F[m];
+        float b = F32[oracle_best_index(M, F32)];
+        if (best) best[g] = b;
+        if (b <= threshold || g == max_gens) break;
+        rc = oracle_step(M, G, E, k, p_cross, p_mut, sigma, seed, gen0 + g, W, F32, Wn);
+        if (rc) break;
+        memcpy(W, Wn, sizeof(float) * (size_t)M * G);
+    }
+    *gens_done = g;
+    free(F);
+    free(Wn);
+    return rc;
+}

@@ -341,3 +341,27 @@ def test_run_best_is_monotone_with_elitism_and_resumable():
         W = oracle.step(W, F, *args, seed=0, gen=g)
     W3, _, _ = oracle.run(cfg.d, cfg.family, X, t, W0, *args, seed=0, gen0=0, n_gens=3)
     assert np.array_equal(W, W3)
+
+
+def test_run_until_stop_rule_against_the_plain_run():
+    """Stop rule: never-reached threshold == oracle.run; +inf stops before the first step; a threshold
+    between two consecutive best values of the plain run stops exactly at the first generation at or below it, with that
+    generation's population and fitness."""
+    import workloads as wl
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=300, M=32)
+    X, t, _ = wl.make_kb(cfg)
+    W0 = oracle.init_population(cfg.M, cfg.G, 9)
+    args = (cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 9, 0)
+    Wf, Ff, best = oracle.run(cfg.d, cfg.family, X, t, W0, *args, 8)
+    W1, F1, b1, done = oracle.run_until(cfg.d, cfg.family, X, t, W0, *args, 8, -1.0)
+    assert done == 8 and np.array_equal(b1, best) and np.array_equal(W1, Wf) and np.array_equal(F1, Ff)
+    W2, F2, b2, done = oracle.run_until(cfg.d, cfg.family, X, t, W0, *args, 8, np.inf)
+    assert done == 0 and np.array_equal(W2, W0) and b2[0] == best[0]
+    drops = [g for g in range(1, 9) if best[g] < best[g - 1]]
+    assert drops, "the run must improve at least once for this pin"
+    g = drops[len(drops) // 2]
+    thr = float(best[g])                                   # first generation whose best is <= thr is g
+    W3, F3, b3, done = oracle.run_until(cfg.d, cfg.family, X, t, W0, *args, 8, thr)
+    assert done == g and np.array_equal(b3, best[:g + 1])
+    Wg, Fg, _ = oracle.run(cfg.d, cfg.family, X, t, W0, *args, g)
+    assert np.array_equal(W3, Wg) and np.array_equal(F3, Fg)
