@@ -143,6 +143,16 @@ int game_step(game_ctx* ctx, uint64_t seed, uint32_t gen);
  * NULL) receives the best (lowest) fitness of each generation's population.  Async. */
 int game_run(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev);
 
+/* game_run with the paper's stop rule ("maximum number of iterations or the learning error threshold",
+ * PAPER.md:128-133 MSE threshold 0.001): generation g's population is final as soon as its best fitness <= threshold.
+ * Nothing synchronises with the host: all max_gens generations are enqueued, a device flag set by the fitness
+ * finalisation makes the remaining kernels return at once (the GA step then carries the population over unchanged).
+ * best_fitness_dev[0..max_gens] (device; entries after the stopping generation are left untouched) and gens_done_dev
+ * (device int32: GA steps performed, 0..max_gens) are required.  Afterwards the current population is the stopping
+ * generation's and fitness_dev is its fitness.  Async. */
+int game_run_until(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t max_gens, float threshold,
+                   float* best_fitness_dev, int32_t* gens_done_dev);
+
 /* n_gens x (eval, step with gen = gen0 + i) with NO trailing evaluation (the population is left one step past its
  * last fitness): the generation loop of PAPER.md:97 as one call, launches only, no host synchronisation.  This is
  * what bench.py times as "K steps".  Async. */

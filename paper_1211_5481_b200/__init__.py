@@ -41,6 +41,7 @@ SIGNATURES = {
     "game_eval_fitness": (C.c_int, [_VP]),
     "game_step": (C.c_int, [_VP, C.c_uint64, C.c_uint32]),
     "game_run": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, _F32P]),
+    "game_run_until": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, C.c_float, _F32P, _VP]),
     "game_evolve": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32]),
     "game_sync": (C.c_int, [_VP]),
     "game_generation_host": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, _F32P, C.c_uint64, C.c_uint32]),
@@ -167,6 +168,11 @@ def game_step(ctx, seed: int, gen: int) -> None:
 
 def game_run(ctx, seed: int, gen0: int, n_gens: int, best_fitness_dev: int | None) -> None:
     _check(ctx, lib().game_run(ctx, seed, gen0, n_gens, best_fitness_dev))
+
+
+def game_run_until(ctx, seed: int, gen0: int, max_gens: int, threshold: float, best_fitness_dev: int,
+                   gens_done_dev: int) -> None:
+    _check(ctx, lib().game_run_until(ctx, seed, gen0, max_gens, threshold, best_fitness_dev, gens_done_dev))
 
 
 def game_evolve(ctx, seed: int, gen0: int, n_gens: int) -> None:

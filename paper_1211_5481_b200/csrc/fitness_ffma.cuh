@@ -29,7 +29,9 @@ __global__ void __launch_bounds__(kFfmaTile) fitness_ffma_kernel(const float* __
                                                                   const float* __restrict__ W,
                                                                   double* __restrict__ part, long long P, int N,
                                                                   int d, int M, int G, int expansion, int act,
-                                                                  int m_stride, long long n_tiles) {
+                                                                  int m_stride, long long n_tiles,
+                                                                  const int* __restrict__ stop) {
+    if (stop != nullptr && *stop != 0) return;
     extern __shared__ float phi[];  // [G][128]
     __shared__ float s_wsum[kFfmaTile / 32][kFfmaMB];
     const int tid = threadIdx.x;

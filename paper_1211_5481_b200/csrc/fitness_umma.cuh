@@ -71,6 +71,7 @@ struct Params {
     const float* W;        // [M][G]: only gene 0 (the bias a_0) is read here, by the epilogue
     const uint8_t* Wimg;   // [m_tiles][steps][8192]: A_hi (2 k-groups x 128 rows x 16 B), then A_lo
     double* part;          // [gridDim.x * 2][m_stride]
+    const int* stop;       // optional: non-zero => the stop rule is met, the kernel returns at once
     long long* stall;      // optional [gridDim.x][4]: cycles the MMA/relay thread stalled on a_full, b_full, acc_empty; total
     long long P;
     int N, d, M, G;
@@ -340,6 +341,7 @@ struct Ring {
 
 template <int EXPANSION, int ACT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
+    if (prm.stop != nullptr && *prm.stop != 0) return;   // uniform over the grid: written by an earlier kernel
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
     const uint32_t bar_a_full = smem_u32(bars), bar_a_empty = bar_a_full + 8 * kStagesTotal;

@@ -52,7 +52,8 @@ struct GaParams {
 //      and the per-gene mutation draws for that slot.
 __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __restrict__ W,
                                                               const float* __restrict__ F,
-                                                              float* __restrict__ Wn, GaParams p) {
+                                                              float* __restrict__ Wn, GaParams p,
+                                                              const int* __restrict__ stop) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
     __shared__ int s_rank;
     __shared__ int s_parent[2];
@@ -60,6 +61,10 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     const int c = blockIdx.x;
     const int tid = threadIdx.x;
     const int M = p.M, G = p.G;
+    if (stop != nullptr && *stop != 0) {   // stop rule already met: the population is final, carry it over unchanged
+        for (int g = tid; g < G; g += kGaThreads) Wn[static_cast<size_t>(c) * G + g] = W[static_cast<size_t>(c) * G + g];
+        return;
+    }
 
     // (1) rank of chromosome c under the order
     const float kc = fit_key(F[c]);
@@ -138,13 +143,15 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
                                                                         float* __restrict__ best_out,
                                                                         float* __restrict__ blk_key,
                                                                         int* __restrict__ blk_idx,
-                                                                        unsigned int* __restrict__ ticket) {
+                                                                        unsigned int* __restrict__ ticket,
+                                                                        int* __restrict__ stop, float threshold, int gen_index) {
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
     __shared__ bool s_last;
     // 32 chromosomes per block x 8 row groups: row group g sums partial rows g, g+8, g+16, ... with four independent
     // accumulators (the loads are L2 latency-bound: one thread walking all ~300 rows took 108 us at M = 4096), then the
     // eight group sums are added in group order -- a fixed order, so the result is bit-stable.
+    if (stop != nullptr && stop[0] != 0) return;   // stop rule met earlier: fitness and best trace stay as they are
     __shared__ double s_grp[kFinGroups][kFinCols];
     const int col = threadIdx.x % kFinCols, grp = threadIdx.x / kFinCols;
     const int m = blockIdx.x * kFinCols + col;
@@ -222,8 +229,13 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         }
         warp_min(key, idx);
         if (threadIdx.x == 0) {
-            *best_out = __ldcg(F + idx);  // the fitness itself (NaN if every chromosome is NaN: idx = 0)
+            const float best = __ldcg(F + idx);  // the fitness itself (NaN if every chromosome is NaN: idx = 0)
+            *best_out = best;
             *ticket = 0u;
+            if (stop != nullptr) {
+                stop[1] = gen_index;                       // GA steps performed so far
+                if (best <= threshold) stop[0] = 1;        // learning-error threshold reached
+            }
         }
     }
 }

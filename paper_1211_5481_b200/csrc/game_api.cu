@@ -35,7 +35,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -56,6 +56,9 @@ struct game_ctx {
     int num_sms = 0;
     unsigned long long launches = 0;
     bool timing = false;
+    int* stop = nullptr;                             // device stop state, non-null only inside game_run_until
+    float stop_threshold = 0.f;
+    int stop_gen_index = 0;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> events;
     cudaStream_t copy_stream = nullptr;              // game_generation_host: H2D of pattern ranges overlapped with compute
     std::vector<cudaEvent_t> copy_events;
@@ -180,6 +183,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         prm.n_b = prm.resident ? prm.stages : umma::kStreamBStages;
         prm.n_a = umma::kStagesTotal - prm.n_b;
         prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
+        prm.stop = c->stop;
         const long long units = static_cast<long long>(p_tiles_all) * prm.m_groups;
         const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);   // the same grid for every range
         n_part = 2 * grid;
@@ -246,7 +250,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         n_part = grid;
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
         fitness_ffma_kernel<<<grid, kFfmaTile, smem, c->stream>>>(c->X, c->t, W, part, c->P, c->N, c->d, c->M, c->G,
-                                                                   c->expansion, c->act, c->m_stride, n_tiles);
+                                                                   c->expansion, c->act, c->m_stride, n_tiles, c->stop);
         if ((rc = check_launch(c, "fitness_ffma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     }
@@ -255,7 +259,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     finalize_fitness_kernel<<<fin_blocks, kFinThreads, 0, c->stream>>>(
         part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket));
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index);
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
     c->fitness_valid = sse_out == nullptr;
     return GAME_OK;
@@ -272,7 +276,7 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     p.t_cross = bernoulli_threshold(c->p_cross);
     p.t_mut = bernoulli_threshold(c->p_mut);
     p.sigma = c->sigma; p.gen = gen; p.key = make_key(seed);
-    ga_step_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p);
+    ga_step_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop);
     if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
     c->cur ^= 1;
     c->fitness_valid = false;
@@ -312,6 +316,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
     c->off_ticket = off; off = align_up(off + sizeof(unsigned int));
     c->off_stall = off; off = align_up(off + sizeof(long long) * 4 * kMaxCtas);
+    c->off_stop = off; off = align_up(off + 2 * sizeof(int));
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
@@ -459,6 +464,29 @@ int game_run(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* 
     return GAME_OK;
 }
 
+int game_run_until(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t max_gens, float threshold, float* best_fitness_dev,
+                   int32_t* gens_done_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!best_fitness_dev || !gens_done_dev) return fail(c, GAME_ERR_INVALID_ARG, "game_run_until needs best_fitness_dev and gens_done_dev");
+    if (!c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_run_until before game_bind_state");
+    int* stop = reinterpret_cast<int*>(c->ws + c->off_stop);
+    GAME_CUDA(cudaMemsetAsync(stop, 0, 2 * sizeof(int), c->stream));
+    c->stop = stop;
+    c->stop_threshold = threshold;
+    int rc = GAME_OK;
+    for (uint32_t i = 0; i <= max_gens && rc == GAME_OK; ++i) {
+        c->stop_gen_index = static_cast<int>(i);
+        rc = eval_internal(c, best_fitness_dev + i);
+        if (rc != GAME_OK || i == max_gens) break;
+        rc = step_internal(c, seed, gen0 + i);
+    }
+    c->stop = nullptr;
+    if (rc != GAME_OK) return rc;
+    GAME_CUDA(cudaMemcpyAsync(gens_done_dev, stop + 1, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
+    c->fitness_valid = true;     // the fitness of the final population (of the stopping generation, or of generation max_gens)
+    return GAME_OK;
+}
+
 int game_evolve(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens) {
     if (!c) return GAME_ERR_INVALID_ARG;
     for (uint32_t i = 0; i < n_gens; ++i) {
@@ -519,7 +547,7 @@ int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_tota
     game::finalize_fitness_kernel<<<fin_blocks, game::kFinThreads, 0, c->stream>>>(
         sse_dev, 1, c->M, c->M, static_cast<double>(P_total), c->fitness, nullptr, best_fitness_dev,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket));
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), nullptr, 0.f, 0);
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
     c->fitness_valid = true;
     return GAME_OK;

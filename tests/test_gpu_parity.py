@@ -422,3 +422,45 @@ def test_pattern_sharded_evaluation_single_device(game, world):
         assert np.array_equal(P_.view(np.uint32), ref.view(np.uint32))
     for G in ranks:
         G.close()
+
+
+# ------------------------------------------------------------------------------------------------ stop rule
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_run_until_stop_rule(game, scheme):
+    """game_run_until: all generations are enqueued with no host sync; the device flag must freeze the
+    population, the fitness and the best trace at the first generation whose best fitness <= threshold -- the same
+    generation, population (bit-exact) and trace as the plain device run cut there, and as the oracle's stop rule."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=600, M=48)
+    X, t, _ = wl.make_kb(cfg)
+    n, seed = 9, 21
+    G = make(game, cfg, scheme); G.load_kb(X, t)
+    G.init_population(seed)
+    plain = torch.full((n + 1,), float("nan"), dtype=torch.float32, device="cuda")
+    G.run(seed, 0, n, plain); G.sync()
+    plain = plain.cpu().numpy()
+    drops = [g for g in range(1, n + 1) if plain[g] < plain[g - 1]]
+    assert drops
+    g_stop = drops[len(drops) // 2]
+    thr = float(plain[g_stop])
+    for threshold, expect in ((thr, g_stop), (-1.0, n), (float("inf"), 0)):
+        G.init_population(seed)
+        best = torch.full((n + 1,), float("nan"), dtype=torch.float32, device="cuda")
+        done = torch.full((1,), -7, dtype=torch.int32, device="cuda")
+        game.game_run_until(G.ctx, seed, 0, n, threshold, best.data_ptr(), done.data_ptr()); G.sync()
+        assert int(done.item()) == expect
+        b = best.cpu().numpy()
+        assert np.array_equal(b[:expect + 1], plain[:expect + 1]) and np.all(np.isnan(b[expect + 1:]))
+        # population and fitness are those of generation `expect`
+        G2 = make(game, cfg, scheme); G2.load_kb(X, t); G2.init_population(seed)
+        G2.run(seed, 0, expect, None); G2.sync()
+        assert np.array_equal(G.get_population().view(np.uint32), G2.get_population().view(np.uint32))
+        assert np.array_equal(G.get_fitness(), G2.get_fitness())
+        G.step(seed, 99); G.sync()            # the fitness is valid for the final population
+        G2.close()
+    # against the oracle's stop rule (free-running: same bar as the trajectories)
+    W0 = oracle.init_population(cfg.M, cfg.G, seed)
+    _, _, b_ref, done_ref = oracle.run_until(cfg.d, cfg.family, X, t, W0, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut,
+                                             cfg.sigma, seed, 0, n, thr)
+    assert done_ref == g_stop and np.all(np.abs(b_ref - plain[:g_stop + 1]) <= 1e-4 * np.abs(b_ref))
+    G.close()
