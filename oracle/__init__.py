@@ -19,6 +19,7 @@ _SRC = os.path.join(_HERE, "game_oracle.c")
 _LIB = os.path.join(_HERE, "libgame_oracle.so")
 
 EXP_CHEBYSHEV, EXP_TRIG = 0, 1
+SEL_TOURNAMENT, SEL_RANKING, SEL_ROULETTE = 0, 1, 2
 ACT_IDENTITY, ACT_SIGMOID, ACT_TANH = 0, 1, 2
 
 
@@ -78,6 +79,15 @@ def lib() -> C.CDLL:
         L.oracle_step.restype = C.c_int
         L.oracle_step.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
                                   C.c_uint64, C.c_uint32, f32p, f32p, f32p]
+        L.oracle_roulette_weight.restype = C.c_uint64
+        L.oracle_roulette_weight.argtypes = [C.c_float]
+        L.oracle_rank_from_word.restype = C.c_int
+        L.oracle_rank_from_word.argtypes = [C.c_uint32, C.c_int]
+        L.oracle_roulette_from_word.restype = C.c_int
+        L.oracle_roulette_from_word.argtypes = [C.c_uint32, C.c_int, C.POINTER(C.c_uint64)]
+        L.oracle_step_sel.restype = C.c_int
+        L.oracle_step_sel.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
+                                      C.c_uint64, C.c_uint32, f32p, f32p, f32p]
         L.oracle_run_until.restype = C.c_int
         L.oracle_run_until.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, f32p, f32p,
                                        C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
@@ -271,3 +281,28 @@ def run_until(d: int, fam: int, X, t, W, E: int, k: int, p_cross: float, p_mut: 
     if rc:
         raise ValueError(f"oracle_run_until failed: {rc}")
     return W, F, best[:done.value + 1], done.value
+
+
+def roulette_weight(f: float) -> int:
+    return lib().oracle_roulette_weight(float(f))
+
+
+def rank_from_word(w: int, M: int) -> int:
+    return lib().oracle_rank_from_word(w, M)
+
+
+def roulette_from_word(w: int, weights) -> int:
+    wt = np.ascontiguousarray(weights, dtype=np.uint64)
+    return lib().oracle_roulette_from_word(w, wt.size, _p(wt, C.c_uint64))
+
+
+def step_sel(W, F, E: int, k: int, selection: int, p_cross: float, p_mut: float, sigma: float, seed: int, gen: int):
+    """One generation with tournament (0), ranking (1) or roulette (2) selection (reading R10)."""
+    W, F = _f32(W), _f32(F)
+    M, G = W.shape
+    Wn = np.empty_like(W)
+    rc = lib().oracle_step_sel(M, G, E, k, selection, p_cross, p_mut, sigma, seed, gen,
+                               _p(W, C.c_float), _p(F, C.c_float), _p(Wn, C.c_float))
+    if rc:
+        raise ValueError(f"oracle_step_sel failed: {rc}")
+    return Wn

@@ -451,3 +451,101 @@ int oracle_run_until(int64_t P, int N, int d, int M, int family, const float *X,
     free(Wn);
     return rc;
 }
+
+/* ---- the paper's own selection methods  ("roulette/ranking", "selection: RANKING and
+ * ROULETTE"; the paper does not define them: DESIGN.md reading R10).  Both pick parent A and parent B of child slot c
+ * independently from words w0 and w1 of ONE Philox call with counter (0, c, gen, TAG_SELECT); everything is integer
+ * arithmetic so that a GPU can reproduce it bit for bit.
+ *
+ * RANKING (linear ranking): chromosomes ordered by `precedes` (rank 0 = best); rank r has weight M - r, total
+ *   T = M (M + 1) / 2;  u = floor(w * T / 2^32);  the selected rank is the smallest r with
+ *   C(r) = (r + 1) M - r (r + 1) / 2 > u;  the parent is the chromosome holding that rank.
+ * ROULETTE (fitness-proportionate on the paper's fitness 1 - error): weight_i =
+ *   floor(clamp(1 - key(F_i), 0, 1) * 2^32) evaluated in double (NaN / +inf fitness -> 0), T = sum of weights;
+ *   u = floor(w * T / 2^32);  the parent is the smallest index i whose prefix sum exceeds u;  T = 0 -> uniform index.
+ */
+enum { SEL_TOURNAMENT = 0, SEL_RANKING = 1, SEL_ROULETTE = 2 };
+
+uint64_t oracle_roulette_weight(float f)
+{
+    float key = fit_key(f);
+    double v = 1.0 - (double)key;
+    if (!(v > 0.0)) return 0;
+    if (v >= 1.0) return (uint64_t)1 << 32;
+    return (uint64_t)floor(v * 4294967296.0);
+}
+
+int oracle_rank_from_word(uint32_t w, int M)
+{
+    uint64_t T = (uint64_t)M * (uint64_t)(M + 1) / 2;
+    uint64_t u = (uint64_t)(((unsigned __int128)w * T) >> 32);
+    for (int r = 0; r < M; ++r) {
+        uint64_t C = (uint64_t)(r + 1) * (uint64_t)M - (uint64_t)r * (uint64_t)(r + 1) / 2;
+        if (C > u) return r;
+    }
+    return M - 1;
+}
+
+int oracle_roulette_from_word(uint32_t w, int M, const uint64_t *weight)
+{
+    uint64_t T = 0;
+    for (int i = 0; i < M; ++i) T += weight[i];
+    if (T == 0) return (int)oracle_index(w, (uint32_t)M);
+    uint64_t u = (uint64_t)(((unsigned __int128)w * T) >> 32);
+    uint64_t acc = 0;
+    for (int i = 0; i < M; ++i) {
+        acc += weight[i];
+        if (acc > u) return i;
+    }
+    return M - 1;
+}
+
+/* One generation as oracle_step, with the selection method chosen by `selection` (crossover, mutation, elitism and
+ * their draws are unchanged; `k` is only used by SEL_TOURNAMENT). */
+int oracle_step_sel(int M, int G, int E, int k, int selection, double p_cross, double p_mut, float sigma,
+                    uint64_t seed, uint32_t gen, const float *W, const float *F, float *Wnext)
+{
+    if (selection == SEL_TOURNAMENT) return oracle_step(M, G, E, k, p_cross, p_mut, sigma, seed, gen, W, F, Wnext);
+    if (M < 1 || G < 1 || E < 0 || E >= M || selection > SEL_ROULETTE) return -1;
+    int *by_rank = (int *)malloc(sizeof(int) * (size_t)M);
+    uint64_t *weight = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)M);
+    if (!by_rank || !weight) { free(by_rank); free(weight); return -2; }
+    for (int m = 0; m < M; ++m) {
+        int r = 0;
+        for (int j = 0; j < M; ++j) r += precedes(F, j, m);
+        by_rank[r] = m;
+        weight[m] = oracle_roulette_weight(F[m]);
+    }
+    for (int s = 0; s < E; ++s)
+        memcpy(Wnext + (size_t)s * G, W + (size_t)by_rank[s] * G, sizeof(float) * (size_t)G);
+    uint64_t Tc = oracle_bernoulli_threshold(p_cross);
+    uint64_t Tm = oracle_bernoulli_threshold(p_mut);
+    for (int c = E; c < M; ++c) {
+        uint32_t r[4];
+        draw(seed, 0u, (uint32_t)c, gen, TAG_SELECT, r);
+        int parent[2];
+        for (int s = 0; s < 2; ++s)
+            parent[s] = selection == SEL_RANKING ? by_rank[oracle_rank_from_word(r[s], M)]
+                                                 : oracle_roulette_from_word(r[s], M, weight);
+        const float *A = W + (size_t)parent[0] * G;
+        const float *B = W + (size_t)parent[1] * G;
+        float *child = Wnext + (size_t)c * G;
+        uint32_t rc[4];
+        draw(seed, 0u, (uint32_t)c, gen, TAG_CROSS, rc);
+        int q = G;
+        if ((uint64_t)rc[0] < Tc && G >= 2) q = 1 + (int)oracle_index(rc[1], (uint32_t)(G - 1));
+        for (int g = 0; g < G; ++g) child[g] = g < q ? A[g] : B[g];
+        for (int g = 0; g < G; ++g) {
+            uint32_t rm[4];
+            draw(seed, (uint32_t)g, (uint32_t)c, gen, TAG_MUTATE, rm);
+            if ((uint64_t)rm[0] < Tm) {
+                float z = oracle_gauss(rm[1], rm[2]);
+                float delta = sigma * z;
+                child[g] = child[g] + delta;
+            }
+        }
+    }
+    free(by_rank);
+    free(weight);
+    return 0;
+}

@@ -365,3 +365,69 @@ def test_run_until_stop_rule_against_the_plain_run():
     assert done == g and np.array_equal(b3, best[:g + 1])
     Wg, Fg, _ = oracle.run(cfg.d, cfg.family, X, t, W0, *args, g)
     assert np.array_equal(W3, Wg) and np.array_equal(F3, Fg)
+
+
+# ------------------------------------------------------------------------------------------------ ranking / roulette (R10)
+def test_ranking_word_map_has_exact_linear_probabilities():
+    """Sweeping w over a grid fine enough to hit every u in [0, T): rank r must be chosen for exactly M - r values of
+    u (linear ranking, best rank weight M, worst weight 1), monotonically in w."""
+    for M in (1, 2, 5, 12):
+        T = M * (M + 1) // 2
+        counts, last = [0] * M, 0
+        for u in range(T):
+            w = -(-(u << 32) // T)                     # smallest 32-bit word with floor(w T / 2^32) == u
+            assert (w * T) >> 32 == u
+            r = oracle.rank_from_word(w, M)
+            assert r >= last
+            last = r
+            counts[r] += 1
+        assert counts == [M - r for r in range(M)]
+    assert oracle.rank_from_word(0, 4096) == 0 and oracle.rank_from_word(2**32 - 1, 4096) == 4095
+
+
+def test_roulette_weights_and_word_map():
+    # weight = floor((1 - F) 2^32) clipped to [0, 2^32]; NaN / inf / F >= 1 -> 0; F <= 0 -> 2^32   (PAPER.md:91)
+    assert oracle.roulette_weight(0.25) == 3 << 30 and oracle.roulette_weight(0.0) == 1 << 32
+    assert oracle.roulette_weight(1.0) == 0 and oracle.roulette_weight(1.5) == 0 and oracle.roulette_weight(-3.0) == 1 << 32
+    assert oracle.roulette_weight(np.nan) == 0 and oracle.roulette_weight(np.inf) == 0
+    assert oracle.roulette_weight(np.float32(0.1)) == int(np.floor((1.0 - float(np.float32(0.1))) * 2**32))
+    # exact proportions on small integer weights: index i is hit for exactly weight_i values of u
+    wts = [3, 0, 5, 1, 0, 7]
+    T = sum(wts)
+    counts = [0] * len(wts)
+    for u in range(T):
+        w = -(-(u << 32) // T)
+        counts[oracle.roulette_from_word(w, wts)] += 1
+    assert counts == wts
+    # all weights zero -> uniform index
+    assert [oracle.roulette_from_word(w, [0, 0, 0, 0]) for w in (0, 2**30, 2**31, 2**32 - 1)] == [0, 1, 2, 3]
+
+
+@pytest.mark.parametrize("selection", [oracle.SEL_RANKING, oracle.SEL_ROULETTE])
+def test_step_sel_invariants(selection):
+    rng = np.random.Generator(np.random.Philox(5))
+    M, G, E = 60, 9, 3
+    W = rng.uniform(-1, 1, (M, G)).astype(np.float32)
+    F = rng.uniform(0, 1, M).astype(np.float32)
+    F[7] = np.nan; F[9] = F[11]
+    # no crossover, no mutation: every child is a bit-copy of a parent chosen by the selection alone
+    Wn = oracle.step_sel(W, F, E, 3, selection, 0.0, 0.0, 0.1, 17, 2)
+    order = sorted(range(M), key=lambda m: (np.inf if np.isnan(F[m]) else F[m], m))
+    assert all(np.array_equal(Wn[s], W[order[s]]) for s in range(E))
+    rows = {W[m].tobytes(): m for m in range(M)}
+    parents = [rows[Wn[c].tobytes()] for c in range(E, M)]
+    assert 7 not in parents or selection == oracle.SEL_RANKING        # zero roulette weight is never selected
+    # the choice is the documented map of word 0 of the SELECT draw
+    for c in (E, E + 1, M - 1):
+        w0 = int(oracle.philox4x32_10([0, c, 2, 1], [17, 0])[0])
+        if selection == oracle.SEL_RANKING:
+            assert rows[Wn[c].tobytes()] == order[oracle.rank_from_word(w0, M)]
+        else:
+            assert rows[Wn[c].tobytes()] == oracle.roulette_from_word(w0, [oracle.roulette_weight(f) for f in F])
+    # better chromosomes are selected more often (both methods are fitness-monotone in expectation)
+    many = np.concatenate([[rows[r.tobytes()] for r in oracle.step_sel(W, F, 0, 3, selection, 0.0, 0.0, 0.1, 17, g)]
+                           for g in range(40)])
+    best_half = set(order[:M // 2])
+    assert np.mean([p in best_half for p in many]) > 0.55
+    # tournament through the same entry point is the plain step
+    assert np.array_equal(oracle.step_sel(W, F, E, 3, 0, 0.9, 0.05, 0.1, 17, 2), oracle.step(W, F, E, 3, 0.9, 0.05, 0.1, 17, 2))
