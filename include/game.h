@@ -109,6 +109,17 @@ int game_bind_state(game_ctx* ctx, float* popA_dev, float* popB_dev, float* fitn
 int game_set_ga_params(game_ctx* ctx, int32_t elite, int32_t tournament, double p_cross, double p_mut,
                        float sigma);
 
+/* Selection method of game_step.  TOURNAMENT (default, BASELINE.json) uses the `tournament` size of game_set_ga_params.
+ * RANKING and ROULETTE are the paper's own methods, defined here with integer arithmetic only
+ * (R10): parents A and B of child slot c come from words 0 and 1 of the Philox draw (0, c, gen, TAG_SELECT);
+ *   RANKING : rank r (0 = best under (fitness, index), NaN worst) has weight M - r, u = floor(w M(M+1)/2 / 2^32), the parent
+ *             holds the smallest rank r with (r+1) M - r (r+1)/2 > u;
+ *   ROULETTE: weight_i = floor(clamp(1 - fitness_i, 0, 1) * 2^32) (PAPER.md:91 fitness = 1 - error; NaN / inf -> 0),
+ *             u = floor(w * sum / 2^32), the parent is the smallest index whose prefix sum exceeds u (sum = 0: uniform).
+ * Elitism, crossover and mutation are unchanged. */
+enum { GAME_SEL_TOURNAMENT = 0, GAME_SEL_RANKING = 1, GAME_SEL_ROULETTE = 2 };
+int game_set_selection(game_ctx* ctx, int32_t selection);
+
 /* Current population <- genes uniform in [-1,1) from Philox4x32-10 with
  * key = seed, counter = (g>>2, m, 0, TAG_INIT), word g&3, w = float(word>>8)*2^-23 - 1  [SURVEY 8(c) R6].
  * Invalidates the fitness.  Async. */

@@ -43,7 +43,89 @@ struct GaParams {
     float sigma;
     uint32_t gen;
     PhiloxKey key;
+    int selection;                        // 0 tournament, 1 ranking, 2 roulette (R10)
+    const int* by_rank;                   // ranking: chromosome holding each rank (rank_kernel)
+    const unsigned long long* prefix;     // roulette: inclusive prefix sums of the integer weights (roulette_prefix_kernel)
 };
+
+// ---- the paper's own selection methods ("ranking", "roulette"; defined by DESIGN.md R10).  Integer
+// arithmetic only, so that the choice is bit-identical on any machine.
+// floor(w * T / 2^32) for a 32-bit word and T < 2^57
+__device__ __forceinline__ unsigned long long scale_word(uint32_t w, unsigned long long T) {
+    return static_cast<unsigned long long>(w) * (T >> 32) + ((static_cast<unsigned long long>(w) * (T & 0xffffffffull)) >> 32);
+}
+// linear ranking: rank r (0 = best) has weight M - r; smallest r with C(r) = (r+1) M - r (r+1) / 2 > u
+__device__ __forceinline__ int rank_from_word(uint32_t w, int M) {
+    const unsigned long long Mu = static_cast<unsigned long long>(M);
+    const unsigned long long u = scale_word(w, Mu * (Mu + 1) / 2);
+    int lo = 0, hi = M - 1;
+    while (lo < hi) {
+        const unsigned long long r = static_cast<unsigned long long>((lo + hi) >> 1);
+        if ((r + 1) * Mu - r * (r + 1) / 2 > u) hi = static_cast<int>(r); else lo = static_cast<int>(r) + 1;
+    }
+    return lo;
+}
+// roulette weight of a fitness: floor(clamp(1 - key(F), 0, 1) * 2^32) in double (PAPER.md:91 fitness = 1 - error)
+__device__ __forceinline__ unsigned long long roulette_weight(float f) {
+    const double v = 1.0 - static_cast<double>(fit_key(f));
+    if (!(v > 0.0)) return 0ull;
+    if (v >= 1.0) return 1ull << 32;
+    return static_cast<unsigned long long>(v * 4294967296.0);
+}
+// smallest index whose inclusive prefix sum exceeds floor(w T / 2^32); T = 0 -> uniform index
+__device__ __forceinline__ int roulette_from_word(uint32_t w, int M, const unsigned long long* __restrict__ prefix) {
+    const unsigned long long T = prefix[M - 1];
+    if (T == 0) return static_cast<int>(index_below(w, static_cast<uint32_t>(M)));
+    const unsigned long long u = scale_word(w, T);
+    int lo = 0, hi = M - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (prefix[mid] > u) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+// by_rank[rank of chromosome c] = c; one block per chromosome (the same count as in ga_step_kernel).
+__global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* __restrict__ F, int M, int* __restrict__ by_rank) {
+    __shared__ int s_warp_cnt[kGaThreads / 32];
+    const int c = blockIdx.x, tid = threadIdx.x;
+    const float kc = fit_key(F[c]);
+    int cnt = 0;
+    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(F[j]), j, kc, c) ? 1 : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((tid & 31) == 0) s_warp_cnt[tid >> 5] = cnt;
+    __syncthreads();
+    if (tid == 0) {
+        int r = 0;
+        for (int w = 0; w < kGaThreads / 32; ++w) r += s_warp_cnt[w];
+        by_rank[r] = c;
+    }
+}
+
+// Inclusive prefix sums of the roulette weights; one block of 1024 threads, each owning a contiguous segment.
+__global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* __restrict__ F, int M,
+                                                               unsigned long long* __restrict__ prefix) {
+    __shared__ unsigned long long s_tot[1024];
+    const int tid = threadIdx.x;
+    const int per = (M + 1023) / 1024;
+    const int i0 = tid * per, i1 = min(M, i0 + per);
+    unsigned long long acc = 0;
+    for (int i = i0; i < i1; ++i) acc += roulette_weight(F[i]);
+    s_tot[tid] = acc;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {               // Hillis-Steele scan of the 1024 segment totals (integers: exact)
+        const unsigned long long v = tid >= o ? s_tot[tid - o] : 0ull;
+        __syncthreads();
+        s_tot[tid] += v;
+        __syncthreads();
+    }
+    acc = tid > 0 ? s_tot[tid - 1] : 0ull;
+    for (int i = i0; i < i1; ++i) {
+        acc += roulette_weight(F[i]);
+        prefix[i] = acc;
+    }
+}
 
 // ---- one generation (R7).  Block c plays two parts, with no grid-wide synchronisation:
 //  (1) as chromosome c of the OLD population it counts how many chromosomes precede it; if that rank is
@@ -92,17 +174,29 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     if (tid == 0) {
         const int k = p.tournament;
         int par[2] = {-1, -1};
-        float pkey[2] = {0.f, 0.f};
-        uint4 r = make_uint4(0, 0, 0, 0);
-        for (int e = 0; e < 2 * k; ++e) {
-            if ((e & 3) == 0)
-                r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
-            const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
-            const float ki = fit_key(F[idx]);
-            const int side = e < k ? 0 : 1;
-            if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
-                par[side] = idx;
-                pkey[side] = ki;
+        if (p.selection == 0) {
+            float pkey[2] = {0.f, 0.f};
+            uint4 r = make_uint4(0, 0, 0, 0);
+            for (int e = 0; e < 2 * k; ++e) {
+                if ((e & 3) == 0)
+                    r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
+                const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
+                const float ki = fit_key(F[idx]);
+                const int side = e < k ? 0 : 1;
+                if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
+                    par[side] = idx;
+                    pkey[side] = ki;
+                }
+            }
+        } else {
+            // ranking / roulette: parents A and B from words 0 and 1 of one SELECT draw
+            const uint4 r = philox4x32_10(0u, static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
+            if (p.selection == 1) {
+                par[0] = p.by_rank[rank_from_word(r.x, M)];
+                par[1] = p.by_rank[rank_from_word(r.y, M)];
+            } else {
+                par[0] = roulette_from_word(r.x, M, p.prefix);
+                par[1] = roulette_from_word(r.y, M, p.prefix);
             }
         }
         s_parent[0] = par[0];

@@ -35,7 +35,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -46,7 +46,7 @@ struct game_ctx {
     bool fitness_valid = false;
     bool ticket_zeroed = false;
     // GA parameters
-    int elite = 2, tournament = 3;
+    int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT;
     double p_cross = 0.9, p_mut = 0.05;
     float sigma = 0.1f;
     // execution
@@ -276,6 +276,17 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     p.t_cross = bernoulli_threshold(c->p_cross);
     p.t_mut = bernoulli_threshold(c->p_mut);
     p.sigma = c->sigma; p.gen = gen; p.key = make_key(seed);
+    p.selection = c->selection;
+    p.by_rank = reinterpret_cast<const int*>(c->ws + c->off_by_rank);
+    p.prefix = reinterpret_cast<const unsigned long long*>(c->ws + c->off_prefix);
+    if (c->selection == GAME_SEL_RANKING) {
+        rank_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->fitness, c->M, reinterpret_cast<int*>(c->ws + c->off_by_rank));
+        if ((rc = check_launch(c, "rank_kernel"))) return rc;
+    } else if (c->selection == GAME_SEL_ROULETTE) {
+        roulette_prefix_kernel<<<1, 1024, 0, c->stream>>>(c->fitness, c->M,
+                                                           reinterpret_cast<unsigned long long*>(c->ws + c->off_prefix));
+        if ((rc = check_launch(c, "roulette_prefix_kernel"))) return rc;
+    }
     ga_step_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop);
     if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
     c->cur ^= 1;
@@ -317,6 +328,8 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_ticket = off; off = align_up(off + sizeof(unsigned int));
     c->off_stall = off; off = align_up(off + sizeof(long long) * 4 * kMaxCtas);
     c->off_stop = off; off = align_up(off + 2 * sizeof(int));
+    c->off_by_rank = off; off = align_up(off + sizeof(int) * static_cast<size_t>(M));
+    c->off_prefix = off; off = align_up(off + sizeof(unsigned long long) * static_cast<size_t>(M));
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
@@ -406,6 +419,13 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
     if (!(sigma >= 0.0f) || !std::isfinite(sigma)) return fail(c, GAME_ERR_INVALID_ARG, "sigma must be finite and >= 0");
     c->elite = elite; c->tournament = tournament;
     c->p_cross = p_cross; c->p_mut = p_mut; c->sigma = sigma;
+    return GAME_OK;
+}
+
+int game_set_selection(game_ctx* c, int32_t selection) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (selection < GAME_SEL_TOURNAMENT || selection > GAME_SEL_ROULETTE) return fail(c, GAME_ERR_INVALID_ARG, "unknown selection %d", selection);
+    c->selection = selection;
     return GAME_OK;
 }
 

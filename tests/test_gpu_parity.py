@@ -464,3 +464,32 @@ def test_run_until_stop_rule(game, scheme):
                                              cfg.sigma, seed, 0, n, thr)
     assert done_ref == g_stop and np.all(np.abs(b_ref - plain[:g_stop + 1]) <= 1e-4 * np.abs(b_ref))
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ ranking / roulette
+@pytest.mark.parametrize("selection", [1, 2])
+@pytest.mark.parametrize("M,N,d,E,pc,pm,sigma,seed,gen", [
+    (64, 4, 3, 2, 0.9, 0.05, 0.1, 0, 0), (512, 10, 6, 4, 0.9, 0.2, 0.1, 1, 7), (4096, 32, 10, 2, 0.9, 0.2, 0.1, 3, 19),
+    (1500, 7, 3, 0, 1.0, 0.0, 0.0, 2**40 + 1, 5), (33, 2, 1, 32, 0.5, 0.5, 1.0, 9, 2**31 + 3)])
+def test_ga_step_ranking_roulette_bit_exact(game, selection, M, N, d, E, pc, pm, sigma, seed, gen):
+    """The paper's own selection methods (crossover 0.9, mutation 0.2, elitism 2 are its settings):
+    same fitness vector and seed in, bit-identical next population out."""
+    rng = np.random.Generator(np.random.Philox(2000 + M + selection))
+    G = game.Game(300, N, d, M, wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    W = rng.uniform(-2, 2, size=(M, G.G)).astype(np.float32)
+    F = rng.uniform(0, 1.2, size=M).astype(np.float32)            # some fitness above 1: zero roulette weight
+    F[rng.integers(0, M, size=max(1, M // 8))] = F[0]
+    F[3] = np.nan; F[5] = np.inf; F[6] = -0.0; F[7] = 1e-30
+    G.set_ga_params(E, 3, pc, pm, sigma)
+    game.game_set_selection(G.ctx, selection)
+    G.set_population(W); G.set_fitness(F)
+    G.step(seed, gen); G.sync()
+    ref = oracle.step_sel(W, F, E, 3, selection, pc, pm, sigma, seed, gen)
+    Wn = G.get_population()
+    assert np.array_equal(Wn.view(np.uint32), ref.view(np.uint32)), \
+        f"{np.count_nonzero(Wn.view(np.uint32) != ref.view(np.uint32))} genes differ"
+    if selection == 2:                                            # all weights zero -> uniform parents
+        G.set_population(W); G.set_fitness(np.full(M, 2.0, np.float32)); G.step(seed, gen); G.sync()
+        ref = oracle.step_sel(W, np.full(M, 2.0, np.float32), E, 3, selection, pc, pm, sigma, seed, gen)
+        assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
+    G.close()
