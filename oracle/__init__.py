@@ -88,6 +88,8 @@ def lib() -> C.CDLL:
         L.oracle_step_sel.restype = C.c_int
         L.oracle_step_sel.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
                                       C.c_uint64, C.c_uint32, f32p, f32p, f32p]
+        L.oracle_immigrate.restype = C.c_int
+        L.oracle_immigrate.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint64, C.c_uint32, f32p]
         L.oracle_run_until.restype = C.c_int
         L.oracle_run_until.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, f32p, f32p,
                                        C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
@@ -305,4 +307,14 @@ def step_sel(W, F, E: int, k: int, selection: int, p_cross: float, p_mut: float,
                                _p(W, C.c_float), _p(F, C.c_float), _p(Wn, C.c_float))
     if rc:
         raise ValueError(f"oracle_step_sel failed: {rc}")
+    return Wn
+
+
+def immigrate(Wn, E: int, R: int, seed: int, gen: int) -> np.ndarray:
+    """Overwrite the last R child slots of a stepped population with fresh random chromosomes (R12)."""
+    Wn = _f32(Wn).copy()
+    M, G = Wn.shape
+    rc = lib().oracle_immigrate(M, G, E, R, seed, gen, _p(Wn, C.c_float))
+    if rc:
+        raise ValueError(f"oracle_immigrate failed: {rc}")
     return Wn

@@ -549,3 +549,22 @@ int oracle_step_sel(int M, int G, int E, int k, int selection, double p_cross, d
     free(weight);
     return 0;
 }
+
+
+/* ---- random replacement  ("a variable number of chromosomes are randomly generated to replace older
+ * individuals"; reading R12).  After a generation step the last R child slots M-R..M-1 (never elite slots:
+ * R <= M - E) are overwritten by fresh random chromosomes, genes uniform in [-1,1) exactly as at initialisation but
+ * drawn with counter (g>>2, c, gen, TAG_IMMIGRANT = 4), word g&3. */
+enum { TAG_IMMIGRANT = 4 };
+
+int oracle_immigrate(int M, int G, int E, int R, uint64_t seed, uint32_t gen, float *Wnext)
+{
+    if (R < 0 || R > M - E) return -1;
+    for (int c = M - R; c < M; ++c)
+        for (int g = 0; g < G; ++g) {
+            uint32_t r[4];
+            draw(seed, (uint32_t)(g >> 2), (uint32_t)c, gen, TAG_IMMIGRANT, r);
+            Wnext[(size_t)c * G + g] = (float)(r[g & 3] >> 8) * 0x1p-23f - 1.0f;
+        }
+    return 0;
+}

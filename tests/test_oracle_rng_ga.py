@@ -431,3 +431,23 @@ def test_step_sel_invariants(selection):
     assert np.mean([p in best_half for p in many]) > 0.55
     # tournament through the same entry point is the plain step
     assert np.array_equal(oracle.step_sel(W, F, E, 3, 0, 0.9, 0.05, 0.1, 17, 2), oracle.step(W, F, E, 3, 0.9, 0.05, 0.1, 17, 2))
+
+
+def test_immigrants_replace_only_the_last_slots_with_init_like_genes():
+    rng = np.random.Generator(np.random.Philox(8))
+    M, G, E, R = 40, 13, 2, 5
+    Wn = rng.uniform(-3, 3, (M, G)).astype(np.float32)
+    out = oracle.immigrate(Wn, E, R, 77, 6)
+    assert np.array_equal(out[:M - R], Wn[:M - R])                      # everything else untouched
+    assert out[M - R:].min() >= -1.0 and out[M - R:].max() < 1.0       # PAPER.md:66 gene range
+    # the documented map: gene g of slot c = word g&3 of Philox(counter (g>>2, c, gen, 4), key seed)
+    for c, g in ((M - R, 0), (M - 1, 12), (M - 2, 5)):
+        w = int(oracle.philox4x32_10([g >> 2, c, 6, 4], [77, 0])[g & 3])
+        assert out[c, g] == np.float32(np.float32(w >> 8) * np.float32(2.0 ** -23) - np.float32(1.0))
+    assert np.array_equal(oracle.immigrate(Wn, E, 0, 77, 6), Wn)
+    assert not np.array_equal(oracle.immigrate(Wn, E, R, 77, 7)[M - R:], out[M - R:])     # fresh draws every generation
+    with pytest.raises(ValueError):
+        oracle.immigrate(Wn, E, M - E + 1, 77, 6)                      # would overwrite an elite slot
+    # ~uniform: mean near 0, variance near 1/3 over many genes
+    big = oracle.immigrate(np.zeros((2000, 64), np.float32), 0, 2000, 1, 0)
+    assert abs(big.mean()) < 0.01 and abs(big.var() - 1 / 3) < 0.01
