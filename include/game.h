@@ -120,6 +120,13 @@ int game_set_ga_params(game_ctx* ctx, int32_t elite, int32_t tournament, double 
 enum { GAME_SEL_TOURNAMENT = 0, GAME_SEL_RANKING = 1, GAME_SEL_ROULETTE = 2 };
 int game_set_selection(game_ctx* ctx, int32_t selection);
 
+/* Random replacement ("a variable number of chromosomes are randomly generated to replace older
+ * individuals"; R12): the last `immigrants` child slots of every game_step (never elite slots:
+ * 0 <= immigrants <= M - elite, checked against the current elite count; clamped again if elite grows later) are
+ * fresh random chromosomes, genes uniform in [-1,1) as at initialisation, Philox counter (g>>2, c, gen, TAG_IMMIGRANT = 4),
+ * word g&3.  Default 0. */
+int game_set_immigrants(game_ctx* ctx, int32_t immigrants);
+
 /* Current population <- genes uniform in [-1,1) from Philox4x32-10 with
  * key = seed, counter = (g>>2, m, 0, TAG_INIT), word g&3, w = float(word>>8)*2^-23 - 1  [SURVEY 8(c) R6].
  * Invalidates the fitness.  Async. */

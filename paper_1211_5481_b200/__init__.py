@@ -36,6 +36,7 @@ SIGNATURES = {
     "game_bind_state": (C.c_int, [_VP, _F32P, _F32P, _F32P, _VP, C.c_size_t]),
     "game_set_ga_params": (C.c_int, [_VP, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_float]),
     "game_set_selection": (C.c_int, [_VP, C.c_int32]),
+    "game_set_immigrants": (C.c_int, [_VP, C.c_int32]),
     "game_init_population": (C.c_int, [_VP, C.c_uint64]),
     "game_current_population": (C.c_int, [_VP, C.POINTER(C.c_void_p)]),
     "game_invalidate_fitness": (C.c_int, [_VP]),
@@ -140,6 +141,10 @@ def game_bind_state(ctx, popA_dev: int, popB_dev: int, fitness_dev: int, workspa
 
 def game_set_ga_params(ctx, elite: int, tournament: int, p_cross: float, p_mut: float, sigma: float) -> None:
     _check(ctx, lib().game_set_ga_params(ctx, elite, tournament, p_cross, p_mut, sigma))
+
+
+def game_set_immigrants(ctx, immigrants: int) -> None:
+    _check(ctx, lib().game_set_immigrants(ctx, immigrants))
 
 
 def game_set_selection(ctx, selection: int) -> None:

@@ -43,6 +43,7 @@ struct GaParams {
     float sigma;
     uint32_t gen;
     PhiloxKey key;
+    int immigrants;                       // last R child slots are replaced by fresh random chromosomes (R12)
     int selection;                        // 0 tournament, 1 ranking, 2 roulette (R10)
     const int* by_rank;                   // ranking: chromosome holding each rank (rank_kernel)
     const unsigned long long* prefix;     // roulette: inclusive prefix sums of the integer weights (roulette_prefix_kernel)
@@ -169,6 +170,15 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
         for (int g = tid; g < G; g += kGaThreads) dst[g] = src[g];
     }
     if (c < p.elite) return;  // slots 0..elite-1 are written by the elites themselves
+    if (c >= M - p.immigrants) {
+        // random replacement: genes uniform in [-1,1) as at initialisation, tag IMMIGRANT
+        float* fresh = Wn + static_cast<size_t>(c) * G;
+        for (int g = tid; g < G; g += kGaThreads) {
+            const uint4 r = philox4x32_10(static_cast<uint32_t>(g >> 2), static_cast<uint32_t>(c), p.gen, kTagImmigrant, p.key);
+            fresh[g] = gene_from_word(word_of(r, g & 3));
+        }
+        return;
+    }
 
     // (2) tournaments: entrants 0..k-1 -> parent A, k..2k-1 -> parent B (with replacement)
     if (tid == 0) {

@@ -46,7 +46,7 @@ struct game_ctx {
     bool fitness_valid = false;
     bool ticket_zeroed = false;
     // GA parameters
-    int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT;
+    int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0;
     double p_cross = 0.9, p_mut = 0.05;
     float sigma = 0.1f;
     // execution
@@ -277,6 +277,7 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     p.t_mut = bernoulli_threshold(c->p_mut);
     p.sigma = c->sigma; p.gen = gen; p.key = make_key(seed);
     p.selection = c->selection;
+    p.immigrants = c->immigrants < c->M - c->elite ? c->immigrants : c->M - c->elite;
     p.by_rank = reinterpret_cast<const int*>(c->ws + c->off_by_rank);
     p.prefix = reinterpret_cast<const unsigned long long*>(c->ws + c->off_prefix);
     if (c->selection == GAME_SEL_RANKING) {
@@ -419,6 +420,14 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
     if (!(sigma >= 0.0f) || !std::isfinite(sigma)) return fail(c, GAME_ERR_INVALID_ARG, "sigma must be finite and >= 0");
     c->elite = elite; c->tournament = tournament;
     c->p_cross = p_cross; c->p_mut = p_mut; c->sigma = sigma;
+    return GAME_OK;
+}
+
+int game_set_immigrants(game_ctx* c, int32_t immigrants) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (immigrants < 0 || immigrants > c->M - c->elite)
+        return fail(c, GAME_ERR_INVALID_ARG, "immigrants must be in [0, M - elite]");
+    c->immigrants = immigrants;
     return GAME_OK;
 }
 

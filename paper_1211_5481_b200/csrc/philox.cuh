@@ -14,7 +14,7 @@
 
 namespace game {
 
-enum : uint32_t { kTagInit = 0u, kTagSelect = 1u, kTagCross = 2u, kTagMutate = 3u };
+enum : uint32_t { kTagInit = 0u, kTagSelect = 1u, kTagCross = 2u, kTagMutate = 3u, kTagImmigrant = 4u };
 
 struct PhiloxKey {
     uint32_t k0, k1;

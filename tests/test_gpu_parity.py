@@ -493,3 +493,22 @@ def test_ga_step_ranking_roulette_bit_exact(game, selection, M, N, d, E, pc, pm,
         ref = oracle.step_sel(W, np.full(M, 2.0, np.float32), E, 3, selection, pc, pm, sigma, seed, gen)
         assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
     G.close()
+
+
+@pytest.mark.parametrize("selection,M,E,R", [(0, 200, 2, 17), (1, 64, 2, 62), (2, 513, 0, 1), (0, 100, 4, 0)])
+def test_ga_step_with_random_immigrants_bit_exact(game, selection, M, E, R):
+    """Random replacement (R12): the last R child slots are fresh random chromosomes, everything else is
+    the plain step; bit-exact against oracle.step_sel + oracle.immigrate."""
+    rng = np.random.Generator(np.random.Philox(3000 + M))
+    G = game.Game(300, 6, 4, M, wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    W = rng.uniform(-2, 2, size=(M, G.G)).astype(np.float32)
+    F = rng.uniform(0, 1, size=M).astype(np.float32)
+    G.set_ga_params(E, 3, 0.9, 0.2, 0.1)
+    game.game_set_selection(G.ctx, selection)
+    game.game_set_immigrants(G.ctx, R)
+    with pytest.raises(game.GameError):
+        game.game_set_immigrants(G.ctx, M - E + 1)
+    G.set_population(W); G.set_fitness(F); G.step(31, 8); G.sync()
+    ref = oracle.immigrate(oracle.step_sel(W, F, E, 3, selection, 0.9, 0.2, 0.1, 31, 8), E, R, 31, 8)
+    assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
+    G.close()
