@@ -61,6 +61,11 @@ CONFIGS = {
     "c3": Config("c3", 4_000_000, 32, 10, 4096, EXP_CHEBYSHEV, ACT_SIGMOID, 4, 3, 0.9, 0.05, 0.1, 20, 1.0, 1.0, 0.05, 3),
 }
 
+# The paper's own experiment shape, as a synthetic stand-in: 2100 patterns x 9 feature
+# columns, polytrigo degree 8, B*N+1 = 19 chromosomes (eq.(4)), crossover 0.9, mutation 0.2, elitism 2,
+# ranking selection, MSE threshold 0.001, thousands of iterations: the latency-bound regime.  Per-feature coefficients (D1).
+PAPER_SHAPE = Config("n1", 2_100, 9, 8, 19, EXP_TRIG, ACT_SIGMOID, 2, 3, 0.9, 0.2, 0.1, 10_000, float(np.pi), 0.3, 0.05, 11)
+
 C4_M = (256, 1024, 4096, 16384)
 C4_P = (100_000, 1_000_000, 10_000_000)
 
