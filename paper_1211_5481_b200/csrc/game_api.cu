@@ -142,7 +142,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (rc) return rc;
     const int scheme = resolved_scheme(c);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers N <= 32 (Chebyshev) / N <= 16 (trig) and d <= 64");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers d <= 64");
     if (!c->ticket_zeroed) {
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
         c->ticket_zeroed = true;
@@ -307,15 +307,15 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     if (expansion > GAME_EXP_TRIG || act > GAME_ACT_TANH) return GAME_ERR_INVALID_ARG;
     if (P > (1ll << 40) || N > 4096 || d > 4096 || M > (1 << 24)) return GAME_ERR_INVALID_ARG;
     const long long G = static_cast<long long>(N) * d * (expansion == GAME_EXP_TRIG ? 2 : 1) + 1;
-    if (G > game::kFfmaMaxG) return GAME_ERR_UNSUPPORTED;
+    const bool umma_ok = d <= 64 && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
+    if (G > (1 << 20) || (!umma_ok && G > game::kFfmaMaxG)) return GAME_ERR_UNSUPPORTED;   // FFMA kernel: G <= 448
     game_ctx* c = new (std::nothrow) game_ctx();
     if (!c) return GAME_ERR_INVALID_ARG;
     c->P = P; c->N = N; c->d = d; c->M = M; c->G = static_cast<int>(G);
     c->expansion = expansion; c->act = act;
     c->m_tiles = 2 * ((M + 2 * game::umma::kBM - 1) / (2 * game::umma::kBM));   // one chromosome tile per CTA of a pair
     c->m_stride = c->m_tiles * game::umma::kBM;
-    c->umma_ok = d <= 64 && (expansion == GAME_EXP_CHEBYSHEV ? N <= 32 : N <= 16) &&
-                 (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
+    c->umma_ok = umma_ok;
     c->chunks = (N + 7) / 8;
     c->steps_per_chunk = expansion == GAME_EXP_CHEBYSHEV ? (d + 1) / 2 : d;
     c->steps = c->chunks * c->steps_per_chunk;
@@ -370,7 +370,9 @@ int game_set_scheme(game_ctx* c, int32_t scheme) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (scheme < GAME_SCHEME_AUTO || scheme > GAME_SCHEME_F16X3) return fail(c, GAME_ERR_INVALID_ARG, "unknown scheme %d", scheme);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers N <= 32 (Chebyshev) / N <= 16 (trig) and d <= 64");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers d <= 64");
+    if (scheme == GAME_SCHEME_FFMA && c->G > game::kFfmaMaxG)
+        return fail(c, GAME_ERR_UNSUPPORTED, "FFMA covers G <= 448");
     c->scheme = scheme;
     return GAME_OK;
 }

@@ -69,7 +69,9 @@ def test_create_rejects_bad_shapes(L, args):
 
 def test_create_unsupported_gene_count(L):
     ctx = C.c_void_p()
-    assert L.game_create(C.byref(ctx), 10, 64, 10, 8, 0x0100) == game.ERR_UNSUPPORTED   # G = 641 > 448
+    assert L.game_create(C.byref(ctx), 10, 10, 70, 8, 0x0100) == game.ERR_UNSUPPORTED   # d > 64 and G = 701 > 448
+    assert L.game_create(C.byref(ctx), 10, 64, 10, 8, 0x0100) == game.OK                # G = 641: tensor-core kernel
+    game.game_destroy(ctx)
 
 
 def test_scheme_resolution(L):
@@ -78,10 +80,16 @@ def test_scheme_resolution(L):
     game.game_set_scheme(ctx, game.SCHEME_FFMA)
     assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
     game.game_destroy(ctx)
-    ctx = game.game_create(1000, 40, 10, 64, 0x0100)          # N > 32: tensor-core kernel does not cover it
+    ctx = game.game_create(1000, 4, 70, 64, 0x0100)           # d > 64: tensor-core kernel does not cover it
     assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
     with pytest.raises(game.GameError) as e:
         game.game_set_scheme(ctx, game.SCHEME_F16X3)
+    assert e.value.code == game.ERR_UNSUPPORTED
+    game.game_destroy(ctx)
+    ctx = game.game_create(1000, 64, 10, 64, 0x0100)          # G = 641: only the tensor-core kernel covers it
+    assert game.game_get_scheme(ctx) == game.SCHEME_F16X3
+    with pytest.raises(game.GameError) as e:
+        game.game_set_scheme(ctx, game.SCHEME_FFMA)
     assert e.value.code == game.ERR_UNSUPPORTED
     game.game_destroy(ctx)
 

@@ -61,6 +61,10 @@ FITNESS_CASES = [
     ("stream_trig", "c2", dict(P=900, N=16, d=12, M=140)),
     # many chromosome tiles per unit with resident phi (reuse across 5 tile pairs), ragged everything
     ("resident_reuse", "c3", dict(P=2100, N=31, d=9, M=1111)),
+    # more features than the old 32 / 16 limits (x is read straight from global memory)
+    ("wide_cheb", "c3", dict(P=900, N=44, d=10, M=140)),
+    ("wide_trig", "c2", dict(P=700, N=27, d=5, M=70)),
+    ("huge_G_641", "c3", dict(P=600, N=64, d=10, M=70)),      # beyond the FFMA kernel's G <= 448: tensor path only
 ]
 
 
@@ -73,6 +77,8 @@ def case_cfg(base, over):
 @pytest.mark.parametrize("name,base,over", FITNESS_CASES, ids=[c[0] for c in FITNESS_CASES])
 def test_fitness_matches_oracle(game, name, base, over, scheme):
     cfg = case_cfg(base, over)
+    if scheme == 1 and cfg.G > 448:
+        pytest.skip("the FFMA kernel covers G <= 448")
     X, t, _ = wl.make_kb(cfg)
     W = wl.uniform_population(cfg.M, cfg.G, seed=100 + cfg.seed)
     G = make(game, cfg, scheme)
