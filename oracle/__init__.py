@@ -88,6 +88,8 @@ def lib() -> C.CDLL:
         L.oracle_step_sel.restype = C.c_int
         L.oracle_step_sel.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_float,
                                       C.c_uint64, C.c_uint32, f32p, f32p, f32p]
+        L.oracle_eval_rmse.restype = C.c_int
+        L.oracle_eval_rmse.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, f32p, f32p, f32p, f64p]
         L.oracle_immigrate.restype = C.c_int
         L.oracle_immigrate.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint64, C.c_uint32, f32p]
         L.oracle_run_until.restype = C.c_int
@@ -318,3 +320,15 @@ def immigrate(Wn, E: int, R: int, seed: int, gen: int) -> np.ndarray:
     if rc:
         raise ValueError(f"oracle_immigrate failed: {rc}")
     return Wn
+
+
+def eval_rmse(d: int, fam: int, X, t, W) -> np.ndarray:
+    """Root-mean-square error per chromosome."""
+    X, t, W = _f32(X), _f32(t), _f32(W)
+    P, N = X.shape
+    M, G = W.shape
+    F = np.empty(M, dtype=np.float64)
+    rc = lib().oracle_eval_rmse(P, N, d, M, fam, _p(X, C.c_float), _p(t, C.c_float), _p(W, C.c_float), _p(F, C.c_double))
+    if rc:
+        raise ValueError(f"oracle_eval_rmse failed: {rc}")
+    return F

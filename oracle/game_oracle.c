@@ -568,3 +568,13 @@ int oracle_immigrate(int M, int G, int E, int R, uint64_t seed, uint32_t gen, fl
         }
     return 0;
 }
+
+
+/* ---- RMSE  ("the MSE or the RMSE may be used"): F_rmse[m] = sqrt((1/P) sum_p (y - t)^2), in double. */
+int oracle_eval_rmse(int64_t P, int N, int d, int M, int family, const float *X, const float *t, const float *W, double *F)
+{
+    int rc = oracle_eval_fitness(P, N, d, M, family, X, t, W, F, NULL);
+    if (rc) return rc;
+    for (int m = 0; m < M; ++m) F[m] = sqrt(F[m]);
+    return 0;
+}

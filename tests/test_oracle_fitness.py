@@ -394,3 +394,18 @@ def test_confusion_counts_brute_force_and_identities():
     assert (tp, fp, tn, fn) == (int(np.sum(pred & (t > 0.5))), int(np.sum(pred & (t <= 0.5))),
                                 int(np.sum(~pred & (t <= 0.5))), int(np.sum(~pred & (t > 0.5))))
     assert tp + fp + tn + fn == 1000 and oracle.confusion(t.astype(np.float64), t, 0.5) == (int(t.sum()), 0, int(1000 - t.sum()), 0)
+
+
+def test_rmse_closed_forms():
+    """RMSE: W = 0 on 0/1 labels -> exactly 0.5; it is the Euclidean norm of the residual / sqrt(P)
+    (numpy.linalg.norm, a library routine) and orders chromosomes exactly as the MSE does."""
+    import workloads as wl
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=500, M=12)
+    X, t, _ = wl.make_kb(cfg)
+    assert np.all(oracle.eval_rmse(cfg.d, cfg.family, X, t, np.zeros((3, cfg.G), np.float32)) == 0.5)
+    W = wl.uniform_population(cfg.M, cfg.G, 2)
+    R = oracle.eval_rmse(cfg.d, cfg.family, X, t, W)
+    for m in range(cfg.M):
+        y = oracle.predict(cfg.d, cfg.family, X, W[m])
+        assert abs(R[m] - np.linalg.norm(y - t) / np.sqrt(cfg.P)) <= 1e-14
+    assert np.array_equal(np.argsort(R, kind="stable"), np.argsort(oracle.eval_fitness(cfg.d, cfg.family, X, t, W), kind="stable"))
