@@ -122,6 +122,12 @@ int game_set_ga_params(game_ctx* ctx, int32_t elite, int32_t tournament, double 
 enum { GAME_SEL_TOURNAMENT = 0, GAME_SEL_RANKING = 1, GAME_SEL_ROULETTE = 2 };
 int game_set_selection(game_ctx* ctx, int32_t selection);
 
+/* Error metric written to fitness_dev ("the MSE or the RMSE may be used"): MSE (default) or
+ * RMSE = sqrt(MSE), taken in fp64 before the single rounding to fp32.  Lower is better either way (the GA order is the
+ * same); the threshold of game_run_until is compared against the chosen metric.  Invalidates the fitness. */
+enum { GAME_ERROR_MSE = 0, GAME_ERROR_RMSE = 1 };
+int game_set_error_metric(game_ctx* ctx, int32_t metric);
+
 /* Random replacement ("a variable number of chromosomes are randomly generated to replace older
  * individuals"; R12): the last `immigrants` child slots of every game_step (never elite slots:
  * 0 <= immigrants <= M - elite, checked against the current elite count; clamped again if elite grows later) are

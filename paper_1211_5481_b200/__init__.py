@@ -17,6 +17,7 @@ EXP_CHEBYSHEV, EXP_TRIG = 0, 1
 ACT_IDENTITY, ACT_SIGMOID, ACT_TANH = 0, 1, 2
 SCHEME_AUTO, SCHEME_FFMA, SCHEME_F16X3 = 0, 1, 2
 SEL_TOURNAMENT, SEL_RANKING, SEL_ROULETTE = 0, 1, 2
+ERROR_MSE, ERROR_RMSE = 0, 1
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_WORKSPACE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -37,6 +38,7 @@ SIGNATURES = {
     "game_set_ga_params": (C.c_int, [_VP, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_float]),
     "game_set_selection": (C.c_int, [_VP, C.c_int32]),
     "game_set_immigrants": (C.c_int, [_VP, C.c_int32]),
+    "game_set_error_metric": (C.c_int, [_VP, C.c_int32]),
     "game_init_population": (C.c_int, [_VP, C.c_uint64]),
     "game_current_population": (C.c_int, [_VP, C.POINTER(C.c_void_p)]),
     "game_invalidate_fitness": (C.c_int, [_VP]),
@@ -141,6 +143,10 @@ def game_bind_state(ctx, popA_dev: int, popB_dev: int, fitness_dev: int, workspa
 
 def game_set_ga_params(ctx, elite: int, tournament: int, p_cross: float, p_mut: float, sigma: float) -> None:
     _check(ctx, lib().game_set_ga_params(ctx, elite, tournament, p_cross, p_mut, sigma))
+
+
+def game_set_error_metric(ctx, metric: int) -> None:
+    _check(ctx, lib().game_set_error_metric(ctx, metric))
 
 
 def game_set_immigrants(ctx, immigrants: int) -> None:

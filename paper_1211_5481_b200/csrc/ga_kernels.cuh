@@ -248,7 +248,7 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
                                                                         float* __restrict__ blk_key,
                                                                         int* __restrict__ blk_idx,
                                                                         unsigned int* __restrict__ ticket,
-                                                                        int* __restrict__ stop, float threshold, int gen_index) {
+                                                                        int* __restrict__ stop, float threshold, int gen_index, int rmse) {
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
     __shared__ bool s_last;
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         if (sse_out != nullptr) {            // pattern-sharded evaluation: hand out the un-normalised sum instead
             sse_out[m] = s;
         } else {
-            const float f = static_cast<float>(s / P_d);
+            const float f = static_cast<float>(rmse ? sqrt(s / P_d) : s / P_d);   // MSE or RMSE
             F[m] = f;
             key = fit_key(f);
             idx = m;

@@ -46,7 +46,7 @@ struct game_ctx {
     bool fitness_valid = false;
     bool ticket_zeroed = false;
     // GA parameters
-    int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0;
+    int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0, rmse = 0;
     double p_cross = 0.9, p_mut = 0.05;
     float sigma = 0.1f;
     // execution
@@ -259,7 +259,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     finalize_fitness_kernel<<<fin_blocks, kFinThreads, 0, c->stream>>>(
         part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index);
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index, c->rmse);
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
     c->fitness_valid = sse_out == nullptr;
     return GAME_OK;
@@ -425,6 +425,14 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
     return GAME_OK;
 }
 
+int game_set_error_metric(game_ctx* c, int32_t metric) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (metric != GAME_ERROR_MSE && metric != GAME_ERROR_RMSE) return fail(c, GAME_ERR_INVALID_ARG, "unknown error metric %d", metric);
+    c->rmse = metric == GAME_ERROR_RMSE ? 1 : 0;
+    c->fitness_valid = false;
+    return GAME_OK;
+}
+
 int game_set_immigrants(game_ctx* c, int32_t immigrants) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (immigrants < 0 || immigrants > c->M - c->elite)
@@ -578,7 +586,7 @@ int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_tota
     game::finalize_fitness_kernel<<<fin_blocks, game::kFinThreads, 0, c->stream>>>(
         sse_dev, 1, c->M, c->M, static_cast<double>(P_total), c->fitness, nullptr, best_fitness_dev,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), nullptr, 0.f, 0);
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), nullptr, 0.f, 0, c->rmse);
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
     c->fitness_valid = true;
     return GAME_OK;

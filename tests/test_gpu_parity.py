@@ -518,3 +518,21 @@ def test_ga_step_with_random_immigrants_bit_exact(game, selection, M, E, R):
     ref = oracle.immigrate(oracle.step_sel(W, F, E, 3, selection, 0.9, 0.2, 0.1, 31, 8), E, R, 31, 8)
     assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
     G.close()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_rmse_metric(game, scheme):
+    """game_set_error_metric(RMSE): fitness_dev = sqrt(MSE) within 1e-5 of the oracle's RMSE; the GA step on
+    it is bit-exact (the operators only see a fitness vector)."""
+    cfg = wl.scaled(wl.CONFIGS["c2"], P=2300, M=140)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 14)
+    G = make(game, cfg, scheme); G.load_kb(X, t); G.set_population(W)
+    game.game_set_error_metric(G.ctx, game.ERROR_RMSE)
+    G.eval_fitness(); G.sync()
+    F = G.get_fitness()
+    assert_fitness_close(F, oracle.eval_rmse(cfg.d, cfg.family, X, t, W), "rmse")
+    G.step(3, 1); G.sync()
+    ref = oracle.step(W, F, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 3, 1)
+    assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
+    G.close()
