@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--scheme", default="auto", choices=["auto", "ffma", "f16x3"])
     ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
                     help="N > 1: independent replicas (default), or ONE population over pattern shards with an all-reduce of M sums per generation")
+    ap.add_argument("--fused", action="store_true",
+                    help="small problems: time game_evolve_fused (the whole generation loop as one persistent kernel)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -211,6 +213,9 @@ def run_ours(args, cfg, rank, world, local_rank):
     sse = torch.zeros(cfg.M, dtype=torch.float64, device=dev) if shard else None
 
     def generations(first_gen, n):
+        if args.fused:
+            game.game_evolve_fused(G.ctx, seed, first_gen, n, None)   # one persistent kernel for all n generations
+            return
         if not shard:
             game.game_evolve(G.ctx, seed, first_gen, n)      # n x (fused fitness eval, GA step): launches only
             return
@@ -281,11 +286,16 @@ def run_ours(args, cfg, rank, world, local_rank):
 
     # ---------------- roofline of the dominant kernel (fused fitness)
     peaks, peaks_src = load_peaks()
-    flops_per_launch = (6.0 * cfg.P * cfg.M * (cfg.G - 1) if G.scheme() == game.SCHEME_F16X3      # 3 MMAs per gene; the bias gene rides on the epilogue
-                        else 2.0 * cfg.P * cfg.M * cfg.G)
+    fused = args.fused
+    if fused:      # one persistent kernel = the whole timed region: fp32 FFMA arithmetic, 2 P M G flop per generation
+        flops_per_launch = 2.0 * cfg.P * cfg.M * cfg.G * args.steps
+        kernel_ms, kernel_n = ms, 1
+    else:
+        flops_per_launch = (6.0 * cfg.P * cfg.M * (cfg.G - 1) if G.scheme() == game.SCHEME_F16X3      # 3 MMAs per gene; the bias gene rides on the epilogue
+                            else 2.0 * cfg.P * cfg.M * cfg.G)
     avg_s = kernel_ms * 1e-3 / max(kernel_n, 1)
     achieved = flops_per_launch / avg_s / 1e12
-    if G.scheme() == game.SCHEME_F16X3:
+    if G.scheme() == game.SCHEME_F16X3 and not fused:
         peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
         peak_note = (f"{peaks_src} bf16_tflops_sustained (fp16 and bf16 share the kind::f16 rate; the kernel is timed "
                      f"inside a {ms / 1e3:.2f} s step loop); burst figure {peaks['bf16_tflops']}")
@@ -295,7 +305,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         peak_note = "derived fp32 FFMA peak: 148 SM x 128 lanes x 2 flop x 1.965 GHz"
         bound = "alu"
     roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel": "fitness_umma_kernel" if bound == "tensor" else "fitness_ffma_kernel",
+                "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel": "ga_fused_kernel" if fused else ("fitness_umma_kernel" if bound == "tensor" else "fitness_ffma_kernel"),
                 "kernel_ms_avg": avg_s * 1e3, "kernel_launches_timed": kernel_n, "kernel_share_of_step": kernel_ms / ms,
                 "flops_per_launch": flops_per_launch, "peak_source": peak_note,
                 "hbm_algorithmic_bytes_per_launch": 4 * (cfg.P * (cfg.N + 1)),

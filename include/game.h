@@ -184,6 +184,16 @@ int game_run_until(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t max_gen
  * what bench.py times as "K steps".  Async. */
 int game_evolve(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens);
 
+/* game_evolve as ONE persistent kernel for the latency-bound regime of the paper's own experiments (PAPER.md:120-136:
+ * 2100 patterns, a few dozen chromosomes, thousands of iterations): a cooperative grid of one CTA per SM expands its
+ * slice of the patterns once, then runs n_gens x (fitness, GA step) with two grid barriers per generation and no kernel
+ * launch in between.  fp32 FFMA arithmetic (the FFMA scheme's accuracy); the GA operators, selection method, immigrants
+ * and RMSE setting are those of game_step, bit for bit, on the fitness the kernel itself computed.  best_fitness_dev
+ * ([n_gens] device, or NULL) receives the best fitness of every evaluated generation; fitness_dev is left holding the
+ * fitness of the LAST evaluated population (the one before the final step).  Covers M <= 1024, P*M*G <= 2e8 and a
+ * per-CTA slice that fits 200 KB of shared memory; otherwise GAME_ERR_UNSUPPORTED (use game_evolve).  Async. */
+int game_evolve_fused(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev);
+
 /* Stream synchronise; returns GAME_ERR_CUDA if any enqueued work failed. */
 int game_sync(game_ctx* ctx);
 

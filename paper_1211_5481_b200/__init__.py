@@ -48,6 +48,7 @@ SIGNATURES = {
     "game_run": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, _F32P]),
     "game_run_until": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, C.c_float, _F32P, _VP]),
     "game_evolve": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32]),
+    "game_evolve_fused": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, _F32P]),
     "game_sync": (C.c_int, [_VP]),
     "game_generation_host": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, _F32P, C.c_uint64, C.c_uint32]),
     "game_eval_sse": (C.c_int, [_VP, _VP]),
@@ -194,6 +195,10 @@ def game_run_until(ctx, seed: int, gen0: int, max_gens: int, threshold: float, b
 
 def game_evolve(ctx, seed: int, gen0: int, n_gens: int) -> None:
     _check(ctx, lib().game_evolve(ctx, seed, gen0, n_gens))
+
+
+def game_evolve_fused(ctx, seed: int, gen0: int, n_gens: int, best_fitness_dev: int | None = None) -> None:
+    _check(ctx, lib().game_evolve_fused(ctx, seed, gen0, n_gens, best_fitness_dev))
 
 
 def game_sync(ctx) -> None:

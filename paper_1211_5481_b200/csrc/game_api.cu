@@ -15,6 +15,7 @@
 #include "fitness_umma.cuh"
 #include "ga_kernels.cuh"
 #include "predict.cuh"
+#include "ga_fused.cuh"
 
 namespace {
 
@@ -35,7 +36,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -331,6 +332,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_stop = off; off = align_up(off + 2 * sizeof(int));
     c->off_by_rank = off; off = align_up(off + sizeof(int) * static_cast<size_t>(M));
     c->off_prefix = off; off = align_up(off + sizeof(unsigned long long) * static_cast<size_t>(M));
+    c->off_fused_bar = off; off = align_up(off + sizeof(unsigned int));
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
@@ -523,6 +525,51 @@ int game_run_until(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t max_gens,
     if (rc != GAME_OK) return rc;
     GAME_CUDA(cudaMemcpyAsync(gens_done_dev, stop + 1, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
     c->fitness_valid = true;     // the fitness of the final population (of the stopping generation, or of generation max_gens)
+    return GAME_OK;
+}
+
+int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev) {
+    using namespace game;
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_fused before game_load_kb");
+    if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_fused before game_bind_state");
+    if (n_gens == 0) return GAME_OK;
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    // few CTAs for tiny problems: the two grid barriers per generation, not the arithmetic, set the pace
+    const double work = static_cast<double>(c->P) * c->M * c->G;
+    int grid = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+    const int by_work = static_cast<int>(work / 65536.0) + 1;
+    const int floor_ctas = c->M < grid ? (c->M < 8 ? 8 : c->M) : grid;      // at least one CTA per child slot
+    if (by_work < grid) grid = by_work < floor_ctas ? floor_ctas : by_work;
+    if (grid > c->P) grid = static_cast<int>(c->P);
+    const int ppc = static_cast<int>((c->P + grid - 1) / grid);
+    const size_t smem = sizeof(float) * (static_cast<size_t>(ppc) * c->G + static_cast<size_t>(c->M) * c->G + ppc + c->M) +
+                        sizeof(int) * static_cast<size_t>(c->M) + 8 + sizeof(unsigned long long) * static_cast<size_t>(c->M);
+    if (c->M > kFusedMaxM || smem > 200u * 1024u || work > 2e8)
+        return fail(c, GAME_ERR_UNSUPPORTED, "game_evolve_fused covers M <= 1024, P*M*G <= 2e8 and %zu KB <= 200 KB of shared memory per CTA", smem >> 10);
+    GAME_CUDA(cudaFuncSetAttribute(ga_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+    FusedParams prm;
+    prm.X = c->X; prm.t = c->t; prm.pop[0] = c->pop[0]; prm.pop[1] = c->pop[1]; prm.F = c->fitness;
+    prm.part = reinterpret_cast<double*>(c->ws + c->off_part);
+    prm.best = best_fitness_dev;
+    prm.barrier = reinterpret_cast<unsigned int*>(c->ws + c->off_fused_bar);
+    prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
+    prm.expansion = c->expansion; prm.act = c->act; prm.rmse = c->rmse;
+    prm.cur = c->cur; prm.n_gens = static_cast<int>(n_gens); prm.ppc = ppc;
+    prm.ga.M = c->M; prm.ga.G = c->G; prm.ga.elite = c->elite; prm.ga.tournament = c->tournament;
+    prm.ga.t_cross = bernoulli_threshold(c->p_cross);
+    prm.ga.t_mut = bernoulli_threshold(c->p_mut);
+    prm.ga.sigma = c->sigma; prm.ga.gen = gen0; prm.ga.key = make_key(seed);
+    prm.ga.selection = c->selection;
+    prm.ga.immigrants = c->immigrants < c->M - c->elite ? c->immigrants : c->M - c->elite;
+    prm.ga.by_rank = nullptr; prm.ga.prefix = nullptr;
+    GAME_CUDA(cudaMemsetAsync(prm.barrier, 0, sizeof(unsigned int), c->stream));
+    void* args[] = {&prm};
+    GAME_CUDA(cudaLaunchCooperativeKernel(reinterpret_cast<void*>(ga_fused_kernel), dim3(grid), dim3(kFusedThreads), args, smem, c->stream));
+    if ((rc = check_launch(c, "ga_fused_kernel"))) return rc;
+    if (n_gens & 1u) c->cur ^= 1;
+    c->fitness_valid = false;
     return GAME_OK;
 }
 

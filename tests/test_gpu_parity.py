@@ -536,3 +536,46 @@ def test_rmse_metric(game, scheme):
     ref = oracle.step(W, F, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 3, 1)
     assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ fused persistent loop
+@pytest.mark.parametrize("base,over,selection,immigrants", [
+    ("c0", {}, 0, 0), ("c0", dict(P=777, M=37), 1, 3), ("n1", {}, 1, 0), ("n1", dict(P=500, M=23), 2, 2),
+    ("c1", dict(P=3001, M=50), 0, 0)])
+def test_evolve_fused_lockstep_and_determinism(game, base, over, selection, immigrants):
+    """game_evolve_fused (one persistent cooperative kernel).  Lock-step, one generation per call: the
+    fitness it leaves in fitness_dev is within 1e-5 of the oracle's for the same population and the next population is
+    bit-identical to the oracle's step on THAT fitness vector; n generations in one launch == n launches of one."""
+    import torch
+    cfg = wl.scaled(wl.PAPER_SHAPE if base == "n1" else wl.CONFIGS[base], **over)
+    X, t, _ = wl.make_kb(cfg)
+    seed, n = 5, 6
+    G = make(game, cfg); G.load_kb(X, t)
+    game.game_set_selection(G.ctx, selection); game.game_set_immigrants(G.ctx, immigrants)
+    G.init_population(seed); G.sync()
+    W = G.get_population()
+    bests = []
+    for g in range(n):
+        game.game_evolve_fused(G.ctx, seed, g, 1, None); G.sync()
+        F = G.get_fitness()
+        assert_fitness_close(F, oracle.eval_fitness(cfg.d, cfg.family, X, t, W), f"fused gen {g}")
+        bests.append(F[oracle.best_index(F)])
+        W = oracle.immigrate(oracle.step_sel(W, F, cfg.elite, cfg.tournament, selection, cfg.p_cross, cfg.p_mut, cfg.sigma,
+                                             seed, g), cfg.elite, immigrants, seed, g)
+        assert np.array_equal(G.get_population().view(np.uint32), W.view(np.uint32)), f"population forked at gen {g}"
+    with pytest.raises(game.GameError):
+        G.step(seed, 0)                                    # the population is one step past its last fitness
+    G.init_population(seed)
+    best = torch.full((n,), float("nan"), dtype=torch.float32, device="cuda")
+    game.game_evolve_fused(G.ctx, seed, 0, n, best.data_ptr()); G.sync()
+    assert np.array_equal(G.get_population().view(np.uint32), W.view(np.uint32))
+    assert np.array_equal(best.cpu().numpy(), np.asarray(bests, np.float32))
+    G.close()
+
+
+def test_evolve_fused_rejects_big_problems(game):
+    G = game.Game(100_000, 10, 6, 512, wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    with pytest.raises(game.GameError) as e:
+        game.game_evolve_fused(G.ctx, 1, 0, 1, None)
+    assert e.value.code == game.ERR_UNSUPPORTED
+    G.close()
