@@ -40,7 +40,7 @@ UNIT = "evals/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists).
-NCU_TRAFFIC_BYTES = {"c3": 544669440}      # profiles/r01c_README.md: 535.2 MB read + 9.5 MB written
+NCU_TRAFFIC_BYTES = {"c3": 546192640}      # profiles/r01d_README.md: 536.5 MB read + 9.7 MB written
 
 
 def parse_args():
