@@ -64,6 +64,8 @@ FITNESS_CASES = [
     # more features than the old 32 / 16 limits (x is read straight from global memory)
     ("wide_cheb", "c3", dict(P=900, N=44, d=10, M=140)),
     ("wide_trig", "c2", dict(P=700, N=27, d=5, M=70)),
+    ("stream_tail", "c3", dict(P=800, N=24, d=14, M=150)),       # streaming, 21 K steps: last stage holds 1 of 4 steps
+    ("stream_tail_trig", "c2", dict(P=800, N=24, d=7, M=150)),   # streaming trig, 21 K steps
     ("huge_G_641", "c3", dict(P=600, N=64, d=10, M=70)),      # beyond the FFMA kernel's G <= 448: tensor path only
 ]
 
