@@ -23,8 +23,9 @@ SEL_TOURNAMENT, SEL_RANKING, SEL_ROULETTE = 0, 1, 2
 ACT_IDENTITY, ACT_SIGMOID, ACT_TANH = 0, 1, 2
 
 
-def family(expansion: int, activation: int) -> int:
-    return expansion | (activation << 8)
+def family(expansion: int, activation: int, shared: bool = False) -> int:
+    """shared = the paper's literal form: one coefficient per degree for ALL features (eq.(2))."""
+    return expansion | (activation << 8) | (int(shared) << 16)
 
 
 def build(force: bool = False) -> str:

@@ -44,9 +44,10 @@
 int oracle_num_genes(int N, int d, int family)
 {
     int expansion = family & 0xff;
-    if (N < 1 || d < 1) return -1;
-    if (expansion == EXP_CHEBYSHEV) return N * d + 1;
-    if (expansion == EXP_TRIG) return N * 2 * d + 1;
+    int shared = (family >> 16) & 1;    /* PAPER.md:52-55 eq.(2) literally: coefficients shared by all features */
+    if (N < 1 || d < 1 || (family >> 17) != 0) return -1;
+    if (expansion == EXP_CHEBYSHEV) return (shared ? 1 : N) * d + 1;
+    if (expansion == EXP_TRIG) return (shared ? 1 : N) * 2 * d + 1;
     return -1;
 }
 
@@ -70,6 +71,33 @@ void oracle_paper_shapes(int N, int d, int B, int *num_chromosomes, int *num_gen
 void oracle_expand(int N, int d, int family, const float *x, double *phi)
 {
     int expansion = family & 0xff;
+    if ((family >> 16) & 1) {
+        /* Shared coefficients, the paper's own form (eq.(2), 75-77 eq.(5), 84-89 eq.(7)):
+         * Out = a_0 + sum_j a_j sum_i g_j(f_i), so the expansion term of gene j is the SUM over the features --
+         * the per-pattern sums of cosines and sines that the paper precomputes once.
+         * Gene order [a_0, a_1..a_d] (Chebyshev) or [a_0, a_1..a_d, b_1..b_d] (trig). */
+        int G = oracle_num_genes(N, d, family);
+        phi[0] = 1.0;
+        for (int g = 1; g < G; ++g) phi[g] = 0.0;
+        for (int i = 0; i < N; ++i) {
+            double xi = (double)x[i];
+            if (expansion == EXP_CHEBYSHEV) {
+                double tjm1 = 1.0, tj = xi;
+                for (int j = 1; j <= d; ++j) {
+                    phi[j] += tj;
+                    double tn = 2.0 * xi * tj - tjm1;
+                    tjm1 = tj;
+                    tj = tn;
+                }
+            } else {
+                for (int k = 1; k <= d; ++k) {
+                    phi[k] += cos((double)k * xi);
+                    phi[d + k] += sin((double)k * xi);
+                }
+            }
+        }
+        return;
+    }
     phi[0] = 1.0;
     if (expansion == EXP_CHEBYSHEV) {
         for (int i = 0; i < N; ++i) {

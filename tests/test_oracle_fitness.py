@@ -409,3 +409,42 @@ def test_rmse_closed_forms():
         y = oracle.predict(cfg.d, cfg.family, X, W[m])
         assert abs(R[m] - np.linalg.norm(y - t) / np.sqrt(cfg.P)) <= 1e-14
     assert np.array_equal(np.argsort(R, kind="stable"), np.argsort(oracle.eval_fitness(cfg.d, cfg.family, X, t, W), kind="stable"))
+
+
+# ------------------------------------------------------------------------------------------------ shared coefficients
+def _golden_example():
+    path = os.path.join(os.path.dirname(__file__), "golden", "paper_worked_example.txt")
+    return dict(l.split(None, 1) for l in open(path) if l.strip() and not l.startswith("#"))
+
+
+def test_shared_mode_is_the_papers_worked_example_shape():
+    """11 features, degree 3, polytrigo (B = 2) -> 7 genes [a0,a1,a2,a3,b1,b2,b3], 23 chromosomes."""
+    ex = _golden_example()
+    N, d = int(ex["features"]), int(ex["degree"])
+    fam = oracle.family(oracle.EXP_TRIG, oracle.ACT_IDENTITY, shared=True)
+    assert oracle.num_genes(N, d, fam) == int(ex["num_genes"]) == 7
+    assert oracle.paper_shapes(N, d, int(ex["B"])) == (int(ex["num_chromosomes"]), int(ex["num_genes"]))
+    assert oracle.num_genes(N, d, oracle.family(oracle.EXP_CHEBYSHEV, 0, shared=True)) == d + 1
+    # gene order: a unit gene at position g picks out the documented term -- a_k -> sum_i cos(k x_i), b_k -> sum_i sin(k x_i)
+    x = np.linspace(-2.5, 2.5, N).astype(np.float32)
+    for g, name in enumerate(ex["gene_order"].split()):
+        w = np.zeros(7, np.float32); w[g] = 1.0
+        k = int(name[1])
+        want = 1.0 if name == "a0" else float(np.sum((np.cos if name[0] == "a" else np.sin)(k * x.astype(np.float64))))
+        assert abs(oracle.output(N, d, fam, x, w) - want) <= 1e-13, name
+
+
+@pytest.mark.parametrize("expansion,act", [(0, 1), (1, 2), (1, 0)])
+def test_shared_mode_equals_per_feature_model_with_tied_genes(expansion, act):
+    """eq.(2) shares a_j across the features: the shared model must equal the per-feature model (BASELINE form, D1)
+    whose genes are tied across features -- two code paths, one number."""
+    rng = np.random.Generator(np.random.Philox(12))
+    P, N, d, M = 300, 6, 4, 5
+    X = rng.uniform(-1, 1, (P, N)).astype(np.float32)
+    t = rng.uniform(0, 1, P).astype(np.float32)
+    B = 2 if expansion == 1 else 1
+    Ws = rng.uniform(-1, 1, (M, B * d + 1)).astype(np.float32)
+    Wp = np.concatenate([Ws[:, :1]] + [Ws[:, 1:]] * N, axis=1)          # [a0 | block | block | ...]
+    Fs = oracle.eval_fitness(d, oracle.family(expansion, act, shared=True), X, t, Ws)
+    Fp = oracle.eval_fitness(d, oracle.family(expansion, act), X, t, Wp)
+    assert np.max(np.abs(Fs - Fp) / Fp) <= 1e-12
