@@ -48,10 +48,15 @@ enum {
     GAME_ERR_UNSUPPORTED = -5  /* shape outside what the kernels cover (stated per call)  */
 };
 
-/* family = expansion | (activation << 8)                                     [DESIGN.md D2]
+/* family = expansion | (activation << 8) | (shared << 16)                    [DESIGN.md D1, D2]
  *   expansion : 0 CHEBYSHEV (T_1..T_d, eq.(1)), 1 TRIG (cos/sin k=1..d, eq.(6))
  *   activation: 0 IDENTITY (the paper's raw sum, eq.(2)), 1 SIGMOID, 2 TANH (BASELINE.json)
+ *   shared    : 0 per-feature coefficients (BASELINE.json: G = N*d+1 / N*2d+1), 1 the paper's literal form (PAPER.md:52-55
+ *               eq.(2), 75-77 eq.(5), 84-89): ONE coefficient per degree for all features, G = d+1 (Chebyshev) or 2d+1
+ *               (trig, gene order [a_0, a_1..a_d, b_1..b_d]); the expansion term of gene j is the sum over the features of
+ *               g_j(f_i) (the per-pattern sums of PAPER.md:110).  Shared mode runs on the FFMA scheme and the fused loop.
  * BASELINE.json configs c0,c1,c3,c4 = 0x0100; c2 = 0x0201. */
+enum { GAME_FAMILY_SHARED = 1 << 16 };
 enum { GAME_EXP_CHEBYSHEV = 0, GAME_EXP_TRIG = 1 };
 enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
 

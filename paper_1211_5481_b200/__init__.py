@@ -85,8 +85,8 @@ def lib() -> C.CDLL:
     return _lib
 
 
-def family(expansion: int, activation: int) -> int:
-    return expansion | (activation << 8)
+def family(expansion: int, activation: int, shared: bool = False) -> int:
+    return expansion | (activation << 8) | (int(shared) << 16)
 
 
 def _check(ctx, rc: int) -> None:
@@ -255,7 +255,7 @@ class Game:
     """
 
     def __init__(self, P: int, N: int, d: int, M: int, expansion: int, activation: int, device="cuda:0",
-                 scheme: int = SCHEME_AUTO):
+                 scheme: int = SCHEME_AUTO, shared: bool = False):
         import torch
 
         if not torch.cuda.is_available():
@@ -263,7 +263,7 @@ class Game:
         self.torch = torch
         self.device = torch.device(device)
         self.P, self.N, self.d, self.M = P, N, d, M
-        self.ctx = game_create(P, N, d, M, family(expansion, activation))
+        self.ctx = game_create(P, N, d, M, family(expansion, activation, shared))
         self.G = game_num_genes(self.ctx)
         with torch.cuda.device(self.device):
             self.X = torch.empty((P, N), dtype=torch.float32, device=self.device)

@@ -24,13 +24,50 @@ __device__ __forceinline__ float activate(int act, float z) {
     return z;
 }
 
+// phi(x) of ONE pattern into dst[g * stride] (gene order of include/game.h).  shared = the paper's literal form
+// (eq.(2), 75-77 eq.(5)): one coefficient per degree for ALL features, so the term of gene j is the sum
+// over the features of g_j(f_i) -- the per-pattern sums of cosines / sines the paper precomputes.
+__device__ __forceinline__ void expand_pattern(const float* __restrict__ xr, bool valid, int N, int d, int expansion,
+                                               int shared, float* __restrict__ dst, int stride) {
+    dst[0] = 1.0f;  // gene 0: bias a_0
+    const int terms = expansion == 0 ? d : 2 * d;
+    if (shared)
+        for (int g = 1; g <= terms; ++g) dst[g * stride] = 0.0f;
+    for (int i = 0; i < N; ++i) {
+        const float x = valid ? xr[i] : 0.0f;
+        float* blk = dst + (1 + (shared ? 0 : i * terms)) * stride;
+        if (expansion == 0) {
+            const float x2 = 2.0f * x;
+            float tm = 1.0f, tc = x;
+            for (int j = 0; j < d; ++j) {
+                blk[j * stride] = shared ? blk[j * stride] + tc : tc;
+                const float tn = fmaf(x2, tc, -tm);
+                tm = tc;
+                tc = tn;
+            }
+        } else {
+            float s1, c1;
+            sincosf(x, &s1, &c1);
+            const float x2 = 2.0f * c1;
+            float cm = 1.0f, cc = c1, sm = 0.0f, sc = s1;
+            for (int k = 0; k < d; ++k) {
+                blk[k * stride] = shared ? blk[k * stride] + cc : cc;
+                blk[(d + k) * stride] = shared ? blk[(d + k) * stride] + sc : sc;
+                const float cn = fmaf(x2, cc, -cm), sn = fmaf(x2, sc, -sm);
+                cm = cc; cc = cn;
+                sm = sc; sc = sn;
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(kFfmaTile) fitness_ffma_kernel(const float* __restrict__ X,
                                                                   const float* __restrict__ t,
                                                                   const float* __restrict__ W,
                                                                   double* __restrict__ part, long long P, int N,
                                                                   int d, int M, int G, int expansion, int act,
                                                                   int m_stride, long long n_tiles,
-                                                                  const int* __restrict__ stop) {
+                                                                  const int* __restrict__ stop, int shared) {
     if (stop != nullptr && *stop != 0) return;
     extern __shared__ float phi[];  // [G][128]
     __shared__ float s_wsum[kFfmaTile / 32][kFfmaMB];
@@ -43,35 +80,7 @@ __global__ void __launch_bounds__(kFfmaTile) fitness_ffma_kernel(const float* __
         const long long p = tile * kFfmaTile + tid;
         const bool valid = p < P;
         const float* xr = X + (valid ? p : 0) * N;
-        phi[tid] = 1.0f;  // gene 0: bias a_0
-        if (expansion == 0) {
-            for (int i = 0; i < N; ++i) {
-                const float x = valid ? xr[i] : 0.0f;
-                const float x2 = 2.0f * x;
-                float tm = 1.0f, tc = x;
-                for (int j = 0; j < d; ++j) {
-                    phi[(1 + i * d + j) * kFfmaTile + tid] = tc;
-                    const float tn = fmaf(x2, tc, -tm);
-                    tm = tc;
-                    tc = tn;
-                }
-            }
-        } else {
-            for (int i = 0; i < N; ++i) {
-                const float x = valid ? xr[i] : 0.0f;
-                float s1, c1;
-                sincosf(x, &s1, &c1);
-                const float x2 = 2.0f * c1;
-                float cm = 1.0f, cc = c1, sm = 0.0f, sc = s1;
-                for (int k = 0; k < d; ++k) {
-                    phi[(1 + i * 2 * d + k) * kFfmaTile + tid] = cc;
-                    phi[(1 + i * 2 * d + d + k) * kFfmaTile + tid] = sc;
-                    const float cn = fmaf(x2, cc, -cm), sn = fmaf(x2, sc, -sm);
-                    cm = cc; cc = cn;
-                    sm = sc; sc = sn;
-                }
-            }
-        }
+        expand_pattern(xr, valid, N, d, expansion, shared, phi + tid, kFfmaTile);
         const float tp = valid ? t[p] : 0.0f;
         __syncthreads();
 

@@ -34,7 +34,7 @@ struct FusedParams {
     float* best;              // [n_gens] best fitness of every evaluated generation, or NULL
     unsigned int* barrier;    // zeroed by the host before the launch
     long long P;
-    int N, d, M, G, expansion, act, rmse;
+    int N, d, M, G, expansion, act, rmse, shared;
     int cur, n_gens, ppc;     // ppc = patterns per CTA (contiguous slices)
     GaParams ga;              // gen = first generation index
 };
@@ -76,33 +76,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) ga_fused_kernel(const FusedP
     // ---- setup: expansion of this CTA's patterns, once (gene order of include/game.h)
     for (int q = tid; q < n_mine; q += kFusedThreads) {
         const float* xr = prm.X + (p_begin + q) * prm.N;
-        float* row = phi + static_cast<size_t>(q) * G;
-        row[0] = 1.0f;
-        for (int i = 0; i < prm.N; ++i) {
-            const float x = __ldg(xr + i);
-            if (prm.expansion == 0) {
-                const float x2 = 2.0f * x;
-                float tm = 1.0f, tc = x;
-                for (int j = 0; j < prm.d; ++j) {
-                    row[1 + i * prm.d + j] = tc;
-                    const float tn = fmaf(x2, tc, -tm);
-                    tm = tc;
-                    tc = tn;
-                }
-            } else {
-                float s1, c1;
-                sincosf(x, &s1, &c1);
-                const float x2 = 2.0f * c1;
-                float cm = 1.0f, cc = c1, sm = 0.0f, sc = s1;
-                for (int k = 0; k < prm.d; ++k) {
-                    row[1 + i * 2 * prm.d + k] = cc;
-                    row[1 + i * 2 * prm.d + prm.d + k] = sc;
-                    const float cn = fmaf(x2, cc, -cm), sn = fmaf(x2, sc, -sm);
-                    cm = cc; cc = cn;
-                    sm = sc; sc = sn;
-                }
-            }
-        }
+        expand_pattern(xr, true, prm.N, prm.d, prm.expansion, prm.shared, phi + static_cast<size_t>(q) * G, 1);
         tl[q] = __ldg(prm.t + p_begin + q);
     }
     __syncthreads();

@@ -31,7 +31,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct game_ctx {
     // shapes
     long long P = 0;
-    int N = 0, d = 0, M = 0, G = 0, expansion = 0, act = 0;
+    int N = 0, d = 0, M = 0, G = 0, expansion = 0, act = 0, shared = 0;
     // tensor-core path geometry
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
@@ -143,7 +143,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (rc) return rc;
     const int scheme = resolved_scheme(c);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers d <= 64");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients with d <= 64");
     if (!c->ticket_zeroed) {
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
         c->ticket_zeroed = true;
@@ -251,7 +251,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         n_part = grid;
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
         fitness_ffma_kernel<<<grid, kFfmaTile, smem, c->stream>>>(c->X, c->t, W, part, c->P, c->N, c->d, c->M, c->G,
-                                                                   c->expansion, c->act, c->m_stride, n_tiles, c->stop);
+                                                                   c->expansion, c->act, c->m_stride, n_tiles, c->stop, c->shared);
         if ((rc = check_launch(c, "fitness_ffma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     }
@@ -303,17 +303,17 @@ extern "C" {
 int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int32_t family) {
     if (!out) return GAME_ERR_INVALID_ARG;
     *out = nullptr;
-    const int expansion = family & 0xff, act = (family >> 8) & 0xff;
-    if (P < 1 || N < 1 || d < 1 || M < 1 || (family >> 16) != 0) return GAME_ERR_INVALID_ARG;
+    const int expansion = family & 0xff, act = (family >> 8) & 0xff, shared = (family >> 16) & 1;
+    if (P < 1 || N < 1 || d < 1 || M < 1 || (family >> 17) != 0) return GAME_ERR_INVALID_ARG;
     if (expansion > GAME_EXP_TRIG || act > GAME_ACT_TANH) return GAME_ERR_INVALID_ARG;
     if (P > (1ll << 40) || N > 4096 || d > 4096 || M > (1 << 24)) return GAME_ERR_INVALID_ARG;
-    const long long G = static_cast<long long>(N) * d * (expansion == GAME_EXP_TRIG ? 2 : 1) + 1;
-    const bool umma_ok = d <= 64 && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
+    const long long G = static_cast<long long>(shared ? 1 : N) * d * (expansion == GAME_EXP_TRIG ? 2 : 1) + 1;
+    const bool umma_ok = !shared && d <= 64 && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
     if (G > (1 << 20) || (!umma_ok && G > game::kFfmaMaxG)) return GAME_ERR_UNSUPPORTED;   // FFMA kernel: G <= 448
     game_ctx* c = new (std::nothrow) game_ctx();
     if (!c) return GAME_ERR_INVALID_ARG;
     c->P = P; c->N = N; c->d = d; c->M = M; c->G = static_cast<int>(G);
-    c->expansion = expansion; c->act = act;
+    c->expansion = expansion; c->act = act; c->shared = shared;
     c->m_tiles = 2 * ((M + 2 * game::umma::kBM - 1) / (2 * game::umma::kBM));   // one chromosome tile per CTA of a pair
     c->m_stride = c->m_tiles * game::umma::kBM;
     c->umma_ok = umma_ok;
@@ -372,7 +372,7 @@ int game_set_scheme(game_ctx* c, int32_t scheme) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (scheme < GAME_SCHEME_AUTO || scheme > GAME_SCHEME_F16X3) return fail(c, GAME_ERR_INVALID_ARG, "unknown scheme %d", scheme);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers d <= 64");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients with d <= 64");
     if (scheme == GAME_SCHEME_FFMA && c->G > game::kFfmaMaxG)
         return fail(c, GAME_ERR_UNSUPPORTED, "FFMA covers G <= 448");
     c->scheme = scheme;
@@ -555,7 +555,7 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
     prm.best = best_fitness_dev;
     prm.barrier = reinterpret_cast<unsigned int*>(c->ws + c->off_fused_bar);
     prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
-    prm.expansion = c->expansion; prm.act = c->act; prm.rmse = c->rmse;
+    prm.expansion = c->expansion; prm.act = c->act; prm.rmse = c->rmse; prm.shared = c->shared;
     prm.cur = c->cur; prm.n_gens = static_cast<int>(n_gens); prm.ppc = ppc;
     prm.ga.M = c->M; prm.ga.G = c->G; prm.ga.elite = c->elite; prm.ga.tournament = c->tournament;
     prm.ga.t_cross = bernoulli_threshold(c->p_cross);
@@ -647,7 +647,7 @@ int game_predict(game_ctx* c, const float* w_dev, const float* X_dev, int64_t Q,
     long long blocks = (Q + game::kPredictThreads - 1) / game::kPredictThreads;
     if (blocks > 8ll * c->num_sms) blocks = 8ll * c->num_sms;
     game::predict_kernel<<<static_cast<unsigned>(blocks), game::kPredictThreads, sizeof(float) * c->G, c->stream>>>(
-        X_dev, w_dev, y_dev, Q, c->N, c->d, c->G, c->expansion, c->act);
+        X_dev, w_dev, y_dev, Q, c->N, c->d, c->G, c->expansion, c->act, c->shared);
     return check_launch(c, "predict_kernel");
 }
 

@@ -13,7 +13,7 @@ constexpr int kPredictThreads = 256;
 
 __global__ void __launch_bounds__(kPredictThreads) predict_kernel(const float* __restrict__ X, const float* __restrict__ w,
                                                                    float* __restrict__ y, long long Q, int N, int d, int G,
-                                                                   int expansion, int act) {
+                                                                   int expansion, int act, int shared) {
     extern __shared__ float s_w[];   // [G]
     for (int g = threadIdx.x; g < G; g += kPredictThreads) s_w[g] = w[g];
     __syncthreads();
@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(kPredictThreads) predict_kernel(const float* _
         if (expansion == 0) {
             for (int i = 0; i < N; ++i) {
                 const float x = __ldg(xr + i), x2 = 2.0f * x;
-                const float* wi = s_w + 1 + i * d;
+                const float* wi = s_w + 1 + (shared ? 0 : i * d);           // shared: the same d coefficients for every feature
                 float tm = 1.0f, tc = x;
                 for (int j = 0; j < d; ++j) {
                     z = fmaf(wi[j], tc, z);
@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(kPredictThreads) predict_kernel(const float* _
                 float s1, c1;
                 sincosf(__ldg(xr + i), &s1, &c1);
                 const float x2 = 2.0f * c1;
-                const float* wi = s_w + 1 + i * 2 * d;
+                const float* wi = s_w + 1 + (shared ? 0 : i * 2 * d);
                 float cm = 1.0f, cc = c1, sm = 0.0f, sc = s1;
                 for (int k = 0; k < d; ++k) {
                     z = fmaf(wi[k], cc, z);

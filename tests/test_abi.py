@@ -59,7 +59,7 @@ def test_num_genes_matches_baseline_configs(L):
 
 @pytest.mark.parametrize("args", [
     (0, 4, 3, 64, 0x0100), (10, 0, 3, 64, 0x0100), (10, 4, 0, 64, 0x0100), (10, 4, 3, 0, 0x0100),
-    (10, 4, 3, 64, 0x0002), (10, 4, 3, 64, 0x0300), (10, 4, 3, 64, 0x10100),
+    (10, 4, 3, 64, 0x0002), (10, 4, 3, 64, 0x0300), (10, 4, 3, 64, 0x20100),
 ])
 def test_create_rejects_bad_shapes(L, args):
     ctx = C.c_void_p()
@@ -139,3 +139,15 @@ def test_fails_loudly_without_a_device(L):
     game.game_destroy(ctx)
     with pytest.raises(RuntimeError):
         game.Game(1000, 4, 3, 64, 0, 1)
+
+
+def test_shared_family_gene_counts(L):
+    """The paper's literal form (eq.(5), 84-89): 11 features, degree 3, polytrigo -> 7 genes."""
+    ctx = game.game_create(200, 11, 3, 23, game.family(game.EXP_TRIG, game.ACT_IDENTITY, shared=True))
+    assert game.game_num_genes(ctx) == 7 and game.game_get_scheme(ctx) == game.SCHEME_FFMA
+    with pytest.raises(game.GameError):
+        game.game_set_scheme(ctx, game.SCHEME_F16X3)
+    game.game_destroy(ctx)
+    ctx = game.game_create(200, 11, 3, 23, game.family(game.EXP_CHEBYSHEV, game.ACT_SIGMOID, shared=True))
+    assert game.game_num_genes(ctx) == 4
+    game.game_destroy(ctx)

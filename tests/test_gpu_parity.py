@@ -581,3 +581,38 @@ def test_evolve_fused_rejects_big_problems(game):
         game.game_evolve_fused(G.ctx, 1, 0, 1, None)
     assert e.value.code == game.ERR_UNSUPPORTED
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ shared coefficients
+@pytest.mark.parametrize("expansion,act,N,d,P,M", [(1, 0, 11, 3, 200, 23), (1, 1, 9, 8, 2100, 19), (0, 1, 7, 5, 1500, 40),
+                                                    (1, 2, 16, 4, 3001, 130)])
+def test_shared_coefficient_mode(game, expansion, act, N, d, P, M):
+    """The paper's literal model (eq.(2),(5),(7): one coefficient per degree for all features; first case = its worked
+    example 11 features, degree 3, 7 genes, 23 chromosomes): fitness, prediction, GA step and the fused loop."""
+    import torch
+    fam = oracle.family(expansion, act, shared=True)
+    rng = np.random.Generator(np.random.Philox(50 + N))
+    X = rng.uniform(-np.pi, np.pi, (P, N)).astype(np.float32) if expansion == 1 else rng.uniform(-1, 1, (P, N)).astype(np.float32)
+    t = (rng.uniform(size=P) > 0.5).astype(np.float32)
+    G = game.Game(P, N, d, M, expansion, act, shared=True)
+    assert G.G == oracle.num_genes(N, d, fam) == (2 * d + 1 if expansion == 1 else d + 1)
+    G.set_ga_params(2, 3, 0.9, 0.2, 0.1)
+    G.load_kb(X, t); G.init_population(3); G.sync()
+    W = G.get_population()
+    G.eval_fitness(); G.sync()
+    F = G.get_fitness()
+    assert_fitness_close(F, oracle.eval_fitness(d, fam, X, t, W), "shared fitness")
+    y = torch.empty(P, dtype=torch.float32, device="cuda")
+    game.game_predict(G.ctx, G.current()[1].data_ptr(), G.X.data_ptr(), P, y.data_ptr()); G.sync()
+    y_ref = oracle.predict(d, fam, X, W[1])
+    assert np.max(np.abs(y.cpu().numpy() - y_ref) / np.maximum(1.0, np.abs(y_ref))) <= 1e-5
+    G.step(3, 0); G.sync()
+    W1 = oracle.step(W, F, 2, 3, 0.9, 0.2, 0.1, 3, 0)
+    assert np.array_equal(G.get_population().view(np.uint32), W1.view(np.uint32))
+    # fused loop, lock-step
+    game.game_evolve_fused(G.ctx, 3, 1, 1, None); G.sync()
+    F1 = G.get_fitness()
+    assert_fitness_close(F1, oracle.eval_fitness(d, fam, X, t, W1), "shared fused fitness")
+    W2 = oracle.step(W1, F1, 2, 3, 0.9, 0.2, 0.1, 3, 1)
+    assert np.array_equal(G.get_population().view(np.uint32), W2.view(np.uint32))
+    G.close()
