@@ -48,7 +48,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS) + ["c4", "n1"])
+    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS) + ["c4", "n1", "n1s"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="auto", choices=["auto", "ffma", "f16x3"])
     ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
@@ -167,7 +167,7 @@ def job_value(P: int, M: int, steps: int, world: int, ms: float) -> float:
 
 def config_dict(cfg, scheme_name, n_gpus):
     return {"workload": (f"{cfg.name}: BASELINE.json configs[{cfg.name[1:]}]" if cfg.name.startswith("c") else
-                         "n1: the paper's own experiment shape (PAPER.md:120-136), synthetic stand-in, ranking selection"), "P": cfg.P, "N": cfg.N, "d": cfg.d,
+                         f"{cfg.name}: the paper's own experiment shape (PAPER.md:120-136), synthetic stand-in, ranking selection" + (", shared coefficients (eq. 2)" if cfg.shared else "")), "P": cfg.P, "N": cfg.N, "d": cfg.d,
             "G": cfg.G, "M": cfg.M, "expansion": "chebyshev" if cfg.expansion == 0 else "trig",
             "activation": ["identity", "sigmoid", "tanh"][cfg.activation], "elite": cfg.elite,
             "tournament": cfg.tournament, "p_cross": cfg.p_cross, "p_mut": cfg.p_mut, "sigma": cfg.sigma,
@@ -194,11 +194,11 @@ def run_ours(args, cfg, rank, world, local_rank):
     torch.cuda.set_device(local_rank)
     scheme = {"auto": game.SCHEME_AUTO, "ffma": game.SCHEME_FFMA, "f16x3": game.SCHEME_F16X3}[args.scheme]
     X, t, _ = wl.make_kb(cfg, seed=cfg.seed + 1000 * rank)           # every replica its own knowledge base
-    G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation, device=dev, scheme=scheme)
+    G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation, device=dev, scheme=scheme, shared=cfg.shared)
     G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
     scheme_name = {game.SCHEME_FFMA: "FFMA fp32", game.SCHEME_F16X3: "F16X3 (3 x tcgen05 kind::f16, 2-term fp16 split, fp32 accumulate)"}[G.scheme()]
     G.load_kb(X, t)
-    if cfg.name == "n1":                      # the paper's settings: ranking selection
+    if cfg.name in ("n1", "n1s"):             # the paper's settings: ranking selection
         game.game_set_selection(G.ctx, game.SEL_RANKING)
     seed = cfg.seed
     G.init_population(seed)
@@ -409,7 +409,7 @@ def main():
         if int(os.environ.get("RANK", "0")) == 0:
             run_c4_sweep(args)
         return
-    cfg = wl.PAPER_SHAPE if args.workload == "n1" else wl.CONFIGS[args.workload]
+    cfg = {"n1": wl.PAPER_SHAPE, "n1s": wl.PAPER_SHAPE_SHARED}.get(args.workload) or wl.CONFIGS[args.workload]
     if args.impl == "reference":
         run_reference(args, cfg, rank, world)
     else:

@@ -43,14 +43,15 @@ class Config:
     w_star_std: float
     noise_std: float
     seed: int
+    shared: bool = False   # the paper's literal form: one coefficient per degree for all features (eq.(2))
 
     @property
     def family(self) -> int:
-        return self.expansion | (self.activation << 8)
+        return self.expansion | (self.activation << 8) | (int(self.shared) << 16)
 
     @property
     def G(self) -> int:
-        return self.N * self.d * (2 if self.expansion == EXP_TRIG else 1) + 1
+        return (1 if self.shared else self.N) * self.d * (2 if self.expansion == EXP_TRIG else 1) + 1
 
 
 # BASELINE.json configs[0..3]; configs[4] is the (M,P) sweep built by c4().
@@ -65,6 +66,9 @@ CONFIGS = {
 # columns, polytrigo degree 8, B*N+1 = 19 chromosomes (eq.(4)), crossover 0.9, mutation 0.2, elitism 2,
 # ranking selection, MSE threshold 0.001, thousands of iterations: the latency-bound regime.  Per-feature coefficients (D1).
 PAPER_SHAPE = Config("n1", 2_100, 9, 8, 19, EXP_TRIG, ACT_SIGMOID, 2, 3, 0.9, 0.2, 0.1, 10_000, float(np.pi), 0.3, 0.05, 11)
+
+# the same with the paper's shared coefficients: G = 2 * 8 + 1 = 17 genes (eq.(5))
+PAPER_SHAPE_SHARED = replace(PAPER_SHAPE, name="n1s", shared=True, w_star_std=0.1)
 
 C4_M = (256, 1024, 4096, 16384)
 C4_P = (100_000, 1_000_000, 10_000_000)
@@ -91,6 +95,8 @@ def _design_matrix(cfg: Config, X64: np.ndarray) -> np.ndarray:
         k = np.arange(1, cfg.d + 1, dtype=np.float64)
         kx = X64[..., None] * k                                            # [rows, N, K]
         blocks = np.concatenate([np.cos(kx), np.sin(kx)], axis=-1).reshape(rows, cfg.N * 2 * cfg.d)
+    if cfg.shared:   # shared coefficients: the term of gene j is the sum over the features
+        blocks = blocks.reshape(rows, cfg.N, -1).sum(axis=1)
     return np.concatenate([np.ones((rows, 1)), blocks], axis=1)
 
 
