@@ -616,3 +616,36 @@ def test_shared_coefficient_mode(game, expansion, act, N, d, P, M):
     W2 = oracle.step(W1, F1, 2, 3, 0.9, 0.2, 0.1, 3, 1)
     assert np.array_equal(G.get_population().view(np.uint32), W2.view(np.uint32))
     G.close()
+
+
+# ------------------------------------------------------------------------------------------------ randomised shapes
+def test_random_shapes_fitness_and_step(game):
+    """Seeded sweep over odd shapes (P, N, d, M not multiples of any tile), both expansions, all activations, all three
+    selection methods: fitness within 1e-5 of the oracle on the AUTO scheme, GA step bit-exact."""
+    rng = np.random.Generator(np.random.Philox(2026))
+    for trial in range(14):
+        expansion = int(rng.integers(0, 2))
+        act = int(rng.integers(0, 3))
+        N = int(rng.integers(1, 41))
+        d = int(rng.integers(1, 8 if expansion else 12))
+        while N * d * (2 if expansion else 1) + 1 > 440:
+            N -= 1
+        P = int(rng.integers(1, 4000))
+        M = int(rng.integers(2, 420))
+        selection = int(rng.integers(0, 3))
+        E = int(rng.integers(0, min(M, 6)))
+        fam = oracle.family(expansion, act)
+        X = rng.uniform(-1, 1, (P, N)).astype(np.float32) * (np.float32(np.pi) if expansion else np.float32(1))
+        t = rng.uniform(0, 1, P).astype(np.float32)
+        W = (rng.uniform(-1, 1, (M, oracle.num_genes(N, d, fam))) * (0.3 if act == 0 else 1.0)).astype(np.float32)
+        G = game.Game(P, N, d, M, expansion, act)
+        G.set_ga_params(E, 3, 0.9, 0.2, 0.1)
+        game.game_set_selection(G.ctx, selection)
+        G.load_kb(X, t); G.set_population(W); G.eval_fitness(); G.sync()
+        F = G.get_fitness()
+        what = f"trial {trial}: exp {expansion} act {act} P {P} N {N} d {d} M {M}"
+        assert_fitness_close(F, oracle.eval_fitness(d, fam, X, t, W), what)
+        G.step(trial, trial + 1); G.sync()
+        ref = oracle.step_sel(W, F, E, 3, selection, 0.9, 0.2, 0.1, trial, trial + 1)
+        assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32)), what
+        G.close()

@@ -451,3 +451,34 @@ def test_immigrants_replace_only_the_last_slots_with_init_like_genes():
     # ~uniform: mean near 0, variance near 1/3 over many genes
     big = oracle.immigrate(np.zeros((2000, 64), np.float32), 0, 2000, 1, 0)
     assert abs(big.mean()) < 0.01 and abs(big.var() - 1 / 3) < 0.01
+
+
+# ------------------------------------------------------------------------------------------------ property tests (hypothesis)
+from hypothesis import given, settings, strategies as st
+
+
+@settings(max_examples=40, deadline=None)
+@given(M=st.integers(2, 40), G=st.integers(1, 20), E_frac=st.floats(0, 0.9), k=st.integers(1, 5),
+       pc=st.sampled_from([0.0, 0.3, 0.9, 1.0]), pm=st.sampled_from([0.0, 0.05, 1.0]), selection=st.integers(0, 2),
+       seed=st.integers(0, 2**64 - 1), gen=st.integers(0, 2**32 - 1))
+def test_step_invariants_on_random_shapes(M, G, E_frac, k, pc, pm, selection, seed, gen):
+    """For any shape and parameters: population size constant; elites = the E best rows in order, bit-copied; with
+    sigma = 0 every child gene equals a gene of SOME chromosome at the same position (crossover only recombines);
+    the step is a pure function of its arguments."""
+    E = min(int(E_frac * M), M - 1)
+    rng = np.random.Generator(np.random.Philox(seed % 2**32))
+    W = rng.uniform(-1, 1, (M, G)).astype(np.float32)
+    F = rng.uniform(0, 1, M).astype(np.float32)
+    if M > 3:
+        F[1] = F[2]
+    Wn = oracle.step_sel(W, F, E, k, selection, pc, pm, 0.0, seed, gen)
+    assert Wn.shape == W.shape
+    order = sorted(range(M), key=lambda m: (F[m], m))
+    for s in range(E):
+        assert np.array_equal(Wn[s], W[order[s]])
+    for g in range(G):
+        assert set(Wn[:, g].tolist()) <= set(W[:, g].tolist())
+    assert np.array_equal(Wn, oracle.step_sel(W, F, E, k, selection, pc, pm, 0.0, seed, gen))
+    if pc == 0.0:
+        rows = {W[m].tobytes() for m in range(M)}
+        assert all(Wn[c].tobytes() in rows for c in range(M))
