@@ -297,18 +297,46 @@ template <int ACT>
 __device__ __forceinline__ float bias_term_of(float a0) {
     return ACT == 1 ? -1.44269504088896340736f * a0 : (ACT == 2 ? 2.88539008177792681472f * a0 : a0);
 }
+// `tq` is the staged target: t itself, or 1 - t for tanh (so that 1 - 2 r - t is one FFMA).
 template <int ACT>
-__device__ __forceinline__ float act_err2(float z, float bias_term, float t) {
-    float y;
+__device__ __forceinline__ float staged_target(float t) { return ACT == 2 ? 1.0f - t : t; }
+template <int ACT>
+__device__ __forceinline__ float act_err2(float z, float bias_term, float tq) {
+    float e;
     if (ACT == 1) {
-        y = rcp_approx(1.0f + ex2_approx(fmaf(z, -1.44269504088896340736f, bias_term)));
+        e = rcp_approx(1.0f + ex2_approx(fmaf(z, -1.44269504088896340736f, bias_term))) - tq;
     } else if (ACT == 2) {
-        y = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(fmaf(z, 2.88539008177792681472f, bias_term))), 1.0f);
+        e = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(fmaf(z, 2.88539008177792681472f, bias_term))), tq);
     } else {
-        y = z + bias_term;
+        e = (z + bias_term) - tq;
     }
-    const float e = y - t;
     return e * e;
+}
+// Two outputs at once with ONE reciprocal: r = 1 / (a0 a1), 1 / a0 = r a1, 1 / a1 = r a0 (the epilogue of the
+// mid-size shapes is bound by the MUFU pipe: 1.5 instead of 2 MUFU operations per output).  The exponent is clamped
+// at 60 so that a0 a1 <= 2^121 stays finite (sigmoid / 1 - tanh below 2^-60 are 0 in fp32 arithmetic on t anyway).
+template <int ACT>
+__device__ __forceinline__ void act_err2_pair(float z0, float z1, float bias_term, float tq0, float tq1, float& acc0,
+                                              float& acc1) {
+    if (ACT == 0) {
+        acc0 += act_err2<ACT>(z0, bias_term, tq0);
+        acc1 += act_err2<ACT>(z1, bias_term, tq1);
+        return;
+    }
+    const float c = ACT == 1 ? -1.44269504088896340736f : 2.88539008177792681472f;
+    const float a0 = 1.0f + ex2_approx(fminf(fmaf(z0, c, bias_term), 60.0f));
+    const float a1 = 1.0f + ex2_approx(fminf(fmaf(z1, c, bias_term), 60.0f));
+    float r = rcp_approx(a0 * a1), e0, e1;
+    if (ACT == 1) {
+        e0 = fmaf(r, a1, -tq0);
+        e1 = fmaf(r, a0, -tq1);
+    } else {
+        r *= -2.0f;
+        e0 = fmaf(r, a1, tq0);
+        e1 = fmaf(r, a0, tq1);
+    }
+    acc0 = fmaf(e0, e0, acc0);
+    acc1 = fmaf(e1, e1, acc1);
 }
 
 // ---------------------------------------------------------------------------------------------- the kernel
@@ -498,7 +526,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");      // everyone is done with the previous tile's t
             {
                 const int gi = q * 32 + lane;
-                ts[gi] = (h * 128 + gi < n_valid) ? __ldg(prm.t + p0 + h * 128 + gi) : 0.0f;
+                ts[gi] = (h * 128 + gi < n_valid) ? staged_target<ACT>(__ldg(prm.t + p0 + h * 128 + gi)) : 0.0f;
             }
             asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
@@ -521,10 +549,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
 #pragma unroll
                         for (int i = 0; i < 8; ++i) {
                             const float4 tv = tp[i];
-                            sum += act_err2<ACT>(__uint_as_float(v[4 * i + 0]), bias, tv.x);
-                            sum1 += act_err2<ACT>(__uint_as_float(v[4 * i + 1]), bias, tv.y);
-                            sum2 += act_err2<ACT>(__uint_as_float(v[4 * i + 2]), bias, tv.z);
-                            sum3 += act_err2<ACT>(__uint_as_float(v[4 * i + 3]), bias, tv.w);
+                            act_err2_pair<ACT>(__uint_as_float(v[4 * i + 0]), __uint_as_float(v[4 * i + 1]), bias, tv.x, tv.y,
+                                               sum, sum1);
+                            act_err2_pair<ACT>(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), bias, tv.z, tv.w,
+                                               sum2, sum3);
                         }
                     } else {
 #pragma unroll
