@@ -68,8 +68,8 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *              (lo.hi, hi.lo, hi.hi; the lo.lo term, <= 2^-22 relative, is dropped), fp32 accumulation in TMEM.
  *              Precondition: |w| and |phi| < 65504 (fp16 range); phi is bounded by 1 for Chebyshev on
  *              |x| <= 1 and for trig; out-of-range values give Inf/NaN fitness, which the GA ranks worst.
- *              Covers any N with d <= 64 (phi of a 256-pattern tile stays resident in shared memory up to 20 K
- *              steps of 16 genes, i.e. ceil(N/8) * ceil(d/2) <= 20 for Chebyshev, ceil(N/8) * d <= 20 for trig; longer K
+ *              Covers any N with d <= 64 (the K axis is the gene order without the bias gene, 16 genes per K step;
+ *              phi of a 256-pattern tile stays resident in shared memory up to 20 K steps, i.e. G - 1 <= 320; longer K
  *              extents are streamed); d > 64 -> GAME_ERR_UNSUPPORTED when F16X3 is forced, FFMA under AUTO.
  *   FFMA covers G <= 448 (its shared-memory tile); forcing it on a larger G -> GAME_ERR_UNSUPPORTED.
  * Both schemes sum each tile's squared errors in fp32 and accumulate tile sums in fp64 in a fixed order

@@ -10,14 +10,16 @@
 //   warp 0      loader   : cp.async.bulk (1-D TMA) of this CTA's pre-split W operand images, 32 KB (4 K steps) per stage
 //   warp 1      MMA      : leader CTA: tcgen05.mma.cta_group::2.kind::f16, M=256 (128 chromosomes per CTA) x
 //                          N=256 patterns (128 generated per CTA) x K=16 genes, three MMAs per K step
-//                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM;
+//                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM; the whole warp runs the
+//                          loop converged and one elected lane issues, so that descriptors stay in uniform registers;
 //                          peer CTA: relays "my stage is full" to the leader's barrier
-//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation, (y-t)^2, private per-chromosome sum
-//                          (TMEM lane = chromosome, so no shuffle is needed); fp64 accumulation per (CTA, m)
-//   warps 10-17 producers: two sets of 4 warps alternating chunks; one pattern per thread; Chebyshev / multiple-angle
-//                          recurrences for 8 features at a time, fp16 hi/lo split, 16-byte stores straight into the
-//                          MMA's canonical layout; phi of a pattern tile stays resident in shared memory and is
-//                          reused by every chromosome-tile pair of the work unit (see "the kernel" below)
+//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation (one reciprocal per two outputs), (y-t)^2,
+//                          private per-chromosome sum (TMEM lane = chromosome, so no shuffle is needed); fp64
+//                          accumulation per (CTA, m)
+//   warps 10-17 producers: two sets of 4 warps alternating pipeline stages; one pattern per thread walking the gene
+//                          order with the Chebyshev / multiple-angle recurrences, fp16 hi/lo split, 16-byte stores
+//                          straight into the MMA's canonical layout; phi of a pattern tile stays resident in shared
+//                          memory and is reused by every chromosome-tile pair of the work unit (see "the kernel")
 //
 // Why a pair: ncu on the single-CTA version (profiles/r01a) showed the shared-memory data pipe, not the tensor
 // pipe, saturating (tensor-core operand reads 46 % + producer stores 28 % + loads 4 % + bulk fills): with
@@ -28,11 +30,10 @@
 // 8-row core matrices packed back to back, i.e. a plain [k_group][row][8 x fp16] array:
 //     byte(row, k) = (k / 8) * rows * 16 + row * 16 + (k % 8) * 2        SBO = 128 B, LBO = rows * 16 B
 // so a producer warp's 32 rows x 16 B are 512 contiguous bytes (conflict-free) and a K step is any pair of
-// k-groups.  The K axis is a PERMUTATION of the genes chosen for the generator (the W images use the same one):
-//   chunk c = features 8c..8c+7;  k-group kg of the chunk holds, for those 8 features,
-//       Chebyshev: T_{kg+1}(x_i)          trig: cos((kg/2+1) x_i) if kg even, sin((kg/2+1) x_i) if kg odd
-//   (padded to an even number of k-groups; absent features / degrees are zeros in the W image).  The bias gene
-//   a_0 is not on the K axis: the epilogue adds it on the FFMA that scales z for ex2.
+// k-groups.  The K axis is the gene order of include/game.h without the bias gene (position q = g - 1, 8 positions
+// per k-group, zero-padded in the W images to a multiple of 16): no padding inside the K extent, so K steps =
+// ceil((G - 1) / 16) (an earlier layout of 8-feature chunks cost c4 9 K steps instead of 8 and c1 6 instead of 4).
+// The bias gene a_0 is not on the K axis: the epilogue adds it on the FFMA that scales z for ex2.
 #pragma once
 #include <cuda_fp16.h>
 
@@ -48,10 +49,10 @@ constexpr int kABytes = 2 * kBM * 16;          // one K step of A, hi or lo: 2 k
 constexpr int kBBytes = 2 * kRows * 16;        // one K step of this CTA's half of B, hi or lo: 4096
 constexpr int kSlotBytes = 2 * kABytes;        // one K step of either operand (hi + lo) = 8192
 static_assert(2 * kBBytes == kSlotBytes, "A and B steps share the slot size");
-constexpr int kKS = 4;                         // K steps per pipeline stage: the issuing thread's fixed cost per
-                                               // stage (poll ~150, commit ~120, fence ~45 cycles, measured) is
-                                               // amortised over 3 * kKS MMAs of 128 cycles each (kKS = 1: 27.6 ms,
-                                               // 2: 22.4 ms, 4: 20.3 ms per c3 evaluation)
+constexpr int kKS = 4;                         // K steps per pipeline stage: the issuing warp's fixed cost per
+                                               // stage (barrier poll, fence, commits) is amortised over 3 * kKS
+                                               // MMAs of 128 cycles each (kKS = 1: 27.6 ms, 2: 22.4 ms, 4: 20.3 ms
+                                               // per c3 evaluation, measured with a one-lane issue loop)
 constexpr int kStageBytes = kKS * kSlotBytes;  // 32768
 constexpr int kStagesTotal = 7;                // 32 KB stages shared by the A ring and the B stages (224 KB)
 constexpr int kMaxResidentStages = 5;          // phi of a whole pattern tile stays in smem up to 20 K steps
@@ -72,7 +73,7 @@ struct Params {
     const uint8_t* Wimg;   // [m_tiles][steps][8192]: A_hi (2 k-groups x 128 rows x 16 B), then A_lo
     double* part;          // [gridDim.x * 2][m_stride]
     const int* stop;       // optional: non-zero => the stop rule is met, the kernel returns at once
-    long long* stall;      // optional [gridDim.x][4]: cycles the MMA/relay thread stalled on a_full, b_full, acc_empty; total
+    long long* stall;      // optional [gridDim.x][4]: cycles the MMA/relay warp waited on a_full, b_full, acc_empty; total
     long long P;
     int N, d, M, G;
     int m_stride;          // m_tiles * 128
@@ -82,11 +83,12 @@ struct Params {
     int zero_part;         // 1: this launch starts the generation (clear this CTA's partial sums first)
     int m_groups;          // work unit = (pattern tile, group of m_pairs_per_group chromosome-tile pairs)
     int m_pairs_per_group;
-    int chunks;            // ceil(N / 8)
-    int steps_per_chunk;   // Chebyshev ceil(d / 2); trig d
-    int steps;             // chunks * steps_per_chunk K steps (the bias gene is added by the epilogue)
+    int dd;                // genes per feature: Chebyshev d, trig 2 d
+    int steps;             // ceil((G - 1) / 16) K steps (the bias gene is added by the epilogue)
+    int span;              // K steps per producer work item (kKS; less when the whole K extent is one stage)
     int stages;            // ceil(steps / kKS) pipeline stages per tile
-    int resident;          // 1: n_b == stages, phi generated once per unit and reused by all its chromosome tiles
+    int resident;          // 1: phi generated once per unit and reused by all its chromosome tiles; n_b == stages, or
+                           //    2 * stages (phi of the next unit is generated while this one is consumed)
     int n_a, n_b;          // A ring stages, B stages (n_a + n_b <= kStagesTotal)
 };
 
@@ -153,11 +155,25 @@ __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
         if (++n > (1u << 24)) __trap();
     } while (!mbar_try_wait(bar, parity));
 }
+// Long waits (the producers of a resident unit wait for a whole unit, ~100 us at c3): exponential back-off up to
+// MAX_NS.  With a fixed 32 ns sleep this loop was more than half of all instructions the kernel executed (ncu source
+// page of a c4 point: 110 M iterations), issue slots and power taken from the working warps.
+template <int MAX_NS>
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+    uint32_t n = 0, ns = 32;
+    do {
+        __nanosleep(ns);
+        ns = min(2 * ns, static_cast<uint32_t>(MAX_NS));
+        if (++n > (1u << 24)) __trap();
+    } while (!mbar_try_wait(bar, parity));
+}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -169,6 +185,29 @@ __device__ __forceinline__ void tmem_alloc_pair(uint32_t dst_smem, uint32_t cols
 }
 __device__ __forceinline__ void tmem_dealloc_pair(uint32_t addr, uint32_t cols) {
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+}
+// One lane of a converged warp (the same lane every time for the same mask).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+// Barrier polls of a converged warp: the elected lane polls, the vote makes the answer warp-uniform.  (All 32 lanes
+// polling the same barrier is ruinous when the poll fails: measured 4x on the whole kernel.)
+__device__ __forceinline__ bool warp_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok = 0;
+    if (elect_one()) ok = mbar_try_wait(bar, parity);
+    return __any_sync(0xffffffffu, ok) != 0;
+}
+__device__ __forceinline__ void warp_wait_spin(uint32_t bar, uint32_t parity) {
+    uint32_t n = 0;
+    while (!warp_try_wait(bar, parity)) {
+        if (++n > (1u << 26)) __trap();
+    }
 }
 // D[tmem, both CTAs] (+)= A[smem of both CTAs] . B[smem of both CTAs]; issued by one thread of the leader CTA.
 __device__ __forceinline__ void umma_f16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -217,24 +256,20 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
 // Instruction descriptor, kind::f16: D = F32 (bit 4), A = B = F16 (0), both K-major, N >> 3 at bit 17,
 // M >> 4 at bit 24 (M = 256: the pair's two 128-row halves).
 constexpr uint32_t kIdesc = (1u << 4) | (static_cast<uint32_t>(kBN >> 3) << 17) | (static_cast<uint32_t>((2 * kBM) >> 4) << 24);
-// ---------------------------------------------------------------------------------------------- K-axis permutation
-// Gene held by (K step s, k-group kg in {0,1}, slot f in 0..7), or -1 for padding.  Used by the W image
-// builder; the producers below generate phi in exactly this order.
-__host__ __device__ inline int gene_at(int s, int kg, int f, int N, int d, int expansion, int steps_per_chunk) {
-    const int c = s / steps_per_chunk, ss = s % steps_per_chunk;
-    const int i = c * 8 + f;
-    if (i >= N) return -1;
-    if (expansion == 0) {
-        const int j = 2 * ss + kg + 1;
-        return j <= d ? 1 + i * d + (j - 1) : -1;
-    }
-    return 1 + i * 2 * d + ss + (kg ? d : 0);
+// ---------------------------------------------------------------------------------------------- K axis
+// The K axis is the gene order of include/game.h without the bias gene: position q = g - 1, k-group = 8 consecutive
+// positions, K step = 2 k-groups; positions >= G - 1 are padding (zero in the W images, so phi there is irrelevant).
+// Gene held by (K step s, k-group kg in {0,1}, slot f in 0..7), or -1 for padding.  Used by the W image builder;
+// the producers below generate phi in exactly this order.
+__host__ __device__ inline int gene_at(int s, int kg, int f, int G) {
+    const int g = 1 + (2 * s + kg) * 8 + f;
+    return g < G ? g : -1;
 }
 
 // W [M][G] fp32 -> per (m_tile, step) 8 KB images: A_hi then A_lo, each [2 k-groups][128 rows][8 fp16].
 // hi = rn_f16(w), lo = rn_f16(w - hi).  One thread per (m_tile, step, k-group, row).
-__global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __restrict__ img, int M, int G, int N, int d,
-                                      int expansion, int steps_per_chunk, int steps, int m_tiles) {
+__global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __restrict__ img, int M, int G, int steps,
+                                      int m_tiles) {
     const long long idx = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     const long long total = static_cast<long long>(m_tiles) * steps * 2 * kBM;
     if (idx >= total) return;
@@ -249,7 +284,7 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
         float w[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const int g = gene_at(s, kg, f2 * 2 + e, N, d, expansion, steps_per_chunk);
+            const int g = gene_at(s, kg, f2 * 2 + e, G);
             w[e] = (g >= 0 && m < M) ? W[static_cast<size_t>(m) * G + g] : 0.0f;
         }
         const __half2 h = __floats2half2_rn(w[0], w[1]);
@@ -285,10 +320,6 @@ __device__ __forceinline__ void split_store(const float (&v)[8], uint8_t* hi_dst
     }
     *reinterpret_cast<uint4*>(hi_dst) = make_uint4(h[0], h[1], h[2], h[3]);
     *reinterpret_cast<uint4*>(lo_dst) = make_uint4(l[0], l[1], l[2], l[3]);
-}
-__device__ __forceinline__ void zero_store(uint8_t* hi_dst, uint8_t* lo_dst) {
-    *reinterpret_cast<uint4*>(hi_dst) = make_uint4(0u, 0u, 0u, 0u);
-    *reinterpret_cast<uint4*>(lo_dst) = make_uint4(0u, 0u, 0u, 0u);
 }
 
 // (act(z + bias) - t)^2.  `bias_term` is the bias gene pre-multiplied so that it rides on the FFMA that scales z for
@@ -379,7 +410,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     float* ts_all = reinterpret_cast<float*>(smem + kSmemBar + kBarBytes);
     const uint32_t smem_base = smem_u32(smem);
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // the warp index through a shuffle: ptxas then knows it is warp-uniform, and so is all control flow that depends
+    // only on it (the producers' walk over the gene order compiles to uniform branches instead of a convergence
+    // barrier per value)
+    const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const uint32_t crank = cluster_ctarank();            // 0 = leader, 1 = peer
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int units = prm.p_tiles * prm.m_groups;
@@ -392,7 +426,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < kStagesTotal; ++s) {
             // K steps held by B stage s (resident: the tile's last stage may hold fewer than kKS)
-            const int ks = resident ? min(kKS, prm.steps - s * kKS) : kKS;
+            const int ks = resident ? min(kKS, prm.steps - (s % stages) * kKS) : kKS;
             mbar_init(bar_a_full + 8 * s, crank == 0 ? 2 : 1);   // leader: own loader + the peer's relay
             mbar_init(bar_a_empty + 8 * s, 1);
             mbar_init(bar_b_full + 8 * s, (kNumProdWarps / 2) * max(ks, 1));
@@ -437,50 +471,54 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            // ====================================== MMA issuer (leader) / relay "my stages are full" (peer)
-            // The issuing thread is the serial resource of the whole kernel (measured per stage: barrier poll ~150
-            // cycles, commit ~120, fence + descriptors ~45, each MMA issue ~60), so a stage carries kKS K steps
-            // (3 * kKS MMAs), the leader waits on ONE barrier per stage -- its a_full[i] counts its own loader and
-            // the peer's relay -- and it polls the next stage's barrier BEFORE issuing this stage's MMAs.
-            Ring ra, rb;
-            uint32_t tile = 0, unit_parity = 0;
-            const uint32_t leader_a_full = map_to_cta(bar_a_full, 0);
-            long long st_a = 0, st_b = 0, st_c = 0;
-            const long long t_begin = clock64();
-            uint32_t ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);
-            for (int u = pair; u < units; u += n_pairs, unit_parity ^= 1) {
-                const int mg = u % prm.m_groups;
-                const int mp0 = mg * prm.m_pairs_per_group;
-                const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
-                for (int mp = mp0; mp < mp1; ++mp, ++tile) {
-                    const bool need_b = !resident || mp == mp0;          // B stages must be (re)filled for this tile
-                    const bool release_b = !resident || mp == mp1 - 1;   // last reader of the B stages
-                    const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
-                    const uint32_t d_tmem = tmem_base + buf * kBN;
-                    if (crank == 0 && !mbar_try_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1)) {
+        // ====================================== MMA issuer (leader) / relay "my stages are full" (peer)
+        // The issuing thread is the serial resource of the whole kernel: every instruction between two MMAs shows up
+        // in the tile time.  The WHOLE warp runs this loop converged (all lanes poll the barriers) and one elected lane
+        // issues the MMAs and commits: everything that feeds them (descriptors, barrier addresses) is then
+        // warp-uniform and lives in uniform registers -- under `if (lane == 0)` ptxas wrapped every tcgen05.mma in an
+        // elect / 5 x R2UR / branch loop.  A stage carries kKS K steps (3 * kKS MMAs); the leader waits on ONE barrier
+        // per stage -- its a_full[i] counts its own loader and the peer's relay -- and polls the next stage's barrier
+        // BEFORE issuing this stage's MMAs.
+        Ring ra, rb, rbu;                    // rbu: first B stage of the current unit (resident mode)
+        uint32_t tile = 0;
+        const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem_base, 0);
+        const uint32_t leader_a_full = map_to_cta(bar_a_full, 0);
+        long long st_a = 0, st_b = 0, st_c = 0;
+        const long long t_begin = clock64();
+        bool ready = warp_try_wait(bar_a_full + 8 * ra.i, ra.phase);
+        for (int u = pair; u < units; u += n_pairs, rbu = rbu.at(stages, n_b)) {
+            const int mg = u % prm.m_groups;
+            const int mp0 = mg * prm.m_pairs_per_group;
+            const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
+            for (int mp = mp0; mp < mp1; ++mp, ++tile) {
+                const bool need_b = !resident || mp == mp0;          // B stages must be (re)filled for this tile
+                const bool release_b = !resident || mp == mp1 - 1;   // last reader of the B stages
+                const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
+                const uint32_t d_tmem = tmem_u + buf * kBN;
+                if (resident) rb = rbu;                               // every tile of the unit reads the same B stages
+                if (crank == 0 && !warp_try_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1)) {
+                    const long long t0 = clock64();
+                    warp_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
+                    st_c += clock64() - t0;
+                }
+                for (int j = 0; j < stages; ++j) {
+                    if (!ready) {
                         const long long t0 = clock64();
-                        mbar_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
-                        st_c += clock64() - t0;
+                        warp_wait_spin(bar_a_full + 8 * ra.i, ra.phase);
+                        st_a += clock64() - t0;
                     }
-                    for (int j = 0; j < stages; ++j) {
-                        if (resident) { rb.i = j; rb.phase = unit_parity; }
-                        if (!ready) {
-                            const long long t0 = clock64();
-                            mbar_wait_spin(bar_a_full + 8 * ra.i, ra.phase);
-                            st_a += clock64() - t0;
-                        }
-                        if (need_b && !mbar_try_wait(bar_b_full + 8 * rb.i, rb.phase)) {
-                            const long long t0 = clock64();
-                            mbar_wait_spin(bar_b_full + 8 * rb.i, rb.phase);
-                            st_b += clock64() - t0;
-                        }
-                        const uint32_t cur = ra.i;
-                        ra.advance(n_a);
-                        ready = mbar_try_wait(bar_a_full + 8 * ra.i, ra.phase);            // next stage's poll, early
-                        if (crank == 0) {
-                            tc_fence_after();
-                            const int nk = min(kKS, prm.steps - j * kKS);
+                    if (need_b && !warp_try_wait(bar_b_full + 8 * rb.i, rb.phase)) {
+                        const long long t0 = clock64();
+                        warp_wait_spin(bar_b_full + 8 * rb.i, rb.phase);
+                        st_b += clock64() - t0;
+                    }
+                    const uint32_t cur = ra.i;
+                    ra.advance(n_a);
+                    ready = warp_try_wait(bar_a_full + 8 * ra.i, ra.phase);            // next stage's poll, early
+                    if (crank == 0) {
+                        tc_fence_after();
+                        const int nk = min(kKS, prm.steps - j * kKS);
+                        if (elect_one()) {
                             for (int k = 0; k < nk; ++k) {
                                 const uint32_t a_hi = smem_base + cur * kStageBytes + k * kSlotBytes, a_lo = a_hi + kABytes;
                                 const uint32_t b_hi = b_base + rb.i * kStageBytes + k * kSlotBytes, b_lo = b_hi + kBBytes;
@@ -492,18 +530,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                             }
                             umma_commit_pair(bar_a_empty + 8 * cur);                        // A stage free in both CTAs
                             if (release_b) umma_commit_pair(bar_b_empty + 8 * rb.i);        // B stage free in both CTAs
-                        } else {
-                            mbar_arrive_cluster(leader_a_full + 8 * cur);                   // relay: my stages are full
+                            if (j == stages - 1) umma_commit_pair(bar_acc_full + 8 * buf);  // accumulators complete
                         }
-                        if (!resident) rb.advance(n_b);
+                        __syncwarp();
+                    } else {
+                        if (elect_one()) mbar_arrive_cluster(leader_a_full + 8 * cur);      // relay: my stages are full
+                        __syncwarp();
                     }
-                    if (crank == 0) umma_commit_pair(bar_acc_full + 8 * buf);               // accumulators complete
+                    rb.advance(n_b);
                 }
             }
-            if (prm.stall != nullptr) {
-                long long* out = prm.stall + static_cast<size_t>(blockIdx.x) * 4;
-                out[0] = st_a; out[1] = st_b; out[2] = st_c; out[3] = clock64() - t_begin;
-            }
+        }
+        if (prm.stall != nullptr && lane == 0) {
+            long long* out = prm.stall + static_cast<size_t>(blockIdx.x) * 4;
+            out[0] = st_a; out[1] = st_b; out[2] = st_c; out[3] = clock64() - t_begin;
         }
     } else if (warp < 2 + kNumEpiWarps) {
         // ============================================================== epilogue
@@ -514,6 +554,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
         const uint32_t leader_acc_empty = map_to_cta(bar_acc_empty, 0);
         uint32_t tile = 0;
+        // this thread's target of a unit (column h * 128 + q * 32 + lane of its pattern tile), staged form; 0 if absent
+        auto target_of = [&](int uu) {
+            if (uu >= units) return 0.0f;
+            const long long pp = static_cast<long long>(prm.p_tile0 + uu / prm.m_groups) * kBN + h * 128 + q * 32 + lane;
+            return pp < prm.P ? staged_target<ACT>(__ldg(prm.t + pp)) : 0.0f;
+        };
+        float t_next = target_of(pair);      // always one unit ahead: its HBM latency is hidden behind a whole unit
         for (int u = pair; u < units; u += n_pairs) {
             const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
@@ -524,16 +571,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             // same for every chromosome tile of the unit); named barrier per half, 128 threads
             float* ts = ts_all + h * 128;
             asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");      // everyone is done with the previous tile's t
-            {
-                const int gi = q * 32 + lane;
-                ts[gi] = (h * 128 + gi < n_valid) ? staged_target<ACT>(__ldg(prm.t + p0 + h * 128 + gi)) : 0.0f;
-            }
+            ts[q * 32 + lane] = t_next;
+            t_next = target_of(u + n_pairs);
             asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                 const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
                 const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
                 // the bias gene a_0 is not part of the contraction: it rides on the epilogue's FFMA
                 const float bias = bias_term_of<ACT>(m < prm.M ? __ldg(prm.W + static_cast<size_t>(m) * prm.G) : 0.0f);
+                // this lane's running sum, fetched before the wait: its L2 round trip is off the tile's critical path
+                const double part_old = __ldcg(my_part + m);
                 mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
@@ -565,20 +612,24 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8 * buf);
-                __stcg(my_part + m, __ldcg(my_part + m) + static_cast<double>(sum));
+                __stcg(my_part + m, part_old + static_cast<double>(sum));
             }
         }
     } else {
         // ============================================================== producers: phi -> this CTA's half of B
-        // Two sets of 4 warps; a set owns whole chunks (8 features: the recurrences restart there) and the sets
-        // alternate chunks.  One proxy fence + the arrivals per batch of up to kBatch K steps (the fence waits for
-        // this warp's stores to land).  x is read straight from global memory (once per unit when resident).
-        constexpr int kBatch = 6;
-        const int pidx = threadIdx.x - (2 + kNumEpiWarps) * 32;
-        const int set = pidx >> 7;              // which warp set
-        const int r = pidx & (kRows - 1);       // pattern row of this thread, 0..127
+        // Two sets of 4 warps; a thread owns one pattern row.  A work item is `span` consecutive K steps (one pipeline
+        // stage) and the sets alternate items.  Within an item a thread walks the flat gene order: it enters the item
+        // at feature i, index j within the feature (re-running the recurrence up to j), emits 8 values per k-group and
+        // moves to the next feature whenever j reaches dd; all of this control is uniform over the warp.  x is read
+        // straight from global memory in blocks of four features, one block ahead (the rows of the NEXT unit are prefetched
+        // into L2 meanwhile).  One proxy fence + the arrivals per item.
+        const int pw = warp - (2 + kNumEpiWarps);       // producer warp 0..7
+        const int set = pw >> 2;                         // which warp set
+        const int r = (pw & 3) * 32 + lane;              // pattern row of this thread, 0..127
+        const int dd = prm.dd, span = prm.span;
+        const int n_items = (prm.steps + span - 1) / span;
         Ring rb;                                // ring position of the current fill's first stage
-        uint32_t item = 0;                      // running chunk counter: chunk goes to set (item & 1)
+        uint32_t item = 0;                      // running item counter: item goes to set (item & 1)
         for (int u = pair; u < units; u += n_pairs) {
             const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
@@ -586,76 +637,103 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const long long p = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows + r;
             const bool valid = p < prm.P;
             const float* xrow = prm.X + (valid ? p : 0) * prm.N;
+            const bool vec4 = (prm.N & 3) == 0;       // rows are 16-byte aligned (X itself is: game_load_kb checks)
+            auto fetch = [&](int i) { return (valid && i < prm.N) ? __ldg(xrow + i) : 0.0f; };
+            auto fetch4 = [&](int i) {                 // features i..i+3, i a multiple of 4; absent ones are 0
+                if (vec4) return (valid && i < prm.N) ? __ldg(reinterpret_cast<const float4*>(xrow + i)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                return make_float4(fetch(i), fetch(i + 1), fetch(i + 2), fetch(i + 3));
+            };
+            // the knowledge base streams from HBM exactly once: pull the next unit's rows into L2 now, so that its first
+            // loads do not pay the HBM latency on the critical path of a short unit
+            if (set == 0 && u + n_pairs < units) {
+                const long long pn = static_cast<long long>(prm.p_tile0 + (u + n_pairs) / prm.m_groups) * kBN +
+                                     static_cast<long long>(crank) * kRows + r;
+                if (pn < prm.P) {
+                    const char* row = reinterpret_cast<const char*>(prm.X + pn * prm.N);
+                    const int bytes = prm.N * 4;
+                    for (int off = 0; off < bytes; off += 128) prefetch_l2(row + off);
+                    prefetch_l2(row + bytes - 4);
+                }
+            }
             const int n_fill = resident ? 1 : mp1 - mp0;        // how many times the K extent is generated
             for (int fill = 0; fill < n_fill; ++fill) {
-                for (int c = 0; c < prm.chunks; ++c, ++item) {
+                for (int w = 0; w < n_items; ++w, ++item) {
                     if ((item & 1u) != static_cast<uint32_t>(set)) continue;
-                    // recurrence state for the 8 features of this chunk
-                    float x2[8], am[8], ac[8], bm[8], bc[8];
-#pragma unroll
-                    for (int f = 0; f < 8; ++f) {
-                        const int i = c * 8 + f;
-                        const float x = (valid && i < prm.N) ? __ldg(xrow + i) : 0.0f;
+                    const int s0 = w * span, s1 = min(prm.steps, s0 + span);
+                    const Ring pos = rb.at(s0 / kKS, n_b);
+                    // where this item enters the gene order
+                    int i = (16 * s0) / dd, j = 16 * s0 - i * dd;
+                    // x in blocks of 4 features (one 16-byte load per block when the rows are 16-byte aligned: a scalar
+                    // load of one feature touches 32 different lines per warp, and those loads were what bounded the
+                    // producers on short units); `cur` is the block of feature i, `nxt` the one after it, already in flight
+                    float4 cur = fetch4(i & ~3), nxt = fetch4((i & ~3) + 4);
+                    auto pick = [&](int ii) {
+                        const int k = ii & 3;
+                        return k == 0 ? cur.x : (k == 1 ? cur.y : (k == 2 ? cur.z : cur.w));
+                    };
+                    // recurrence state: cp, cc = T_j, T_{j+1} (or cos jx, cos (j+1)x); sp, sc = sin jx, sin (j+1)x
+                    float x2, cp, cc, sp = 0.0f, sc = 0.0f;
+                    auto enter = [&](float x) {
                         if (EXPANSION == 0) {
-                            x2[f] = 2.0f * x; am[f] = 1.0f; ac[f] = x;       // T_0, T_1
-                            bm[f] = 0.0f; bc[f] = 0.0f;
+                            x2 = 2.0f * x; cp = 1.0f; cc = x;
                         } else {
                             float sn, cs;
                             sincosf(x, &sn, &cs);
-                            x2[f] = 2.0f * cs; am[f] = 1.0f; ac[f] = cs;     // cos 0x, cos 1x
-                            bm[f] = 0.0f; bc[f] = sn;                        // sin 0x, sin 1x
+                            x2 = 2.0f * cs; cp = 1.0f; cc = cs; sp = 0.0f; sc = sn;
+                        }
+                    };
+                    // value of index jj within the feature (Chebyshev T_{jj+1}; trig cos (jj+1)x for jj < d, else
+                    // sin (jj-d+1)x), advancing the recurrence that produced it
+                    auto next = [&](int jj) {
+                        float out;
+                        if (EXPANSION == 0 || jj < prm.d) {
+                            out = cc;
+                            const float t = fmaf(x2, cc, -cp);
+                            cp = cc; cc = t;
+                        } else {
+                            out = sc;
+                            const float t = fmaf(x2, sc, -sp);
+                            sp = sc; sc = t;
+                        }
+                        return out;
+                    };
+                    enter(pick(i));
+                    if (EXPANSION == 0 || j <= prm.d) {
+                        for (int jj = 0; jj < j; ++jj) next(jj);
+                    } else {
+                        for (int jj = prm.d; jj < j; ++jj) next(jj);
+                    }
+                    mbar_wait_backoff<512>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
+                    // (A compact one-value-per-iteration loop with a sliding 8-value window was tried against the
+                    // instruction-cache misses this unrolled body causes: 2400 instead of 3800 SASS instructions, but
+                    // its serial chain made an item 25 % slower.)
+                    for (int st = s0; st < s1; ++st) {
+                        uint8_t* b_hi = smem + (n_a + pos.i) * kStageBytes + (st % kKS) * kSlotBytes + r * 16;
+                        uint8_t* b_lo = b_hi + kBBytes;
+#pragma unroll
+                        for (int kg = 0; kg < 2; ++kg) {
+                            float v[8];
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                if (j == dd) {
+                                    ++i; j = 0;
+                                    if ((i & 3) == 0) { cur = nxt; nxt = fetch4(i + 4); }
+                                    enter(pick(i));
+                                }
+                                v[e] = next(j);
+                                ++j;
+                            }
+                            split_store(v, b_hi + kg * (kRows * 16), b_lo + kg * (kRows * 16));
                         }
                     }
-                    const int s_chunk = c * prm.steps_per_chunk;           // first K step of this chunk in the tile
-                    for (int ss0 = 0; ss0 < prm.steps_per_chunk; ss0 += kBatch) {
-                        const int nb = min(kBatch, prm.steps_per_chunk - ss0);
-                        for (int jb = 0; jb < nb; ++jb) {
-                            const int ss = ss0 + jb, s = s_chunk + ss;
-                            const Ring pos = rb.at(s / kKS, n_b);
-                            if (!mbar_try_wait(bar_b_empty + 8 * pos.i, pos.phase ^ 1))
-                                mbar_wait_sleep<32>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
-                            uint8_t* b_hi = smem + (n_a + pos.i) * kStageBytes + (s % kKS) * kSlotBytes + r * 16;
-                            uint8_t* b_lo = b_hi + kBBytes;
-                            float v0[8], v1[8];
-                            if (EXPANSION == 0) {
-                                // k-group 0: T_{2ss+1}, k-group 1: T_{2ss+2}
-#pragma unroll
-                                for (int f = 0; f < 8; ++f) {
-                                    v0[f] = ac[f];
-                                    v1[f] = fmaf(x2[f], ac[f], -am[f]);
-                                    ac[f] = fmaf(x2[f], v1[f], -ac[f]);
-                                    am[f] = v1[f];
-                                }
-                            } else {
-                                // k-group 0: cos((ss+1) x), k-group 1: sin((ss+1) x)
-#pragma unroll
-                                for (int f = 0; f < 8; ++f) {
-                                    v0[f] = ac[f];
-                                    v1[f] = bc[f];
-                                    const float cn = fmaf(x2[f], ac[f], -am[f]);
-                                    const float sn = fmaf(x2[f], bc[f], -bm[f]);
-                                    am[f] = ac[f]; ac[f] = cn;
-                                    bm[f] = bc[f]; bc[f] = sn;
-                                }
-                            }
-                            split_store(v0, b_hi, b_lo);
-                            if (EXPANSION == 0 && 2 * ss + 2 > prm.d) {
-                                zero_store(b_hi + kRows * 16, b_lo + kRows * 16);      // odd d: last k-group is padding
-                            } else {
-                                split_store(v1, b_hi + kRows * 16, b_lo + kRows * 16);
-                            }
-                        }
-                        fence_proxy_async_smem();
-                        __syncwarp();
-                        if (lane == 0) {
-                            for (int jb = 0; jb < nb; ++jb) {
-                                const int s = s_chunk + ss0 + jb;
-                                const Ring pos = rb.at(s / kKS, n_b);
-                                mbar_arrive(bar_b_full + 8 * pos.i);
-                                // streaming ring stages always expect kKS K steps: stand in for the missing ones
-                                if (!resident && s == prm.steps - 1)
-                                    for (int e = prm.steps % kKS; e != 0 && e < kKS; ++e) mbar_arrive(bar_b_full + 8 * pos.i);
-                            }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) {
+                        for (int st = s0; st < s1; ++st) {
+                            mbar_arrive(bar_b_full + 8 * pos.i);
+                            // streaming ring stages always expect kKS K steps: stand in for the missing ones
+                            if (!resident && st == prm.steps - 1)
+                                for (int e = prm.steps % kKS; e != 0 && e < kKS; ++e) mbar_arrive(bar_b_full + 8 * pos.i);
                         }
                     }
                 }

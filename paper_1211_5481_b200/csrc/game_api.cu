@@ -34,7 +34,7 @@ struct game_ctx {
     int N = 0, d = 0, M = 0, G = 0, expansion = 0, act = 0, shared = 0;
     // tensor-core path geometry
     bool umma_ok = false;
-    int m_tiles = 0, m_stride = 0, chunks = 0, steps_per_chunk = 0, steps = 0;
+    int m_tiles = 0, m_stride = 0, steps = 0;
     // workspace layout (byte offsets)
     size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
@@ -161,7 +161,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         uint8_t* img = c->ws + c->off_img;
         const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
         umma::build_w_images_kernel<<<static_cast<unsigned>((n_thr + 255) / 256), 256, 0, c->stream>>>(
-            W, img, c->M, c->G, c->N, c->d, c->expansion, c->steps_per_chunk, c->steps, c->m_tiles);
+            W, img, c->M, c->G, c->steps, c->m_tiles);
         if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
         umma::Params prm;
         prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.part = part;
@@ -178,10 +178,15 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         if (want > m_pairs) want = m_pairs;
         prm.m_pairs_per_group = static_cast<int>((m_pairs + want - 1) / want);
         prm.m_groups = (m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
-        prm.chunks = c->chunks; prm.steps_per_chunk = c->steps_per_chunk; prm.steps = c->steps;
+        prm.dd = c->expansion == GAME_EXP_CHEBYSHEV ? c->d : 2 * c->d;
+        prm.steps = c->steps;
         prm.stages = (c->steps + umma::kKS - 1) / umma::kKS;
+        prm.span = prm.stages > 1 ? umma::kKS : (c->steps + 1) / 2;      // one stage only: half of it per producer set
         prm.resident = prm.stages <= umma::kMaxResidentStages ? 1 : 0;
-        prm.n_b = prm.resident ? prm.stages : umma::kStreamBStages;
+        // phi of a pattern tile stays in shared memory when it fits, twice over when that fits too (the producers
+        // then work one unit ahead of the MMAs)
+        prm.n_b = !prm.resident ? umma::kStreamBStages
+                                : (2 * prm.stages <= umma::kMaxResidentStages ? 2 * prm.stages : prm.stages);
         prm.n_a = umma::kStagesTotal - prm.n_b;
         prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
         prm.stop = c->stop;
@@ -317,9 +322,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->m_tiles = 2 * ((M + 2 * game::umma::kBM - 1) / (2 * game::umma::kBM));   // one chromosome tile per CTA of a pair
     c->m_stride = c->m_tiles * game::umma::kBM;
     c->umma_ok = umma_ok;
-    c->chunks = (N + 7) / 8;
-    c->steps_per_chunk = expansion == GAME_EXP_CHEBYSHEV ? (d + 1) / 2 : d;
-    c->steps = c->chunks * c->steps_per_chunk;
+    c->steps = static_cast<int>((G - 1 + 15) / 16);   // K steps of 16 genes; the bias gene is not part of the contraction
     size_t off = 0;
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
     c->off_img = off;
