@@ -310,7 +310,7 @@ def run_ours(args, cfg, rank, world, local_rank):
                 "flops_per_launch": flops_per_launch, "peak_source": peak_note,
                 "hbm_algorithmic_bytes_per_launch": 4 * (cfg.P * (cfg.N + 1)),
                 "mufu_frac_at_max_clock": (0.0 if cfg.activation == wl.ACT_IDENTITY or fused else
-                                           1.5 * cfg.P * cfg.M / avg_s / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6)),
+                                           1.25 * cfg.P * cfg.M / avg_s / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6)),
                 "hbm_frac_of_measured": 4 * (cfg.P * (cfg.N + 1)) / avg_s / 1e9 / float(peaks["hbm_gbs"])}
 
     # ---------------- CPU baseline: the oracle as it stands, one thread, bounded sample
@@ -374,8 +374,8 @@ def run_c4_sweep(args):
             sweep.append({"M": M, "P": P, "ms_per_eval": ms, "evals_per_s": P * M / (ms * 1e-3), "kernel_ms": kms / kn,
                           "tensor_tflops": tf, "tensor_frac": tf / float(peaks["bf16_tflops"]),
                           "hbm_frac": 4.0 * P * (big.N + 1) / (kms / kn * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
-                          # epilogue: 1.5 MUFU per evaluation (ex2 each, one rcp per two), 16 MUFU lanes per SM per clock
-                          "mufu_frac_at_max_clock": 1.5 * P * M / (kms / kn * 1e-3) / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6),
+                          # epilogue: 1.25 MUFU per evaluation (ex2 each, one rcp per four), 16 MUFU lanes per SM per clock
+                          "mufu_frac_at_max_clock": 1.25 * P * M / (kms / kn * 1e-3) / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6),
                           "l2": "X larger than L2" if P * big.N * 4 > 126e6 else "X fits L2 (not flushed)"})
             G.close()
     clocks = sampler.stop()

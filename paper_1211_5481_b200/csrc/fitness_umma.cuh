@@ -13,7 +13,7 @@
 //                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM; the whole warp runs the
 //                          loop converged and one elected lane issues, so that descriptors stay in uniform registers;
 //                          peer CTA: relays "my stage is full" to the leader's barrier
-//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation (one reciprocal per two outputs), (y-t)^2,
+//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation (one reciprocal per four outputs), (y-t)^2,
 //                          private per-chromosome sum (TMEM lane = chromosome, so no shuffle is needed); fp64
 //                          accumulation per (CTA, m)
 //   warps 10-17 producers: two sets of 4 warps alternating pipeline stages; one pattern per thread walking the gene
@@ -349,31 +349,36 @@ __device__ __forceinline__ float act_err2(float z, float bias_term, float tq) {
     }
     return e * e;
 }
-// Two outputs at once with ONE reciprocal: r = 1 / (a0 a1), 1 / a0 = r a1, 1 / a1 = r a0 (the epilogue of the
-// mid-size shapes is bound by the MUFU pipe: 1.5 instead of 2 MUFU operations per output).  The exponent is clamped
-// at 60 so that a0 a1 <= 2^121 stays finite (sigmoid / 1 - tanh below 2^-60 are 0 in fp32 arithmetic on t anyway).
+// Four outputs at once with ONE reciprocal: r = 1 / (a0 a1 a2 a3), 1 / (a0 a1) = r (a2 a3), 1 / a0 = a1 / (a0 a1), ...
+// The epilogue of the mid-size shapes is bound by the MUFU pipe (16 lanes per SM per clock): this is 1.25 MUFU
+// operations per output instead of 2 (1.5 with pairs) for 1.25 extra FMULs.  The exponent is clamped at 30 so that the
+// product stays finite (<= 2^121); sigmoid / 1 - tanh below 2^-30 are below fp32 resolution of the error against t.
 template <int ACT>
-__device__ __forceinline__ void act_err2_pair(float z0, float z1, float bias_term, float tq0, float tq1, float& acc0,
-                                              float& acc1) {
+__device__ __forceinline__ void act_err2_quad(float z0, float z1, float z2, float z3, float bias_term, float4 tq, float& acc0,
+                                              float& acc1, float& acc2, float& acc3) {
     if (ACT == 0) {
-        acc0 += act_err2<ACT>(z0, bias_term, tq0);
-        acc1 += act_err2<ACT>(z1, bias_term, tq1);
+        acc0 += act_err2<ACT>(z0, bias_term, tq.x);
+        acc1 += act_err2<ACT>(z1, bias_term, tq.y);
+        acc2 += act_err2<ACT>(z2, bias_term, tq.z);
+        acc3 += act_err2<ACT>(z3, bias_term, tq.w);
         return;
     }
     const float c = ACT == 1 ? -1.44269504088896340736f : 2.88539008177792681472f;
-    const float a0 = 1.0f + ex2_approx(fminf(fmaf(z0, c, bias_term), 60.0f));
-    const float a1 = 1.0f + ex2_approx(fminf(fmaf(z1, c, bias_term), 60.0f));
-    float r = rcp_approx(a0 * a1), e0, e1;
-    if (ACT == 1) {
-        e0 = fmaf(r, a1, -tq0);
-        e1 = fmaf(r, a0, -tq1);
-    } else {
-        r *= -2.0f;
-        e0 = fmaf(r, a1, tq0);
-        e1 = fmaf(r, a0, tq1);
-    }
+    const float a0 = 1.0f + ex2_approx(fminf(fmaf(z0, c, bias_term), 30.0f));
+    const float a1 = 1.0f + ex2_approx(fminf(fmaf(z1, c, bias_term), 30.0f));
+    const float a2 = 1.0f + ex2_approx(fminf(fmaf(z2, c, bias_term), 30.0f));
+    const float a3 = 1.0f + ex2_approx(fminf(fmaf(z3, c, bias_term), 30.0f));
+    const float p01 = a0 * a1, p23 = a2 * a3;
+    float r = rcp_approx(p01 * p23);
+    if (ACT == 2) r *= -2.0f;                      // tanh = 1 - 2 / a: tq holds 1 - t
+    const float r01 = r * p23, r23 = r * p01;      // (-2) / (a0 a1), (-2) / (a2 a3)
+    const float s = ACT == 1 ? -1.0f : 1.0f;       // sigmoid: e = 1/a - t; tanh: e = (1 - t) - 2/a
+    const float e0 = fmaf(r01, a1, s * tq.x), e1 = fmaf(r01, a0, s * tq.y);
+    const float e2 = fmaf(r23, a3, s * tq.z), e3 = fmaf(r23, a2, s * tq.w);
     acc0 = fmaf(e0, e0, acc0);
     acc1 = fmaf(e1, e1, acc1);
+    acc2 = fmaf(e2, e2, acc2);
+    acc3 = fmaf(e3, e3, acc3);
 }
 
 // ---------------------------------------------------------------------------------------------- the kernel
@@ -601,6 +606,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
+                // (16 columns at a time with the next chunk's TMEM load in flight was measured twice: 3 % slower.)
 #pragma unroll 1
                 for (int cc = 0; cc < 4; ++cc) {
                     const int col0 = h * 128 + cc * 32;
@@ -611,13 +617,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     tmem_ld_wait();
                     if (col0 + 32 <= n_valid) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            const float4 tv = tp[i];
-                            act_err2_pair<ACT>(__uint_as_float(v[4 * i + 0]), __uint_as_float(v[4 * i + 1]), bias, tv.x, tv.y,
-                                               sum, sum1);
-                            act_err2_pair<ACT>(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), bias, tv.z, tv.w,
+                        for (int i = 0; i < 8; ++i)
+                            act_err2_quad<ACT>(__uint_as_float(v[4 * i + 0]), __uint_as_float(v[4 * i + 1]),
+                                               __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), bias, tp[i], sum, sum1,
                                                sum2, sum3);
-                        }
                     } else {
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
