@@ -68,9 +68,11 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *              (lo.hi, hi.lo, hi.hi; the lo.lo term, <= 2^-22 relative, is dropped), fp32 accumulation in TMEM.
  *              Precondition: |w| and |phi| < 65504 (fp16 range); phi is bounded by 1 for Chebyshev on
  *              |x| <= 1 and for trig; out-of-range values give Inf/NaN fitness, which the GA ranks worst.
- *              Covers any N with d <= 64 (the K axis is the gene order without the bias gene, 16 genes per K step;
- *              phi of a 256-pattern tile stays resident in shared memory up to 20 K steps, i.e. G - 1 <= 320; longer K
- *              extents are streamed); d > 64 -> GAME_ERR_UNSUPPORTED when F16X3 is forced, FFMA under AUTO.
+ *              Covers any N and d for Chebyshev, d <= 128 for the trigonometric family (the fp32 multiple-angle
+ *              recurrence leaves the 1e-5 fitness bound beyond that: 2e-6 at d = 100, 2e-5 at d = 400).  The K axis
+ *              is the gene order without the bias gene, 16 genes per K step; phi of a 256-pattern tile stays resident
+ *              in shared memory up to 20 K steps, i.e. G - 1 <= 320; longer K extents are streamed.  Trigonometric
+ *              d > 128 -> GAME_ERR_UNSUPPORTED when F16X3 is forced, FFMA under AUTO.
  *   FFMA covers G <= 448 (its shared-memory tile); forcing it on a larger G -> GAME_ERR_UNSUPPORTED.
  * Both schemes sum each tile's squared errors in fp32 and accumulate tile sums in fp64 in a fixed order
  * (run-to-run bit-stable; equal chromosomes get equal fitness in any slot). */
@@ -78,7 +80,7 @@ enum { GAME_SCHEME_AUTO = 0, GAME_SCHEME_FFMA = 1, GAME_SCHEME_F16X3 = 2 };
 
 /* Create a context for a knowledge base of P patterns x N features, expansion degree d, population of
  * M chromosomes.  Validates: P >= 1, N >= 1, d >= 1, M >= 1, known family -> GAME_ERR_INVALID_ARG;
- * a shape no kernel covers (d > 64 together with G > 448) -> GAME_ERR_UNSUPPORTED.
+ * a shape no kernel covers (trigonometric d > 128, or shared coefficients, together with G > 448) -> GAME_ERR_UNSUPPORTED.
  * Host only; touches no device memory. */
 int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int32_t family);
 

@@ -143,7 +143,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (rc) return rc;
     const int scheme = resolved_scheme(c);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients with d <= 64");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients (trigonometric family: d <= 128)");
     if (!c->ticket_zeroed) {
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
         c->ticket_zeroed = true;
@@ -313,7 +313,10 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     if (expansion > GAME_EXP_TRIG || act > GAME_ACT_TANH) return GAME_ERR_INVALID_ARG;
     if (P > (1ll << 40) || N > 4096 || d > 4096 || M > (1 << 24)) return GAME_ERR_INVALID_ARG;
     const long long G = static_cast<long long>(shared ? 1 : N) * d * (expansion == GAME_EXP_TRIG ? 2 : 1) + 1;
-    const bool umma_ok = !shared && d <= 64 && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
+    // the tensor-core kernel walks the gene order, so any degree works; for the trigonometric family the fp32 multiple-angle
+    // recurrence limits it (fitness error against the fp64 oracle: 2e-6 at d = 100, 2e-5 at d = 400; bound 1e-5)
+    const int d_max_umma = expansion == GAME_EXP_TRIG ? 128 : 4096;
+    const bool umma_ok = !shared && d <= d_max_umma && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
     if (G > (1 << 20) || (!umma_ok && G > game::kFfmaMaxG)) return GAME_ERR_UNSUPPORTED;   // FFMA kernel: G <= 448
     game_ctx* c = new (std::nothrow) game_ctx();
     if (!c) return GAME_ERR_INVALID_ARG;
@@ -375,7 +378,7 @@ int game_set_scheme(game_ctx* c, int32_t scheme) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (scheme < GAME_SCHEME_AUTO || scheme > GAME_SCHEME_F16X3) return fail(c, GAME_ERR_INVALID_ARG, "unknown scheme %d", scheme);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients with d <= 64");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients (trigonometric family: d <= 128)");
     if (scheme == GAME_SCHEME_FFMA && c->G > game::kFfmaMaxG)
         return fail(c, GAME_ERR_UNSUPPORTED, "FFMA covers G <= 448");
     c->scheme = scheme;

@@ -69,7 +69,9 @@ def test_create_rejects_bad_shapes(L, args):
 
 def test_create_unsupported_gene_count(L):
     ctx = C.c_void_p()
-    assert L.game_create(C.byref(ctx), 10, 10, 70, 8, 0x0100) == game.ERR_UNSUPPORTED   # d > 64 and G = 701 > 448
+    assert L.game_create(C.byref(ctx), 10, 2, 200, 8, 0x0101) == game.ERR_UNSUPPORTED   # trig d > 128 and G = 801 > 448
+    assert L.game_create(C.byref(ctx), 10, 10, 70, 8, 0x0100) == game.OK                # Chebyshev: any degree, G = 701
+    game.game_destroy(ctx)
     assert L.game_create(C.byref(ctx), 10, 64, 10, 8, 0x0100) == game.OK                # G = 641: tensor-core kernel
     game.game_destroy(ctx)
 
@@ -80,7 +82,7 @@ def test_scheme_resolution(L):
     game.game_set_scheme(ctx, game.SCHEME_FFMA)
     assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
     game.game_destroy(ctx)
-    ctx = game.game_create(1000, 4, 70, 64, 0x0100)           # d > 64: tensor-core kernel does not cover it
+    ctx = game.game_create(1000, 1, 200, 64, 0x0101)          # trig d > 128 (G = 401): tensor-core kernel does not cover it
     assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
     with pytest.raises(game.GameError) as e:
         game.game_set_scheme(ctx, game.SCHEME_F16X3)

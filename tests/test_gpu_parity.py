@@ -67,6 +67,11 @@ FITNESS_CASES = [
     ("stream_tail", "c3", dict(P=800, N=24, d=14, M=150)),       # streaming, 21 K steps: last stage holds 1 of 4 steps
     ("stream_tail_trig", "c2", dict(P=800, N=24, d=7, M=150)),   # streaming trig, 21 K steps
     ("huge_G_641", "c3", dict(P=600, N=64, d=10, M=70)),      # beyond the FFMA kernel's G <= 448: tensor path only
+    # degrees far beyond a K step: a feature spans several k-groups, the producers enter items in mid-feature
+    ("deg70_cheb", "c1", dict(P=1500, N=6, d=70, M=140)),
+    ("deg100_cheb", "c1", dict(P=1500, N=10, d=100, M=140)),  # G = 1001, streaming
+    ("deg300_cheb", "c3", dict(P=900, N=3, d=300, M=70)),
+    ("deg100_trig", "c2", dict(P=900, N=3, d=100, M=70)),     # G = 601
 ]
 
 
