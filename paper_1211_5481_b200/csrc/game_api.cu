@@ -218,9 +218,25 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
             GAME_CUDA(cudaStreamWaitEvent(c->copy_stream, c->copy_events[n_ranges], 0));
         }
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
+        // Range boundaries in whole rounds of the persistent grid (a launch that ends in mid-round idles part of the
+        // grid), the first range short: its copy is the only one the kernel has to wait for.
+        int bound[9];
+        {
+            const long long per_round = pair_cap / prm.m_groups > 0 ? pair_cap / prm.m_groups : 1;   // pattern tiles per round
+            const long long rounds = (p_tiles_all + per_round - 1) / per_round;
+            const long long first = rounds / 32 > 0 ? rounds / 32 : 1;
+            bound[0] = 0;
+            for (int k = 1; k <= n_ranges; ++k) {
+                const long long e = n_ranges == 1 ? rounds : first + (rounds - first) * (k - 1) / (n_ranges - 1);
+                const long long tl = e * per_round;
+                bound[k] = static_cast<int>(tl < p_tiles_all ? tl : p_tiles_all);
+            }
+            bound[n_ranges] = p_tiles_all;
+        }
+        bool first_launch = true;
         for (int k = 0; k < n_ranges; ++k) {
-            const int tile0 = static_cast<int>(static_cast<long long>(p_tiles_all) * k / n_ranges);
-            const int tile1 = static_cast<int>(static_cast<long long>(p_tiles_all) * (k + 1) / n_ranges);
+            const int tile0 = bound[k], tile1 = bound[k + 1];
+            if (tile1 <= tile0) continue;
             if (hk != nullptr) {
                 const long long p0 = static_cast<long long>(tile0) * umma::kBN;
                 long long p1 = static_cast<long long>(tile1) * umma::kBN;
@@ -232,7 +248,8 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
                 GAME_CUDA(cudaEventRecord(c->copy_events[k], c->copy_stream));
                 GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[k], 0));
             }
-            prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = k == 0 ? 1 : 0;
+            prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = first_launch ? 1 : 0;
+            first_launch = false;
 #define GAME_LAUNCH(E, A) umma::fitness_umma_kernel<E, A><<<grid, umma::kThreads, umma::kSmemBytes, c->stream>>>(prm)
             const int sel = c->expansion * 3 + c->act;
             switch (sel) {
