@@ -16,7 +16,7 @@
 //   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation (one reciprocal per four outputs), (y-t)^2,
 //                          private per-chromosome sum (TMEM lane = chromosome, so no shuffle is needed); fp64
 //                          accumulation per (CTA, m)
-//   warps 10-17 producers: two sets of 4 warps alternating pipeline stages; one pattern per thread walking the gene
+//   warps 10-17 producers: four sets of 2 warps taking pipeline stages in turn; two patterns per thread walking the gene
 //                          order with the Chebyshev / multiple-angle recurrences, fp16 hi/lo split, 16-byte stores
 //                          straight into the MMA's canonical layout; phi of a pattern tile stays resident in shared
 //                          memory and is reused by every chromosome-tile pair of the work unit (see "the kernel")
@@ -58,6 +58,10 @@ constexpr int kStagesTotal = 7;                // 32 KB stages shared by the A r
 constexpr int kMaxResidentStages = 5;          // phi of a whole pattern tile stays in smem up to 20 K steps
 constexpr int kStreamBStages = 3;              // B ring when phi does not fit (regenerated per chromosome tile)
 constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4 warps (128 rows each)
+constexpr int kRPT = 2;                        // pattern rows per producer thread: two independent recurrences share one
+                                               // walk over the gene order (the walk's control was most of a value's cost)
+constexpr int kSetWarps = kRows / (32 * kRPT); // warps that cover the 128 rows of this CTA once: 2
+constexpr int kNumSets = kNumProdWarps / kSetWarps;   // producer sets, each takes whole work items: 4
 constexpr int kThreads = (2 + kNumEpiWarps + kNumProdWarps) * 32;   // 576
 constexpr int kSmemBar = kStagesTotal * kStageBytes;  // barriers start here
 constexpr int kAKS = 2;                        // K steps per A ring slot: the A ring is refilled in HALF stages (16 KB), so
@@ -394,7 +398,7 @@ __device__ __forceinline__ void act_err2_quad(float z0, float z1, float z2, floa
 //   a_full[i]    1 + tx : the loader's bulk copy of A slot i has landed; on the leader +1: the peer's relay
 //                         ("my A slot i, and the B stage it pairs with, are full")
 //   a_empty[i]   1      : tcgen05.commit of the MMAs that read A slot i, multicast to both CTAs
-//   b_full[i]    4 * (K steps in the stage): the 4 producer warps that own each of its K steps have written it
+//   b_full[i]    2 * (K steps in the stage): the 2 producer warps that own each of its K steps have written it
 //   b_empty[i]   1      : tcgen05.commit (multicast) of the last MMAs that will read B stage i
 //   acc_full[b]  1      : tcgen05.commit after a tile's last MMA, multicast to both CTAs
 //   acc_empty[b] 16     : leader only; the 8 epilogue warps of BOTH CTAs have drained accumulator b
@@ -446,7 +450,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         for (int s = 0; s < kStagesTotal; ++s) {
             // K steps held by B stage s (resident: the tile's last stage may hold fewer than kKS)
             const int ks = resident ? min(kKS, prm.steps - (s % stages) * kKS) : kKS;
-            mbar_init(bar_b_full + 8 * s, (kNumProdWarps / 2) * max(ks, 1));
+            mbar_init(bar_b_full + 8 * s, kSetWarps * max(ks, 1));
             mbar_init(bar_b_empty + 8 * s, 1);
         }
         for (int b = 0; b < 2; ++b) {
@@ -637,15 +641,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         }
     } else {
         // ============================================================== producers: phi -> this CTA's half of B
-        // Two sets of 4 warps; a thread owns one pattern row.  A work item is `span` consecutive K steps (one pipeline
-        // stage) and the sets alternate items.  Within an item a thread walks the flat gene order: it enters the item
+        // Four sets of 2 warps; a thread owns two pattern rows (r and r + 64: two independent recurrences under one walk).
+        // A work item is `span` consecutive K steps (one pipeline stage) and the sets take the items in turn.  Within an item a thread walks the flat gene order: it enters the item
         // at feature i, index j within the feature (re-running the recurrence up to j), emits 8 values per k-group and
         // moves to the next feature whenever j reaches dd; all of this control is uniform over the warp.  x is read
         // straight from global memory in blocks of four features, one block ahead (the rows of the NEXT unit are prefetched
         // into L2 meanwhile).  One proxy fence + the arrivals per item.
         const int pw = warp - (2 + kNumEpiWarps);       // producer warp 0..7
-        const int set = pw >> 2;                         // which warp set
-        const int r = (pw & 3) * 32 + lane;              // pattern row of this thread, 0..127
+        const int set = pw / kSetWarps;                  // which warp set
+        const int r = (pw % kSetWarps) * 32 + lane;      // first pattern row of this thread; it also owns r + 64
         const int dd = prm.dd, span = prm.span;
         const int n_items = (prm.steps + span - 1) / span;
         Ring rb;                                // ring position of the current fill's first stage
@@ -654,103 +658,130 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
             const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
-            const long long p = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows + r;
-            const bool valid = p < prm.P;
-            const float* xrow = prm.X + (valid ? p : 0) * prm.N;
-            // x in blocks of 4 features.  Block b of this row; b and the feature indices are clamped into the row, so a
+            // x in blocks of 4 features.  Block b of a row; b and the feature indices are clamped into the row, so a
             // load never leaves it (features past N only exist in the zero-padded tail of the K axis, where phi is
             // multiplied by W image zeros: any finite value of the SAME row will do there, and a row that holds a
             // non-finite value has a non-finite z anyway).  Rows of a pattern past P read row 0 (masked by the epilogue).
+            const float* xrow[kRPT];
+#pragma unroll
+            for (int q = 0; q < kRPT; ++q) {
+                const long long p = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows + r + q * (kRows / kRPT);
+                xrow[q] = prm.X + (p < prm.P ? p : 0) * prm.N;
+            }
             const bool vec4 = (prm.N & 3) == 0;       // rows are 16-byte aligned (X itself is: game_load_kb checks)
             const int last_blk = (prm.N - 1) >> 2, last_i = prm.N - 1;
-            auto fetch4 = [&](int b) {
+            auto fetch4 = [&](const float* row, int b) {
                 b = min(b, last_blk);
-                if (vec4) return __ldg(reinterpret_cast<const float4*>(xrow) + b);
+                if (vec4) return __ldg(reinterpret_cast<const float4*>(row) + b);
                 const int i0 = 4 * b;
-                return make_float4(__ldg(xrow + i0), __ldg(xrow + min(i0 + 1, last_i)), __ldg(xrow + min(i0 + 2, last_i)),
-                                   __ldg(xrow + min(i0 + 3, last_i)));
+                return make_float4(__ldg(row + i0), __ldg(row + min(i0 + 1, last_i)), __ldg(row + min(i0 + 2, last_i)),
+                                   __ldg(row + min(i0 + 3, last_i)));
             };
             // the knowledge base streams from HBM exactly once: pull the next unit's rows into L2 now, so that its first
             // loads do not pay the HBM latency on the critical path of a short unit
             if (set == 0 && u + n_pairs < units) {
-                const long long pn = static_cast<long long>(prm.p_tile0 + (u + n_pairs) / prm.m_groups) * kBN +
-                                     static_cast<long long>(crank) * kRows + r;
-                if (pn < prm.P) {
-                    const char* row = reinterpret_cast<const char*>(prm.X + pn * prm.N);
-                    const int bytes = prm.N * 4;
-                    for (int off = 0; off < bytes; off += 128) prefetch_l2(row + off);
-                    prefetch_l2(row + bytes - 4);
+#pragma unroll
+                for (int q = 0; q < kRPT; ++q) {
+                    const long long pn = static_cast<long long>(prm.p_tile0 + (u + n_pairs) / prm.m_groups) * kBN +
+                                         static_cast<long long>(crank) * kRows + r + q * (kRows / kRPT);
+                    if (pn < prm.P) {
+                        const char* row = reinterpret_cast<const char*>(prm.X + pn * prm.N);
+                        const int bytes = prm.N * 4;
+                        for (int off = 0; off < bytes; off += 128) prefetch_l2(row + off);
+                        prefetch_l2(row + bytes - 4);
+                    }
                 }
             }
             const int n_fill = resident ? 1 : mp1 - mp0;        // how many times the K extent is generated
             for (int fill = 0; fill < n_fill; ++fill) {
                 for (int w = 0; w < n_items; ++w, ++item) {
-                    if ((item & 1u) != static_cast<uint32_t>(set)) continue;
                     const int s0 = w * span, s1 = min(prm.steps, s0 + span);
                     const Ring pos = rb.at(s0 / kKS, n_b);
+                    if (item % kNumSets != static_cast<uint32_t>(set)) {
+                        // Not this set's item, but still wait for its stage to have been emptied: an mbarrier wait only
+                        // tells one phase from the next, so a set must watch EVERY lap of every stage go by (with more
+                        // sets than ring stages it would otherwise skip a lap and take a stale phase for the one it
+                        // needs).  Stages are released in item order, so this never delays the set's own item.
+                        mbar_wait_backoff<512>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
+                        continue;
+                    }
                     // where this item enters the gene order
                     int i = (16 * s0) / dd, j = 16 * s0 - i * dd;
                     // x in blocks of 4 features (one 16-byte load per block when the rows are 16-byte aligned: a scalar
                     // load of one feature touches 32 different lines per warp, and those loads were what bounded the
                     // producers on short units); `cur` is the block of feature i, `nxt` the one after it, already in flight
-                    float4 cur = fetch4(i >> 2), nxt = fetch4((i >> 2) + 1);
-                    auto pick = [&](int ii) {
+                    float4 cur[kRPT], nxt[kRPT];
+#pragma unroll
+                    for (int q = 0; q < kRPT; ++q) {
+                        cur[q] = fetch4(xrow[q], i >> 2);
+                        nxt[q] = fetch4(xrow[q], (i >> 2) + 1);
+                    }
+                    auto pick = [&](const float4& c4, int ii) {
                         const int k = ii & 3;
-                        return k == 0 ? cur.x : (k == 1 ? cur.y : (k == 2 ? cur.z : cur.w));
+                        return k == 0 ? c4.x : (k == 1 ? c4.y : (k == 2 ? c4.z : c4.w));
                     };
-                    // recurrence state: cp, cc = T_j, T_{j+1} (or cos jx, cos (j+1)x); sp, sc = sin jx, sin (j+1)x
-                    float x2, cp, cc, sp = 0.0f, sc = 0.0f;
-                    auto enter = [&](float x) {
-                        if (EXPANSION == 0) {
-                            x2 = 2.0f * x; cp = 1.0f; cc = x;
-                        } else {
-                            float sn, cs;
-                            sincosf(x, &sn, &cs);
-                            x2 = 2.0f * cs; cp = 1.0f; cc = cs; sp = 0.0f; sc = sn;
+                    // recurrence state per row: cp, cc = T_j, T_{j+1} (or cos jx, cos (j+1)x); sp, sc = sin jx, sin (j+1)x
+                    float x2[kRPT], cp[kRPT], cc[kRPT], sp[kRPT], sc[kRPT];
+                    auto enter = [&]() {                      // both rows start feature i
+#pragma unroll
+                        for (int q = 0; q < kRPT; ++q) {
+                            const float x = pick(cur[q], i);
+                            if (EXPANSION == 0) {
+                                x2[q] = 2.0f * x; cp[q] = 1.0f; cc[q] = x; sp[q] = 0.0f; sc[q] = 0.0f;
+                            } else {
+                                float sn, cs;
+                                sincosf(x, &sn, &cs);
+                                x2[q] = 2.0f * cs; cp[q] = 1.0f; cc[q] = cs; sp[q] = 0.0f; sc[q] = sn;
+                            }
                         }
                     };
                     // value of index jj within the feature (Chebyshev T_{jj+1}; trig cos (jj+1)x for jj < d, else
-                    // sin (jj-d+1)x), advancing the recurrence that produced it
-                    auto next = [&](int jj) {
+                    // sin (jj-d+1)x) of row q, advancing the recurrence that produced it
+                    auto next = [&](int q, int jj) {
                         float out;
                         if (EXPANSION == 0 || jj < prm.d) {
-                            out = cc;
-                            const float t = fmaf(x2, cc, -cp);
-                            cp = cc; cc = t;
+                            out = cc[q];
+                            const float t = fmaf(x2[q], cc[q], -cp[q]);
+                            cp[q] = cc[q]; cc[q] = t;
                         } else {
-                            out = sc;
-                            const float t = fmaf(x2, sc, -sp);
-                            sp = sc; sc = t;
+                            out = sc[q];
+                            const float t = fmaf(x2[q], sc[q], -sp[q]);
+                            sp[q] = sc[q]; sc[q] = t;
                         }
                         return out;
                     };
-                    enter(pick(i));
-                    if (EXPANSION == 0 || j <= prm.d) {
-                        for (int jj = 0; jj < j; ++jj) next(jj);
-                    } else {
-                        for (int jj = prm.d; jj < j; ++jj) next(jj);
+                    enter();
+                    for (int jj = (EXPANSION == 0 || j <= prm.d) ? 0 : prm.d; jj < j; ++jj) {
+#pragma unroll
+                        for (int q = 0; q < kRPT; ++q) next(q, jj);
                     }
                     mbar_wait_backoff<512>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
-                    // One k-group (8 values, one 16-byte row of hi and of lo) per iteration of a loop that is NOT unrolled:
-                    // unrolled over the 16 values of a K step the body was 25 KB of code, a quarter of the producers'
-                    // stall samples were instruction-cache misses (ncu source page of an M = 256 point) and 21 warp
-                    // instructions were executed per value.  (A one-value-per-iteration loop with a sliding 8-value window
-                    // was smaller still, but its serial chain made an item 25 % slower.)
+                    // One k-group (8 values, one 16-byte row of hi and of lo, for each of the thread's rows) per iteration
+                    // of a loop that is NOT unrolled: unrolled over the 16 values of a K step the body was 25 KB of code, a
+                    // quarter of the producers' stall samples were instruction-cache misses (ncu source page of an M = 256
+                    // point) and 21 warp instructions were executed per value.  (A one-value-per-iteration loop with a
+                    // sliding 8-value window was smaller still, but its serial chain made an item 25 % slower.)
                     uint8_t* dst = smem + (n_a + pos.i) * kStageBytes + (s0 % kKS) * kSlotBytes + r * 16;
 #pragma unroll 1
                     for (int g8 = 0; g8 < 2 * (s1 - s0); ++g8) {
-                        float v[8];
+                        float v[kRPT][8];
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
                             if (j == dd) {
                                 ++i; j = 0;
-                                if ((i & 3) == 0) { cur = nxt; nxt = fetch4((i >> 2) + 1); }
-                                enter(pick(i));
+                                if ((i & 3) == 0) {
+#pragma unroll
+                                    for (int q = 0; q < kRPT; ++q) { cur[q] = nxt[q]; nxt[q] = fetch4(xrow[q], (i >> 2) + 1); }
+                                }
+                                enter();
                             }
-                            v[e] = next(j);
+#pragma unroll
+                            for (int q = 0; q < kRPT; ++q) v[q][e] = next(q, j);
                             ++j;
                         }
-                        split_store(v, dst, dst + kBBytes);
+#pragma unroll
+                        for (int q = 0; q < kRPT; ++q)
+                            split_store(v[q], dst + q * (kRows / kRPT) * 16, dst + q * (kRows / kRPT) * 16 + kBBytes);
                         dst += (g8 & 1) ? kRows * 16 + kBBytes : kRows * 16;   // next k-group; after the odd one skip the lo half
                     }
                     fence_proxy_async_smem();
