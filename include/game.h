@@ -72,7 +72,8 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *              recurrence leaves the 1e-5 fitness bound beyond that: 2e-6 at d = 100, 2e-5 at d = 400).  The K axis
  *              is the gene order without the bias gene, 16 genes per K step; phi of a 256-pattern tile stays resident
  *              in shared memory up to 20 K steps, i.e. G - 1 <= 320; longer K extents are streamed.  Trigonometric
- *              d > 128 -> GAME_ERR_UNSUPPORTED when F16X3 is forced, FFMA under AUTO.
+ *              d > 128 -> GAME_ERR_UNSUPPORTED when F16X3 is forced, FFMA under AUTO.  Shared coefficients
+ *              (GAME_FAMILY_SHARED): covered for G - 1 <= 64 terms, FFMA beyond.
  *   FFMA covers G <= 448 (its shared-memory tile); forcing it on a larger G -> GAME_ERR_UNSUPPORTED.
  * Both schemes sum each tile's squared errors in fp32 and accumulate tile sums in fp64 in a fixed order
  * (run-to-run bit-stable; equal chromosomes get equal fitness in any slot). */
@@ -80,7 +81,7 @@ enum { GAME_SCHEME_AUTO = 0, GAME_SCHEME_FFMA = 1, GAME_SCHEME_F16X3 = 2 };
 
 /* Create a context for a knowledge base of P patterns x N features, expansion degree d, population of
  * M chromosomes.  Validates: P >= 1, N >= 1, d >= 1, M >= 1, known family -> GAME_ERR_INVALID_ARG;
- * a shape no kernel covers (trigonometric d > 128, or shared coefficients, together with G > 448) -> GAME_ERR_UNSUPPORTED.
+ * a shape no kernel covers (trigonometric d > 128, or more than 64 shared terms, together with G > 448) -> GAME_ERR_UNSUPPORTED.
  * Host only; touches no device memory. */
 int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int32_t family);
 

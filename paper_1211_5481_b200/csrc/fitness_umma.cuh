@@ -94,6 +94,8 @@ struct Params {
     int m_groups;          // work unit = (pattern tile, group of m_pairs_per_group chromosome-tile pairs)
     int m_pairs_per_group;
     int dd;                // genes per feature: Chebyshev d, trig 2 d
+    int shared;            // 1: the paper's literal model: ONE coefficient set for all features, the term of
+                           //    index jj is the SUM over the features; G = dd + 1
     int steps;             // ceil((G - 1) / 16) K steps (the bias gene is added by the epilogue)
     int span;              // K steps per producer work item (kKS; less when the whole K extent is one stage)
     int stages;            // ceil(steps / kKS) pipeline stages per tile
@@ -705,6 +707,67 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                         mbar_wait_backoff<512>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
                         continue;
                     }
+                    if (prm.shared) {
+                        // ---- shared coefficients: term jj of a pattern = sum over its features of T_{jj+1}(x_i) (or cos / sin).
+                        // One k-group (8 consecutive jj) at a time: for every feature the recurrence is run from its start
+                        // up to the k-group and the 8 values are added up; the K extent is short (dd <= 64), so re-running
+                        // the head of the recurrence costs less than keeping dd accumulators per row would.
+                        mbar_wait_backoff<512>(bar_b_empty + 8 * pos.i, pos.phase ^ 1);
+                        uint8_t* dst = smem + (n_a + pos.i) * kStageBytes + (s0 % kKS) * kSlotBytes + r * 16;
+#pragma unroll 1
+                        for (int g8 = 0; g8 < 2 * (s1 - s0); ++g8) {
+                            const int jbase = 8 * (2 * s0 + g8);
+                            float acc[kRPT][8];
+#pragma unroll
+                            for (int q = 0; q < kRPT; ++q)
+#pragma unroll
+                                for (int e = 0; e < 8; ++e) acc[q][e] = 0.0f;
+                            float4 blk[kRPT];
+#pragma unroll 1
+                            for (int i = 0; i < prm.N; ++i) {
+                                float x2[kRPT], cp[kRPT], cc[kRPT], sp[kRPT], sc[kRPT];
+#pragma unroll
+                                for (int q = 0; q < kRPT; ++q) {
+                                    if ((i & 3) == 0) blk[q] = fetch4(xrow[q], i >> 2);
+                                    const int k = i & 3;
+                                    const float x = k == 0 ? blk[q].x : (k == 1 ? blk[q].y : (k == 2 ? blk[q].z : blk[q].w));
+                                    if (EXPANSION == 0) {
+                                        x2[q] = 2.0f * x; cp[q] = 1.0f; cc[q] = x; sp[q] = 0.0f; sc[q] = 0.0f;
+                                    } else {
+                                        float sn, cs;
+                                        sincosf(x, &sn, &cs);
+                                        x2[q] = 2.0f * cs; cp[q] = 1.0f; cc[q] = cs; sp[q] = 0.0f; sc[q] = sn;
+                                    }
+                                }
+                                auto step = [&](int q, int jj) {
+                                    float out;
+                                    if (EXPANSION == 0 || jj < prm.d) {
+                                        out = cc[q];
+                                        const float t = fmaf(x2[q], cc[q], -cp[q]);
+                                        cp[q] = cc[q]; cc[q] = t;
+                                    } else {
+                                        out = sc[q];
+                                        const float t = fmaf(x2[q], sc[q], -sp[q]);
+                                        sp[q] = sc[q]; sc[q] = t;
+                                    }
+                                    return out;
+                                };
+                                for (int jj = 0; jj < jbase; ++jj) {
+#pragma unroll
+                                    for (int q = 0; q < kRPT; ++q) step(q, jj);
+                                }
+#pragma unroll
+                                for (int e = 0; e < 8; ++e) {
+#pragma unroll
+                                    for (int q = 0; q < kRPT; ++q) acc[q][e] += step(q, jbase + e);
+                                }
+                            }
+#pragma unroll
+                            for (int q = 0; q < kRPT; ++q)
+                                split_store(acc[q], dst + q * (kRows / kRPT) * 16, dst + q * (kRows / kRPT) * 16 + kBBytes);
+                            dst += (g8 & 1) ? kRows * 16 + kBBytes : kRows * 16;
+                        }
+                    } else {
                     // where this item enters the gene order
                     int i = (16 * s0) / dd, j = 16 * s0 - i * dd;
                     // x in blocks of 4 features (one 16-byte load per block when the rows are 16-byte aligned: a scalar
@@ -784,6 +847,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                             split_store(v[q], dst + q * (kRows / kRPT) * 16, dst + q * (kRows / kRPT) * 16 + kBBytes);
                         dst += (g8 & 1) ? kRows * 16 + kBBytes : kRows * 16;   // next k-group; after the odd one skip the lo half
                     }
+                    }   // per-feature coefficients
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) {

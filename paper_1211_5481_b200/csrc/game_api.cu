@@ -143,7 +143,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (rc) return rc;
     const int scheme = resolved_scheme(c);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients (trigonometric family: d <= 128)");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers trigonometric degrees d <= 128 and, with shared coefficients, G - 1 <= 64");
     if (!c->ticket_zeroed) {
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
         c->ticket_zeroed = true;
@@ -189,6 +189,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         prm.m_pairs_per_group = best_tpu;
         prm.m_groups = (m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
         prm.dd = c->expansion == GAME_EXP_CHEBYSHEV ? c->d : 2 * c->d;
+        prm.shared = c->shared;
         prm.steps = c->steps;
         prm.stages = (c->steps + umma::kKS - 1) / umma::kKS;
         prm.span = prm.stages > 1 ? umma::kKS : (c->steps + 1) / 2;      // one stage only: half of it per producer set
@@ -343,7 +344,10 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     // the tensor-core kernel walks the gene order, so any degree works; for the trigonometric family the fp32 multiple-angle
     // recurrence limits it (fitness error against the fp64 oracle: 2e-6 at d = 100, 2e-5 at d = 400; bound 1e-5)
     const int d_max_umma = expansion == GAME_EXP_TRIG ? 128 : 4096;
-    const bool umma_ok = !shared && d <= d_max_umma && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
+    // shared coefficients: the producers re-run the head of every feature's recurrence per k-group, fine for the short K
+    // extents the paper's model has (G - 1 = d or 2 d <= 64)
+    const bool shared_ok = !shared || d * (expansion == GAME_EXP_TRIG ? 2 : 1) <= 64;
+    const bool umma_ok = shared_ok && d <= d_max_umma && (P + game::umma::kBN - 1) / game::umma::kBN < (1ll << 30);
     if (G > (1 << 20) || (!umma_ok && G > game::kFfmaMaxG)) return GAME_ERR_UNSUPPORTED;   // FFMA kernel: G <= 448
     game_ctx* c = new (std::nothrow) game_ctx();
     if (!c) return GAME_ERR_INVALID_ARG;
@@ -405,7 +409,7 @@ int game_set_scheme(game_ctx* c, int32_t scheme) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (scheme < GAME_SCHEME_AUTO || scheme > GAME_SCHEME_F16X3) return fail(c, GAME_ERR_INVALID_ARG, "unknown scheme %d", scheme);
     if (scheme == GAME_SCHEME_F16X3 && !c->umma_ok)
-        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers per-feature coefficients (trigonometric family: d <= 128)");
+        return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers trigonometric degrees d <= 128 and, with shared coefficients, G - 1 <= 64");
     if (scheme == GAME_SCHEME_FFMA && c->G > game::kFfmaMaxG)
         return fail(c, GAME_ERR_UNSUPPORTED, "FFMA covers G <= 448");
     c->scheme = scheme;

@@ -146,7 +146,12 @@ def test_fails_loudly_without_a_device(L):
 def test_shared_family_gene_counts(L):
     """The paper's literal form (eq.(5), 84-89): 11 features, degree 3, polytrigo -> 7 genes."""
     ctx = game.game_create(200, 11, 3, 23, game.family(game.EXP_TRIG, game.ACT_IDENTITY, shared=True))
-    assert game.game_num_genes(ctx) == 7 and game.game_get_scheme(ctx) == game.SCHEME_FFMA
+    assert game.game_num_genes(ctx) == 7 and game.game_get_scheme(ctx) == game.SCHEME_F16X3
+    game.game_set_scheme(ctx, game.SCHEME_FFMA)
+    assert game.game_get_scheme(ctx) == game.SCHEME_FFMA
+    game.game_destroy(ctx)
+    ctx = game.game_create(200, 11, 40, 23, game.family(game.EXP_TRIG, game.ACT_IDENTITY, shared=True))   # 80 terms > 64
+    assert game.game_num_genes(ctx) == 81 and game.game_get_scheme(ctx) == game.SCHEME_FFMA
     with pytest.raises(game.GameError):
         game.game_set_scheme(ctx, game.SCHEME_F16X3)
     game.game_destroy(ctx)

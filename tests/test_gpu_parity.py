@@ -589,9 +589,10 @@ def test_evolve_fused_rejects_big_problems(game):
 
 
 # ------------------------------------------------------------------------------------------------ shared coefficients
+@pytest.mark.parametrize("scheme", [1, 2])
 @pytest.mark.parametrize("expansion,act,N,d,P,M", [(1, 0, 11, 3, 200, 23), (1, 1, 9, 8, 2100, 19), (0, 1, 7, 5, 1500, 40),
-                                                    (1, 2, 16, 4, 3001, 130)])
-def test_shared_coefficient_mode(game, expansion, act, N, d, P, M):
+                                                    (1, 2, 16, 4, 3001, 130), (0, 2, 5, 33, 700, 300), (1, 1, 3, 32, 900, 70)])
+def test_shared_coefficient_mode(game, expansion, act, N, d, P, M, scheme):
     """The paper's literal model (eq.(2),(5),(7): one coefficient per degree for all features; first case = its worked
     example 11 features, degree 3, 7 genes, 23 chromosomes): fitness, prediction, GA step and the fused loop."""
     import torch
@@ -599,7 +600,7 @@ def test_shared_coefficient_mode(game, expansion, act, N, d, P, M):
     rng = np.random.Generator(np.random.Philox(50 + N))
     X = rng.uniform(-np.pi, np.pi, (P, N)).astype(np.float32) if expansion == 1 else rng.uniform(-1, 1, (P, N)).astype(np.float32)
     t = (rng.uniform(size=P) > 0.5).astype(np.float32)
-    G = game.Game(P, N, d, M, expansion, act, shared=True)
+    G = game.Game(P, N, d, M, expansion, act, shared=True, scheme=scheme)
     assert G.G == oracle.num_genes(N, d, fam) == (2 * d + 1 if expansion == 1 else d + 1)
     G.set_ga_params(2, 3, 0.9, 0.2, 0.1)
     G.load_kb(X, t); G.init_population(3); G.sync()
