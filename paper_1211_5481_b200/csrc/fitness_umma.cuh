@@ -387,6 +387,61 @@ __device__ __forceinline__ void act_err2_quad(float z0, float z1, float z2, floa
     acc3 = fmaf(e3, e3, acc3);
 }
 
+// Packed FP32 pairs (sm_100: FFMA2 / FADD2 / FMUL2 do two IEEE fp32 operations per issued instruction).  The epilogue is
+// bound by issue slots and latency, not by the FMA pipe, so halving the FP32 instruction count is what counts.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+// Eight outputs: two interleaved quads (columns 0,2,4,6 and 1,3,5,7), one in each half of the packed operations, each with
+// ONE reciprocal per four outputs as in act_err2_quad.  tA, tB: staged targets of columns 0..3 and 4..7.  acc: two packed
+// running sums (four scalar sums).
+template <int ACT>
+__device__ __forceinline__ void act_err2_oct(const uint32_t* v, float bias_term, const float4& tA, const float4& tB, f32x2& acc0,
+                                             f32x2& acc1) {
+    const float c = ACT == 1 ? -1.44269504088896340736f : 2.88539008177792681472f;
+    const f32x2 c2 = pack2(c, c), b2 = pack2(bias_term, bias_term), one2 = pack2(1.0f, 1.0f);
+    f32x2 a[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const f32x2 s = fma2(pack2(__uint_as_float(v[2 * k]), __uint_as_float(v[2 * k + 1])), c2, b2);
+        float s0, s1;
+        unpack2(s, s0, s1);
+        a[k] = add2(pack2(ex2_approx(fminf(s0, 30.0f)), ex2_approx(fminf(s1, 30.0f))), one2);
+    }
+    const f32x2 p01 = mul2(a[0], a[1]), p23 = mul2(a[2], a[3]);
+    float q0, q1;
+    unpack2(mul2(p01, p23), q0, q1);
+    f32x2 r = pack2(rcp_approx(q0), rcp_approx(q1));
+    if (ACT == 2) r = mul2(r, pack2(-2.0f, -2.0f));          // tanh = 1 - 2 / a: the staged target is 1 - t
+    const f32x2 r01 = mul2(r, p23), r23 = mul2(r, p01);
+    const float sg = ACT == 1 ? -1.0f : 1.0f;                 // sigmoid: e = 1/a - t; tanh: e = (1 - t) - 2/a
+    const f32x2 e0 = fma2(r01, a[1], pack2(sg * tA.x, sg * tA.y)), e1 = fma2(r01, a[0], pack2(sg * tA.z, sg * tA.w));
+    const f32x2 e2 = fma2(r23, a[3], pack2(sg * tB.x, sg * tB.y)), e3 = fma2(r23, a[2], pack2(sg * tB.z, sg * tB.w));
+    acc0 = fma2(e0, e0, acc0);
+    acc1 = fma2(e1, e1, acc1);
+    acc0 = fma2(e2, e2, acc0);
+    acc1 = fma2(e3, e3, acc1);
+}
+
 // ---------------------------------------------------------------------------------------------- the kernel
 // Shared memory: kStagesTotal stages of 32 KB (kKS = 4 K steps each).  Stages [0, n_a) are the A ring (W operand
 // images streamed from L2 by the loader), used as 2 * n_a slots of kAKS = 2 K steps (16 KB); stages
@@ -612,6 +667,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
+                f32x2 pacc0 = 0ull, pacc1 = 0ull;      // packed running sums of the full 32-column chunks (sigmoid / tanh)
                 // (16 columns at a time with the next chunk's TMEM load in flight was measured twice: 3 % slower.)
 #pragma unroll 1
                 for (int cc = 0; cc < 4; ++cc) {
@@ -622,11 +678,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     const float4* tp = reinterpret_cast<const float4*>(ts + cc * 32);
                     tmem_ld_wait();
                     if (col0 + 32 <= n_valid) {
+                        if (ACT == 0) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i)
-                            act_err2_quad<ACT>(__uint_as_float(v[4 * i + 0]), __uint_as_float(v[4 * i + 1]),
-                                               __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), bias, tp[i], sum, sum1,
-                                               sum2, sum3);
+                            for (int i = 0; i < 8; ++i)
+                                act_err2_quad<ACT>(__uint_as_float(v[4 * i + 0]), __uint_as_float(v[4 * i + 1]),
+                                                   __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), bias, tp[i], sum, sum1,
+                                                   sum2, sum3);
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) act_err2_oct<ACT>(v + 8 * i, bias, tp[2 * i], tp[2 * i + 1], pacc0, pacc1);
+                        }
                     } else {
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
@@ -634,7 +695,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                         }
                     }
                 }
-                sum = (sum + sum1) + (sum2 + sum3);
+                {
+                    float p0, p1, p2, p3;
+                    unpack2(pacc0, p0, p1);
+                    unpack2(pacc1, p2, p3);
+                    sum = ((sum + sum1) + (sum2 + sum3)) + ((p0 + p1) + (p2 + p3));
+                }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8 * buf);
