@@ -13,7 +13,7 @@
 //                          (W_lo.phi_hi, W_hi.phi_lo, W_hi.phi_hi), fp32 accumulators in TMEM; the whole warp runs the
 //                          loop converged and one elected lane issues, so that descriptors stay in uniform registers;
 //                          peer CTA: relays "my stage is full" to the leader's barrier
-//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation (one reciprocal per four outputs), (y-t)^2,
+//   warps 2-9   epilogue : tcgen05.ld 32 columns at a time; activation (packed FP32 pairs, one reciprocal per four outputs), (y-t)^2,
 //                          private per-chromosome sum (TMEM lane = chromosome, so no shuffle is needed); fp64
 //                          accumulation per (CTA, m)
 //   warps 10-17 producers: four sets of 2 warps taking pipeline stages in turn; two patterns per thread walking the gene
