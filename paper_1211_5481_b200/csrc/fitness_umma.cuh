@@ -57,7 +57,7 @@ constexpr int kStageBytes = kKS * kSlotBytes;  // 32768
 constexpr int kStagesTotal = 7;                // 32 KB stages shared by the A ring and the B stages (224 KB)
 constexpr int kMaxResidentStages = 5;          // phi of a whole pattern tile stays in smem up to 20 K steps
 constexpr int kStreamBStages = 3;              // B ring when phi does not fit (regenerated per chromosome tile)
-constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: two sets of 4 warps (128 rows each)
+constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: kNumSets sets of kSetWarps warps (128 rows each)
 constexpr int kRPT = 2;                        // pattern rows per producer thread: two independent recurrences share one
                                                // walk over the gene order (the walk's control was most of a value's cost)
 constexpr int kSetWarps = kRows / (32 * kRPT); // warps that cover the 128 rows of this CTA once: 2
