@@ -655,3 +655,37 @@ def test_random_shapes_fitness_and_step(game):
         ref = oracle.step_sel(W, F, E, 3, selection, 0.9, 0.2, 0.1, trial, trial + 1)
         assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32)), what
         G.close()
+
+
+def test_random_shapes_tensor_path_wide(game):
+    """Seeded sweep of the tensor-core kernel over the corners the fixed cases do not reach together: shared and
+    per-feature coefficients, degrees far beyond a K step, streaming K extents, M and P around the tile edges.  Fitness
+    within 1e-5 of the oracle (IDENTITY activation is kept to G <= 1200: DESIGN.md section 5, measured limit of the scheme)."""
+    import torch
+    rng = np.random.Generator(np.random.Philox(4096))
+    done = 0
+    while done < 24:
+        expansion = int(rng.integers(0, 2)); act = int(rng.integers(0, 3)); shared = bool(rng.integers(0, 3) == 0)
+        if shared:
+            N = int(rng.integers(1, 20)); d = int(rng.integers(1, 33 if expansion else 65))
+        else:
+            N = int(rng.integers(1, 60)); d = int(rng.integers(1, 30 if expansion else 80))
+            while N * d * (2 if expansion else 1) > (1200 if act == 0 else 2000):
+                N = max(1, N // 2); d = max(1, d - 1)
+        P = int(rng.choice([255, 256, 257, 700, 1500, 4000])) + int(rng.integers(0, 3))
+        M = int(rng.choice([1, 2, 127, 128, 129, 255, 256, 257, 700, 1300])) + int(rng.integers(0, 2))
+        Gn = (1 if shared else N) * d * (2 if expansion else 1) + 1
+        if P * M * Gn > 3e8:
+            continue
+        fam = oracle.family(expansion, act, shared=shared)
+        X = (rng.uniform(-np.pi, np.pi, (P, N)) if expansion else rng.uniform(-1, 1, (P, N))).astype(np.float32)
+        t = (rng.uniform(size=P) > 0.5).astype(np.float32) if act == 1 else rng.uniform(-1, 1, P).astype(np.float32)
+        scale = 1.0 / max(1.0, np.sqrt(Gn / 8.0) * (N if shared else 1) ** 0.5)
+        W = (rng.uniform(-1, 1, (M, Gn)) * scale).astype(np.float32)
+        G = game.Game(P, N, d, M, expansion, act, shared=shared, scheme=game.SCHEME_F16X3)
+        G.load_kb(X, t); G.set_population(torch.from_numpy(W).cuda()); G.eval_fitness(); G.sync()
+        F = G.get_fitness()
+        G.close()
+        assert_fitness_close(F, oracle.eval_fitness(d, fam, X, t, W),
+                             f"exp={expansion} act={act} shared={shared} N={N} d={d} P={P} M={M} G={Gn}")
+        done += 1
