@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgame.so")
 SOURCES = [os.path.join(CSRC, "game_api.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("philox.cuh", "ga_kernels.cuh", "fitness_ffma.cuh", "fitness_umma.cuh", "predict.cuh", "ga_fused.cuh")]
+HEADERS = [os.path.join(CSRC, f) for f in ("pdl.cuh", "philox.cuh", "ga_kernels.cuh", "fitness_ffma.cuh", "fitness_umma.cuh", "predict.cuh", "ga_fused.cuh")]
 HEADERS.append(os.path.join(os.path.dirname(HERE), "include", "game.h"))
 
 NVCC_FLAGS = [

@@ -8,6 +8,8 @@
 #pragma once
 #include <cstdint>
 
+#include "pdl.cuh"
+
 namespace game {
 
 constexpr int kFfmaTile = 128;   // patterns per tile == threads per block
@@ -68,6 +70,8 @@ __global__ void __launch_bounds__(kFfmaTile) fitness_ffma_kernel(const float* __
                                                                   int d, int M, int G, int expansion, int act,
                                                                   int m_stride, long long n_tiles,
                                                                   const int* __restrict__ stop, int shared) {
+    pdl_wait();                // W, the partial sums and the stop flag are complete (pdl.cuh)
+    pdl_launch_dependents();
     if (stop != nullptr && *stop != 0) return;
     extern __shared__ float phi[];  // [G][128]
     __shared__ float s_wsum[kFfmaTile / 32][kFfmaMB];

@@ -39,6 +39,8 @@
 
 #include <cstdint>
 
+#include "pdl.cuh"
+
 namespace game {
 namespace umma {
 
@@ -285,6 +287,8 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
     const long long idx = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     const long long total = static_cast<long long>(m_tiles) * steps * 2 * kBM;
     if (idx >= total) return;
+    pdl_wait();                // W (the GA step's children) is complete, and so is the fitness kernel that read the old images
+    pdl_launch_dependents();
     const int row = static_cast<int>(idx % kBM);
     const int kg = static_cast<int>((idx / kBM) % 2);
     const int s = static_cast<int>((idx / (2 * kBM)) % steps);
@@ -474,7 +478,6 @@ struct Ring {
 
 template <int EXPANSION, int ACT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
-    if (prm.stop != nullptr && *prm.stop != 0) return;   // uniform over the grid: written by an earlier kernel
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
     const uint32_t bar_a_full = smem_u32(bars), bar_a_empty = bar_a_full + 8 * kMaxASlots;
@@ -490,7 +493,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const uint32_t crank = cluster_ctarank();            // 0 = leader, 1 = peer
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
-    const int units = prm.p_tiles * prm.m_groups;
+    int units = prm.p_tiles * prm.m_groups;
     const int m_pairs = prm.m_tiles >> 1;
     const uint32_t n_a = prm.n_a, n_b = prm.n_b;
     const uint32_t n_as = 2 * n_a;               // A ring slots of kAKS K steps
@@ -522,6 +525,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     cluster_sync_all();          // both CTAs' barriers are initialised before any remote arrive / multicast commit
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+
+    // Everything above (barriers, TMEM, the cluster handshake) touches no global memory and overlaps the tail of the
+    // preceding kernel (pdl.cuh).  From here on the W images, W, the partial sums and the stop flag are complete.
+    pdl_wait();
+    pdl_launch_dependents();
+    const bool stopped = prm.stop != nullptr && *prm.stop != 0;   // uniform over the grid: written by an earlier kernel
+    if (stopped) units = 0;    // stop rule met: no work, no writes; fall through to the teardown (TMEM is allocated)
 
     if (warp == 0) {
         // ============================================================== loader: W operand images -> A ring
@@ -633,7 +643,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         const int q = warp & 3;                 // TMEM lane quarter this warp may access
         const int h = (warp - 2) >> 2;          // column half
         double* my_part = prm.part + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
-        if (prm.zero_part)
+        if (prm.zero_part && !stopped)
             for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
         const uint32_t leader_acc_empty = map_to_cta(bar_acc_empty, 0);
         uint32_t tile = 0;

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdint>
 
+#include "pdl.cuh"
 #include "philox.cuh"
 
 namespace game {
@@ -144,6 +145,8 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     const int c = blockIdx.x;
     const int tid = threadIdx.x;
     const int M = p.M, G = p.G;
+    pdl_wait();                            // F (finalize), W and, for ranking / roulette, by_rank / prefix are complete
+    pdl_launch_dependents();
     if (stop != nullptr && *stop != 0) {   // stop rule already met: the population is final, carry it over unchanged
         for (int g = tid; g < G; g += kGaThreads) Wn[static_cast<size_t>(c) * G + g] = W[static_cast<size_t>(c) * G + g];
         return;
@@ -255,6 +258,8 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
     // 32 chromosomes per block x 8 row groups: row group g sums partial rows g, g+8, g+16, ... with four independent
     // accumulators (the loads are L2 latency-bound: one thread walking all ~300 rows took 108 us at M = 4096), then the
     // eight group sums are added in group order -- a fixed order, so the result is bit-stable.
+    pdl_wait();                                    // the fitness kernel's partial sums are complete
+    pdl_launch_dependents();
     if (stop != nullptr && stop[0] != 0) return;   // stop rule met earlier: fitness and best trace stay as they are
     __shared__ double s_grp[kFinGroups][kFinCols];
     const int col = threadIdx.x % kFinCols, grp = threadIdx.x / kFinCols;

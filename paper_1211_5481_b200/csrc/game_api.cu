@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -48,6 +49,7 @@ struct game_ctx {
     bool ticket_zeroed = false;
     // GA parameters
     int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0, rmse = 0;
+    bool pdl = true;   // programmatic dependent launch along the generation's kernel chain (pdl.cuh); GAME_PDL=0 turns it off
     double p_cross = 0.9, p_mut = 0.05;
     float sigma = 0.1f;
     // execution
@@ -160,8 +162,8 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (scheme == GAME_SCHEME_F16X3) {
         uint8_t* img = c->ws + c->off_img;
         const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
-        umma::build_w_images_kernel<<<static_cast<unsigned>((n_thr + 255) / 256), 256, 0, c->stream>>>(
-            W, img, c->M, c->G, c->steps, c->m_tiles);
+        launch_chain(c->pdl, umma::build_w_images_kernel, dim3(static_cast<unsigned>((n_thr + 255) / 256)), dim3(256), 0, c->stream,
+                     W, img, c->M, c->G, c->steps, c->m_tiles);
         if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
         umma::Params prm;
         prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.part = part;
@@ -251,7 +253,8 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
             }
             prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = first_launch ? 1 : 0;
             first_launch = false;
-#define GAME_LAUNCH(E, A) umma::fitness_umma_kernel<E, A><<<grid, umma::kThreads, umma::kSmemBytes, c->stream>>>(prm)
+#define GAME_LAUNCH(E, A) \
+    launch_chain(c->pdl && hk == nullptr, umma::fitness_umma_kernel<E, A>, dim3(grid), dim3(umma::kThreads), umma::kSmemBytes, c->stream, prm)
             const int sel = c->expansion * 3 + c->act;
             switch (sel) {
                 case 0: GAME_LAUNCH(0, 0); break;
@@ -283,14 +286,14 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         const int grid = static_cast<int>(grid_ll);
         n_part = grid;
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
-        fitness_ffma_kernel<<<grid, kFfmaTile, smem, c->stream>>>(c->X, c->t, W, part, c->P, c->N, c->d, c->M, c->G,
-                                                                   c->expansion, c->act, c->m_stride, n_tiles, c->stop, c->shared);
+        launch_chain(c->pdl && hk == nullptr, fitness_ffma_kernel, dim3(grid), dim3(kFfmaTile), smem, c->stream,
+                     c->X, c->t, W, part, c->P, c->N, c->d, c->M, c->G, c->expansion, c->act, c->m_stride, n_tiles, c->stop, c->shared);
         if ((rc = check_launch(c, "fitness_ffma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     }
     if (timed) c->events.emplace_back(ev0, ev1);
     const int fin_blocks = (c->M + kFinCols - 1) / kFinCols;
-    finalize_fitness_kernel<<<fin_blocks, kFinThreads, 0, c->stream>>>(
+    launch_chain(c->pdl, finalize_fitness_kernel, dim3(fin_blocks), dim3(kFinThreads), 0, c->stream,
         part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
         reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index, c->rmse);
@@ -322,7 +325,8 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
                                                            reinterpret_cast<unsigned long long*>(c->ws + c->off_prefix));
         if ((rc = check_launch(c, "roulette_prefix_kernel"))) return rc;
     }
-    ga_step_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop);
+    launch_chain(c->pdl, ga_step_kernel, dim3(c->M), dim3(kGaThreads), 0, c->stream,
+                 c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop);
     if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
     c->cur ^= 1;
     c->fitness_valid = false;
@@ -356,6 +360,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->m_tiles = 2 * ((M + 2 * game::umma::kBM - 1) / (2 * game::umma::kBM));   // one chromosome tile per CTA of a pair
     c->m_stride = c->m_tiles * game::umma::kBM;
     c->umma_ok = umma_ok;
+    if (const char* e = std::getenv("GAME_PDL")) c->pdl = e[0] != '0';   // A/B switch for measurements; default on
     c->steps = static_cast<int>((G - 1 + 15) / 16);   // K steps of 16 genes; the bias gene is not part of the contraction
     size_t off = 0;
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
