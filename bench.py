@@ -362,6 +362,7 @@ def run_c4_sweep(args):
             torch.cuda.synchronize()
             game.game_time_fitness_kernel(G.ctx, True)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            launches0 = G.launch_count()
             e0.record()
             for _ in range(args.steps):
                 game.game_eval_fitness(G.ctx)
@@ -369,7 +370,7 @@ def run_c4_sweep(args):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / args.steps
             kms, kn = game.game_fitness_kernel_ms(G.ctx)
-            launches += 3 * args.steps
+            launches += G.launch_count() - launches0      # the library's own count (fitness + finalize per evaluation)
             tf = 6.0 * P * M * (big.G - 1) / (kms / kn * 1e-3) / 1e12
             sweep.append({"M": M, "P": P, "ms_per_eval": ms, "evals_per_s": P * M / (ms * 1e-3), "kernel_ms": kms / kn,
                           "tensor_tflops": tf, "tensor_frac": tf / float(peaks["bf16_tflops"]),

@@ -153,7 +153,10 @@ int game_init_population(game_ctx* ctx, uint64_t seed);
 /* Which of popA/popB is current (device pointer), e.g. to upload or download a population with a
  * plain device copy.  Writing through it is allowed between calls (call game_invalidate_fitness after). */
 int game_current_population(const game_ctx* ctx, float** pop_dev);
-/* Mark the fitness stale (after the caller wrote the current population). */
+/* Mark the fitness stale (after the caller wrote the current population).  REQUIRED after every such write, also when
+ * the fitness is stale already: the tensor-core scheme keeps fp16 hi/lo operand images of the current population in the
+ * workspace (game_step updates them gene by gene as it writes the children, so a generation loop runs no image pass),
+ * and this call is what tells the library to rebuild them from the population at the next evaluation. */
 int game_invalidate_fitness(game_ctx* ctx);
 /* Mark fitness_dev as valid without evaluating (after the caller wrote fitness_dev itself, e.g. to
  * feed the GA operators a given fitness vector -- the "same fitness vector and seed" parity hook). */

@@ -313,6 +313,22 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
     *reinterpret_cast<uint4*>(base + kABytes) = *reinterpret_cast<const uint4*>(lo);
 }
 
+// One gene of chromosome m straight into the W operand images: the same split and the same address as
+// build_w_images_kernel, so that the GA step can keep the images of the population it writes up to date and the
+// generation loop needs no separate image pass.  Gene 0 (the bias) is not on the K axis.  The zero padding (genes past
+// G, rows past M) is written once by build_w_images_kernel and never touched here.
+__device__ __forceinline__ void store_w_image_gene(uint8_t* __restrict__ img, int steps, int m, int g, float w) {
+    if (g < 1) return;
+    const int q = g - 1, kgi = q >> 3, f = q & 7;
+    const int s = kgi >> 1, kg = kgi & 1;
+    const int mt = m / kBM, row = m % kBM;
+    const __half hi = __float2half_rn(w);
+    const __half lo = __float2half_rn(w - __half2float(hi));
+    uint8_t* base = img + (static_cast<size_t>(mt) * steps + s) * (2 * kABytes) + kg * (kBM * 16) + row * 16 + f * 2;
+    *reinterpret_cast<__half*>(base) = hi;
+    *reinterpret_cast<__half*>(base + kABytes) = lo;
+}
+
 // ---------------------------------------------------------------------------------------------- producer helpers
 // lo = v - hi in ONE instruction: the sm_100 mixed-precision FMA (SASS FHFMA) takes the fp16 hi straight from
 // the packed register: fma.rn.f32.f16 d = hi * (-1) + v (exact: v - hi is representable).

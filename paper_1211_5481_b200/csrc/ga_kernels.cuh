@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdint>
 
+#include "fitness_umma.cuh"
 #include "pdl.cuh"
 #include "philox.cuh"
 
@@ -134,10 +135,14 @@ __global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* __re
 //      below `elite` it copies its row, unchanged, to slot `rank` of the new population (elitism);
 //  (2) as child slot c >= elite of the NEW population it runs the two tournaments, the crossover draw
 //      and the per-gene mutation draws for that slot.
+// With `img` != nullptr (tensor-core scheme, images of the OLD population valid) every gene written to the new population
+// is also split into the W operand images of fitness_umma_kernel, which then needs no image pass of its own; under the
+// stop rule rows carry over in place and their images stay as they are.
 __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __restrict__ W,
                                                               const float* __restrict__ F,
                                                               float* __restrict__ Wn, GaParams p,
-                                                              const int* __restrict__ stop) {
+                                                              const int* __restrict__ stop,
+                                                              uint8_t* __restrict__ img, int img_steps) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
     __shared__ int s_rank;
     __shared__ int s_parent[2];
@@ -170,7 +175,11 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     if (rank < p.elite) {
         const float* src = W + static_cast<size_t>(c) * G;
         float* dst = Wn + static_cast<size_t>(rank) * G;
-        for (int g = tid; g < G; g += kGaThreads) dst[g] = src[g];
+        for (int g = tid; g < G; g += kGaThreads) {
+            const float v = src[g];
+            dst[g] = v;
+            if (img != nullptr) umma::store_w_image_gene(img, img_steps, rank, g, v);
+        }
     }
     if (c < p.elite) return;  // slots 0..elite-1 are written by the elites themselves
     if (c >= M - p.immigrants) {
@@ -178,7 +187,9 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
         float* fresh = Wn + static_cast<size_t>(c) * G;
         for (int g = tid; g < G; g += kGaThreads) {
             const uint4 r = philox4x32_10(static_cast<uint32_t>(g >> 2), static_cast<uint32_t>(c), p.gen, kTagImmigrant, p.key);
-            fresh[g] = gene_from_word(word_of(r, g & 3));
+            const float v = gene_from_word(word_of(r, g & 3));
+            fresh[g] = v;
+            if (img != nullptr) umma::store_w_image_gene(img, img_steps, c, g, v);
         }
         return;
     }
@@ -235,6 +246,7 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
             v = __fadd_rn(v, __fmul_rn(p.sigma, z));
         }
         child[g] = v;
+        if (img != nullptr) umma::store_w_image_gene(img, img_steps, c, g, v);
     }
 }
 

@@ -46,6 +46,7 @@ struct game_ctx {
     unsigned char* ws = nullptr;
     int cur = 0;
     bool fitness_valid = false;
+    bool img_valid = false;   // the W operand images in the workspace are those of the current population
     bool ticket_zeroed = false;
     // GA parameters
     int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0, rmse = 0;
@@ -162,9 +163,12 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (scheme == GAME_SCHEME_F16X3) {
         uint8_t* img = c->ws + c->off_img;
         const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
-        launch_chain(c->pdl, umma::build_w_images_kernel, dim3(static_cast<unsigned>((n_thr + 255) / 256)), dim3(256), 0, c->stream,
-                     W, img, c->M, c->G, c->steps, c->m_tiles);
-        if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
+        if (!c->img_valid) {   // inside a generation loop the GA step keeps the images up to date (ga_step_kernel)
+            launch_chain(c->pdl, umma::build_w_images_kernel, dim3(static_cast<unsigned>((n_thr + 255) / 256)), dim3(256), 0,
+                         c->stream, W, img, c->M, c->G, c->steps, c->m_tiles);
+            if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
+            c->img_valid = true;
+        }
         umma::Params prm;
         prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.part = part;
         prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
@@ -326,7 +330,8 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
         if ((rc = check_launch(c, "roulette_prefix_kernel"))) return rc;
     }
     launch_chain(c->pdl, ga_step_kernel, dim3(c->M), dim3(kGaThreads), 0, c->stream,
-                 c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop);
+                 c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop,
+                 c->img_valid ? c->ws + c->off_img : static_cast<uint8_t*>(nullptr), c->steps);
     if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
     c->cur ^= 1;
     c->fitness_valid = false;
@@ -453,6 +458,7 @@ int game_bind_state(game_ctx* c, float* popA_dev, float* popB_dev, float* fitnes
     c->ws = static_cast<unsigned char*>(workspace_dev);
     c->cur = 0;
     c->fitness_valid = false;
+    c->img_valid = false;
     c->ticket_zeroed = false;
     return GAME_OK;
 }
@@ -502,6 +508,7 @@ int game_init_population(game_ctx* c, uint64_t seed) {
                                                                                                game::make_key(seed));
     if ((rc = check_launch(c, "init_population_kernel"))) return rc;
     c->fitness_valid = false;
+    c->img_valid = false;
     return GAME_OK;
 }
 
@@ -515,6 +522,7 @@ int game_current_population(const game_ctx* c, float** pop_dev) {
 int game_invalidate_fitness(game_ctx* c) {
     if (!c) return GAME_ERR_INVALID_ARG;
     c->fitness_valid = false;
+    c->img_valid = false;     // the caller wrote the population: the W operand images are rebuilt by the next evaluation
     return GAME_OK;
 }
 
@@ -612,6 +620,7 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
     if ((rc = check_launch(c, "ga_fused_kernel"))) return rc;
     if (n_gens & 1u) c->cur ^= 1;
     c->fitness_valid = false;
+    c->img_valid = false;
     return GAME_OK;
 }
 
@@ -642,6 +651,7 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     const size_t wb = sizeof(float) * static_cast<size_t>(c->M) * c->G;
     GAME_CUDA(cudaMemcpyAsync(c->pop[c->cur], W_host, wb, cudaMemcpyHostToDevice, c->stream));
     c->fitness_valid = false;
+    c->img_valid = false;
     const HostKb hk{X_host, t_host};
     int rc = ensure_device(c);
     if (rc) return rc;

@@ -545,6 +545,33 @@ def test_rmse_metric(game, scheme):
     G.close()
 
 
+@pytest.mark.parametrize("base,over,selection,immigrants", [
+    ("c1", dict(P=1500, M=300), 0, 0), ("c3", dict(P=600, M=257), 1, 5), ("c2", dict(P=900, M=131), 2, 3),
+    ("c0", dict(P=300, M=37), 0, 2)])
+def test_step_keeps_w_images(game, base, over, selection, immigrants):
+    """Inside a generation loop the GA step writes the W operand images of the tensor-core kernel itself (elites,
+    children, immigrants), and the next evaluation runs no image pass.  The fitness it then computes must be
+    bit-identical to the one computed from images rebuilt from scratch for the same population (set_population
+    invalidates them), generation after generation; and it stays within 1e-5 of the oracle."""
+    cfg = wl.scaled(wl.CONFIGS[base], **over)
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg, game.SCHEME_F16X3); G.load_kb(X, t)
+    game.game_set_selection(G.ctx, selection); game.game_set_immigrants(G.ctx, immigrants)
+    H = make(game, cfg, game.SCHEME_F16X3); H.load_kb(X, t)       # every evaluation from rebuilt images
+    G.init_population(9)
+    for gen in range(4):
+        n0 = G.launch_count()
+        G.eval_fitness(); G.sync()
+        assert G.launch_count() - n0 == (3 if gen == 0 else 2)     # image pass only before the first generation
+        F = G.get_fitness()
+        W = G.get_population()
+        H.set_population(W); H.eval_fitness(); H.sync()
+        assert np.array_equal(F.view(np.uint32), H.get_fitness().view(np.uint32)), f"generation {gen}"
+        G.step(21, gen); G.sync()
+    assert_fitness_close(F, oracle.eval_fitness(cfg.d, cfg.family, X, t, W), "after three in-step image updates")
+    G.close(); H.close()
+
+
 # ------------------------------------------------------------------------------------------------ fused persistent loop
 @pytest.mark.parametrize("base,over,selection,immigrants", [
     ("c0", {}, 0, 0), ("c0", dict(P=777, M=37), 1, 3), ("n1", {}, 1, 0), ("n1", dict(P=500, M=23), 2, 2),
