@@ -253,7 +253,7 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
 // ---- fitness finalisation: F[m] = (sum over partial rows, in row order) / P in fp64, rounded to fp32
 // (PAPER.md:63 MSE).  Optionally the best (lowest, NaN worst, ties -> lower index) fitness of the
 // population is written to *best_out by the last block to finish (R8).
-constexpr int kFinThreads = 256, kFinCols = 32, kFinGroups = kFinThreads / kFinCols;
+constexpr int kFinThreads = 1024, kFinCols = 32, kFinGroups = kFinThreads / kFinCols;
 
 __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* __restrict__ part,
                                                                         int n_part, int m_stride, int M,
@@ -267,9 +267,10 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
     __shared__ bool s_last;
-    // 32 chromosomes per block x 8 row groups: row group g sums partial rows g, g+8, g+16, ... with four independent
-    // accumulators (the loads are L2 latency-bound: one thread walking all ~300 rows took 108 us at M = 4096), then the
-    // eight group sums are added in group order -- a fixed order, so the result is bit-stable.
+    // 32 chromosomes per block x 32 row groups: row group g sums partial rows g, g+32, g+64, ... with four independent
+    // accumulators (the loads are L2 latency-bound: one thread walking all ~300 rows took 108 us at M = 4096; 8 groups
+    // 15 us, of which ten dependent L2 round trips), then the 32 group sums are added in group order -- a fixed order, so the
+    // result is bit-stable.
     pdl_wait();                                    // the fitness kernel's partial sums are complete
     pdl_launch_dependents();
     if (stop != nullptr && stop[0] != 0) return;   // stop rule met earlier: fitness and best trace stay as they are
@@ -285,7 +286,9 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
 #pragma unroll
             for (int i = 0; i < 4; ++i) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
         }
-        for (int i = 0; r < n_part; r += kFinGroups, ++i) acc[i] += __ldcg(part + static_cast<size_t>(r) * m_stride + m);
+#pragma unroll
+        for (int i = 0; i < 3; ++i)      // the tail: at most three rows, same accumulator per position as above
+            if (r + i * kFinGroups < n_part) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
     }
     s_grp[grp][col] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
     __syncthreads();
