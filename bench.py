@@ -40,7 +40,7 @@ UNIT = "evals/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists).
-NCU_TRAFFIC_BYTES = {"c3": 548385024}      # profiles/r01h_README.md: 535.5 MB read + 12.9 MB written
+NCU_TRAFFIC_BYTES = {"c3": 546093312}      # profiles/r01i_README.md: 536.5 MB read + 9.6 MB written
 
 
 def parse_args():
