@@ -572,6 +572,32 @@ def test_step_keeps_w_images(game, base, over, selection, immigrants):
     G.close(); H.close()
 
 
+@pytest.mark.parametrize("base,over,scheme,selection", [
+    ("c0", {}, 2, 0), ("c1", dict(P=6000, M=300), 2, 1), ("c2", dict(P=2500, M=131), 2, 2), ("c1", dict(P=3000, M=64), 1, 0)])
+def test_dependent_launch_chain_is_race_free(game, base, over, scheme, selection, monkeypatch):
+    """The generation's kernels run under programmatic dependent launch (csrc/pdl.cuh): each one is launched while its
+    predecessor still runs and parks in griddepcontrol.wait.  A missing or misplaced wait would let a kernel read what its
+    predecessor has not written yet, so 40 generations enqueued back to back must give the same populations, fitness
+    vectors and best-fitness trace, bit for bit, as the same run with plain stream-ordered launches (GAME_PDL=0)."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS[base], **over)
+    X, t, _ = wl.make_kb(cfg)
+    n = 40
+    out = []
+    for pdl in ("0", "1", "1"):
+        monkeypatch.setenv("GAME_PDL", pdl)                 # read by game_create
+        G = make(game, cfg, scheme); G.load_kb(X, t)
+        game.game_set_selection(G.ctx, selection); game.game_set_immigrants(G.ctx, 2)
+        best = torch.zeros(n + 1, dtype=torch.float32, device="cuda")
+        G.init_population(17); G.run(17, 0, n, best); G.sync()
+        out.append((G.get_population().view(np.uint32), G.get_fitness().view(np.uint32), best.cpu().numpy().view(np.uint32)))
+        G.close()
+    for a, b in zip(out[0], out[1]):
+        assert np.array_equal(a, b)
+    for a, b in zip(out[1], out[2]):
+        assert np.array_equal(a, b)
+
+
 # ------------------------------------------------------------------------------------------------ fused persistent loop
 @pytest.mark.parametrize("base,over,selection,immigrants", [
     ("c0", {}, 0, 0), ("c0", dict(P=777, M=37), 1, 3), ("n1", {}, 1, 0), ("n1", dict(P=500, M=23), 2, 2),
