@@ -54,7 +54,8 @@ enum {
  *   shared    : 0 per-feature coefficients (BASELINE.json: G = N*d+1 / N*2d+1), 1 the paper's literal form (PAPER.md:52-55
  *               eq.(2), 75-77 eq.(5), 84-89): ONE coefficient per degree for all features, G = d+1 (Chebyshev) or 2d+1
  *               (trig, gene order [a_0, a_1..a_d, b_1..b_d]); the expansion term of gene j is the sum over the features of
- *               g_j(f_i) (the per-pattern sums of PAPER.md:110).  Shared mode runs on the FFMA scheme and the fused loop.
+ *               g_j(f_i) (the per-pattern sums of PAPER.md:110).  Shared mode runs on every path: the tensor-core scheme up to 64 terms
+ *               (G - 1 <= 64), the FFMA scheme and the fused loop.
  * BASELINE.json configs c0,c1,c3,c4 = 0x0100; c2 = 0x0201. */
 enum { GAME_FAMILY_SHARED = 1 << 16 };
 enum { GAME_EXP_CHEBYSHEV = 0, GAME_EXP_TRIG = 1 };

@@ -63,16 +63,16 @@ __device__ __forceinline__ void expand_pattern(const float* __restrict__ xr, boo
     }
 }
 
+// X and t are never written by the library's kernels (non-coherent loads are fine); W and the stop flag are written by
+// earlier kernels of the launch chain (pdl.cuh) and are read with ld.global.cg after griddepcontrol.wait.
 __global__ void __launch_bounds__(kFfmaTile) fitness_ffma_kernel(const float* __restrict__ X,
                                                                   const float* __restrict__ t,
-                                                                  const float* __restrict__ W,
-                                                                  double* __restrict__ part, long long P, int N,
+                                                                  const float* W, double* part, long long P, int N,
                                                                   int d, int M, int G, int expansion, int act,
-                                                                  int m_stride, long long n_tiles,
-                                                                  const int* __restrict__ stop, int shared) {
+                                                                  int m_stride, long long n_tiles, const int* stop, int shared) {
     pdl_wait();                // W, the partial sums and the stop flag are complete (pdl.cuh)
     pdl_launch_dependents();
-    if (stop != nullptr && *stop != 0) return;
+    if (stop != nullptr && __ldcg(stop) != 0) return;
     extern __shared__ float phi[];  // [G][128]
     __shared__ float s_wsum[kFfmaTile / 32][kFfmaMB];
     const int tid = threadIdx.x;
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(kFfmaTile) fitness_ffma_kernel(const float* __
             for (int g = 0; g < G; ++g) {
                 const float ph = phi[g * kFfmaTile + tid];
 #pragma unroll
-                for (int i = 0; i < kFfmaMB; ++i) z[i] = fmaf(__ldg(wrow[i] + g), ph, z[i]);
+                for (int i = 0; i < kFfmaMB; ++i) z[i] = fmaf(__ldcg(wrow[i] + g), ph, z[i]);
             }
 #pragma unroll
             for (int i = 0; i < kFfmaMB; ++i) {

@@ -59,6 +59,11 @@ constexpr int kStageBytes = kKS * kSlotBytes;  // 32768
 constexpr int kStagesTotal = 7;                // 32 KB stages shared by the A ring and the B stages (224 KB)
 constexpr int kMaxResidentStages = 5;          // phi of a whole pattern tile stays in smem up to 20 K steps
 constexpr int kStreamBStages = 3;              // B ring when phi does not fit (regenerated per chromosome tile)
+constexpr int kFlushStages = 5;                // streaming mode: the K extent is accumulated in chunks of 5 stages (20 K steps,
+                                               // 60 MMAs) and the chunks are added in fp32 by the epilogue.  The tensor core
+                                               // adds into the TMEM accumulator with truncation, which shrinks |z| by ~1.6e-8 per
+                                               // MMA (measured: 1.25e-5 after the 450 MMAs of G = 2401, identity output); with
+                                               // the chunks the shrink is that of one chunk, whatever G is
 constexpr int kNumEpiWarps = 8, kNumProdWarps = 8;   // producers: kNumSets sets of kSetWarps warps (128 rows each)
 constexpr int kRPT = 2;                        // pattern rows per producer thread: two independent recurrences share one
                                                // walk over the gene order (the walk's control was most of a value's cost)
@@ -77,12 +82,25 @@ constexpr int kTsBytes = kBN * 4;                 // targets of the current patt
 constexpr int kSmemBytes = kSmemBar + kBarBytes + kTsBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
 static_assert(kSmemBytes <= 232448, "shared memory budget");
+// Operand pre-scaling (both powers of two, so exact, and undone by the epilogue's FFMA constant).  An fp16 hi/lo split is
+// only RELATIVE down to 2^-14: below that the lo half is an fp16 subnormal (quantum 2^-24) and an operand of magnitude
+// 1e-5 would carry an absolute error of 3e-8.  So each chromosome row is scaled so that its largest gene lands in
+// [2^13, 2^14) (a gene 2^15 times smaller than the row's largest still has a normal lo half; below that the absolute
+// error is 2^-38 of the row's largest gene), and phi (|phi| <= 1 for Chebyshev on |x| <= 1 and for the trigonometric
+// family) is generated times 16 by starting its recurrence from 16 instead of 1 (range: |phi| < 4094).
+constexpr int kPhiScaleLog2 = 4;
+constexpr float kPhiScale = 16.0f;
+constexpr int kRowTargetExp = 13;
 
 struct Params {
     const float* X;        // [P][N]
     const float* t;        // [P]
     const float* W;        // [M][G]: only gene 0 (the bias a_0) is read here, by the epilogue
     const uint8_t* Wimg;   // [m_tiles][steps][8192]: A_hi (2 k-groups x 128 rows x 16 B), then A_lo
+    const float* wscale;   // [m_stride]: what the accumulated z of a row has to be multiplied by (row and phi scales undone,
+                           //             times the row's calibrated accumulation correction, see calibrate_kernel)
+    float* zdump;          // calibration launch only (else NULL): [m_stride][256] raw accumulated z of pattern tile p_tile0;
+                           //             no error sums are formed
     double* part;          // [gridDim.x * 2][m_stride]
     const int* stop;       // optional: non-zero => the stop rule is met, the kernel returns at once
     long long* stall;      // optional [gridDim.x][4]: cycles the MMA/relay warp waited on a_full, b_full, acc_empty; total
@@ -104,6 +122,8 @@ struct Params {
     int resident;          // 1: phi generated once per unit and reused by all its chromosome tiles; n_b == stages, or
                            //    2 * stages (phi of the next unit is generated while this one is consumed)
     int n_a, n_b;          // A ring stages, B stages (n_a + n_b <= kStagesTotal)
+    int flush;             // 1 (streaming mode): accumulate kFlushStages stages at a time, chunk 0 into accumulator 0, the later
+                           //    chunks into accumulator 1, which the epilogue adds to accumulator 0 (fp32, round to nearest)
 };
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -150,12 +170,24 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return done;
 }
+// The bound of every wait is 20 s of globaltimer, looked at every 2^16 failed polls (a poll count alone could trip under
+// time-slicing, MPS or a debugger).
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void wait_watchdog(uint32_t& n, unsigned long long& t0) {
+    if ((++n & 0xffffu) != 0) return;
+    const unsigned long long now = global_timer_ns();
+    if (t0 == 0) t0 = now;
+    else if (now - t0 > 20000000000ull) __trap();
+}
 // Critical-path waits (MMA issuer, relay, loader): tight poll, three instructions per iteration.
 __device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
     uint32_t n = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if (++n > (1u << 26)) __trap();
-    }
+    unsigned long long t0 = 0;
+    while (!mbar_try_wait(bar, parity)) wait_watchdog(n, t0);
 }
 // Waits of warps that are ahead of the pipeline (producers on a full ring, epilogue on an accumulator still
 // being computed): back off with nanosleep so that polling does not steal issue slots from the working warps
@@ -164,9 +196,10 @@ template <int NS>
 __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     uint32_t n = 0;
+    unsigned long long t0 = 0;
     do {
         __nanosleep(NS);
-        if (++n > (1u << 24)) __trap();
+        wait_watchdog(n, t0);
     } while (!mbar_try_wait(bar, parity));
 }
 // Long waits (the producers of a resident unit wait for a whole unit, ~100 us at c3): exponential back-off up to
@@ -176,10 +209,11 @@ template <int MAX_NS>
 __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     uint32_t n = 0, ns = 32;
+    unsigned long long t0 = 0;
     do {
         __nanosleep(ns);
         ns = min(2 * ns, static_cast<uint32_t>(MAX_NS));
-        if (++n > (1u << 24)) __trap();
+        wait_watchdog(n, t0);
     } while (!mbar_try_wait(bar, parity));
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
@@ -219,9 +253,8 @@ __device__ __forceinline__ bool warp_try_wait(uint32_t bar, uint32_t parity) {
 }
 __device__ __forceinline__ void warp_wait_spin(uint32_t bar, uint32_t parity) {
     uint32_t n = 0;
-    while (!warp_try_wait(bar, parity)) {
-        if (++n > (1u << 26)) __trap();
-    }
+    unsigned long long t0 = 0;
+    while (!warp_try_wait(bar, parity)) wait_watchdog(n, t0);
 }
 // D[tmem, both CTAs] (+)= A[smem of both CTAs] . B[smem of both CTAs]; issued by one thread of the leader CTA.
 __device__ __forceinline__ void umma_f16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -250,6 +283,17 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
         : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+        "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]),
+        "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]),
+        "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -280,20 +324,46 @@ __host__ __device__ inline int gene_at(int s, int kg, int f, int G) {
     return g < G ? g : -1;
 }
 
+// Power-of-two scale of a chromosome row from the largest magnitude among its genes 1..G-1 (the bias gene is not on the K
+// axis): 2^k amax in [2^13, 2^14).  Rows without a finite positive maximum (all zero, Inf, NaN) are left unscaled, so
+// that non-finite genes still propagate to a non-finite fitness.  k is clamped so that 2^k and 2^-k / 16 stay normal.
+__device__ __forceinline__ int row_scale_exp(float amax) {
+    if (!(amax > 0.0f) || !(amax < INFINITY)) return 0;
+    const int k = kRowTargetExp - ilogbf(amax);
+    return max(-100, min(100, k));
+}
+// the factor the epilogue applies to the accumulated z of such a row: 2^-k / kPhiScale
+__device__ __forceinline__ float row_unscale(int k) { return ldexpf(1.0f, -k - kPhiScaleLog2); }
+__device__ __forceinline__ float row_scale_of_unscale(float f) { return 1.0f / (f * kPhiScale); }   // 2^k back from 2^-k / 16: exact
+
+// wscale[m] for every row of the padded population (rows >= M: unscaled).  One warp per row.
+__global__ void row_scale_kernel(const float* W, float* wscale, int M, int G, int m_stride) {
+    pdl_wait();                // W is complete, and so is the fitness kernel that read the old scales
+    pdl_launch_dependents();
+    const int m = static_cast<int>((static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (m >= m_stride) return;
+    float amax = 0.0f;
+    if (m < M)
+        for (int g = 1 + lane; g < G; g += 32) amax = fmaxf(amax, fabsf(__ldcg(W + static_cast<size_t>(m) * G + g)));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    if (lane == 0) wscale[m] = row_unscale(row_scale_exp(amax));
+}
+
 // W [M][G] fp32 -> per (m_tile, step) 8 KB images: A_hi then A_lo, each [2 k-groups][128 rows][8 fp16].
 // hi = rn_f16(w), lo = rn_f16(w - hi).  One thread per (m_tile, step, k-group, row).
-__global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __restrict__ img, int M, int G, int steps,
-                                      int m_tiles) {
+__global__ void build_w_images_kernel(const float* W, const float* wscale, uint8_t* img, int M, int G, int steps, int m_tiles) {
     const long long idx = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     const long long total = static_cast<long long>(m_tiles) * steps * 2 * kBM;
     if (idx >= total) return;
-    pdl_wait();                // W (the GA step's children) is complete, and so is the fitness kernel that read the old images
+    pdl_wait();                // W and the row scales are complete, and so is the fitness kernel that read the old images
     pdl_launch_dependents();
     const int row = static_cast<int>(idx % kBM);
     const int kg = static_cast<int>((idx / kBM) % 2);
     const int s = static_cast<int>((idx / (2 * kBM)) % steps);
     const int mt = static_cast<int>(idx / (2ll * kBM * steps));
     const int m = mt * kBM + row;
+    const float scale = row_scale_of_unscale(__ldcg(wscale + m));
     __half2 hi[4], lo[4];
 #pragma unroll
     for (int f2 = 0; f2 < 4; ++f2) {
@@ -301,7 +371,7 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const int g = gene_at(s, kg, f2 * 2 + e, G);
-            w[e] = (g >= 0 && m < M) ? W[static_cast<size_t>(m) * G + g] : 0.0f;
+            w[e] = (g >= 0 && m < M) ? __ldcg(W + static_cast<size_t>(m) * G + g) * scale : 0.0f;
         }
         const __half2 h = __floats2half2_rn(w[0], w[1]);
         const float2 hf = __half22float2(h);
@@ -313,11 +383,11 @@ __global__ void build_w_images_kernel(const float* __restrict__ W, uint8_t* __re
     *reinterpret_cast<uint4*>(base + kABytes) = *reinterpret_cast<const uint4*>(lo);
 }
 
-// One gene of chromosome m straight into the W operand images: the same split and the same address as
-// build_w_images_kernel, so that the GA step can keep the images of the population it writes up to date and the
-// generation loop needs no separate image pass.  Gene 0 (the bias) is not on the K axis.  The zero padding (genes past
-// G, rows past M) is written once by build_w_images_kernel and never touched here.
-__device__ __forceinline__ void store_w_image_gene(uint8_t* __restrict__ img, int steps, int m, int g, float w) {
+// One gene of chromosome m, already multiplied by its row's scale, straight into the W operand images: the same split
+// and the same address as build_w_images_kernel, so that the GA step can keep the images of the population it writes up
+// to date and the generation loop needs no separate image pass.  Gene 0 (the bias) is not on the K axis.  The zero padding
+// (genes past G, rows past M) is written once by build_w_images_kernel and never touched here.
+__device__ __forceinline__ void store_w_image_gene(uint8_t* img, int steps, int m, int g, float w) {
     if (g < 1) return;
     const int q = g - 1, kgi = q >> 3, f = q & 7;
     const int s = kgi >> 1, kg = kgi & 1;
@@ -327,6 +397,90 @@ __device__ __forceinline__ void store_w_image_gene(uint8_t* __restrict__ img, in
     uint8_t* base = img + (static_cast<size_t>(mt) * steps + s) * (2 * kABytes) + kg * (kBM * 16) + row * 16 + f * 2;
     *reinterpret_cast<__half*>(base) = hi;
     *reinterpret_cast<__half*>(base + kABytes) = lo;
+}
+
+// ---------------------------------------------------------------------------------------------- calibration
+// The tensor core adds into its fp32 accumulator with TRUNCATION (round toward zero), so every MMA shrinks |z| a little:
+// z_tensor = z (1 - eps), eps ~ 1.6e-8 per MMA (measured: 3.9e-7 for the 24 MMAs of G = 121, 1.25e-5 for the 450 of
+// G = 2401).  For a classifier that is far inside the 1e-5 fitness bound, but the error is SYSTEMATIC: on a regression fit
+// whose residual r = y - t is small against z it does not average out over the patterns, dF/F = -2 eps <z r> / <r r>,
+// up to eps sqrt<z z> / sigma for residual noise sigma (measured 8.9e-5 at sigma = 0.01, identity output).
+// So for the regression activations (identity, tanh) the shrink of every chromosome row is MEASURED before each
+// evaluation: one extra launch of the fitness kernel hands out the raw accumulators of the first pattern tile
+// (Params::zdump), this kernel recomputes the same z for those <= 256 patterns on the CUDA cores (fp32 expansion as in the
+// producers, products and sum in fp64) and fits z_exact = (1 + eps_m) z_tensor by least squares; the evaluation then runs
+// with the row's un-scaling factor times (1 + eps_m).  One block per chromosome, one thread per sample pattern.
+constexpr int kCalThreads = kBN;         // one thread per sample pattern
+template <int EXPANSION>
+__global__ void __launch_bounds__(kCalThreads) calibrate_kernel(const float* __restrict__ X, const float* W, const float* zdump,
+                                                                const float* wscale, float* zcorr, const int* stop, long long P,
+                                                                int N, int d, int M, int G, int shared, int stage_w) {
+    extern __shared__ float cal_w[];       // [G] when stage_w: this chromosome (longer ones are read through the caches)
+    __shared__ double s_num[kCalThreads / 32], s_den[kCalThreads / 32];
+    pdl_wait();                // the calibration launch's accumulators, W and the row scales are complete
+    pdl_launch_dependents();
+    if (stop != nullptr && __ldcg(stop) != 0) return;
+    const int m = blockIdx.x, p = threadIdx.x;      // one block per chromosome row of the padded population
+    const float f = __ldcg(wscale + m);
+    if (m >= M) {
+        if (p == 0) zcorr[m] = f;
+        return;
+    }
+    const float* w = W + static_cast<size_t>(m) * G;
+    if (stage_w) {
+        for (int g = p; g < G; g += kCalThreads) cal_w[g] = __ldcg(w + g);
+        __syncthreads();
+        w = cal_w;
+    }
+    const int n = static_cast<int>(min(static_cast<long long>(kBN), P));
+    const int dd = EXPANSION == 0 ? d : 2 * d;
+    double num = 0.0, den = 0.0;
+    if (p < n) {
+        const float* xr = X + static_cast<size_t>(p) * N;
+        double z = 0.0;
+        for (int i = 0; i < N; ++i) {
+            const float x = __ldg(xr + i);
+            const float* wi = w + 1 + (shared ? 0 : i * dd);
+            if (EXPANSION == 0) {
+                const float x2 = 2.0f * x;
+                float tm = 1.0f, tc = x;
+                for (int j = 0; j < d; ++j) {
+                    z += static_cast<double>(wi[j]) * static_cast<double>(tc);
+                    const float tn = fmaf(x2, tc, -tm);
+                    tm = tc; tc = tn;
+                }
+            } else {
+                float s1, c1;
+                sincosf(x, &s1, &c1);
+                const float x2 = 2.0f * c1;
+                float cm = 1.0f, cc = c1, sm = 0.0f, sc = s1;
+                for (int k = 0; k < d; ++k) {
+                    z += static_cast<double>(wi[k]) * static_cast<double>(cc);
+                    z += static_cast<double>(wi[d + k]) * static_cast<double>(sc);
+                    const float cn = fmaf(x2, cc, -cm), sn = fmaf(x2, sc, -sm);
+                    cm = cc; cc = cn;
+                    sm = sc; sc = sn;
+                }
+            }
+        }
+        const double zt = static_cast<double>(__ldcg(zdump + static_cast<size_t>(m) * kBN + p)) * static_cast<double>(f);
+        num = (z - zt) * zt;
+        den = zt * zt;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        num += __shfl_xor_sync(0xffffffffu, num, o);
+        den += __shfl_xor_sync(0xffffffffu, den, o);
+    }
+    if ((p & 31) == 0) { s_num[p >> 5] = num; s_den[p >> 5] = den; }
+    __syncthreads();
+    if (p == 0) {
+        num = 0.0; den = 0.0;
+        for (int wv = 0; wv < kCalThreads / 32; ++wv) { num += s_num[wv]; den += s_den[wv]; }   // fixed order: bit-stable
+        double eps = den > 0.0 ? num / den : 0.0;
+        if (!(fabs(eps) <= 1e-4)) eps = 0.0;       // non-finite rows, or a row the model does not describe: leave it alone
+        zcorr[m] = static_cast<float>(static_cast<double>(f) * (1.0 + eps));
+    }
 }
 
 // ---------------------------------------------------------------------------------------------- producer helpers
@@ -363,15 +517,21 @@ __device__ __forceinline__ float bias_term_of(float a0) {
 // `tq` is the staged target: t itself, or 1 - t for tanh (so that 1 - 2 r - t is one FFMA).
 template <int ACT>
 __device__ __forceinline__ float staged_target(float t) { return ACT == 2 ? 1.0f - t : t; }
+// `zs` turns the accumulated (pre-scaled) z into the argument: row and phi scales undone, times -log2(e) (sigmoid),
+// 2 log2(e) (tanh) or 1 (identity); a power of two times that constant, so no rounding is added.
 template <int ACT>
-__device__ __forceinline__ float act_err2(float z, float bias_term, float tq) {
+__device__ __forceinline__ float zscale_of(float unscale) {
+    return ACT == 1 ? -1.44269504088896340736f * unscale : (ACT == 2 ? 2.88539008177792681472f * unscale : unscale);
+}
+template <int ACT>
+__device__ __forceinline__ float act_err2(float z, float zs, float bias_term, float tq) {
     float e;
     if (ACT == 1) {
-        e = rcp_approx(1.0f + ex2_approx(fmaf(z, -1.44269504088896340736f, bias_term))) - tq;
+        e = rcp_approx(1.0f + ex2_approx(fmaf(z, zs, bias_term))) - tq;
     } else if (ACT == 2) {
-        e = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(fmaf(z, 2.88539008177792681472f, bias_term))), tq);
+        e = fmaf(-2.0f, rcp_approx(1.0f + ex2_approx(fmaf(z, zs, bias_term))), tq);
     } else {
-        e = (z + bias_term) - tq;
+        e = fmaf(z, zs, bias_term) - tq;
     }
     return e * e;
 }
@@ -380,16 +540,15 @@ __device__ __forceinline__ float act_err2(float z, float bias_term, float tq) {
 // operations per output instead of 2 (1.5 with pairs) for 1.25 extra FMULs.  The exponent is clamped at 30 so that the
 // product stays finite (<= 2^121); sigmoid / 1 - tanh below 2^-30 are below fp32 resolution of the error against t.
 template <int ACT>
-__device__ __forceinline__ void act_err2_quad(float z0, float z1, float z2, float z3, float bias_term, float4 tq, float& acc0,
+__device__ __forceinline__ void act_err2_quad(float z0, float z1, float z2, float z3, float c, float bias_term, float4 tq, float& acc0,
                                               float& acc1, float& acc2, float& acc3) {
     if (ACT == 0) {
-        acc0 += act_err2<ACT>(z0, bias_term, tq.x);
-        acc1 += act_err2<ACT>(z1, bias_term, tq.y);
-        acc2 += act_err2<ACT>(z2, bias_term, tq.z);
-        acc3 += act_err2<ACT>(z3, bias_term, tq.w);
+        acc0 += act_err2<ACT>(z0, c, bias_term, tq.x);
+        acc1 += act_err2<ACT>(z1, c, bias_term, tq.y);
+        acc2 += act_err2<ACT>(z2, c, bias_term, tq.z);
+        acc3 += act_err2<ACT>(z3, c, bias_term, tq.w);
         return;
     }
-    const float c = ACT == 1 ? -1.44269504088896340736f : 2.88539008177792681472f;
     const float a0 = 1.0f + ex2_approx(fminf(fmaf(z0, c, bias_term), 30.0f));
     const float a1 = 1.0f + ex2_approx(fminf(fmaf(z1, c, bias_term), 30.0f));
     const float a2 = 1.0f + ex2_approx(fminf(fmaf(z2, c, bias_term), 30.0f));
@@ -435,9 +594,8 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
 // ONE reciprocal per four outputs as in act_err2_quad.  tA, tB: staged targets of columns 0..3 and 4..7.  acc: two packed
 // running sums (four scalar sums).
 template <int ACT>
-__device__ __forceinline__ void act_err2_oct(const uint32_t* v, float bias_term, const float4& tA, const float4& tB, f32x2& acc0,
+__device__ __forceinline__ void act_err2_oct(const uint32_t* v, float c, float bias_term, const float4& tA, const float4& tB, f32x2& acc0,
                                              f32x2& acc1) {
-    const float c = ACT == 1 ? -1.44269504088896340736f : 2.88539008177792681472f;
     const f32x2 c2 = pack2(c, c), b2 = pack2(bias_term, bias_term), one2 = pack2(1.0f, 1.0f);
     f32x2 a[4];
 #pragma unroll
@@ -546,7 +704,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     // preceding kernel (pdl.cuh).  From here on the W images, W, the partial sums and the stop flag are complete.
     pdl_wait();
     pdl_launch_dependents();
-    const bool stopped = prm.stop != nullptr && *prm.stop != 0;   // uniform over the grid: written by an earlier kernel
+    const bool stopped = prm.stop != nullptr && __ldcg(prm.stop) != 0;   // uniform over the grid: written by an earlier kernel
     if (stopped) units = 0;    // stop rule met: no work, no writes; fall through to the teardown (TMEM is allocated)
 
     if (warp == 0) {
@@ -586,6 +744,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         // this slot's MMAs.
         Ring ra, rb, rbu;                    // rbu: first B stage of the current unit (resident mode)
         uint32_t tile = 0;
+        uint32_t uses0 = 0, uses1 = 0;       // how often each accumulator has been handed to the epilogue so far
+        const bool flush = prm.flush != 0;
         const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem_base, 0);
         const uint32_t leader_a_full = map_to_cta(bar_a_full, 0);
         long long st_a = 0, st_b = 0, st_c = 0;
@@ -598,15 +758,24 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                 const bool need_b = !resident || mp == mp0;          // B stages must be (re)filled for this tile
                 const bool release_b = !resident || mp == mp1 - 1;   // last reader of the B stages
-                const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
-                const uint32_t d_tmem = tmem_u + buf * kBN;
+                uint32_t buf = 0, d_tmem = 0;
+                int k_first = 0;                                      // first K step of the current accumulation chunk
                 if (resident) rb = rbu;                               // every tile of the unit reads the same B stages
-                if (crank == 0 && !warp_try_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1)) {
-                    const long long t0 = clock64();
-                    warp_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
-                    st_c += clock64() - t0;
-                }
                 for (int j = 0; j < stages; ++j) {
+                    if (j == 0 || (flush && j % kFlushStages == 0)) {
+                        // a new accumulation: the whole tile (alternating accumulators), or the next chunk of its K extent
+                        buf = flush ? (j == 0 ? 0u : 1u) : (tile & 1);
+                        d_tmem = tmem_u + buf * kBN;
+                        k_first = j * kKS;
+                        const uint32_t acc_phase = (buf ? uses1 : uses0) & 1;
+                        if (crank == 0 && !warp_try_wait(bar_acc_empty + 8 * buf, acc_phase ^ 1)) {
+                            const long long t0 = clock64();
+                            warp_wait_spin(bar_acc_empty + 8 * buf, acc_phase ^ 1);
+                            st_c += clock64() - t0;
+                        }
+                        if (buf) ++uses1; else ++uses0;
+                    }
+                    const bool acc_done = j == stages - 1 || (flush && (j + 1) % kFlushStages == 0);   // this stage ends the accumulation
                     if (need_b && !warp_try_wait(bar_b_full + 8 * rb.i, rb.phase)) {
                         const long long t0 = clock64();
                         warp_wait_spin(bar_b_full + 8 * rb.i, rb.phase);
@@ -632,13 +801,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                                     const uint32_t b_hi = b_base + rb.i * kStageBytes + (k - j * kKS) * kSlotBytes, b_lo = b_hi + kBBytes;
                                     const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
                                     const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
-                                    umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, k != 0 ? 1u : 0u);   // small terms first
+                                    umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, k != k_first ? 1u : 0u);   // small terms first
                                     umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
                                     umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
                                 }
                                 umma_commit_pair(bar_a_empty + 8 * cur);                                    // A slot free in both CTAs
                                 if (last_of_stage && release_b) umma_commit_pair(bar_b_empty + 8 * rb.i);   // B stage free in both CTAs
-                                if (k1 == prm.steps) umma_commit_pair(bar_acc_full + 8 * buf);              // accumulators complete
+                                if (last_of_stage && acc_done) umma_commit_pair(bar_acc_full + 8 * buf);    // accumulation complete
                             }
                             __syncwarp();
                         } else {
@@ -659,10 +828,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         const int q = warp & 3;                 // TMEM lane quarter this warp may access
         const int h = (warp - 2) >> 2;          // column half
         double* my_part = prm.part + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
-        if (prm.zero_part && !stopped)
+        if (prm.zero_part && !stopped && prm.zdump == nullptr)
             for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
         const uint32_t leader_acc_empty = map_to_cta(bar_acc_empty, 0);
         uint32_t tile = 0;
+        uint32_t uses0 = 0, uses1 = 0;          // accumulators taken over from the MMA warp so far (barrier phases)
+        const bool flush = prm.flush != 0;
+        const int n_chunks = flush ? (stages + kFlushStages - 1) / kFlushStages : 1;
         // this thread's target of a unit (column h * 128 + q * 32 + lane of its pattern tile), staged form; 0 if absent
         auto target_of = [&](int uu) {
             if (uu >= units) return 0.0f;
@@ -684,13 +856,39 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             t_next = target_of(u + n_pairs);
             asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
-                const uint32_t buf = tile & 1, acc_phase = (tile >> 1) & 1;
+                const uint32_t buf = flush ? 0u : (tile & 1);
                 const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
                 // the bias gene a_0 is not part of the contraction: it rides on the epilogue's FFMA
-                const float bias = bias_term_of<ACT>(m < prm.M ? __ldg(prm.W + static_cast<size_t>(m) * prm.G) : 0.0f);
+                const float bias = bias_term_of<ACT>(m < prm.M ? __ldcg(prm.W + static_cast<size_t>(m) * prm.G) : 0.0f);
+                const float zs = zscale_of<ACT>(__ldcg(prm.wscale + m));     // this row's scale and phi's, undone on the same FFMA
                 // this lane's running sum, fetched before the wait: its L2 round trip is off the tile's critical path
-                const double part_old = __ldcg(my_part + m);
-                mbar_wait_sleep<256>(bar_acc_full + 8 * buf, acc_phase);
+                const double part_old = prm.zdump == nullptr ? __ldcg(my_part + m) : 0.0;
+                // streaming mode: accumulator 1 receives the K extent's later chunks one after the other; add each of them to
+                // accumulator 0 (chunk 0, then the running sum) with round-to-nearest fp32 adds and hand accumulator 1 back
+                for (int chunk = 1; chunk < n_chunks; ++chunk) {
+                    mbar_wait_sleep<256>(bar_acc_full + 8, uses1 & 1);
+                    ++uses1;
+                    tc_fence_after();
+#pragma unroll 1
+                    for (int cc = 0; cc < 4; ++cc) {
+                        const int col0 = h * 128 + cc * 32;
+                        if (col0 >= n_valid) break;
+                        const uint32_t ta = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + col0;
+                        uint32_t v0[32], v1[32];
+                        tmem_ld32(ta, v0);
+                        tmem_ld32(ta + kBN, v1);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v0[i] = __float_as_uint(__uint_as_float(v0[i]) + __uint_as_float(v1[i]));
+                        tmem_st32(ta, v0);
+                    }
+                    tmem_st_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8);
+                }
+                mbar_wait_sleep<256>(bar_acc_full + 8 * buf, (buf ? uses1 : uses0) & 1);   // (complete already if chunks were merged)
+                if (buf) ++uses1; else ++uses0;
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
                 f32x2 pacc0 = 0ull, pacc1 = 0ull;      // packed running sums of the full 32-column chunks (sigmoid / tanh)
@@ -703,21 +901,27 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     tmem_ld32(tmem_base + (static_cast<uint32_t>(q * 32) << 16) + buf * kBN + col0, v);
                     const float4* tp = reinterpret_cast<const float4*>(ts + cc * 32);
                     tmem_ld_wait();
+                    if (prm.zdump != nullptr) {       // calibration launch: hand out the accumulators as they are
+                        uint4* zd = reinterpret_cast<uint4*>(prm.zdump + static_cast<size_t>(m) * kBN + col0);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) __stcg(zd + i, make_uint4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]));
+                        continue;
+                    }
                     if (col0 + 32 <= n_valid) {
                         if (ACT == 0) {
 #pragma unroll
                             for (int i = 0; i < 8; ++i)
                                 act_err2_quad<ACT>(__uint_as_float(v[4 * i + 0]), __uint_as_float(v[4 * i + 1]),
-                                                   __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), bias, tp[i], sum, sum1,
+                                                   __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]), zs, bias, tp[i], sum, sum1,
                                                    sum2, sum3);
                         } else {
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) act_err2_oct<ACT>(v + 8 * i, bias, tp[2 * i], tp[2 * i + 1], pacc0, pacc1);
+                            for (int i = 0; i < 4; ++i) act_err2_oct<ACT>(v + 8 * i, zs, bias, tp[2 * i], tp[2 * i + 1], pacc0, pacc1);
                         }
                     } else {
 #pragma unroll
                         for (int i = 0; i < 32; ++i) {
-                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), bias, ts[cc * 32 + i]);
+                            if (col0 + i < n_valid) sum += act_err2<ACT>(__uint_as_float(v[i]), zs, bias, ts[cc * 32 + i]);
                         }
                     }
                 }
@@ -730,7 +934,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8 * buf);
-                __stcg(my_part + m, part_old + static_cast<double>(sum));
+                if (prm.zdump == nullptr) __stcg(my_part + m, part_old + static_cast<double>(sum));
             }
         }
     } else {
@@ -823,12 +1027,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                                     if ((i & 3) == 0) blk[q] = fetch4(xrow[q], i >> 2);
                                     const int k = i & 3;
                                     const float x = k == 0 ? blk[q].x : (k == 1 ? blk[q].y : (k == 2 ? blk[q].z : blk[q].w));
-                                    if (EXPANSION == 0) {
-                                        x2[q] = 2.0f * x; cp[q] = 1.0f; cc[q] = x; sp[q] = 0.0f; sc[q] = 0.0f;
+                                    if (EXPANSION == 0) {      // the recurrences are linear: started from kPhiScale they yield kPhiScale * phi
+                                        x2[q] = 2.0f * x; cp[q] = kPhiScale; cc[q] = kPhiScale * x; sp[q] = 0.0f; sc[q] = 0.0f;
                                     } else {
                                         float sn, cs;
                                         sincosf(x, &sn, &cs);
-                                        x2[q] = 2.0f * cs; cp[q] = 1.0f; cc[q] = cs; sp[q] = 0.0f; sc[q] = sn;
+                                        x2[q] = 2.0f * cs; cp[q] = kPhiScale; cc[q] = kPhiScale * cs; sp[q] = 0.0f; sc[q] = kPhiScale * sn;
                                     }
                                 }
                                 auto step = [&](int q, int jj) {
@@ -881,12 +1085,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
 #pragma unroll
                         for (int q = 0; q < kRPT; ++q) {
                             const float x = pick(cur[q], i);
-                            if (EXPANSION == 0) {
-                                x2[q] = 2.0f * x; cp[q] = 1.0f; cc[q] = x; sp[q] = 0.0f; sc[q] = 0.0f;
+                            if (EXPANSION == 0) {      // started from kPhiScale the (linear) recurrences yield kPhiScale * phi
+                                x2[q] = 2.0f * x; cp[q] = kPhiScale; cc[q] = kPhiScale * x; sp[q] = 0.0f; sc[q] = 0.0f;
                             } else {
                                 float sn, cs;
                                 sincosf(x, &sn, &cs);
-                                x2[q] = 2.0f * cs; cp[q] = 1.0f; cc[q] = cs; sp[q] = 0.0f; sc[q] = sn;
+                                x2[q] = 2.0f * cs; cp[q] = kPhiScale; cc[q] = kPhiScale * cs; sp[q] = 0.0f; sc[q] = kPhiScale * sn;
                             }
                         }
                     };

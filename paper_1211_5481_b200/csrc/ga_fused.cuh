@@ -39,7 +39,14 @@ struct FusedParams {
     GaParams ga;              // gen = first generation index
 };
 
-// All CTAs arrive; thread 0 of each spins (bounded) until everyone of this epoch has.
+// All CTAs arrive; thread 0 of each spins until everyone of this epoch has.  The counter only grows within a launch
+// (the host zeroes it and caps a launch at 2^20 generations, so it cannot wrap); the wait is bounded in TIME (20 s of
+// globaltimer: a protocol bug traps instead of hanging the GPU, time-slicing or a debugger cannot trip it).
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& epoch) {
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -47,8 +54,13 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
         epoch += gridDim.x;
         atomicAdd(counter, 1u);
         unsigned int n = 0;
+        unsigned long long t0 = 0;
         while (*reinterpret_cast<volatile unsigned int*>(counter) < epoch) {
-            if (++n > (1u << 27)) __trap();
+            if ((++n & 0xffffu) == 0) {
+                const unsigned long long now = global_timer_ns();
+                if (t0 == 0) t0 = now;
+                else if (now - t0 > 20000000000ull) __trap();
+            }
         }
         __threadfence();
     }

@@ -76,7 +76,9 @@ __device__ __forceinline__ unsigned long long roulette_weight(float f) {
     return static_cast<unsigned long long>(v * 4294967296.0);
 }
 // smallest index whose inclusive prefix sum exceeds floor(w T / 2^32); T = 0 -> uniform index
-__device__ __forceinline__ int roulette_from_word(uint32_t w, int M, const unsigned long long* __restrict__ prefix) {
+// (`prefix` and `by_rank` are generic pointers: global memory written by an earlier kernel of the chain in ga_step_kernel,
+// shared memory in ga_fused_kernel -- plain loads, which are coherent after griddepcontrol.wait.)
+__device__ __forceinline__ int roulette_from_word(uint32_t w, int M, const unsigned long long* prefix) {
     const unsigned long long T = prefix[M - 1];
     if (T == 0) return static_cast<int>(index_below(w, static_cast<uint32_t>(M)));
     const unsigned long long u = scale_word(w, T);
@@ -89,12 +91,12 @@ __device__ __forceinline__ int roulette_from_word(uint32_t w, int M, const unsig
 }
 
 // by_rank[rank of chromosome c] = c; one block per chromosome (the same count as in ga_step_kernel).
-__global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* __restrict__ F, int M, int* __restrict__ by_rank) {
+__global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* F, int M, int* by_rank) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
     const int c = blockIdx.x, tid = threadIdx.x;
-    const float kc = fit_key(F[c]);
+    const float kc = fit_key(__ldcg(F + c));
     int cnt = 0;
-    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(F[j]), j, kc, c) ? 1 : 0;
+    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(__ldcg(F + j)), j, kc, c) ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if ((tid & 31) == 0) s_warp_cnt[tid >> 5] = cnt;
@@ -107,14 +109,13 @@ __global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* __restric
 }
 
 // Inclusive prefix sums of the roulette weights; one block of 1024 threads, each owning a contiguous segment.
-__global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* __restrict__ F, int M,
-                                                               unsigned long long* __restrict__ prefix) {
+__global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* F, int M, unsigned long long* prefix) {
     __shared__ unsigned long long s_tot[1024];
     const int tid = threadIdx.x;
     const int per = (M + 1023) / 1024;
     const int i0 = tid * per, i1 = min(M, i0 + per);
     unsigned long long acc = 0;
-    for (int i = i0; i < i1; ++i) acc += roulette_weight(F[i]);
+    for (int i = i0; i < i1; ++i) acc += roulette_weight(__ldcg(F + i));
     s_tot[tid] = acc;
     __syncthreads();
     for (int o = 1; o < 1024; o <<= 1) {               // Hillis-Steele scan of the 1024 segment totals (integers: exact)
@@ -125,7 +126,7 @@ __global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* __re
     }
     acc = tid > 0 ? s_tot[tid - 1] : 0ull;
     for (int i = i0; i < i1; ++i) {
-        acc += roulette_weight(F[i]);
+        acc += roulette_weight(__ldcg(F + i));
         prefix[i] = acc;
     }
 }
@@ -138,12 +139,33 @@ __global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* __re
 // With `img` != nullptr (tensor-core scheme, images of the OLD population valid) every gene written to the new population
 // is also split into the W operand images of fitness_umma_kernel, which then needs no image pass of its own; under the
 // stop rule rows carry over in place and their images stay as they are.
-__global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __restrict__ W,
-                                                              const float* __restrict__ F,
-                                                              float* __restrict__ Wn, GaParams p,
-                                                              const int* __restrict__ stop,
-                                                              uint8_t* __restrict__ img, int img_steps) {
+// W, F, stop, by_rank and prefix are written by earlier kernels of the launch chain, which may still be running when this
+// grid starts (pdl.cuh): they are read with ld.global.cg after griddepcontrol.wait, never through the non-coherent path
+// (no __ldg, no const __restrict__: ld.global.nc requires data that is read-only for the kernel's whole lifetime).
+// The images hold every row times its own power-of-two scale (fitness_umma.cuh: the largest gene of the row lands in
+// [2^13, 2^14)), so a row's images are written in a second pass, once the block knows the row's largest gene.
+__device__ __forceinline__ void store_row_images(uint8_t* img, float* wscale, int img_steps, int m, const float* row, int G,
+                                                 float amax, float* s_red) {
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    __syncthreads();                                   // s_red may still be read from an earlier row of this block
+    if ((tid & 31) == 0) s_red[tid >> 5] = amax;
+    __syncthreads();
+    amax = s_red[0];
+#pragma unroll
+    for (int w = 1; w < kGaThreads / 32; ++w) amax = fmaxf(amax, s_red[w]);
+    const int k = umma::row_scale_exp(amax);
+    const float scale = ldexpf(1.0f, k);
+    if (tid == 0) wscale[m] = umma::row_unscale(k);
+    // every thread re-reads the genes it wrote itself (same thread, same address: no synchronisation needed)
+    for (int g = 1 + tid; g < G; g += kGaThreads) umma::store_w_image_gene(img, img_steps, m, g, row[g] * scale);
+}
+
+__global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, const float* F, float* Wn, GaParams p,
+                                                              const int* stop, uint8_t* img, float* wscale, int img_steps) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
+    __shared__ float s_red[kGaThreads / 32];
     __shared__ int s_rank;
     __shared__ int s_parent[2];
     __shared__ int s_cut;
@@ -152,15 +174,15 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     const int M = p.M, G = p.G;
     pdl_wait();                            // F (finalize), W and, for ranking / roulette, by_rank / prefix are complete
     pdl_launch_dependents();
-    if (stop != nullptr && *stop != 0) {   // stop rule already met: the population is final, carry it over unchanged
-        for (int g = tid; g < G; g += kGaThreads) Wn[static_cast<size_t>(c) * G + g] = W[static_cast<size_t>(c) * G + g];
+    if (stop != nullptr && __ldcg(stop) != 0) {   // stop rule already met: the population is final, carry it over unchanged
+        for (int g = tid; g < G; g += kGaThreads) Wn[static_cast<size_t>(c) * G + g] = __ldcg(W + static_cast<size_t>(c) * G + g);
         return;
     }
 
     // (1) rank of chromosome c under the order
-    const float kc = fit_key(F[c]);
+    const float kc = fit_key(__ldcg(F + c));
     int cnt = 0;
-    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(F[j]), j, kc, c) ? 1 : 0;
+    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(__ldcg(F + j)), j, kc, c) ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if ((tid & 31) == 0) s_warp_cnt[tid >> 5] = cnt;
@@ -175,22 +197,26 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     if (rank < p.elite) {
         const float* src = W + static_cast<size_t>(c) * G;
         float* dst = Wn + static_cast<size_t>(rank) * G;
+        float amax = 0.0f;
         for (int g = tid; g < G; g += kGaThreads) {
-            const float v = src[g];
+            const float v = __ldcg(src + g);
             dst[g] = v;
-            if (img != nullptr) umma::store_w_image_gene(img, img_steps, rank, g, v);
+            if (g >= 1) amax = fmaxf(amax, fabsf(v));
         }
+        if (img != nullptr) store_row_images(img, wscale, img_steps, rank, dst, G, amax, s_red);
     }
     if (c < p.elite) return;  // slots 0..elite-1 are written by the elites themselves
     if (c >= M - p.immigrants) {
         // random replacement: genes uniform in [-1,1) as at initialisation, tag IMMIGRANT
         float* fresh = Wn + static_cast<size_t>(c) * G;
+        float amax = 0.0f;
         for (int g = tid; g < G; g += kGaThreads) {
             const uint4 r = philox4x32_10(static_cast<uint32_t>(g >> 2), static_cast<uint32_t>(c), p.gen, kTagImmigrant, p.key);
             const float v = gene_from_word(word_of(r, g & 3));
             fresh[g] = v;
-            if (img != nullptr) umma::store_w_image_gene(img, img_steps, c, g, v);
+            if (g >= 1) amax = fmaxf(amax, fabsf(v));
         }
+        if (img != nullptr) store_row_images(img, wscale, img_steps, c, fresh, G, amax, s_red);
         return;
     }
 
@@ -205,7 +231,7 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
                 if ((e & 3) == 0)
                     r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
                 const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
-                const float ki = fit_key(F[idx]);
+                const float ki = fit_key(__ldcg(F + idx));
                 const int side = e < k ? 0 : 1;
                 if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
                     par[side] = idx;
@@ -238,16 +264,18 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
     const int q = s_cut;
     float* child = Wn + static_cast<size_t>(c) * G;
     // per-gene Gaussian mutation, no clamping (D6)
+    float amax = 0.0f;
     for (int g = tid; g < G; g += kGaThreads) {
-        float v = g < q ? A[g] : B[g];
+        float v = __ldcg(g < q ? A + g : B + g);
         const uint4 rm = philox4x32_10(static_cast<uint32_t>(g), static_cast<uint32_t>(c), p.gen, kTagMutate, p.key);
         if (static_cast<unsigned long long>(rm.x) < p.t_mut) {
             const float z = gauss_from_words(rm.y, rm.z);
             v = __fadd_rn(v, __fmul_rn(p.sigma, z));
         }
         child[g] = v;
-        if (img != nullptr) umma::store_w_image_gene(img, img_steps, c, g, v);
+        if (g >= 1) amax = fmaxf(amax, fabsf(v));
     }
+    if (img != nullptr) store_row_images(img, wscale, img_steps, c, child, G, amax, s_red);
 }
 
 // ---- fitness finalisation: F[m] = (sum over partial rows, in row order) / P in fp64, rounded to fp32
@@ -255,15 +283,10 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* __rest
 // population is written to *best_out by the last block to finish (R8).
 constexpr int kFinThreads = 1024, kFinCols = 32, kFinGroups = kFinThreads / kFinCols;
 
-__global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* __restrict__ part,
-                                                                        int n_part, int m_stride, int M,
-                                                                        double P_d, float* __restrict__ F,
-                                                                        double* __restrict__ sse_out,
-                                                                        float* __restrict__ best_out,
-                                                                        float* __restrict__ blk_key,
-                                                                        int* __restrict__ blk_idx,
-                                                                        unsigned int* __restrict__ ticket,
-                                                                        int* __restrict__ stop, float threshold, int gen_index, int rmse) {
+__global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* part, int n_part, int m_stride, int M,
+                                                                        double P_d, float* F, double* sse_out, float* best_out,
+                                                                        float* blk_key, int* blk_idx, unsigned int* ticket,
+                                                                        int* stop, float threshold, int gen_index, int rmse) {
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
     __shared__ bool s_last;
@@ -273,7 +296,7 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
     // result is bit-stable.
     pdl_wait();                                    // the fitness kernel's partial sums are complete
     pdl_launch_dependents();
-    if (stop != nullptr && stop[0] != 0) return;   // stop rule met earlier: fitness and best trace stay as they are
+    if (stop != nullptr && __ldcg(stop) != 0) return;   // stop rule met earlier: fitness and best trace stay as they are
     __shared__ double s_grp[kFinGroups][kFinCols];
     const int col = threadIdx.x % kFinCols, grp = threadIdx.x / kFinCols;
     const int m = blockIdx.x * kFinCols + col;

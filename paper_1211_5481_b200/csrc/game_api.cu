@@ -24,6 +24,8 @@ constexpr int kMaxCtas = 160;            // persistent grid cap (B200: 148 SMs)
 constexpr int kMaxPartRows = 2 * kMaxCtas;
 constexpr size_t kAlign = 256;
 constexpr size_t kMaxTimedLaunches = 8192;
+constexpr size_t kPredictMaxSmem = 227u * 1024u;
+constexpr size_t kCalMaxSmem = 200u * 1024u;       // calibrate_kernel stages one chromosome in shared memory up to this size   // predict_kernel stages the chromosome in shared memory up to this size
 
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
@@ -37,7 +39,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -50,6 +52,7 @@ struct game_ctx {
     bool ticket_zeroed = false;
     // GA parameters
     int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0, rmse = 0;
+    bool calibrate = true;   // regression activations on the tensor-core scheme: measure each row's accumulation shrink (calibrate_kernel)
     bool pdl = true;   // programmatic dependent launch along the generation's kernel chain (pdl.cuh); GAME_PDL=0 turns it off
     double p_cross = 0.9, p_mut = 0.05;
     float sigma = 0.1f;
@@ -58,6 +61,7 @@ struct game_ctx {
     int scheme = GAME_SCHEME_AUTO;
     bool device_checked = false;
     int num_sms = 0;
+    int device = -1;                                 // ordinal of the device the bound buffers live on (-1: unknown, use the current one)
     unsigned long long launches = 0;
     bool timing = false;
     int* stop = nullptr;                             // device stop state, non-null only inside game_run_until
@@ -93,6 +97,31 @@ int cuda_fail(game_ctx* c, cudaError_t e, const char* what) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// The device a pointer lives on, or -1 (host pointer, no driver, unknown): errors are swallowed, this is only a hint.
+int device_of(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return -1;
+    }
+    return (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) ? at.device : -1;
+}
+
+// Every compute entry runs on the device of the bound buffers, whatever the caller's current device is (the stream
+// handle, the kernels' attributes and the sm_100 check all belong to that device), and restores the caller's device.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 int resolved_scheme(const game_ctx* c) {
     if (c->scheme == GAME_SCHEME_AUTO) return c->umma_ok ? GAME_SCHEME_F16X3 : GAME_SCHEME_FFMA;
     return c->scheme;
@@ -114,6 +143,9 @@ int ensure_device(game_ctx* c) {
     c->num_sms = prop.multiProcessorCount;
     using namespace game;
     GAME_CUDA(cudaFuncSetAttribute(fitness_ffma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kFfmaMaxG * kFfmaTile * 4));
+    GAME_CUDA(cudaFuncSetAttribute(predict_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kPredictMaxSmem)));
+    GAME_CUDA(cudaFuncSetAttribute(umma::calibrate_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kCalMaxSmem)));
+    GAME_CUDA(cudaFuncSetAttribute(umma::calibrate_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kCalMaxSmem)));
 #define GAME_SET_SMEM(E, A) \
     GAME_CUDA(cudaFuncSetAttribute(umma::fitness_umma_kernel<E, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, umma::kSmemBytes))
     GAME_SET_SMEM(0, 0); GAME_SET_SMEM(0, 1); GAME_SET_SMEM(0, 2);
@@ -142,6 +174,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     using namespace game;
     if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_load_kb");
     if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness before game_bind_state");
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     const int scheme = resolved_scheme(c);
@@ -163,14 +196,18 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     if (scheme == GAME_SCHEME_F16X3) {
         uint8_t* img = c->ws + c->off_img;
         const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
+        float* wscale = reinterpret_cast<float*>(c->ws + c->off_wscale);
         if (!c->img_valid) {   // inside a generation loop the GA step keeps the images up to date (ga_step_kernel)
+            launch_chain(c->pdl, umma::row_scale_kernel, dim3(static_cast<unsigned>((c->m_stride * 32ll + 255) / 256)), dim3(256), 0,
+                         c->stream, W, wscale, c->M, c->G, c->m_stride);
+            if ((rc = check_launch(c, "row_scale_kernel"))) return rc;
             launch_chain(c->pdl, umma::build_w_images_kernel, dim3(static_cast<unsigned>((n_thr + 255) / 256)), dim3(256), 0,
-                         c->stream, W, img, c->M, c->G, c->steps, c->m_tiles);
+                         c->stream, W, wscale, img, c->M, c->G, c->steps, c->m_tiles);
             if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
             c->img_valid = true;
         }
         umma::Params prm;
-        prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.part = part;
+        prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.wscale = wscale; prm.zdump = nullptr; prm.part = part;
         prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
         prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
         const int p_tiles_all = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
@@ -205,6 +242,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         prm.n_b = !prm.resident ? umma::kStreamBStages
                                 : (2 * prm.stages <= umma::kMaxResidentStages ? 2 * prm.stages : prm.stages);
         prm.n_a = umma::kStagesTotal - prm.n_b;
+        prm.flush = prm.resident ? 0 : 1;
         prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
         prm.stop = c->stop;
         const long long units = static_cast<long long>(p_tiles_all) * prm.m_groups;
@@ -254,6 +292,39 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
                                           cudaMemcpyHostToDevice, c->copy_stream));
                 GAME_CUDA(cudaEventRecord(c->copy_events[k], c->copy_stream));
                 GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[k], 0));
+            }
+            if (first_launch && c->calibrate && c->act != GAME_ACT_SIGMOID) {
+                // regression activations: measure every row's accumulation shrink on the first pattern tile (calibrate_kernel)
+                float* zdump = reinterpret_cast<float*>(c->ws + c->off_zdump);
+                float* zcorr = reinterpret_cast<float*>(c->ws + c->off_zcorr);
+                umma::Params cal = prm;
+                cal.p_tile0 = 0; cal.p_tiles = 1; cal.zero_part = 0; cal.zdump = zdump; cal.stall = nullptr;
+                cal.m_pairs_per_group = 1; cal.m_groups = m_pairs;          // one chromosome-tile pair per CTA pair: shortest launch
+                const int cal_grid = 2 * (m_pairs < pair_cap ? m_pairs : pair_cap);
+                const int sel = c->expansion * 3 + c->act;
+#define GAME_LAUNCH_CAL(E, A) \
+    launch_chain(c->pdl && hk == nullptr, umma::fitness_umma_kernel<E, A>, dim3(cal_grid), dim3(umma::kThreads), umma::kSmemBytes, c->stream, cal)
+                switch (sel) {
+                    case 0: GAME_LAUNCH_CAL(0, 0); break;
+                    case 2: GAME_LAUNCH_CAL(0, 2); break;
+                    case 3: GAME_LAUNCH_CAL(1, 0); break;
+                    default: GAME_LAUNCH_CAL(1, 2); break;
+                }
+#undef GAME_LAUNCH_CAL
+                if ((rc = check_launch(c, "fitness_umma_kernel (calibration)"))) return rc;
+                const size_t w_bytes = sizeof(float) * static_cast<size_t>(c->G);
+                const int stage_w = w_bytes <= kCalMaxSmem ? 1 : 0;
+                if (c->expansion == GAME_EXP_CHEBYSHEV)
+                    launch_chain(c->pdl && hk == nullptr, umma::calibrate_kernel<0>, dim3(c->m_stride), dim3(umma::kCalThreads),
+                                 stage_w ? w_bytes : 0, c->stream, c->X, W, zdump, wscale, zcorr, c->stop, c->P, c->N, c->d, c->M, c->G,
+                                 c->shared, stage_w);
+                else
+                    launch_chain(c->pdl && hk == nullptr, umma::calibrate_kernel<1>, dim3(c->m_stride), dim3(umma::kCalThreads),
+                                 stage_w ? w_bytes : 0, c->stream, c->X, W, zdump, wscale, zcorr, c->stop, c->P, c->N, c->d, c->M, c->G,
+                                 c->shared, stage_w);
+                if ((rc = check_launch(c, "calibrate_kernel"))) return rc;
+                prm.wscale = zcorr;
+                if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));      // the roofline figure times the evaluation proper
             }
             prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = first_launch ? 1 : 0;
             first_launch = false;
@@ -310,6 +381,7 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     using namespace game;
     if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_step before game_bind_state");
     if (!c->fitness_valid) return fail(c, GAME_ERR_BAD_STATE, "game_step needs a fresh fitness (game_eval_fitness first)");
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     GaParams p;
@@ -331,7 +403,8 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     }
     launch_chain(c->pdl, ga_step_kernel, dim3(c->M), dim3(kGaThreads), 0, c->stream,
                  c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop,
-                 c->img_valid ? c->ws + c->off_img : static_cast<uint8_t*>(nullptr), c->steps);
+                 c->img_valid ? c->ws + c->off_img : static_cast<uint8_t*>(nullptr), reinterpret_cast<float*>(c->ws + c->off_wscale),
+                 c->steps);
     if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
     c->cur ^= 1;
     c->fitness_valid = false;
@@ -366,11 +439,16 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->m_stride = c->m_tiles * game::umma::kBM;
     c->umma_ok = umma_ok;
     if (const char* e = std::getenv("GAME_PDL")) c->pdl = e[0] != '0';   // A/B switch for measurements; default on
+    if (const char* e = std::getenv("GAME_CALIBRATE")) c->calibrate = e[0] != '0';   // A/B switch; default on
     c->steps = static_cast<int>((G - 1 + 15) / 16);   // K steps of 16 genes; the bias gene is not part of the contraction
     size_t off = 0;
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
     c->off_img = off;
     if (c->umma_ok) off = align_up(off + static_cast<size_t>(c->m_tiles) * c->steps * 2 * game::umma::kABytes);
+    c->off_wscale = off; off = align_up(off + sizeof(float) * static_cast<size_t>(c->m_stride));
+    c->off_zcorr = off; off = align_up(off + sizeof(float) * static_cast<size_t>(c->m_stride));
+    c->off_zdump = off;       // calibration samples (regression activations on the tensor-core scheme only)
+    if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(float) * static_cast<size_t>(c->m_stride) * game::umma::kBN);
     const size_t fin_blocks = (static_cast<size_t>(M) + game::kFinCols - 1) / game::kFinCols;
     c->off_blk_key = off; off = align_up(off + fin_blocks * sizeof(float));
     c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
@@ -439,6 +517,7 @@ int game_load_kb(game_ctx* c, const float* X_dev, const float* t_dev) {
     c->X = X_dev;
     c->t = t_dev;
     c->fitness_valid = false;
+    if (c->device < 0) c->device = device_of(X_dev);
     return GAME_OK;
 }
 
@@ -456,6 +535,10 @@ int game_bind_state(game_ctx* c, float* popA_dev, float* popB_dev, float* fitnes
     c->pop[1] = popB_dev;
     c->fitness = fitness_dev;
     c->ws = static_cast<unsigned char*>(workspace_dev);
+    {
+        const int dev = device_of(workspace_dev);
+        if (dev >= 0 && dev != c->device) { c->device = dev; c->device_checked = false; }
+    }
     c->cur = 0;
     c->fitness_valid = false;
     c->img_valid = false;
@@ -501,6 +584,7 @@ int game_set_selection(game_ctx* c, int32_t selection) {
 int game_init_population(game_ctx* c, uint64_t seed) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_init_population before game_bind_state");
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     const long long n = static_cast<long long>(c->M) * ((c->G + 3) / 4);
@@ -560,6 +644,7 @@ int game_run_until(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t max_gens,
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!best_fitness_dev || !gens_done_dev) return fail(c, GAME_ERR_INVALID_ARG, "game_run_until needs best_fitness_dev and gens_done_dev");
     if (!c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_run_until before game_bind_state");
+    DeviceGuard guard(c->device);
     int* stop = reinterpret_cast<int*>(c->ws + c->off_stop);
     GAME_CUDA(cudaMemsetAsync(stop, 0, 2 * sizeof(int), c->stream));
     c->stop = stop;
@@ -584,6 +669,7 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
     if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_fused before game_load_kb");
     if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_fused before game_bind_state");
     if (n_gens == 0) return GAME_OK;
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     // few CTAs for tiny problems: the two grid barriers per generation, not the arithmetic, set the pace
@@ -606,7 +692,7 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
     prm.barrier = reinterpret_cast<unsigned int*>(c->ws + c->off_fused_bar);
     prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
     prm.expansion = c->expansion; prm.act = c->act; prm.rmse = c->rmse; prm.shared = c->shared;
-    prm.cur = c->cur; prm.n_gens = static_cast<int>(n_gens); prm.ppc = ppc;
+    prm.ppc = ppc;
     prm.ga.M = c->M; prm.ga.G = c->G; prm.ga.elite = c->elite; prm.ga.tournament = c->tournament;
     prm.ga.t_cross = bernoulli_threshold(c->p_cross);
     prm.ga.t_mut = bernoulli_threshold(c->p_mut);
@@ -614,11 +700,21 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
     prm.ga.selection = c->selection;
     prm.ga.immigrants = c->immigrants < c->M - c->elite ? c->immigrants : c->M - c->elite;
     prm.ga.by_rank = nullptr; prm.ga.prefix = nullptr;
-    GAME_CUDA(cudaMemsetAsync(prm.barrier, 0, sizeof(unsigned int), c->stream));
-    void* args[] = {&prm};
-    GAME_CUDA(cudaLaunchCooperativeKernel(reinterpret_cast<void*>(ga_fused_kernel), dim3(grid), dim3(kFusedThreads), args, smem, c->stream));
-    if ((rc = check_launch(c, "ga_fused_kernel"))) return rc;
-    if (n_gens & 1u) c->cur ^= 1;
+    // The grid barrier counts arrivals in 32 bits (2 x grid per generation): at most 2^20 generations per launch, longer
+    // runs are several launches back to back on the stream (same result: the loop carries no state but the buffers).
+    constexpr uint32_t kMaxGensPerLaunch = 1u << 20;
+    for (uint32_t done = 0; done < n_gens;) {
+        const uint32_t n = n_gens - done < kMaxGensPerLaunch ? n_gens - done : kMaxGensPerLaunch;
+        prm.cur = c->cur; prm.n_gens = static_cast<int>(n);
+        prm.ga.gen = gen0 + done;
+        prm.best = best_fitness_dev ? best_fitness_dev + done : nullptr;
+        GAME_CUDA(cudaMemsetAsync(prm.barrier, 0, sizeof(unsigned int), c->stream));
+        void* args[] = {&prm};
+        GAME_CUDA(cudaLaunchCooperativeKernel(reinterpret_cast<void*>(ga_fused_kernel), dim3(grid), dim3(kFusedThreads), args, smem, c->stream));
+        if ((rc = check_launch(c, "ga_fused_kernel"))) return rc;
+        if (n & 1u) c->cur ^= 1;
+        done += n;
+    }
     c->fitness_valid = false;
     c->img_valid = false;
     return GAME_OK;
@@ -637,6 +733,7 @@ int game_evolve(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens) {
 
 int game_sync(game_ctx* c) {
     if (!c) return GAME_ERR_INVALID_ARG;
+    DeviceGuard guard(c->device);
     GAME_CUDA(cudaStreamSynchronize(c->stream));
     GAME_CUDA(cudaGetLastError());
     return GAME_OK;
@@ -648,6 +745,7 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     if (!X_host || !t_host || !W_host) return fail(c, GAME_ERR_INVALID_ARG, "null host input");
     if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "game_generation_host before game_load_kb");
     if (!c->pop[0]) return fail(c, GAME_ERR_BAD_STATE, "game_generation_host before game_bind_state");
+    DeviceGuard guard(c->device);
     const size_t wb = sizeof(float) * static_cast<size_t>(c->M) * c->G;
     GAME_CUDA(cudaMemcpyAsync(c->pop[c->cur], W_host, wb, cudaMemcpyHostToDevice, c->stream));
     c->fitness_valid = false;
@@ -675,6 +773,7 @@ int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_tota
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!sse_dev || P_total < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_set_fitness_from_sse: null sse_dev or P_total < 1");
     if (!c->fitness || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_set_fitness_from_sse before game_bind_state");
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     if (!c->ticket_zeroed) {
@@ -694,18 +793,22 @@ int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_tota
 int game_predict(game_ctx* c, const float* w_dev, const float* X_dev, int64_t Q, float* y_dev) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!w_dev || !X_dev || !y_dev || Q < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_predict: null pointer or Q < 1");
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     long long blocks = (Q + game::kPredictThreads - 1) / game::kPredictThreads;
     if (blocks > 8ll * c->num_sms) blocks = 8ll * c->num_sms;
-    game::predict_kernel<<<static_cast<unsigned>(blocks), game::kPredictThreads, sizeof(float) * c->G, c->stream>>>(
-        X_dev, w_dev, y_dev, Q, c->N, c->d, c->G, c->expansion, c->act, c->shared);
+    const size_t w_bytes = sizeof(float) * static_cast<size_t>(c->G);
+    const int stage_w = w_bytes <= kPredictMaxSmem ? 1 : 0;        // opted in up to 227 KB by ensure_device
+    game::predict_kernel<<<static_cast<unsigned>(blocks), game::kPredictThreads, stage_w ? w_bytes : 0, c->stream>>>(
+        X_dev, w_dev, y_dev, Q, c->N, c->d, c->G, c->expansion, c->act, c->shared, stage_w);
     return check_launch(c, "predict_kernel");
 }
 
 int game_confusion(game_ctx* c, const float* y_dev, const float* t_dev, int64_t Q, float threshold, uint64_t* counts_dev) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!y_dev || !t_dev || !counts_dev || Q < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_confusion: null pointer or Q < 1");
+    DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
     GAME_CUDA(cudaMemsetAsync(counts_dev, 0, 4 * sizeof(uint64_t), c->stream));
@@ -735,6 +838,7 @@ int game_time_fitness_kernel(game_ctx* c, int32_t enable) {
 
 int game_fitness_kernel_ms(game_ctx* c, double* total_ms, uint64_t* launches) {
     if (!c || !total_ms || !launches) return GAME_ERR_INVALID_ARG;
+    DeviceGuard guard(c->device);
     double sum = 0.0;
     for (auto& ev : c->events) {
         GAME_CUDA(cudaEventSynchronize(ev.second));

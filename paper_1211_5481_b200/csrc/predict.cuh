@@ -13,10 +13,15 @@ constexpr int kPredictThreads = 256;
 
 __global__ void __launch_bounds__(kPredictThreads) predict_kernel(const float* __restrict__ X, const float* __restrict__ w,
                                                                    float* __restrict__ y, long long Q, int N, int d, int G,
-                                                                   int expansion, int act, int shared) {
-    extern __shared__ float s_w[];   // [G]
-    for (int g = threadIdx.x; g < G; g += kPredictThreads) s_w[g] = w[g];
-    __syncthreads();
+                                                                   int expansion, int act, int shared, int stage_w) {
+    extern __shared__ float s_stage[];   // [G] when stage_w: the chromosome staged in shared memory (G up to 57 K genes);
+                                         // longer chromosomes are read through L1 / L2 (every thread walks the same genes)
+    const float* s_w = w;
+    if (stage_w) {
+        for (int g = threadIdx.x; g < G; g += kPredictThreads) s_stage[g] = w[g];
+        __syncthreads();
+        s_w = s_stage;
+    }
     for (long long q = static_cast<long long>(blockIdx.x) * kPredictThreads + threadIdx.x; q < Q;
          q += static_cast<long long>(gridDim.x) * kPredictThreads) {
         const float* xr = X + q * N;

@@ -400,6 +400,27 @@ def test_predict_and_confusion_match_oracle(game, base, over):
     G.close()
 
 
+@pytest.mark.parametrize("N,d", [(130, 100), (600, 100)])
+def test_predict_long_chromosomes(game, N, d):
+    """game_predict with chromosomes beyond 48 KB (G = 13 001: staged in opted-in shared memory) and beyond what shared
+    memory holds (G = 60 001: read through the caches): the trained model can be applied wherever training is accepted."""
+    import torch
+    Q = 700
+    rng = np.random.Generator(np.random.Philox(90 + N))
+    G = game.Game(8, N, d, 4, wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    fam = oracle.family(wl.EXP_CHEBYSHEV, wl.ACT_SIGMOID)
+    assert G.G == N * d + 1
+    X = rng.uniform(-1, 1, (Q, N)).astype(np.float32)
+    w = (rng.uniform(-1, 1, G.G) / np.sqrt(G.G / 8.0)).astype(np.float32)
+    y = torch.empty(Q, dtype=torch.float32, device="cuda")
+    wd, Xd = torch.from_numpy(w).cuda(), torch.from_numpy(X).cuda()
+    game.game_predict(G.ctx, wd.data_ptr(), Xd.data_ptr(), Q, y.data_ptr())
+    G.sync()
+    y_ref = oracle.predict(d, fam, X, w)
+    assert np.max(np.abs(y.cpu().numpy() - y_ref)) <= 1e-5
+    G.close()
+
+
 # ------------------------------------------------------------------------------------------------ pattern sharding (N3)
 @pytest.mark.parametrize("world", [2, 3])
 def test_pattern_sharded_evaluation_single_device(game, world):
@@ -562,7 +583,8 @@ def test_step_keeps_w_images(game, base, over, selection, immigrants):
     for gen in range(4):
         n0 = G.launch_count()
         G.eval_fitness(); G.sync()
-        assert G.launch_count() - n0 == (3 if gen == 0 else 2)     # image pass only before the first generation
+        cal = 2 if cfg.activation != wl.ACT_SIGMOID else 0        # regression activations: calibration launch + calibrate_kernel
+        assert G.launch_count() - n0 == (4 if gen == 0 else 2) + cal   # row scales + image pass only before the first generation
         F = G.get_fitness()
         W = G.get_population()
         H.set_population(W); H.eval_fitness(); H.sync()

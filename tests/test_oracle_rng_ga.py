@@ -138,6 +138,49 @@ def test_gauss_is_sqrt_times_cos_in_binary32():
     assert np.all(np.abs(z) <= math.sqrt(2 * 23 * math.log(2)) + 1e-5)
 
 
+def _gauss_gold():
+    g = {}
+    for line in open(os.path.join(GOLD, "gauss_worked_example.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            g[line[0]] = int(line[1], 16)
+    return g
+
+
+def test_gauss_worked_example_bit_patterns():
+    """SURVEY 8(c) P-GAUSS: every intermediate of the R5 sampler and of one mutation w' = w + sigma z, bit for bit
+    (tests/golden/gauss_worked_example.txt; values computed for the survey independently of the oracle).  The accuracy
+    tests above pin the constants to ~4e-7 only: a last-digit slip in a high-order Taylor coefficient passes them and
+    fails here."""
+    g = _gauss_gold()
+    bits = lambda v: int(np.float32(v).view(np.uint32))
+    t = oracle.neg2ln_u1(g["a"])
+    assert bits(t) == g["t"]
+    r = np.sqrt(np.float32(t))                            # IEEE binary32 sqrt (numpy: correctly rounded)
+    assert bits(r) == g["r"]
+    c = oracle.cos_angle(g["b"])
+    assert bits(c) == g["c"] and g["b"] >> 30 == 2
+    z = oracle.gauss(g["a"], g["b"])
+    assert bits(z) == g["z"] == bits(np.float32(r) * np.float32(c))
+    sigma = np.uint32(g["sigma"]).view(np.float32)
+    assert sigma == np.float32(0.1)
+    delta = np.float32(sigma * z)
+    assert bits(delta) == g["delta"]
+    w = np.uint32(g["w"]).view(np.float32)
+    assert bits(np.float32(w + delta)) == g["w_mutated"]
+    # the same mutation through the oracle's GA step: one chromosome, one gene besides ... is not constructible with
+    # these words (they are the zero block's, the step draws from counter (g, c, gen, 3)); the step's use of
+    # child + sigma * z is pinned by test_mutation_count_value_and_independence from the raw Philox stream.
+    t1 = oracle.neg2ln_u1(g["a_one"])
+    assert bits(t1) == g["t_one"] and abs(float(oracle.gauss(g["a_one"], g["b"]))) == 0.0
+    t0 = oracle.neg2ln_u1(g["a_min"])
+    assert bits(t0) == g["t_min"] and bits(np.sqrt(np.float32(t0))) == g["r_min"]
+    # w is the init gene of word 0 of the zero Philox block (R6): float(word >> 8) * 2^-23 - 1
+    word0 = int(oracle.philox4x32_10([0, 0, 0, 0], [0, 0])[0])
+    assert bits(np.float32(np.float32(word0 >> 8) * np.float32(2.0 ** -23) - np.float32(1.0))) == g["w"]
+    assert [int(x) for x in oracle.philox4x32_10([0, 0, 0, 0], [0, 0])[1:3]] == [g["a"], g["b"]]
+
+
 def test_gauss_distribution():
     n = 400000
     words = np.stack([oracle.philox4x32_10([i, 0, 0, 9], [42, 0]) for i in range(n // 2)])
