@@ -38,9 +38,29 @@ import workloads as wl
 METRIC = "chromosome_pattern_fitness_evals_per_s"
 UNIT = "evals/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture of that workload exists).
-NCU_TRAFFIC_BYTES = {"c3": 546093312}      # profiles/r01i_README.md: 536.5 MB read + 9.6 MB written
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused fitness kernel, from the `ncu --set full`
+# captures summarised in profiles/ (a bench run cannot measure DRAM traffic itself: numbers taken under a profiler are not
+# bench values).  Each entry names the capture it comes from and the sha-256 prefix of csrc/fitness_umma.cuh at capture
+# time: when the kernel source has changed since, the figure is withheld (traffic = null) rather than repeated.
+NCU_TRAFFIC = {
+    "c3": {"bytes": 546093312, "source": "profiles/r01i_README.md (536.5 MB read + 9.6 MB written)", "kernel_sha": "r01i"},
+}
+TENSOR_FLOP_PER_CLK_PER_SM = 8192          # dense fp16/bf16 tcgen05 rate (2.25 PFLOP/s nominal = 8192 x 148 SMs x 1.86 GHz)
+
+
+def kernel_sha() -> str:
+    import hashlib
+    with open(os.path.join(ROOT, "paper_1211_5481_b200", "csrc", "fitness_umma.cuh"), "rb") as f:
+        return hashlib.sha256(f.read()).hexdigest()[:12]
+
+
+def traffic_entry(name):
+    e = NCU_TRAFFIC.get(name)
+    if e is None:
+        return None, "no ncu --set full capture of this workload"
+    if e["kernel_sha"] != kernel_sha():
+        return None, f"withheld: {e['source']} is a capture of another version of the kernel ({e['kernel_sha']} != {kernel_sha()})"
+    return e["bytes"], f"{e['source']} (ncu --set full), not measured in this run"
 
 
 def parse_args():
@@ -57,6 +77,8 @@ def parse_args():
                     help="small problems: time game_evolve_fused (the whole generation loop as one persistent kernel)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true",
+                    help="default c3 line: leave out the `sweep` key (c0, c1, c2 and the configs[4] grid in the same process)")
     return ap.parse_args()
 
 
@@ -177,6 +199,137 @@ def config_dict(cfg, scheme_name, n_gpus):
                   else "L2 flushed between timed steps is not possible inside a no-sync generation loop; inputs fit L2"}
 
 
+def roofline_of(cfg, game, scheme, fused, kernel_ms, kernel_n, loop_ms, steps, peaks, peaks_src, clocks):
+    """Roofline object of the dominant kernel.  `peak` is the measured figure the contract names (sustained bf16 = fp16
+    rate for a kernel timed inside a long step loop); because a run under the power cap can exceed a cuBLAS-derived
+    figure, the fractions against the burst figure and against the clock-scaled hardware rate are printed beside it."""
+    if fused:      # one persistent kernel = the whole timed region: fp32 FFMA arithmetic, 2 P M G flop per generation
+        flops_per_launch = 2.0 * cfg.P * cfg.M * cfg.G * steps
+        kernel_ms, kernel_n = loop_ms, 1
+    elif scheme == game.SCHEME_F16X3:
+        flops_per_launch = 6.0 * cfg.P * cfg.M * (cfg.G - 1)     # 3 MMAs per gene; the bias gene rides on the epilogue
+    else:
+        flops_per_launch = 2.0 * cfg.P * cfg.M * cfg.G
+    avg_s = kernel_ms * 1e-3 / max(kernel_n, 1)
+    achieved = flops_per_launch / avg_s / 1e12 if avg_s > 0 else 0.0
+    tensor = scheme == game.SCHEME_F16X3 and not fused
+    sm_mhz = (clocks or {}).get("sm_mhz") or float(peaks.get("sm_max_mhz", 1965.0))
+    if tensor:
+        peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+        burst = float(peaks["bf16_tflops"])
+        clock_peak = TENSOR_FLOP_PER_CLK_PER_SM * 148 * sm_mhz * 1e6 / 1e12
+        peak_note = (f"{peaks_src} bf16_tflops_sustained (fp16 and bf16 share the kind::f16 rate; kernel timed inside a step loop)")
+        bound = "tensor"
+        extra = {"frac_of_burst": achieved / burst, "peak_burst": burst,
+                 "frac_of_clock_scaled_peak": achieved / clock_peak, "peak_clock_scaled": clock_peak,
+                 "peak_clock_scaled_note": f"{TENSOR_FLOP_PER_CLK_PER_SM} flop/clk/SM x 148 SMs x the SM clock sampled in the step loop ({sm_mhz:.0f} MHz): the ceiling at this clock",
+                 "useful_tflops": achieved / 3.0}
+    else:
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        peak_note = "derived fp32 FFMA peak: 148 SM x 128 lanes x 2 flop x 1.965 GHz"
+        bound = "alu"
+        extra = {}
+    traffic, traffic_source = traffic_entry(cfg.name) if tensor else (None, "not captured")
+    mufu_per_eval = 0.0 if (cfg.activation == wl.ACT_IDENTITY or fused) else 1.25
+    fr = {"tensor": achieved / peak if tensor else 0.0,
+          "mufu": mufu_per_eval * cfg.P * cfg.M / avg_s / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6) if avg_s > 0 else 0.0,
+          "hbm": 4 * (cfg.P * (cfg.N + 1)) / avg_s / 1e9 / float(peaks["hbm_gbs"]) if avg_s > 0 else 0.0}
+    out = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+           "traffic": traffic, "traffic_source": traffic_source,
+           "kernel": "ga_fused_kernel" if fused else ("fitness_umma_kernel" if tensor else "fitness_ffma_kernel"),
+           "kernel_ms_avg": avg_s * 1e3, "kernel_launches_timed": kernel_n,
+           "kernel_share_of_step": (avg_s * 1e3) / (loop_ms / steps) if loop_ms > 0 else None,
+           "flops_per_launch": flops_per_launch, "peak_source": peak_note,
+           "hbm_algorithmic_bytes_per_launch": 4 * (cfg.P * (cfg.N + 1)),
+           "mufu_frac_at_max_clock": fr["mufu"], "hbm_frac_of_measured": fr["hbm"],
+           "binding_unit": max(fr, key=fr.get) if tensor else "alu"}
+    out.update(extra)
+    return out
+
+
+def sweep_points(args, game, torch, peaks, peaks_src):
+    """The other BASELINE.json configurations in the same process: c0, c1, c2 as generation loops (device-resident,
+    uninstrumented loop + an instrumented pass for the kernel time) and the configs[4] fitness-kernel grid."""
+    pts = []
+    for name, steps, warmup in (("c0", 400, 40), ("c1", 400, 40), ("c2", 100, 10)):
+        cfg = wl.CONFIGS[name]
+        X, t, _ = wl.make_kb(cfg)
+        G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation)
+        G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+        G.load_kb(X, t)
+        G.init_population(cfg.seed)
+        game.game_evolve(G.ctx, cfg.seed, 0, warmup)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = G.launch_count()
+        e0.record()
+        game.game_evolve(G.ctx, cfg.seed, warmup, steps)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        launches = G.launch_count() - l0
+        clocks = sampler.stop()
+        game.game_time_fitness_kernel(G.ctx, True)
+        game.game_evolve(G.ctx, cfg.seed, warmup + steps, min(steps, 50))
+        torch.cuda.synchronize()
+        kms, kn = game.game_fitness_kernel_ms(G.ctx)
+        game.game_time_fitness_kernel(G.ctx, False)
+        rf = roofline_of(cfg, game, G.scheme(), False, kms, kn, ms, steps, peaks, peaks_src, clocks)
+        pts.append({"workload": f"{name}: BASELINE.json configs[{name[1:]}]", "P": cfg.P, "G": cfg.G, "M": cfg.M, "steps": steps,
+                    "evals_per_s": cfg.P * cfg.M * steps / (ms * 1e-3), "generations_per_s": steps / (ms * 1e-3),
+                    "ms_per_step": ms / steps, "gpu_launches": int(launches), "kernel_ms": rf["kernel_ms_avg"],
+                    "tensor_tflops": rf["achieved"], "tensor_frac_of_sustained": rf["frac"], "tensor_frac_of_burst": rf.get("frac_of_burst"),
+                    "mufu_frac_at_max_clock": rf["mufu_frac_at_max_clock"], "hbm_frac": rf["hbm_frac_of_measured"],
+                    "binding_unit": "launch latency" if name in ("c0", "c1") else rf["binding_unit"], "clocks": clocks,
+                    "l2": "X fits L2 (not flushed: the loop has no host sync)"})
+        G.close()
+    # configs[4]: fitness kernel only, M x P grid
+    big = wl.c4(max(wl.C4_M), max(wl.C4_P))
+    X, t, _ = wl.make_kb(big)
+    Xd, td = torch.from_numpy(X).cuda(), torch.from_numpy(t).cuda()
+    for M in wl.C4_M:
+        W = torch.from_numpy(wl.uniform_population(M, big.G, seed=4)).cuda()
+        for P in wl.C4_P:
+            pts.append(c4_point(game, torch, big, M, P, Xd, td, W, max(args.warmup, 3), 5, peaks))
+    return pts
+
+
+def c4_point(game, torch, big, M, P, Xd, td, W, warmup, steps, peaks):
+    G = game.Game(P, big.N, big.d, M, big.expansion, big.activation)
+    G.X.copy_(Xd[:P]); G.t.copy_(td[:P]); G.set_population(W)
+    for _ in range(warmup):
+        game.game_eval_fitness(G.ctx)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    game.game_time_fitness_kernel(G.ctx, True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = G.launch_count()
+    e0.record()
+    for _ in range(steps):
+        game.game_eval_fitness(G.ctx)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    kms, kn = game.game_fitness_kernel_ms(G.ctx)
+    game.game_time_fitness_kernel(G.ctx, False)
+    clocks = sampler.stop()
+    launches = G.launch_count() - launches0      # the library's own count (fitness + finalize per evaluation)
+    tf = 6.0 * P * M * (big.G - 1) / (kms / kn * 1e-3) / 1e12
+    fr = {"tensor": tf / float(peaks["bf16_tflops"]),
+          # epilogue: 1.25 MUFU per evaluation (ex2 each, one rcp per four), 16 MUFU lanes per SM per clock
+          "mufu": 1.25 * P * M / (kms / kn * 1e-3) / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6),
+          "hbm": 4.0 * P * (big.N + 1) / (kms / kn * 1e-3) / 1e9 / float(peaks["hbm_gbs"])}
+    G.close()
+    return {"workload": "c4: BASELINE.json configs[4] (fitness kernel only)", "M": M, "P": P, "G": big.G, "ms_per_eval": ms,
+            "evals_per_s": P * M / (ms * 1e-3), "kernel_ms": kms / kn, "gpu_launches": int(launches),
+            "tensor_tflops": tf, "tensor_frac_of_burst": fr["tensor"], "tensor_frac": fr["tensor"],
+            "mufu_frac_at_max_clock": fr["mufu"], "hbm_frac": fr["hbm"], "binding_unit": max(fr, key=fr.get),
+            "sm_mhz": clocks.get("sm_mhz"), "l2": "X larger than L2" if P * big.N * 4 > 126e6 else "X fits L2 (not flushed)"}
+
+
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
     import paper_1211_5481_b200 as game
@@ -225,27 +378,35 @@ def run_ours(args, cfg, rank, world, local_rank):
             game.game_set_fitness_from_sse(G.ctx, sse.data_ptr(), cfg.P * world, None)
             game.game_step(G.ctx, seed, first_gen + i)
 
-    # ---------------- device-resident leg
+    # ---------------- device-resident leg: NO instrumentation inside the timed region (the generation loop is replayed from
+    # a CUDA graph / runs under programmatic dependent launch; per-kernel events would sit inside the chain they overlap)
     generations(0, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     launches0 = G.launch_count()
-    game.game_time_fitness_kernel(G.ctx, True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     generations(args.warmup, args.steps)
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
-    kernel_ms, kernel_n = game.game_fitness_kernel_ms(G.ctx)
-    game.game_time_fitness_kernel(G.ctx, False)
     launches = G.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
     ms = max_over_ranks(ms, dist, dev)
     units = cfg.P * cfg.M * args.steps * world
     value = job_value(cfg.P, cfg.M, args.steps, world, ms)
+    # ---------------- the dominant kernel's own duration: a second, instrumented pass over the same steps (CUDA events on
+    # the library's stream around every launch of the fused fitness kernel; plain launches, no graph)
+    kernel_ms, kernel_n = 0.0, 0
+    if not args.fused and not shard:
+        n_k = min(args.steps, 50)
+        game.game_time_fitness_kernel(G.ctx, True)
+        generations(args.warmup + args.steps, n_k)
+        barrier()
+        kernel_ms, kernel_n = game.game_fitness_kernel_ms(G.ctx)
+        game.game_time_fitness_kernel(G.ctx, False)
 
     # ---------------- end-to-end leg: host buffers through game_generation_host
     e2e = None
@@ -287,31 +448,8 @@ def run_ours(args, cfg, rank, world, local_rank):
     # ---------------- roofline of the dominant kernel (fused fitness)
     peaks, peaks_src = load_peaks()
     fused = args.fused
-    if fused:      # one persistent kernel = the whole timed region: fp32 FFMA arithmetic, 2 P M G flop per generation
-        flops_per_launch = 2.0 * cfg.P * cfg.M * cfg.G * args.steps
-        kernel_ms, kernel_n = ms, 1
-    else:
-        flops_per_launch = (6.0 * cfg.P * cfg.M * (cfg.G - 1) if G.scheme() == game.SCHEME_F16X3      # 3 MMAs per gene; the bias gene rides on the epilogue
-                            else 2.0 * cfg.P * cfg.M * cfg.G)
-    avg_s = kernel_ms * 1e-3 / max(kernel_n, 1)
-    achieved = flops_per_launch / avg_s / 1e12
-    if G.scheme() == game.SCHEME_F16X3 and not fused:
-        peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
-        peak_note = (f"{peaks_src} bf16_tflops_sustained (fp16 and bf16 share the kind::f16 rate; the kernel is timed "
-                     f"inside a {ms / 1e3:.2f} s step loop); burst figure {peaks['bf16_tflops']}")
-        bound = "tensor"
-    else:
-        peak = 148 * 128 * 2 * 1.965e9 / 1e12
-        peak_note = "derived fp32 FFMA peak: 148 SM x 128 lanes x 2 flop x 1.965 GHz"
-        bound = "alu"
-    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel": "ga_fused_kernel" if fused else ("fitness_umma_kernel" if bound == "tensor" else "fitness_ffma_kernel"),
-                "kernel_ms_avg": avg_s * 1e3, "kernel_launches_timed": kernel_n, "kernel_share_of_step": kernel_ms / ms,
-                "flops_per_launch": flops_per_launch, "peak_source": peak_note,
-                "hbm_algorithmic_bytes_per_launch": 4 * (cfg.P * (cfg.N + 1)),
-                "mufu_frac_at_max_clock": (0.0 if cfg.activation == wl.ACT_IDENTITY or fused else
-                                           1.25 * cfg.P * cfg.M / avg_s / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6)),
-                "hbm_frac_of_measured": 4 * (cfg.P * (cfg.N + 1)) / avg_s / 1e9 / float(peaks["hbm_gbs"])}
+    roofline = roofline_of(cfg, game, G.scheme(), fused, kernel_ms, kernel_n, ms, args.steps, peaks, peaks_src, clocks)
+    bound = roofline["bound"]
 
     # ---------------- CPU baseline: the oracle as it stands, one thread, bounded sample
     cpu = None
@@ -329,9 +467,17 @@ def run_ours(args, cfg, rank, world, local_rank):
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f16x3->f32" if bound == "tensor" else "f32", "data": "synthetic",
             "config": config_dict(cfg, scheme_name, world), "generations_per_s": args.steps / (ms * 1e-3),
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
-    print(json.dumps(line), flush=True)
+            "e2e": e2e, "gpu_launches": int(launches), "graph_replays": int(game.game_graph_replays(G.ctx)),
+            "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
     G.close()
+    # ---------------- the other BASELINE.json configurations, same process, same box (default c3 line, one GPU only)
+    if world == 1 and cfg.name == "c3" and not args.no_sweep and not args.fused:
+        del X, t
+        line["sweep"] = sweep_points(args, game, torch, peaks, peaks_src)
+        line["sweep_note"] = ("c0/c1/c2: generation loops (game_evolve, device-resident, no instrumentation in the timed loop; kernel_ms "
+                              "from a separate instrumented pass); c4: game_eval_fitness only, every point timed alone against the burst peak; "
+                              "peaks: " + peaks_src + " MEASURED_PEAKS.json")
+    print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -350,36 +496,15 @@ def run_c4_sweep(args):
     X, t, _ = wl.make_kb(big)
     Xd, td = torch.from_numpy(X).cuda(), torch.from_numpy(t).cuda()
     sweep, launches = [], 0
-    sampler = ClockSampler(0)
-    sampler.start()
     for M in wl.C4_M:
         W = torch.from_numpy(wl.uniform_population(M, big.G, seed=4)).cuda()
         for P in wl.C4_P:
-            G = game.Game(P, big.N, big.d, M, big.expansion, big.activation)
-            G.X.copy_(Xd[:P]); G.t.copy_(td[:P]); G.set_population(W)
-            for _ in range(max(args.warmup, 3)):
-                game.game_eval_fitness(G.ctx)
-            torch.cuda.synchronize()
-            game.game_time_fitness_kernel(G.ctx, True)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            launches0 = G.launch_count()
-            e0.record()
-            for _ in range(args.steps):
-                game.game_eval_fitness(G.ctx)
-            e1.record()
-            torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1) / args.steps
-            kms, kn = game.game_fitness_kernel_ms(G.ctx)
-            launches += G.launch_count() - launches0      # the library's own count (fitness + finalize per evaluation)
-            tf = 6.0 * P * M * (big.G - 1) / (kms / kn * 1e-3) / 1e12
-            sweep.append({"M": M, "P": P, "ms_per_eval": ms, "evals_per_s": P * M / (ms * 1e-3), "kernel_ms": kms / kn,
-                          "tensor_tflops": tf, "tensor_frac": tf / float(peaks["bf16_tflops"]),
-                          "hbm_frac": 4.0 * P * (big.N + 1) / (kms / kn * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
-                          # epilogue: 1.25 MUFU per evaluation (ex2 each, one rcp per four), 16 MUFU lanes per SM per clock
-                          "mufu_frac_at_max_clock": 1.25 * P * M / (kms / kn * 1e-3) / (148 * 16 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6),
-                          "l2": "X larger than L2" if P * big.N * 4 > 126e6 else "X fits L2 (not flushed)"})
-            G.close()
-    clocks = sampler.stop()
+            pt = c4_point(game, torch, big, M, P, Xd, td, W, max(args.warmup, 3), args.steps, peaks)
+            launches += pt["gpu_launches"]
+            sweep.append(pt)
+    mhz = [p_["sm_mhz"] for p_ in sweep if p_.get("sm_mhz")]
+    clocks = {"sm_mhz": float(np.median(mhz)) if mhz else None, "sm_max_mhz": float(peaks.get("sm_max_mhz", 1965.0)),
+              "reasons": ["per-point clocks in sweep[].sm_mhz"]}
     last = sweep[-1]
     line = {"metric": METRIC, "value": last["evals_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": last["ms_per_eval"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -245,6 +245,21 @@ int game_confusion(game_ctx* ctx, const float* y_dev, const float* t_dev, int64_
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 int game_launch_count(const game_ctx* ctx, uint64_t* launches);
 
+/* Diagnostics of the LAST tensor-core fitness launch (what the profiles/ summaries quote): the share of its issue loop the
+ * MMA-issuing warp spent waiting for a W operand slot (a_full), for the generated phi stage (b_full) and for a free TMEM
+ * accumulator (acc_empty), averaged over the leader CTAs.  Synchronises the stream.  raw_host (or NULL) receives up to
+ * raw_slots of the per-CTA records, 16 int64 each: the three waits and the loop's length in SM cycles, then -- in a library
+ * built with -DGAME_PROFILE_PHASES -- globaltimer stamps (ns) of kernel entry, prologue done, predecessor complete, last MMA
+ * issued, cluster through, exit. */
+int game_mma_stall(game_ctx* ctx, double* frac_a_full, double* frac_b_full, double* frac_acc_empty, int64_t* raw_host,
+                   int32_t raw_slots);
+
+/* Number of CUDA-graph replays this context has issued so far: game_run / game_evolve capture the launch chain of 16
+ * generations once (seed, generation index and best-fitness slot live in device memory, so the graph needs no per-generation
+ * argument) and replay it; every replay adds its kernel count to game_launch_count.  0 when the graph path is off
+ * (GAME_GRAPH=0 in the environment at game_create), unavailable, or the run was shorter than 16 generations. */
+int game_graph_replays(const game_ctx* ctx, uint64_t* replays);
+
 /* Timing hook for the roofline line: when enabled, game_eval_fitness brackets the fused fitness kernel
  * with CUDA events on the context's stream; game_fitness_kernel_ms returns the sum of the recorded
  * durations (milliseconds) and the number of launches since the hook was (re)enabled, after

@@ -56,6 +56,8 @@ SIGNATURES = {
     "game_predict": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, _F32P]),
     "game_confusion": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, C.c_float, _VP]),
     "game_launch_count": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
+    "game_graph_replays": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
+    "game_mma_stall": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), _VP, C.c_int32]),
     "game_time_fitness_kernel": (C.c_int, [_VP, C.c_int32]),
     "game_fitness_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
     "game_last_error": (C.c_char_p, [_VP]),
@@ -229,6 +231,21 @@ def game_confusion(ctx, y_dev: int, t_dev: int, Q: int, threshold: float, counts
 def game_launch_count(ctx) -> int:
     n = C.c_uint64()
     _check(ctx, lib().game_launch_count(ctx, C.byref(n)))
+    return n.value
+
+
+def game_mma_stall(ctx, raw=None):
+    """(a_full, b_full, acc_empty) wait shares of the MMA warp in the last tensor-core fitness launch; `raw`: optional
+    numpy int64 array that receives the per-CTA records."""
+    a, b, e = C.c_double(), C.c_double(), C.c_double()
+    _check(ctx, lib().game_mma_stall(ctx, C.byref(a), C.byref(b), C.byref(e), None if raw is None else raw.ctypes.data,
+                                     0 if raw is None else raw.size))
+    return a.value, b.value, e.value
+
+
+def game_graph_replays(ctx) -> int:
+    n = C.c_uint64()
+    _check(ctx, lib().game_graph_replays(ctx, C.byref(n)))
     return n.value
 
 

@@ -81,6 +81,11 @@ constexpr int kBarBytes = (2 * kMaxASlots + 2 * kStagesTotal + 4) * 8 + 16;
 constexpr int kTsBytes = kBN * 4;                 // targets of the current pattern tile, staged once per unit
 constexpr int kSmemBytes = kSmemBar + kBarBytes + kTsBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
+constexpr int kStallSlots = 16;                // diagnostic slots per CTA (Params::stall)
+#ifndef GAME_POLY_PAIRS
+#define GAME_POLY_PAIRS 1
+#endif
+constexpr int kPolyPairs = GAME_POLY_PAIRS;    // of every four packed pairs of the epilogue, how many take 2^s from the FMA pipe
 static_assert(kSmemBytes <= 232448, "shared memory budget");
 // Operand pre-scaling (both powers of two, so exact, and undone by the epilogue's FFMA constant).  An fp16 hi/lo split is
 // only RELATIVE down to 2^-14: below that the lo half is an fp16 subnormal (quantum 2^-24) and an operand of magnitude
@@ -101,9 +106,11 @@ struct Params {
                            //             times the row's calibrated accumulation correction, see calibrate_kernel)
     float* zdump;          // calibration launch only (else NULL): [m_stride][256] raw accumulated z of pattern tile p_tile0;
                            //             no error sums are formed
-    double* part;          // [gridDim.x * 2][m_stride]
+    double* part;          // [gridDim.x * 2][m_stride] slots of 8 bytes, each holding the running sum as a float-float pair
+                           //             (hi, lo): see the epilogue
     const int* stop;       // optional: non-zero => the stop rule is met, the kernel returns at once
-    long long* stall;      // optional [gridDim.x][4]: cycles the MMA/relay warp waited on a_full, b_full, acc_empty; total
+    long long* stall;      // optional [gridDim.x][kStallSlots]: cycles the MMA/relay warp waited on a_full, b_full, acc_empty; its total;
+                           //          slots 4..: globaltimer stamps of the kernel's phases when built with -DGAME_PROFILE_PHASES
     long long P;
     int N, d, M, G;
     int m_stride;          // m_tiles * 128
@@ -195,6 +202,21 @@ __device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
 template <int NS>
 __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
+    uint32_t n = 0;
+    unsigned long long t0 = 0;
+    do {
+        __nanosleep(NS);
+        wait_watchdog(n, t0);
+    } while (!mbar_try_wait(bar, parity));
+}
+// The epilogue's accumulator wait: short on the mid-size shapes (the epilogue is the slower side there and a 256 ns nap
+// costs ~500 cycles of hand-off), long on the tensor-bound ones (where a spinning warp takes issue slots from the MMA
+// warp): poll a few times first, then sleep.
+template <int SPINS, int NS>
+__device__ __forceinline__ void mbar_wait_spin_then_sleep(uint32_t bar, uint32_t parity) {
+#pragma unroll 1
+    for (int i = 0; i < SPINS; ++i)
+        if (mbar_try_wait(bar, parity)) return;
     uint32_t n = 0;
     unsigned long long t0 = 0;
     do {
@@ -304,12 +326,37 @@ __device__ __forceinline__ float rcp_approx(float x) {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// NaN-propagating clamps (fminf / fmaxf return the other operand for a NaN, which would turn a NaN z into a finite error).
+__device__ __forceinline__ float min_nan(float a, float b) {
+    float r;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ float max_nan(float a, float b) {
+    float r;
+    asm("max.NaN.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
+}
 
 // Shared-memory matrix descriptor: K-major, SWIZZLE_NONE; start address, LBO (k-group stride) and SBO
 // (8-row group stride) in 16-byte units; descriptor version 1 (sm_100).
 __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
     return static_cast<uint64_t>((saddr & 0x3FFFFu) >> 4) | (static_cast<uint64_t>(lbo_bytes >> 4) << 16) |
            (static_cast<uint64_t>(sbo_bytes >> 4) << 32) | (1ull << 46);
+}
+// The same descriptor in two words: the low one holds the start address (bits 0-13, 16-byte units; shared memory is
+// < 256 KB, so adding a byte offset / 16 never carries out of the field) and the k-group stride LBO = 128 rows x 16 B
+// (both operands); the high one is constant (SBO = 128 B, descriptor version 1).
+static_assert(kBM == kRows, "A and B share the k-group stride");
+constexpr uint32_t kDescHiWord = (128u >> 4) | (1u << 14);
+constexpr uint32_t kLoHalf = kABytes >> 4;        // hi image -> lo image of the same K step
+constexpr uint32_t kNextStep = kSlotBytes >> 4;   // next K step
+static_assert(kABytes == kBBytes, "A and B share the image size");
+__device__ __forceinline__ uint32_t desc_lo_word(uint32_t saddr) { return ((saddr & 0x3FFFFu) >> 4) | (static_cast<uint32_t>((kBM * 16) >> 4) << 16); }
+__device__ __forceinline__ uint64_t desc_from_lo(uint32_t lo) {
+    uint64_t d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "r"(lo), "r"(kDescHiWord));
+    return d;
 }
 // Instruction descriptor, kind::f16: D = F32 (bit 4), A = B = F16 (0), both K-major, N >> 3 at bit 17,
 // M >> 4 at bit 24 (M = 256: the pair's two 128-row halves).
@@ -407,79 +454,119 @@ __device__ __forceinline__ void store_w_image_gene(uint8_t* img, int steps, int 
 // up to eps sqrt<z z> / sigma for residual noise sigma (measured 8.9e-5 at sigma = 0.01, identity output).
 // So for the regression activations (identity, tanh) the shrink of every chromosome row is MEASURED before each
 // evaluation: one extra launch of the fitness kernel hands out the raw accumulators of the first pattern tile
-// (Params::zdump), this kernel recomputes the same z for those <= 256 patterns on the CUDA cores (fp32 expansion as in the
-// producers, products and sum in fp64) and fits z_exact = (1 + eps_m) z_tensor by least squares; the evaluation then runs
-// with the row's un-scaling factor times (1 + eps_m).  One block per chromosome, one thread per sample pattern.
+// (Params::zdump), cal_phi_kernel + calibrate_kernel recompute the same z for those <= 256 patterns on the CUDA cores (fp32
+// expansion as in the producers, products and sum in fp64) and fits z_exact = (1 + eps_m) z_tensor by least squares; the evaluation then runs
+// with the row's un-scaling factor times (1 + eps_m).
 constexpr int kCalThreads = kBN;         // one thread per sample pattern
+constexpr int kCalRows = 8;              // chromosome rows per block of calibrate_kernel (fewer when G is long)
+constexpr int kCalUnroll = 16;           // phi loads in flight per thread
+
+// phi of the <= 256 sample patterns (the first pattern tile), as the producers generate it (fp32 recurrences), widened to
+// fp64 once: phi_s[(g - 1) * 256 + p] for genes g = 1..G-1.  One thread per pattern.
 template <int EXPANSION>
-__global__ void __launch_bounds__(kCalThreads) calibrate_kernel(const float* __restrict__ X, const float* W, const float* zdump,
-                                                                const float* wscale, float* zcorr, const int* stop, long long P,
-                                                                int N, int d, int M, int G, int shared, int stage_w) {
-    extern __shared__ float cal_w[];       // [G] when stage_w: this chromosome (longer ones are read through the caches)
-    __shared__ double s_num[kCalThreads / 32], s_den[kCalThreads / 32];
-    pdl_wait();                // the calibration launch's accumulators, W and the row scales are complete
+__global__ void __launch_bounds__(kCalThreads) cal_phi_kernel(const float* __restrict__ X, double* phi_s, const int* stop, long long P,
+                                                              int N, int d, int shared) {
+    pdl_wait();
     pdl_launch_dependents();
     if (stop != nullptr && __ldcg(stop) != 0) return;
-    const int m = blockIdx.x, p = threadIdx.x;      // one block per chromosome row of the padded population
-    const float f = __ldcg(wscale + m);
-    if (m >= M) {
-        if (p == 0) zcorr[m] = f;
-        return;
-    }
-    const float* w = W + static_cast<size_t>(m) * G;
-    if (stage_w) {
-        for (int g = p; g < G; g += kCalThreads) cal_w[g] = __ldcg(w + g);
-        __syncthreads();
-        w = cal_w;
-    }
-    const int n = static_cast<int>(min(static_cast<long long>(kBN), P));
+    const int p = threadIdx.x;
     const int dd = EXPANSION == 0 ? d : 2 * d;
-    double num = 0.0, den = 0.0;
-    if (p < n) {
-        const float* xr = X + static_cast<size_t>(p) * N;
-        double z = 0.0;
-        for (int i = 0; i < N; ++i) {
-            const float x = __ldg(xr + i);
-            const float* wi = w + 1 + (shared ? 0 : i * dd);
-            if (EXPANSION == 0) {
-                const float x2 = 2.0f * x;
-                float tm = 1.0f, tc = x;
-                for (int j = 0; j < d; ++j) {
-                    z += static_cast<double>(wi[j]) * static_cast<double>(tc);
-                    const float tn = fmaf(x2, tc, -tm);
-                    tm = tc; tc = tn;
-                }
+    const float* xr = X + static_cast<size_t>(p < P ? p : 0) * N;
+    if (shared)
+        for (int jj = 0; jj < dd; ++jj) phi_s[static_cast<size_t>(jj) * kBN + p] = 0.0;
+    // per-feature coefficients: one block per feature; shared coefficients: one block adds up all features
+    const int i_begin = shared ? 0 : blockIdx.x, i_end = shared ? N : blockIdx.x + 1;
+    for (int i = i_begin; i < i_end; ++i) {
+        const float x = __ldg(xr + i);
+        double* out = phi_s + static_cast<size_t>(shared ? 0 : i * dd) * kBN + p;
+        float x2, cm = 1.0f, cc, sm = 0.0f, sc = 0.0f;
+        if (EXPANSION == 0) {
+            x2 = 2.0f * x; cc = x;
+        } else {
+            float s1, c1;
+            sincosf(x, &s1, &c1);
+            x2 = 2.0f * c1; cc = c1; sc = s1;
+        }
+        for (int k = 0; k < d; ++k) {
+            if (shared) {
+                out[static_cast<size_t>(k) * kBN] += static_cast<double>(cc);
+                if (EXPANSION == 1) out[static_cast<size_t>(d + k) * kBN] += static_cast<double>(sc);
             } else {
-                float s1, c1;
-                sincosf(x, &s1, &c1);
-                const float x2 = 2.0f * c1;
-                float cm = 1.0f, cc = c1, sm = 0.0f, sc = s1;
-                for (int k = 0; k < d; ++k) {
-                    z += static_cast<double>(wi[k]) * static_cast<double>(cc);
-                    z += static_cast<double>(wi[d + k]) * static_cast<double>(sc);
-                    const float cn = fmaf(x2, cc, -cm), sn = fmaf(x2, sc, -sm);
-                    cm = cc; cc = cn;
-                    sm = sc; sc = sn;
-                }
+                out[static_cast<size_t>(k) * kBN] = static_cast<double>(cc);
+                if (EXPANSION == 1) out[static_cast<size_t>(d + k) * kBN] = static_cast<double>(sc);
+            }
+            const float cn = fmaf(x2, cc, -cm);
+            cm = cc; cc = cn;
+            if (EXPANSION == 1) {
+                const float sn = fmaf(x2, sc, -sm);
+                sm = sc; sc = sn;
             }
         }
-        const double zt = static_cast<double>(__ldcg(zdump + static_cast<size_t>(m) * kBN + p)) * static_cast<double>(f);
-        num = (z - zt) * zt;
-        den = zt * zt;
+    }
+}
+
+// zcorr[m] = wscale[m] (1 + eps_m), eps_m from the least-squares fit z_exact = (1 + eps_m) z_tensor over the sample
+// patterns.  A block takes `rows` consecutive chromosomes (their genes staged in shared memory as fp64) and all sample
+// patterns (one per thread): a small fp64 contraction, phi_s streamed once per block.
+__global__ void __launch_bounds__(kCalThreads) calibrate_kernel(const float* W, const double* phi_s, const float* zdump,
+                                                                const float* wscale, float* zcorr, const int* stop, long long P,
+                                                                int M, int G, int m_stride, int rows) {
+    extern __shared__ double cal_w[];      // [rows][Kp]: the rows' genes 1..G-1 in fp64, zero-padded to a multiple of kCalUnroll
+    __shared__ double s_num[kCalRows][kCalThreads / 32], s_den[kCalRows][kCalThreads / 32];
+    pdl_wait();                // the calibration launch's accumulators, phi_s, W and the row scales are complete
+    pdl_launch_dependents();
+    if (stop != nullptr && __ldcg(stop) != 0) return;
+    const int m0 = blockIdx.x * rows, p = threadIdx.x, K = G - 1;
+    const int Kp = (K + kCalUnroll - 1) / kCalUnroll * kCalUnroll;
+    for (int r = 0; r < rows; ++r) {
+        const int m = m0 + r;
+        for (int g = p; g < Kp; g += kCalThreads)
+            cal_w[static_cast<size_t>(r) * Kp + g] =
+                (m < M && g < K) ? static_cast<double>(__ldcg(W + static_cast<size_t>(m) * G + 1 + g)) : 0.0;
+    }
+    __syncthreads();
+    const int n = static_cast<int>(min(static_cast<long long>(kBN), P));
+    double z[kCalRows];
+#pragma unroll
+    for (int r = 0; r < kCalRows; ++r) z[r] = 0.0;
+    if (p < n) {
+        // kCalUnroll loads of phi in flight at a time: one block per SM cannot hide an L2 round trip per gene otherwise
+        for (int g0 = 0; g0 < Kp; g0 += kCalUnroll) {
+            double ph[kCalUnroll];
+#pragma unroll
+            for (int u = 0; u < kCalUnroll; ++u) ph[u] = g0 + u < K ? __ldcg(phi_s + static_cast<size_t>(g0 + u) * kBN + p) : 0.0;
+#pragma unroll
+            for (int u = 0; u < kCalUnroll; ++u)
+#pragma unroll
+                for (int r = 0; r < kCalRows; ++r)
+                    if (r < rows) z[r] = fma(cal_w[static_cast<size_t>(r) * Kp + g0 + u], ph[u], z[r]);
+        }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        num += __shfl_xor_sync(0xffffffffu, num, o);
-        den += __shfl_xor_sync(0xffffffffu, den, o);
+    for (int r = 0; r < kCalRows; ++r) {
+        if (r >= rows) break;
+        const int m = m0 + r;
+        double num = 0.0, den = 0.0;
+        if (p < n && m < m_stride) {
+            const double zt = static_cast<double>(__ldcg(zdump + static_cast<size_t>(m) * kBN + p)) * static_cast<double>(__ldcg(wscale + m));
+            num = (z[r] - zt) * zt;
+            den = zt * zt;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            num += __shfl_xor_sync(0xffffffffu, num, o);
+            den += __shfl_xor_sync(0xffffffffu, den, o);
+        }
+        if ((p & 31) == 0) { s_num[r][p >> 5] = num; s_den[r][p >> 5] = den; }
     }
-    if ((p & 31) == 0) { s_num[p >> 5] = num; s_den[p >> 5] = den; }
     __syncthreads();
-    if (p == 0) {
-        num = 0.0; den = 0.0;
-        for (int wv = 0; wv < kCalThreads / 32; ++wv) { num += s_num[wv]; den += s_den[wv]; }   // fixed order: bit-stable
+    if (p < rows && m0 + p < m_stride) {
+        const int m = m0 + p;
+        double num = 0.0, den = 0.0;
+        for (int wv = 0; wv < kCalThreads / 32; ++wv) { num += s_num[p][wv]; den += s_den[p][wv]; }   // fixed order: bit-stable
         double eps = den > 0.0 ? num / den : 0.0;
-        if (!(fabs(eps) <= 1e-4)) eps = 0.0;       // non-finite rows, or a row the model does not describe: leave it alone
-        zcorr[m] = static_cast<float>(static_cast<double>(f) * (1.0 + eps));
+        if (!(fabs(eps) <= 1e-4) || m >= M) eps = 0.0;   // non-finite rows, or a row the model does not describe: leave it alone
+        zcorr[m] = static_cast<float>(static_cast<double>(__ldcg(wscale + m)) * (1.0 + eps));
     }
 }
 
@@ -549,10 +636,10 @@ __device__ __forceinline__ void act_err2_quad(float z0, float z1, float z2, floa
         acc3 += act_err2<ACT>(z3, c, bias_term, tq.w);
         return;
     }
-    const float a0 = 1.0f + ex2_approx(fminf(fmaf(z0, c, bias_term), 30.0f));
-    const float a1 = 1.0f + ex2_approx(fminf(fmaf(z1, c, bias_term), 30.0f));
-    const float a2 = 1.0f + ex2_approx(fminf(fmaf(z2, c, bias_term), 30.0f));
-    const float a3 = 1.0f + ex2_approx(fminf(fmaf(z3, c, bias_term), 30.0f));
+    const float a0 = 1.0f + ex2_approx(min_nan(fmaf(z0, c, bias_term), 30.0f));
+    const float a1 = 1.0f + ex2_approx(min_nan(fmaf(z1, c, bias_term), 30.0f));
+    const float a2 = 1.0f + ex2_approx(min_nan(fmaf(z2, c, bias_term), 30.0f));
+    const float a3 = 1.0f + ex2_approx(min_nan(fmaf(z3, c, bias_term), 30.0f));
     const float p01 = a0 * a1, p23 = a2 * a3;
     float r = rcp_approx(p01 * p23);
     if (ACT == 2) r *= -2.0f;                      // tanh = 1 - 2 / a: tq holds 1 - t
@@ -590,6 +677,30 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
+// 2^s for a pair of arguments on the FMA pipe (packed FP32) instead of the 16-lane MUFU pipe, which is what bounds the
+// epilogue of the mid-size shapes (ncu: XU pipe 80 % busy inside the epilogue's arithmetic).  s in [-126, 30] (clamped by
+// the caller): n = round(s) through the 1.5 * 2^23 trick, r = s - n in [-1/2, 1/2], 2^r by a degree-6 minimax polynomial
+// (Remez fit on [-1/2, 1/2]; in fp32 Horner form max relative error 9.3e-8, mean 1e-10 -- ex2.approx is 1.7e-7), times
+// 2^n built in the exponent field; returns 1 + 2^s (the caller's next step) on the last FMA.  A NaN stays a NaN.
+__device__ __forceinline__ f32x2 one_plus_exp2_poly2(f32x2 s2) {
+    const float magic = 12582912.0f;                                   // 1.5 * 2^23
+    const f32x2 t2 = add2(s2, pack2(magic, magic));
+    const f32x2 n2 = add2(t2, pack2(-magic, -magic));
+    const f32x2 r2 = add2(s2, mul2(n2, pack2(-1.0f, -1.0f)));
+    f32x2 p = fma2(pack2(0x1.41d334p-13f, 0x1.41d334p-13f), r2, pack2(0x1.5f456ap-10f, 0x1.5f456ap-10f));
+    p = fma2(p, r2, pack2(0x1.3b2dbcp-7f, 0x1.3b2dbcp-7f));
+    p = fma2(p, r2, pack2(0x1.c6aed4p-5f, 0x1.c6aed4p-5f));
+    p = fma2(p, r2, pack2(0x1.ebfbdap-3f, 0x1.ebfbdap-3f));
+    p = fma2(p, r2, pack2(0x1.62e430p-1f, 0x1.62e430p-1f));
+    p = fma2(p, r2, pack2(1.0f, 1.0f));
+    float t0, t1;
+    unpack2(t2, t0, t1);
+    // the low mantissa bits of t hold n (two's complement): 2^n = bits((n + 127) << 23)
+    const float sc0 = __uint_as_float((__float_as_uint(t0) << 23) + 0x3f800000u);
+    const float sc1 = __uint_as_float((__float_as_uint(t1) << 23) + 0x3f800000u);
+    return fma2(p, pack2(sc0, sc1), pack2(1.0f, 1.0f));
+}
+
 // Eight outputs: two interleaved quads (columns 0,2,4,6 and 1,3,5,7), one in each half of the packed operations, each with
 // ONE reciprocal per four outputs as in act_err2_quad.  tA, tB: staged targets of columns 0..3 and 4..7.  acc: two packed
 // running sums (four scalar sums).
@@ -603,7 +714,10 @@ __device__ __forceinline__ void act_err2_oct(const uint32_t* v, float c, float b
         const f32x2 s = fma2(pack2(__uint_as_float(v[2 * k]), __uint_as_float(v[2 * k + 1])), c2, b2);
         float s0, s1;
         unpack2(s, s0, s1);
-        a[k] = add2(pack2(ex2_approx(fminf(s0, 30.0f)), ex2_approx(fminf(s1, 30.0f))), one2);
+        if (k < kPolyPairs)      // this many of the four pairs take their 2^s from the FMA pipe, the others from the MUFU pipe
+            a[k] = one_plus_exp2_poly2(pack2(max_nan(min_nan(s0, 30.0f), -126.0f), max_nan(min_nan(s1, 30.0f), -126.0f)));
+        else
+            a[k] = add2(pack2(ex2_approx(min_nan(s0, 30.0f)), ex2_approx(min_nan(s1, 30.0f))), one2);
     }
     const f32x2 p01 = mul2(a[0], a[1]), p23 = mul2(a[2], a[3]);
     float q0, q1;
@@ -653,6 +767,12 @@ struct Ring {
 template <int EXPANSION, int ACT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness_umma_kernel(const Params prm) {
     extern __shared__ __align__(1024) uint8_t smem[];
+#ifdef GAME_PROFILE_PHASES
+    const unsigned long long ph_entry = global_timer_ns();
+#define GAME_PHASE(slot) do { if (prm.stall != nullptr && threadIdx.x == 32) prm.stall[static_cast<size_t>(blockIdx.x) * kStallSlots + (slot)] = static_cast<long long>(global_timer_ns()); } while (0)
+#else
+#define GAME_PHASE(slot) do { } while (0)
+#endif
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSmemBar);
     const uint32_t bar_a_full = smem_u32(bars), bar_a_empty = bar_a_full + 8 * kMaxASlots;
     const uint32_t bar_b_full = bar_a_empty + 8 * kMaxASlots, bar_b_empty = bar_b_full + 8 * kStagesTotal;
@@ -699,11 +819,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     cluster_sync_all();          // both CTAs' barriers are initialised before any remote arrive / multicast commit
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+#ifdef GAME_PROFILE_PHASES
+    if (prm.stall != nullptr && threadIdx.x == 32) prm.stall[static_cast<size_t>(blockIdx.x) * kStallSlots + 4] = static_cast<long long>(ph_entry);
+#endif
+    GAME_PHASE(5);             // barriers, TMEM and the cluster handshake done
 
     // Everything above (barriers, TMEM, the cluster handshake) touches no global memory and overlaps the tail of the
     // preceding kernel (pdl.cuh).  From here on the W images, W, the partial sums and the stop flag are complete.
     pdl_wait();
     pdl_launch_dependents();
+    GAME_PHASE(6);             // the preceding kernel has completed
     const bool stopped = prm.stop != nullptr && __ldcg(prm.stop) != 0;   // uniform over the grid: written by an earlier kernel
     if (stopped) units = 0;    // stop rule met: no work, no writes; fall through to the teardown (TMEM is allocated)
 
@@ -796,14 +921,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                             const int k1 = min(k0 + kAKS, prm.steps);
                             const bool last_of_stage = k1 == min((j + 1) * kKS, prm.steps);
                             if (elect_one()) {
-                                for (int k = k0; k < k1; ++k) {
-                                    const uint32_t a_hi = smem_base + cur * kASlotBytes + (k - k0) * kSlotBytes, a_lo = a_hi + kABytes;
-                                    const uint32_t b_hi = b_base + rb.i * kStageBytes + (k - j * kKS) * kSlotBytes, b_lo = b_hi + kBBytes;
-                                    const uint64_t da_hi = make_desc(a_hi, kBM * 16, 128), da_lo = make_desc(a_lo, kBM * 16, 128);
-                                    const uint64_t db_hi = make_desc(b_hi, kRows * 16, 128), db_lo = make_desc(b_lo, kRows * 16, 128);
-                                    umma_f16_pair(d_tmem, da_lo, db_hi, kIdesc, k != k_first ? 1u : 0u);   // small terms first
-                                    umma_f16_pair(d_tmem, da_hi, db_lo, kIdesc, 1u);
-                                    umma_f16_pair(d_tmem, da_hi, db_hi, kIdesc, 1u);
+                                // The descriptors of a slot differ only in their start-address field (low word, 16-byte units):
+                                // one base per operand and constant increments -- lo half + kABytes / 16, next K step +
+                                // kSlotBytes / 16.  (Built from scratch per MMA this was 36 instructions per K step in the one
+                                // warp whose instruction stream paces the tensor pipe.)
+                                const uint32_t a0 = desc_lo_word(smem_base + cur * kASlotBytes);
+                                const uint32_t b0 = desc_lo_word(b_base + rb.i * kStageBytes + (k0 - j * kKS) * kSlotBytes);
+                                umma_f16_pair(d_tmem, desc_from_lo(a0 + kLoHalf), desc_from_lo(b0), kIdesc, k0 != k_first ? 1u : 0u);   // small terms first
+                                umma_f16_pair(d_tmem, desc_from_lo(a0), desc_from_lo(b0 + kLoHalf), kIdesc, 1u);
+                                umma_f16_pair(d_tmem, desc_from_lo(a0), desc_from_lo(b0), kIdesc, 1u);
+                                if (k1 - k0 > 1) {
+                                    static_assert(kAKS == 2, "the issue loop is written out for two K steps per A slot");
+                                    const uint32_t a1 = a0 + kNextStep, b1 = b0 + kNextStep;
+                                    umma_f16_pair(d_tmem, desc_from_lo(a1 + kLoHalf), desc_from_lo(b1), kIdesc, 1u);
+                                    umma_f16_pair(d_tmem, desc_from_lo(a1), desc_from_lo(b1 + kLoHalf), kIdesc, 1u);
+                                    umma_f16_pair(d_tmem, desc_from_lo(a1), desc_from_lo(b1), kIdesc, 1u);
                                 }
                                 umma_commit_pair(bar_a_empty + 8 * cur);                                    // A slot free in both CTAs
                                 if (last_of_stage && release_b) umma_commit_pair(bar_b_empty + 8 * rb.i);   // B stage free in both CTAs
@@ -820,16 +952,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             }
         }
         if (prm.stall != nullptr && lane == 0) {
-            long long* out = prm.stall + static_cast<size_t>(blockIdx.x) * 4;
+            long long* out = prm.stall + static_cast<size_t>(blockIdx.x) * kStallSlots;
             out[0] = st_a; out[1] = st_b; out[2] = st_c; out[3] = clock64() - t_begin;
         }
     } else if (warp < 2 + kNumEpiWarps) {
         // ============================================================== epilogue
         const int q = warp & 3;                 // TMEM lane quarter this warp may access
         const int h = (warp - 2) >> 2;          // column half
-        double* my_part = prm.part + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
+        // The running sum of a (CTA, column half, chromosome) slot is a float-float pair (hi, lo), hi + lo carrying ~48 bits:
+        // a tile's fp32 sum is added with an error-free TwoSum (six fp32 adds).  An fp64 add per tile did the same job, but
+        // DADD is a slow pipe on this chip (ncu: 6 % of the epilogue warps' samples were that one instruction).
+        float2* my_part = reinterpret_cast<float2*>(prm.part) + (static_cast<size_t>(blockIdx.x) * 2 + h) * prm.m_stride;
         if (prm.zero_part && !stopped && prm.zdump == nullptr)
-            for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, 0.0);
+            for (int m = q * 32 + lane; m < prm.m_stride; m += kBM) __stcg(my_part + m, make_float2(0.0f, 0.0f));
         const uint32_t leader_acc_empty = map_to_cta(bar_acc_empty, 0);
         uint32_t tile = 0;
         uint32_t uses0 = 0, uses1 = 0;          // accumulators taken over from the MMA warp so far (barrier phases)
@@ -842,6 +977,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             return pp < prm.P ? staged_target<ACT>(__ldg(prm.t + pp)) : 0.0f;
         };
         float t_next = target_of(pair);      // always one unit ahead: its HBM latency is hidden behind a whole unit
+        // The per-tile scalars of this thread's chromosome row -- bias gene, un-scaling factor, running partial sum -- are
+        // fetched ONE TILE AHEAD: loaded at the top of a tile they sat on its critical path (ncu source page of a c4 point:
+        // 9 % of the epilogue warps' samples were the first use of the bias, an L2 round trip per tile).
+        const bool sums = prm.zdump == nullptr;
+        auto row_of = [&](int mp) { return (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane; };
+        auto first_mp_of = [&](int uu) { return (uu % prm.m_groups) * prm.m_pairs_per_group; };
+        int m_nx = pair < units ? row_of(first_mp_of(pair)) : 0;
+        float a0_nx = 0.0f, f_nx = 0.0f;          // RAW loaded values: their first use (a multiply) is a tile later
+        float2 part_nx = make_float2(0.0f, 0.0f);
+        auto fetch_row = [&](int mm) {
+            a0_nx = mm < prm.M ? __ldcg(prm.W + static_cast<size_t>(mm) * prm.G) : 0.0f;
+            f_nx = __ldcg(prm.wscale + mm);
+            if (sums) part_nx = __ldcg(my_part + mm);
+        };
+        if (pair < units) fetch_row(m_nx);
         for (int u = pair; u < units; u += n_pairs) {
             const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
@@ -857,16 +1007,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             asm volatile("bar.sync %0, 128;" ::"r"(2 + h) : "memory");
             for (int mp = mp0; mp < mp1; ++mp, ++tile) {
                 const uint32_t buf = flush ? 0u : (tile & 1);
-                const int m = (2 * mp + static_cast<int>(crank)) * kBM + q * 32 + lane;
-                // the bias gene a_0 is not part of the contraction: it rides on the epilogue's FFMA
-                const float bias = bias_term_of<ACT>(m < prm.M ? __ldcg(prm.W + static_cast<size_t>(m) * prm.G) : 0.0f);
-                const float zs = zscale_of<ACT>(__ldcg(prm.wscale + m));     // this row's scale and phi's, undone on the same FFMA
-                // this lane's running sum, fetched before the wait: its L2 round trip is off the tile's critical path
-                const double part_old = prm.zdump == nullptr ? __ldcg(my_part + m) : 0.0;
+                const int m = m_nx;
+                // the bias gene a_0 is not part of the contraction: it rides on the epilogue's FFMA, together
+                // with the row's un-scaling factor; part_old is this lane's running sum
+                const float bias = bias_term_of<ACT>(a0_nx), zs = zscale_of<ACT>(f_nx);
+                const float2 part_old = part_nx;
+                // the next tile's row (of this unit, or the first of this CTA pair's next unit)
+                const bool more = mp + 1 < mp1 || u + n_pairs < units;
+                m_nx = mp + 1 < mp1 ? row_of(mp + 1) : (u + n_pairs < units ? row_of(first_mp_of(u + n_pairs)) : m);
+                const bool same_row = m_nx == m;        // one chromosome tile per unit (M <= 256): carry the sum in the register
+                if (more && !same_row) fetch_row(m_nx);
                 // streaming mode: accumulator 1 receives the K extent's later chunks one after the other; add each of them to
                 // accumulator 0 (chunk 0, then the running sum) with round-to-nearest fp32 adds and hand accumulator 1 back
                 for (int chunk = 1; chunk < n_chunks; ++chunk) {
-                    mbar_wait_sleep<256>(bar_acc_full + 8, uses1 & 1);
+                    mbar_wait_spin_then_sleep<32, 128>(bar_acc_full + 8, uses1 & 1);
                     ++uses1;
                     tc_fence_after();
 #pragma unroll 1
@@ -887,7 +1041,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8);
                 }
-                mbar_wait_sleep<256>(bar_acc_full + 8 * buf, (buf ? uses1 : uses0) & 1);   // (complete already if chunks were merged)
+                mbar_wait_spin_then_sleep<32, 128>(bar_acc_full + 8 * buf, (buf ? uses1 : uses0) & 1);   // (complete already if chunks were merged)
                 if (buf) ++uses1; else ++uses0;
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
@@ -934,7 +1088,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8 * buf);
-                if (prm.zdump == nullptr) __stcg(my_part + m, part_old + static_cast<double>(sum));
+                if (sums) {
+                    const float hi = __fadd_rn(part_old.x, sum);                       // TwoSum: hi + err == part_old.x + sum exactly
+                    const float bv = __fadd_rn(hi, -part_old.x);
+                    const float err = __fadd_rn(__fadd_rn(part_old.x, -__fadd_rn(hi, -bv)), __fadd_rn(sum, -bv));
+                    const float2 part_new = make_float2(hi, __fadd_rn(part_old.y, err));
+                    __stcg(my_part + m, part_new);
+                    if (same_row) part_nx = part_new;
+                }
             }
         }
     } else {
@@ -1160,16 +1321,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         }
     }
 
+    GAME_PHASE(7);             // the MMA warp has issued everything
     // ---- teardown: everything issued has been consumed once both epilogues have drained the last accumulator;
     // neither CTA may exit (or free TMEM) while the other can still signal its barriers or read its operands.
     tc_fence_before();
     __syncthreads();
     cluster_sync_all();
     tc_fence_after();
+    GAME_PHASE(8);             // both CTAs are through
     if (warp == 1) {
         __syncwarp();
         tmem_dealloc_pair(tmem_base, kTmemCols);
     }
+    GAME_PHASE(9);
+#undef GAME_PHASE
 }
 
 }  // namespace umma

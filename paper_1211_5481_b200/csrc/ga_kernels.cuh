@@ -39,6 +39,25 @@ __global__ void init_population_kernel(float* __restrict__ W, int M, int G, Phil
     }
 }
 
+// Device-resident state of a generation loop (game_run / game_evolve): with the seed, the first generation index, the
+// running generation count and the best-fitness trace pointer in device memory, the kernels of a generation take no
+// per-generation argument from the host, so the chain of one (or sixteen) generations can be captured ONCE in a CUDA graph
+// and replayed (one stream, no per-generation host work).  `evals` counts the fitness finalisations of the
+// run: finalisation i writes best[i] and then bumps it; the GA step that follows is step i = evals - 1.
+struct RunState {
+    PhiloxKey key;
+    uint32_t gen0;
+    int evals;
+    float* best;        // [n + 1] best fitness per generation, or NULL
+};
+
+__global__ void set_run_state_kernel(RunState* run, PhiloxKey key, uint32_t gen0, float* best) {
+    run->key = key;
+    run->gen0 = gen0;
+    run->evals = 0;
+    run->best = best;
+}
+
 struct GaParams {
     int M, G, elite, tournament;
     unsigned long long t_cross, t_mut;  // Bernoulli thresholds floor(p * 2^32)
@@ -163,7 +182,8 @@ __device__ __forceinline__ void store_row_images(uint8_t* img, float* wscale, in
 }
 
 __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, const float* F, float* Wn, GaParams p,
-                                                              const int* stop, uint8_t* img, float* wscale, int img_steps) {
+                                                              const int* stop, uint8_t* img, float* wscale, int img_steps,
+                                                              const RunState* run) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
     __shared__ float s_red[kGaThreads / 32];
     __shared__ int s_rank;
@@ -174,6 +194,11 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
     const int M = p.M, G = p.G;
     pdl_wait();                            // F (finalize), W and, for ranking / roulette, by_rank / prefix are complete
     pdl_launch_dependents();
+    if (run != nullptr) {                  // generation loop replayed from a graph: seed and generation index live on the device
+        p.key.k0 = __ldcg(&run->key.k0);
+        p.key.k1 = __ldcg(&run->key.k1);
+        p.gen = __ldcg(&run->gen0) + static_cast<uint32_t>(__ldcg(&run->evals) - 1);
+    }
     if (stop != nullptr && __ldcg(stop) != 0) {   // stop rule already met: the population is final, carry it over unchanged
         for (int g = tid; g < G; g += kGaThreads) Wn[static_cast<size_t>(c) * G + g] = __ldcg(W + static_cast<size_t>(c) * G + g);
         return;
@@ -286,7 +311,8 @@ constexpr int kFinThreads = 1024, kFinCols = 32, kFinGroups = kFinThreads / kFin
 __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* part, int n_part, int m_stride, int M,
                                                                         double P_d, float* F, double* sse_out, float* best_out,
                                                                         float* blk_key, int* blk_idx, unsigned int* ticket,
-                                                                        int* stop, float threshold, int gen_index, int rmse) {
+                                                                        int* stop, float threshold, int gen_index, int rmse,
+                                                                        RunState* run, int part_ff) {
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
     __shared__ bool s_last;
@@ -303,15 +329,22 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
     float key = INFINITY;
     int idx = 0x7fffffff;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    // a partial row holds fp64 sums (FFMA kernel) or float-float pairs hi + lo in the same 8 bytes (tensor-core kernel)
+    auto slot = [&](int row) {
+        const double* a = part + static_cast<size_t>(row) * m_stride + m;
+        if (!part_ff) return __ldcg(a);
+        const float2 v = __ldcg(reinterpret_cast<const float2*>(a));
+        return static_cast<double>(v.x) + static_cast<double>(v.y);
+    };
     if (m < M) {
         int r = grp;
         for (; r + 3 * kFinGroups < n_part; r += 4 * kFinGroups) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
+            for (int i = 0; i < 4; ++i) acc[i] += slot(r + i * kFinGroups);
         }
 #pragma unroll
         for (int i = 0; i < 3; ++i)      // the tail: at most three rows, same accumulator per position as above
-            if (r + i * kFinGroups < n_part) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
+            if (r + i * kFinGroups < n_part) acc[i] += slot(r + i * kFinGroups);
     }
     s_grp[grp][col] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
     __syncthreads();
@@ -329,7 +362,11 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         }
     }
     if (sse_out != nullptr) return;
-    if (best_out == nullptr) return;
+    if (run != nullptr) {                          // graph replay: the trace slot comes from the device-side generation count
+        float* base = reinterpret_cast<float*>(__ldcg(reinterpret_cast<unsigned long long*>(&run->best)));
+        best_out = base != nullptr ? base + __ldcg(&run->evals) : nullptr;
+    }
+    if (best_out == nullptr && run == nullptr) return;
     __threadfence();  // F[m] visible device-wide before this block takes its ticket
     auto warp_min = [](float& k, int& i) {
 #pragma unroll
@@ -377,7 +414,8 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         warp_min(key, idx);
         if (threadIdx.x == 0) {
             const float best = __ldcg(F + idx);  // the fitness itself (NaN if every chromosome is NaN: idx = 0)
-            *best_out = best;
+            if (best_out != nullptr) *best_out = best;
+            if (run != nullptr) run->evals = __ldcg(&run->evals) + 1;     // nobody reads it until the next kernel of the chain
             *ticket = 0u;
             if (stop != nullptr) {
                 stop[1] = gen_index;                       // GA steps performed so far

@@ -39,7 +39,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_run = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -63,7 +63,18 @@ struct game_ctx {
     int num_sms = 0;
     int device = -1;                                 // ordinal of the device the bound buffers live on (-1: unknown, use the current one)
     unsigned long long launches = 0;
+    int last_umma_grid = 0;                          // CTAs of the last tensor-core fitness launch (game_mma_stall)
     bool timing = false;
+    game::RunState* run = nullptr;                   // device run state, non-null only inside a graph-replayed generation loop
+    // generation loop as a CUDA graph (run_generations): kGraphGens generations captured once, replayed
+    cudaGraphExec_t graph_exec = nullptr;
+    unsigned long long graph_epoch = ~0ull;          // config_epoch the graph was captured under
+    int graph_cur = -1;                              // population buffer that was current at capture
+    unsigned long long graph_nodes = 0;              // kernel launches per replay
+    unsigned long long graph_replays = 0;            // graph launches so far (game_graph_replays)
+    bool graph_ok = true;                            // false after a failed capture: plain launches from then on
+    unsigned long long config_epoch = 0;             // bumped by every call that changes what a generation launches
+    bool use_graph = true;                           // GAME_GRAPH=0 turns the graph path off (A/B measurements)
     int* stop = nullptr;                             // device stop state, non-null only inside game_run_until
     float stop_threshold = 0.f;
     int stop_gen_index = 0;
@@ -144,8 +155,7 @@ int ensure_device(game_ctx* c) {
     using namespace game;
     GAME_CUDA(cudaFuncSetAttribute(fitness_ffma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kFfmaMaxG * kFfmaTile * 4));
     GAME_CUDA(cudaFuncSetAttribute(predict_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kPredictMaxSmem)));
-    GAME_CUDA(cudaFuncSetAttribute(umma::calibrate_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kCalMaxSmem)));
-    GAME_CUDA(cudaFuncSetAttribute(umma::calibrate_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kCalMaxSmem)));
+    GAME_CUDA(cudaFuncSetAttribute(umma::calibrate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kCalMaxSmem)));
 #define GAME_SET_SMEM(E, A) \
     GAME_CUDA(cudaFuncSetAttribute(umma::fitness_umma_kernel<E, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, umma::kSmemBytes))
     GAME_SET_SMEM(0, 0); GAME_SET_SMEM(0, 1); GAME_SET_SMEM(0, 2);
@@ -248,6 +258,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         const long long units = static_cast<long long>(p_tiles_all) * prm.m_groups;
         const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);   // the same grid for every range
         n_part = 2 * grid;
+        c->last_umma_grid = grid;
         // pattern ranges: one launch, or (host knowledge base >= 64 MB) 8 ranges pipelined against their H2D copies
         const size_t kb_bytes = sizeof(float) * static_cast<size_t>(c->P) * (c->N + 1);
         const int n_ranges = (hk != nullptr && kb_bytes >= (64u << 20) && p_tiles_all >= 64) ? 8 : 1;
@@ -293,7 +304,7 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
                 GAME_CUDA(cudaEventRecord(c->copy_events[k], c->copy_stream));
                 GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[k], 0));
             }
-            if (first_launch && c->calibrate && c->act != GAME_ACT_SIGMOID) {
+            if (first_launch && c->calibrate && c->act != GAME_ACT_SIGMOID && sizeof(double) * (static_cast<size_t>(c->G) + umma::kCalUnroll) <= kCalMaxSmem) {
                 // regression activations: measure every row's accumulation shrink on the first pattern tile (calibrate_kernel)
                 float* zdump = reinterpret_cast<float*>(c->ws + c->off_zdump);
                 float* zcorr = reinterpret_cast<float*>(c->ws + c->off_zcorr);
@@ -312,16 +323,19 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
                 }
 #undef GAME_LAUNCH_CAL
                 if ((rc = check_launch(c, "fitness_umma_kernel (calibration)"))) return rc;
-                const size_t w_bytes = sizeof(float) * static_cast<size_t>(c->G);
-                const int stage_w = w_bytes <= kCalMaxSmem ? 1 : 0;
+                double* phi_s = reinterpret_cast<double*>(c->ws + c->off_calphi);
                 if (c->expansion == GAME_EXP_CHEBYSHEV)
-                    launch_chain(c->pdl && hk == nullptr, umma::calibrate_kernel<0>, dim3(c->m_stride), dim3(umma::kCalThreads),
-                                 stage_w ? w_bytes : 0, c->stream, c->X, W, zdump, wscale, zcorr, c->stop, c->P, c->N, c->d, c->M, c->G,
-                                 c->shared, stage_w);
+                    launch_chain(c->pdl && hk == nullptr, umma::cal_phi_kernel<0>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, c->X,
+                                 phi_s, c->stop, c->P, c->N, c->d, c->shared);
                 else
-                    launch_chain(c->pdl && hk == nullptr, umma::calibrate_kernel<1>, dim3(c->m_stride), dim3(umma::kCalThreads),
-                                 stage_w ? w_bytes : 0, c->stream, c->X, W, zdump, wscale, zcorr, c->stop, c->P, c->N, c->d, c->M, c->G,
-                                 c->shared, stage_w);
+                    launch_chain(c->pdl && hk == nullptr, umma::cal_phi_kernel<1>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, c->X,
+                                 phi_s, c->stop, c->P, c->N, c->d, c->shared);
+                if ((rc = check_launch(c, "cal_phi_kernel"))) return rc;
+                const size_t row_bytes = sizeof(double) * ((static_cast<size_t>(c->G - 1) + umma::kCalUnroll - 1) / umma::kCalUnroll * umma::kCalUnroll);
+                int rows = static_cast<int>(kCalMaxSmem / (row_bytes ? row_bytes : 1));
+                rows = rows > umma::kCalRows ? umma::kCalRows : (rows < 1 ? 1 : rows);
+                launch_chain(c->pdl && hk == nullptr, umma::calibrate_kernel, dim3((c->m_stride + rows - 1) / rows), dim3(umma::kCalThreads),
+                             rows * row_bytes, c->stream, W, phi_s, zdump, wscale, zcorr, c->stop, c->P, c->M, c->G, c->m_stride, rows);
                 if ((rc = check_launch(c, "calibrate_kernel"))) return rc;
                 prm.wscale = zcorr;
                 if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));      // the roofline figure times the evaluation proper
@@ -371,7 +385,8 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
     launch_chain(c->pdl, finalize_fitness_kernel, dim3(fin_blocks), dim3(kFinThreads), 0, c->stream,
         part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index, c->rmse);
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index, c->rmse,
+        sse_out == nullptr ? c->run : static_cast<RunState*>(nullptr), scheme == GAME_SCHEME_F16X3 ? 1 : 0);
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
     c->fitness_valid = sse_out == nullptr;
     return GAME_OK;
@@ -404,11 +419,102 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     launch_chain(c->pdl, ga_step_kernel, dim3(c->M), dim3(kGaThreads), 0, c->stream,
                  c->pop[c->cur], c->fitness, c->pop[c->cur ^ 1], p, c->stop,
                  c->img_valid ? c->ws + c->off_img : static_cast<uint8_t*>(nullptr), reinterpret_cast<float*>(c->ws + c->off_wscale),
-                 c->steps);
+                 c->steps, static_cast<const RunState*>(c->run));
     if ((rc = check_launch(c, "ga_step_kernel"))) return rc;
     c->cur ^= 1;
     c->fitness_valid = false;
     return GAME_OK;
+}
+
+// n x (eval, step) [+ a final eval] on the device-resident run state.  Generations are replayed from a CUDA graph of
+// kGraphGens generations (the launch chain captured once, programmatic-dependent-launch edges included), so that the host
+// issues one graph launch per 16 generations instead of three or more kernel launches per generation; what does not fill
+// a graph, and everything when the graph path is off or unavailable, goes out as plain launches on the same run state.
+constexpr uint32_t kGraphGens = 16;
+
+int plain_generation(game_ctx* c) {
+    int rc = eval_internal(c, nullptr);
+    if (rc) return rc;
+    return step_internal(c, 0, 0);      // seed and generation index come from the device run state
+}
+
+int ensure_graph(game_ctx* c) {
+    if (c->graph_exec && c->graph_epoch == c->config_epoch && c->graph_cur == c->cur) return GAME_OK;
+    if (c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+    const unsigned long long launches0 = c->launches;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        c->graph_ok = false;
+        return GAME_OK;
+    }
+    int rc = GAME_OK;
+    for (uint32_t i = 0; i < kGraphGens && rc == GAME_OK; ++i) rc = plain_generation(c);
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    c->graph_nodes = c->launches - launches0;
+    c->launches = launches0;                      // nothing has run yet
+    if (rc != GAME_OK || e != cudaSuccess || graph == nullptr) {
+        cudaGetLastError();
+        if (graph) cudaGraphDestroy(graph);
+        c->graph_ok = false;
+        return rc != GAME_OK ? rc : GAME_OK;
+    }
+    const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) {
+        cudaGetLastError();
+        c->graph_exec = nullptr;
+        c->graph_ok = false;
+        return GAME_OK;
+    }
+    c->graph_epoch = c->config_epoch;
+    c->graph_cur = c->cur;                        // kGraphGens is even: the capture leaves c->cur where it was
+    return GAME_OK;
+}
+
+int run_generations(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_dev, bool final_eval) {
+    using namespace game;
+    if (!c->X || !c->t) return fail(c, GAME_ERR_BAD_STATE, "generation loop before game_load_kb");
+    if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "generation loop before game_bind_state");
+    DeviceGuard guard(c->device);
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    RunState* run = reinterpret_cast<RunState*>(c->ws + c->off_run);
+    set_run_state_kernel<<<1, 1, 0, c->stream>>>(run, make_key(seed), gen0, best_dev);
+    if ((rc = check_launch(c, "set_run_state_kernel"))) return rc;
+    c->run = run;
+    if (!c->ticket_zeroed) {
+        GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
+        c->ticket_zeroed = true;
+    }
+    uint32_t done = 0;
+    const bool graphable = c->use_graph && c->graph_ok && !c->timing && c->stop == nullptr && n_gens >= kGraphGens;
+    if (graphable) {
+        // the graph holds no image pass: bring the W operand images up to date first (one plain generation does)
+        if (resolved_scheme(c) == GAME_SCHEME_F16X3 && !c->img_valid) {
+            rc = plain_generation(c);
+            done = 1;
+        }
+        // a plain generation flips the population buffer; the graph is captured for whichever one is current now
+        if (rc == GAME_OK) rc = ensure_graph(c);
+        while (rc == GAME_OK && c->graph_exec != nullptr && n_gens - done >= kGraphGens) {
+            if (cudaGraphLaunch(c->graph_exec, c->stream) != cudaSuccess) {
+                rc = cuda_fail(c, cudaGetLastError(), "cudaGraphLaunch");
+                break;
+            }
+            c->launches += c->graph_nodes;
+            c->graph_replays += 1;
+            done += kGraphGens;
+            c->fitness_valid = false;               // as after the last captured GA step
+        }
+    }
+    for (; rc == GAME_OK && done < n_gens; ++done) rc = plain_generation(c);
+    if (rc == GAME_OK && final_eval) rc = eval_internal(c, nullptr);
+    c->run = nullptr;
+    return rc;
 }
 
 }  // namespace
@@ -440,6 +546,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->umma_ok = umma_ok;
     if (const char* e = std::getenv("GAME_PDL")) c->pdl = e[0] != '0';   // A/B switch for measurements; default on
     if (const char* e = std::getenv("GAME_CALIBRATE")) c->calibrate = e[0] != '0';   // A/B switch; default on
+    if (const char* e = std::getenv("GAME_GRAPH")) c->use_graph = e[0] != '0';       // A/B switch; default on
     c->steps = static_cast<int>((G - 1 + 15) / 16);   // K steps of 16 genes; the bias gene is not part of the contraction
     size_t off = 0;
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
@@ -449,15 +556,18 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_zcorr = off; off = align_up(off + sizeof(float) * static_cast<size_t>(c->m_stride));
     c->off_zdump = off;       // calibration samples (regression activations on the tensor-core scheme only)
     if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(float) * static_cast<size_t>(c->m_stride) * game::umma::kBN);
+    c->off_calphi = off;      // fp64 phi of the sample patterns
+    if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(double) * static_cast<size_t>(G) * game::umma::kBN);
     const size_t fin_blocks = (static_cast<size_t>(M) + game::kFinCols - 1) / game::kFinCols;
     c->off_blk_key = off; off = align_up(off + fin_blocks * sizeof(float));
     c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
     c->off_ticket = off; off = align_up(off + sizeof(unsigned int));
-    c->off_stall = off; off = align_up(off + sizeof(long long) * 4 * kMaxCtas);
+    c->off_stall = off; off = align_up(off + sizeof(long long) * game::umma::kStallSlots * kMaxCtas);
     c->off_stop = off; off = align_up(off + 2 * sizeof(int));
     c->off_by_rank = off; off = align_up(off + sizeof(int) * static_cast<size_t>(M));
     c->off_prefix = off; off = align_up(off + sizeof(unsigned long long) * static_cast<size_t>(M));
     c->off_fused_bar = off; off = align_up(off + sizeof(unsigned int));
+    c->off_run = off; off = align_up(off + sizeof(game::RunState));
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
@@ -469,6 +579,7 @@ int game_destroy(game_ctx* c) {
         cudaEventDestroy(ev.first);
         cudaEventDestroy(ev.second);
     }
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     for (auto& e : c->copy_events) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
@@ -489,6 +600,7 @@ int game_workspace_bytes(const game_ctx* c, size_t* bytes) {
 
 int game_set_stream(game_ctx* c, void* cuda_stream) {
     if (!c) return GAME_ERR_INVALID_ARG;
+    c->config_epoch += 1;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     return GAME_OK;
 }
@@ -500,6 +612,7 @@ int game_set_scheme(game_ctx* c, int32_t scheme) {
         return fail(c, GAME_ERR_UNSUPPORTED, "F16X3 covers trigonometric degrees d <= 128 and, with shared coefficients, G - 1 <= 64");
     if (scheme == GAME_SCHEME_FFMA && c->G > game::kFfmaMaxG)
         return fail(c, GAME_ERR_UNSUPPORTED, "FFMA covers G <= 448");
+    c->config_epoch += 1;
     c->scheme = scheme;
     return GAME_OK;
 }
@@ -514,6 +627,7 @@ int game_load_kb(game_ctx* c, const float* X_dev, const float* t_dev) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!X_dev || !t_dev) return fail(c, GAME_ERR_INVALID_ARG, "null knowledge-base pointer");
     if (!aligned16(X_dev) || !aligned16(t_dev)) return fail(c, GAME_ERR_INVALID_ARG, "knowledge-base pointers must be 16-byte aligned");
+    c->config_epoch += 1;
     c->X = X_dev;
     c->t = t_dev;
     c->fitness_valid = false;
@@ -531,6 +645,7 @@ int game_bind_state(game_ctx* c, float* popA_dev, float* popB_dev, float* fitnes
         return fail(c, GAME_ERR_INVALID_ARG, "state pointers must be 16-byte aligned (workspace: 256)");
     if (workspace_bytes < c->ws_bytes)
         return fail(c, GAME_ERR_WORKSPACE, "workspace has %zu bytes, game_workspace_bytes says %zu", workspace_bytes, c->ws_bytes);
+    c->config_epoch += 1;
     c->pop[0] = popA_dev;
     c->pop[1] = popB_dev;
     c->fitness = fitness_dev;
@@ -553,6 +668,7 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
     if (!(p_cross >= 0.0 && p_cross <= 1.0) || !(p_mut >= 0.0 && p_mut <= 1.0))
         return fail(c, GAME_ERR_INVALID_ARG, "probabilities must be in [0, 1]");
     if (!(sigma >= 0.0f) || !std::isfinite(sigma)) return fail(c, GAME_ERR_INVALID_ARG, "sigma must be finite and >= 0");
+    c->config_epoch += 1;
     c->elite = elite; c->tournament = tournament;
     c->p_cross = p_cross; c->p_mut = p_mut; c->sigma = sigma;
     return GAME_OK;
@@ -561,6 +677,7 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
 int game_set_error_metric(game_ctx* c, int32_t metric) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (metric != GAME_ERROR_MSE && metric != GAME_ERROR_RMSE) return fail(c, GAME_ERR_INVALID_ARG, "unknown error metric %d", metric);
+    c->config_epoch += 1;
     c->rmse = metric == GAME_ERROR_RMSE ? 1 : 0;
     c->fitness_valid = false;
     return GAME_OK;
@@ -570,6 +687,7 @@ int game_set_immigrants(game_ctx* c, int32_t immigrants) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (immigrants < 0 || immigrants > c->M - c->elite)
         return fail(c, GAME_ERR_INVALID_ARG, "immigrants must be in [0, M - elite]");
+    c->config_epoch += 1;
     c->immigrants = immigrants;
     return GAME_OK;
 }
@@ -577,6 +695,7 @@ int game_set_immigrants(game_ctx* c, int32_t immigrants) {
 int game_set_selection(game_ctx* c, int32_t selection) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (selection < GAME_SEL_TOURNAMENT || selection > GAME_SEL_ROULETTE) return fail(c, GAME_ERR_INVALID_ARG, "unknown selection %d", selection);
+    c->config_epoch += 1;
     c->selection = selection;
     return GAME_OK;
 }
@@ -629,14 +748,7 @@ int game_step(game_ctx* c, uint64_t seed, uint32_t gen) {
 
 int game_run(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev) {
     if (!c) return GAME_ERR_INVALID_ARG;
-    for (uint32_t i = 0; i <= n_gens; ++i) {
-        int rc = eval_internal(c, best_fitness_dev ? best_fitness_dev + i : nullptr);
-        if (rc) return rc;
-        if (i == n_gens) break;
-        rc = step_internal(c, seed, gen0 + i);
-        if (rc) return rc;
-    }
-    return GAME_OK;
+    return run_generations(c, seed, gen0, n_gens, best_fitness_dev, true);
 }
 
 int game_run_until(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t max_gens, float threshold, float* best_fitness_dev,
@@ -722,13 +834,7 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
 
 int game_evolve(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens) {
     if (!c) return GAME_ERR_INVALID_ARG;
-    for (uint32_t i = 0; i < n_gens; ++i) {
-        int rc = eval_internal(c, nullptr);
-        if (rc) return rc;
-        rc = step_internal(c, seed, gen0 + i);
-        if (rc) return rc;
-    }
-    return GAME_OK;
+    return run_generations(c, seed, gen0, n_gens, nullptr, false);
 }
 
 int game_sync(game_ctx* c) {
@@ -784,7 +890,7 @@ int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_tota
     game::finalize_fitness_kernel<<<fin_blocks, game::kFinThreads, 0, c->stream>>>(
         sse_dev, 1, c->M, c->M, static_cast<double>(P_total), c->fitness, nullptr, best_fitness_dev,
         reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), nullptr, 0.f, 0, c->rmse);
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), nullptr, 0.f, 0, c->rmse, static_cast<game::RunState*>(nullptr), 0);
     if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
     c->fitness_valid = true;
     return GAME_OK;
@@ -822,6 +928,32 @@ int game_confusion(game_ctx* c, const float* y_dev, const float* t_dev, int64_t 
 int game_launch_count(const game_ctx* c, uint64_t* launches) {
     if (!c || !launches) return GAME_ERR_INVALID_ARG;
     *launches = c->launches;
+    return GAME_OK;
+}
+
+int game_mma_stall(game_ctx* c, double* frac_a_full, double* frac_b_full, double* frac_acc_empty, int64_t* raw_host, int32_t raw_slots) {
+    if (!c || !frac_a_full || !frac_b_full || !frac_acc_empty) return GAME_ERR_INVALID_ARG;
+    if (!c->ws || c->last_umma_grid <= 0) return fail(c, GAME_ERR_BAD_STATE, "game_mma_stall: no tensor-core fitness launch yet");
+    DeviceGuard guard(c->device);
+    GAME_CUDA(cudaStreamSynchronize(c->stream));
+    std::vector<long long> h(static_cast<size_t>(c->last_umma_grid) * game::umma::kStallSlots);
+    GAME_CUDA(cudaMemcpy(h.data(), c->ws + c->off_stall, h.size() * sizeof(long long), cudaMemcpyDeviceToHost));
+    double a = 0, b = 0, e = 0, t = 0;
+    for (int cta = 0; cta < c->last_umma_grid; cta += 2) {      // leader CTAs issue the MMAs
+        const long long* r = h.data() + static_cast<size_t>(cta) * game::umma::kStallSlots;
+        a += r[0]; b += r[1]; e += r[2]; t += r[3];
+    }
+    *frac_a_full = t > 0 ? a / t : 0.0;
+    *frac_b_full = t > 0 ? b / t : 0.0;
+    *frac_acc_empty = t > 0 ? e / t : 0.0;
+    if (raw_host != nullptr)
+        for (size_t i = 0; i < h.size() && i < static_cast<size_t>(raw_slots > 0 ? raw_slots : 0); ++i) raw_host[i] = h[i];
+    return GAME_OK;
+}
+
+int game_graph_replays(const game_ctx* c, uint64_t* replays) {
+    if (!c || !replays) return GAME_ERR_INVALID_ARG;
+    *replays = c->graph_replays;
     return GAME_OK;
 }
 

@@ -146,8 +146,9 @@ def test_fitness_is_deterministic_and_schemes_agree(game):
     assert np.max(np.abs(out[1] - out[2]) / out[1]) < 2e-6
 
 
-def test_nan_and_inf_propagate(game):
-    cfg = wl.scaled(wl.CONFIGS["c0"], P=600, M=20)
+@pytest.mark.parametrize("P", [600, 512])       # a ragged last tile, and whole tiles only (the packed epilogue path alone)
+def test_nan_and_inf_propagate(game, P):
+    cfg = wl.scaled(wl.CONFIGS["c0"], P=P, M=20)
     X, t, _ = wl.make_kb(cfg)
     W = wl.uniform_population(cfg.M, cfg.G, 3)
     W[4, 2] = np.nan
@@ -583,7 +584,7 @@ def test_step_keeps_w_images(game, base, over, selection, immigrants):
     for gen in range(4):
         n0 = G.launch_count()
         G.eval_fitness(); G.sync()
-        cal = 2 if cfg.activation != wl.ACT_SIGMOID else 0        # regression activations: calibration launch + calibrate_kernel
+        cal = 3 if cfg.activation != wl.ACT_SIGMOID else 0        # regression activations: calibration launch, cal_phi_kernel, calibrate_kernel
         assert G.launch_count() - n0 == (4 if gen == 0 else 2) + cal   # row scales + image pass only before the first generation
         F = G.get_fitness()
         W = G.get_population()
@@ -600,24 +601,26 @@ def test_dependent_launch_chain_is_race_free(game, base, over, scheme, selection
     """The generation's kernels run under programmatic dependent launch (csrc/pdl.cuh): each one is launched while its
     predecessor still runs and parks in griddepcontrol.wait.  A missing or misplaced wait would let a kernel read what its
     predecessor has not written yet, so 40 generations enqueued back to back must give the same populations, fitness
-    vectors and best-fitness trace, bit for bit, as the same run with plain stream-ordered launches (GAME_PDL=0)."""
+    vectors and best-fitness trace, bit for bit, as the same run with plain stream-ordered launches (GAME_PDL=0).  The same
+    holds for the loop replayed from a CUDA graph of 16 generations (GAME_GRAPH, the default; seed and generation index in
+    device memory): 40 = 2 replays + 8 plain generations + the final evaluation."""
     import torch
     cfg = wl.scaled(wl.CONFIGS[base], **over)
     X, t, _ = wl.make_kb(cfg)
     n = 40
     out = []
-    for pdl in ("0", "1", "1"):
+    for pdl, graph in (("0", "0"), ("1", "0"), ("1", "1"), ("0", "1")):      # plain launches / PDL chain / both replayed from a CUDA graph
         monkeypatch.setenv("GAME_PDL", pdl)                 # read by game_create
+        monkeypatch.setenv("GAME_GRAPH", graph)
         G = make(game, cfg, scheme); G.load_kb(X, t)
         game.game_set_selection(G.ctx, selection); game.game_set_immigrants(G.ctx, 2)
         best = torch.zeros(n + 1, dtype=torch.float32, device="cuda")
         G.init_population(17); G.run(17, 0, n, best); G.sync()
         out.append((G.get_population().view(np.uint32), G.get_fitness().view(np.uint32), best.cpu().numpy().view(np.uint32)))
         G.close()
-    for a, b in zip(out[0], out[1]):
-        assert np.array_equal(a, b)
-    for a, b in zip(out[1], out[2]):
-        assert np.array_equal(a, b)
+    for other in out[1:]:
+        for a, b in zip(out[0], other):
+            assert np.array_equal(a, b)
 
 
 # ------------------------------------------------------------------------------------------------ fused persistent loop
