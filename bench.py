@@ -68,7 +68,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS) + ["c4", "n1", "n1s"])
+    ap.add_argument("--workload", default="c3", choices=sorted(wl.CONFIGS) + ["c4", "n1", "n1s", "n1grid"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="auto", choices=["auto", "ffma", "f16x3"])
     ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
@@ -363,7 +363,10 @@ def run_ours(args, cfg, rank, world, local_rank):
         torch.cuda.synchronize()
 
     shard = dist is not None and args.multi == "shard"
-    sse = torch.zeros(cfg.M, dtype=torch.float64, device=dev) if shard else None
+    if shard:
+        ident = [game.game_comm_unique_id() if rank == 0 else None]
+        dist.broadcast_object_list(ident, src=0)
+        game.game_comm_init(G.ctx, ident[0], rank, world)
 
     def generations(first_gen, n):
         if args.fused:
@@ -372,11 +375,9 @@ def run_ours(args, cfg, rank, world, local_rank):
         if not shard:
             game.game_evolve(G.ctx, seed, first_gen, n)      # n x (fused fitness eval, GA step): launches only
             return
-        for i in range(n):                                   # one population, patterns sharded over the ranks
-            game.game_eval_sse(G.ctx, sse.data_ptr())
-            dist.all_reduce(sse, op=dist.ReduceOp.SUM)       # M doubles per generation over NVLink
-            game.game_set_fitness_from_sse(G.ctx, sse.data_ptr(), cfg.P * world, None)
-            game.game_step(G.ctx, seed, first_gen + i)
+        # one population, patterns sharded over the ranks: the whole loop runs inside the library -- per generation the
+        # evaluation kernels, ONE ncclAllReduce of M doubles on the library's stream, finalisation, GA step; no Python
+        game.game_evolve_sharded(G.ctx, seed, first_gen, n, cfg.P * world, None)
 
     # ---------------- device-resident leg: NO instrumentation inside the timed region (the generation loop is replayed from
     # a CUDA graph / runs under programmatic dependent launch; per-kernel events would sit inside the chain they overlap)
@@ -438,6 +439,36 @@ def run_ours(args, cfg, rank, world, local_rank):
                "d2h_bytes_per_step": 4 * (cfg.M + cfg.M * cfg.G) * world, "ms_per_step": ms_e2e / args.steps,
                "api": "game_generation_host (pinned host buffers; H2D X,t,W + eval + step + D2H F,W' per step)"}
 
+    # ---------------- out-of-core leg: the same evaluation with the knowledge base in pinned
+    # host memory and only a 64 MB ring of device buffers, game_eval_fitness_streamed
+    out_of_core = None
+    if not args.no_e2e and world == 1 and cfg.name == "c3" and G.scheme() == game.SCHEME_F16X3:
+        n_slots = 3
+        quantum = 256 * 74
+        slot_rows = max(quantum, (64 << 20) // (4 * (cfg.N + 1)) // n_slots // quantum * quantum)
+        Xr = torch.empty((n_slots * slot_rows, cfg.N), dtype=torch.float32, device=dev)
+        tr = torch.empty((n_slots * slot_rows,), dtype=torch.float32, device=dev)
+        F_res = None
+        game.game_eval_fitness(G.ctx); G.sync(); F_res = G.get_fitness()
+
+        def streamed(n):
+            for _ in range(n):
+                game.game_eval_fitness_streamed(G.ctx, Xh.data_ptr(), th.data_ptr(), Xr.data_ptr(), tr.data_ptr(), slot_rows, n_slots)
+        streamed(2)
+        barrier()
+        n_ev = max(3, min(args.steps, 10))
+        e0.record()
+        streamed(n_ev)
+        e1.record()
+        barrier()
+        ms_oc = e0.elapsed_time(e1) / n_ev
+        out_of_core = {"api": "game_eval_fitness_streamed (fitness evaluation only; knowledge base in pinned host memory)",
+                       "ring_bytes": int(Xr.numel() * 4 + tr.numel() * 4), "slots": n_slots, "slot_rows": int(slot_rows),
+                       "kb_bytes": 4 * cfg.P * (cfg.N + 1), "ms_per_eval": ms_oc, "evals_per_s": cfg.P * cfg.M / (ms_oc * 1e-3),
+                       "h2d_gb_per_s": 4 * cfg.P * (cfg.N + 1) / (ms_oc * 1e-3) / 1e9,
+                       "bit_identical_to_resident": bool(np.array_equal(G.get_fitness().view(np.uint32), F_res.view(np.uint32)))}
+        del Xr, tr
+
     if rank != 0:
         G.close()
         if dist is not None:
@@ -469,6 +500,8 @@ def run_ours(args, cfg, rank, world, local_rank):
             "config": config_dict(cfg, scheme_name, world), "generations_per_s": args.steps / (ms * 1e-3),
             "e2e": e2e, "gpu_launches": int(launches), "graph_replays": int(game.game_graph_replays(G.ctx)),
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+    if out_of_core is not None:
+        line["out_of_core"] = out_of_core
     G.close()
     # ---------------- the other BASELINE.json configurations, same process, same box (default c3 line, one GPU only)
     if world == 1 and cfg.name == "c3" and not args.no_sweep and not args.fused:
@@ -518,6 +551,53 @@ def run_c4_sweep(args):
     print(json.dumps(line), flush=True)
 
 
+def run_n1_grid(args):
+    """the paper's own experiment grid as generations/s -- P = 2100 synthetic patterns,
+    N in {7, 9} feature columns, polytrigo degree in {1, 2, 4, 8}, RANKING and ROULETTE selection,
+    crossover 0.9, mutation 0.2, elitism 2, B N + 1 chromosomes (B = 2), per-feature coefficients (BASELINE.json's form) and
+    the paper's shared coefficients; both execution paths: the launch chain replayed from a CUDA graph (game_evolve) and the
+    persistent whole-GA kernel (game_evolve_fused)."""
+    import torch
+    import paper_1211_5481_b200 as game
+    from paper_1211_5481_b200 import build as game_build
+    from dataclasses import replace
+
+    game_build.build()
+    rows = []
+    steps, warmup = max(args.steps, 2000), 200
+    for N in (7, 9):
+        for d in (1, 2, 4, 8):
+            for shared in (False, True):
+                cfg = replace(wl.PAPER_SHAPE, name="n1grid", N=N, d=d, M=2 * N + 1, shared=shared, w_star_std=0.1 if shared else 0.3)
+                X, t, _ = wl.make_kb(cfg)
+                for sel_name, sel in (("ranking", game.SEL_RANKING), ("roulette", game.SEL_ROULETTE)):
+                    G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation, shared=shared)
+                    G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+                    game.game_set_selection(G.ctx, sel)
+                    G.load_kb(X, t)
+                    res = {}
+                    for path in ("graph", "fused"):
+                        G.init_population(cfg.seed)
+                        fn = (lambda g0, n: game.game_evolve(G.ctx, cfg.seed, g0, n)) if path == "graph" else \
+                             (lambda g0, n: game.game_evolve_fused(G.ctx, cfg.seed, g0, n, None))
+                        fn(0, warmup)
+                        torch.cuda.synchronize()
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record(); fn(warmup, steps); e1.record()
+                        torch.cuda.synchronize()
+                        res[path] = steps / (e0.elapsed_time(e1) * 1e-3)
+                    rows.append({"N": N, "degree": d, "G": cfg.G, "M": cfg.M, "coefficients": "shared" if shared else "per-feature",
+                                 "selection": sel_name, "generations_per_s_graph": res["graph"], "generations_per_s_fused": res["fused"],
+                                 "us_per_40000_iterations_fused": 40000 / res["fused"] * 1e6})
+                    G.close()
+    best = max(r["generations_per_s_fused"] for r in rows)
+    line = {"metric": "generations_per_s", "value": best, "unit": "generations/s", "n_gpus": 1, "steps": steps, "warmup": warmup,
+            "ms_per_step": 1e3 / best, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": {"workload": "n1grid: the paper's experiment grid (PAPER.md:128-136), synthetic stand-in, P = 2100"},
+            "e2e": None, "gpu_launches": None, "grid": rows, "roofline": None, "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -534,6 +614,10 @@ def main():
     if args.workload == "c4":
         if int(os.environ.get("RANK", "0")) == 0:
             run_c4_sweep(args)
+        return
+    if args.workload == "n1grid":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_n1_grid(args)
         return
     cfg = {"n1": wl.PAPER_SHAPE, "n1s": wl.PAPER_SHAPE_SHARED}.get(args.workload) or wl.CONFIGS[args.workload]
     if args.impl == "reference":

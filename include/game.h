@@ -135,8 +135,14 @@ int game_set_selection(game_ctx* ctx, int32_t selection);
 
 /* Error metric written to fitness_dev ("the MSE or the RMSE may be used"): MSE (default) or
  * RMSE = sqrt(MSE), taken in fp64 before the single rounding to fp32.  Lower is better either way (the GA order is the
- * same); the threshold of game_run_until is compared against the chosen metric.  Invalidates the fitness. */
-enum { GAME_ERROR_MSE = 0, GAME_ERROR_RMSE = 1 };
+ * same); the threshold of game_run_until is compared against the chosen metric.
+ * GAME_ERROR_ONE_MINUS_MSE is the paper's literal fitness ("the fitness is calculated as the complement of the
+ * error (i.e. 1-error)"): fitness_dev[m] = float(1 - MSE), HIGHER is better and the best-fitness trace holds maxima.  The
+ * GA operators then work on the error e = 1 - fitness_dev (one fp32 subtraction): elitism, tournaments, ranking and the
+ * roulette weights (which are floor(clamp(1 - e, 0, 1) 2^32), i.e. the fitness itself) are the functions of an error vector
+ * documented above, and the threshold of game_run_until is still a learning-ERROR threshold (stop when 1 - best <= it).
+ * Invalidates the fitness. */
+enum { GAME_ERROR_MSE = 0, GAME_ERROR_RMSE = 1, GAME_ERROR_ONE_MINUS_MSE = 2 };
 int game_set_error_metric(game_ctx* ctx, int32_t metric);
 
 /* Random replacement ("a variable number of chromosomes are randomly generated to replace older
@@ -221,6 +227,21 @@ int game_sync(game_ctx* ctx);
 int game_generation_host(game_ctx* ctx, const float* X_host, const float* t_host, const float* W_host,
                          float* F_host, float* W_next_host, uint64_t seed, uint32_t gen);
 
+/* OUT-OF-CORE evaluation ("the dataset can be very large ... requires greater attention to GPU memory
+ * management, in terms of scheduling and data transfers host-to-device"): the knowledge base stays in HOST memory
+ * (X_host[P][N], t_host[P], P as given to game_create -- it may exceed device memory; pinned memory for full bandwidth) and
+ * passes through a ring of n_slots (2..8) device buffers of slot_rows patterns each: X_ring_dev[n_slots * slot_rows][N],
+ * t_ring_dev[n_slots * slot_rows] (caller-owned, 16-byte aligned, slot_rows a multiple of 256).  One plain asynchronous
+ * copy per pattern range on a library-owned copy stream, n_slots - 1 ranges ahead of the fused fitness kernel, which is
+ * launched once per range and carries its partial sums across the launches; fitness_dev is then the fitness of the current
+ * population over all P patterns, marked valid (game_step may follow).  A slot is used in whole rounds of the kernel's
+ * persistent grid, so every pattern tile is evaluated by the same CTA pair in the same order as in a resident
+ * game_eval_fitness: the result is BIT-IDENTICAL to it.  Needs game_bind_state, not game_load_kb.  Tensor-core scheme
+ * only (GAME_ERR_UNSUPPORTED otherwise); slots too small for one round of the grid -> GAME_ERR_INVALID_ARG (the message
+ * says how many patterns a slot needs).  Async. */
+int game_eval_fitness_streamed(game_ctx* ctx, const float* X_host, const float* t_host, float* X_ring_dev, float* t_ring_dev,
+                               int64_t slot_rows, int32_t n_slots);
+
 /* Pattern-sharded evaluation (PAPER.md:172 future work (iii) multi-GPU; "massive data sets"): each
  * rank binds ITS shard of the knowledge base (P = shard size) and the same population.  game_eval_sse writes the
  * un-normalised sums sse_dev[m] = sum over this shard of (act(z) - t)^2 (device, fp64 [M]) instead of a fitness; the caller
@@ -230,6 +251,18 @@ int game_generation_host(game_ctx* ctx, const float* X_host, const float* t_host
  * give identical populations on all ranks, no broadcast.  Async. */
 int game_eval_sse(game_ctx* ctx, double* sse_dev);
 int game_set_fitness_from_sse(game_ctx* ctx, const double* sse_dev, int64_t P_total, float* best_fitness_dev);
+
+/* The pattern-sharded GENERATION LOOP with the exchange inside the library (no host code between generations): every rank
+ * (one process per GPU) has bound its shard and the same population; per generation game_eval_sse's kernels, ONE
+ * ncclAllReduce(sum) of M doubles on the context's stream (NVLink / NVSwitch: 32 KB at M = 4096, latency only), the
+ * finalisation with P_total and the GA step, n_gens times, all enqueued at once.  best_fitness_dev ([n_gens] device, or
+ * NULL) receives the best fitness of every generation (identical on all ranks).  NCCL is loaded at run time
+ * (libnccl.so.2, the copy the process already has); game_comm_unique_id fills a 128-byte id on ONE rank, which the caller
+ * passes to all ranks (e.g. torch.distributed broadcast) for game_comm_init(id, rank, world).  GAME_ERR_UNSUPPORTED if NCCL
+ * cannot be loaded; a world of 1 is valid (the all-reduce is then a copy).  Async. */
+int game_comm_unique_id(void* id128_host);
+int game_comm_init(game_ctx* ctx, const void* id128_host, int32_t rank, int32_t world);
+int game_evolve_sharded(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, int64_t P_total, float* best_fitness_dev);
 
 /* Test / validation use case: outputs of ONE chromosome w_dev[G] (device; e.g. a row of the current
  * population) on Q patterns X_dev[Q][N] (device, any Q >= 1, independent of the bound knowledge base):

@@ -17,7 +17,7 @@ EXP_CHEBYSHEV, EXP_TRIG = 0, 1
 ACT_IDENTITY, ACT_SIGMOID, ACT_TANH = 0, 1, 2
 SCHEME_AUTO, SCHEME_FFMA, SCHEME_F16X3 = 0, 1, 2
 SEL_TOURNAMENT, SEL_RANKING, SEL_ROULETTE = 0, 1, 2
-ERROR_MSE, ERROR_RMSE = 0, 1
+ERROR_MSE, ERROR_RMSE, ERROR_ONE_MINUS_MSE = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_WORKSPACE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -51,8 +51,12 @@ SIGNATURES = {
     "game_evolve_fused": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, _F32P]),
     "game_sync": (C.c_int, [_VP]),
     "game_generation_host": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, _F32P, C.c_uint64, C.c_uint32]),
+    "game_eval_fitness_streamed": (C.c_int, [_VP, _F32P, _F32P, _F32P, _F32P, C.c_int64, C.c_int32]),
     "game_eval_sse": (C.c_int, [_VP, _VP]),
     "game_set_fitness_from_sse": (C.c_int, [_VP, _VP, C.c_int64, _F32P]),
+    "game_comm_unique_id": (C.c_int, [_VP]),
+    "game_comm_init": (C.c_int, [_VP, _VP, C.c_int32, C.c_int32]),
+    "game_evolve_sharded": (C.c_int, [_VP, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int64, _F32P]),
     "game_predict": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, _F32P]),
     "game_confusion": (C.c_int, [_VP, _F32P, _F32P, C.c_int64, C.c_float, _VP]),
     "game_launch_count": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
@@ -212,12 +216,33 @@ def game_generation_host(ctx, X_host: int, t_host: int, W_host: int, F_host: int
     _check(ctx, lib().game_generation_host(ctx, X_host, t_host, W_host, F_host, W_next_host, seed, gen))
 
 
+def game_eval_fitness_streamed(ctx, X_host: int, t_host: int, X_ring_dev: int, t_ring_dev: int, slot_rows: int, n_slots: int) -> None:
+    _check(ctx, lib().game_eval_fitness_streamed(ctx, X_host, t_host, X_ring_dev, t_ring_dev, slot_rows, n_slots))
+
+
 def game_eval_sse(ctx, sse_dev: int) -> None:
     _check(ctx, lib().game_eval_sse(ctx, sse_dev))
 
 
 def game_set_fitness_from_sse(ctx, sse_dev: int, P_total: int, best_fitness_dev: int | None = None) -> None:
     _check(ctx, lib().game_set_fitness_from_sse(ctx, sse_dev, P_total, best_fitness_dev))
+
+
+def game_comm_unique_id() -> bytes:
+    buf = C.create_string_buffer(128)
+    rc = lib().game_comm_unique_id(buf)
+    if rc != OK:
+        raise GameError(rc, "game_comm_unique_id: NCCL unavailable")
+    return buf.raw
+
+
+def game_comm_init(ctx, id128: bytes, rank: int, world: int) -> None:
+    buf = C.create_string_buffer(bytes(id128), 128)
+    _check(ctx, lib().game_comm_init(ctx, buf, rank, world))
+
+
+def game_evolve_sharded(ctx, seed: int, gen0: int, n_gens: int, P_total: int, best_fitness_dev: int | None = None) -> None:
+    _check(ctx, lib().game_evolve_sharded(ctx, seed, gen0, n_gens, P_total, best_fitness_dev))
 
 
 def game_predict(ctx, w_dev: int, X_dev: int, Q: int, y_dev: int) -> None:
@@ -272,7 +297,7 @@ class Game:
     """
 
     def __init__(self, P: int, N: int, d: int, M: int, expansion: int, activation: int, device="cuda:0",
-                 scheme: int = SCHEME_AUTO, shared: bool = False):
+                 scheme: int = SCHEME_AUTO, shared: bool = False, resident_kb: bool = True):
         import torch
 
         if not torch.cuda.is_available():
@@ -283,14 +308,17 @@ class Game:
         self.ctx = game_create(P, N, d, M, family(expansion, activation, shared))
         self.G = game_num_genes(self.ctx)
         with torch.cuda.device(self.device):
-            self.X = torch.empty((P, N), dtype=torch.float32, device=self.device)
-            self.t = torch.empty((P,), dtype=torch.float32, device=self.device)
+            # resident_kb = False: the knowledge base stays in host memory (game_eval_fitness_streamed), nothing of size P
+            # is allocated on the device
+            self.X = torch.empty((P, N), dtype=torch.float32, device=self.device) if resident_kb else None
+            self.t = torch.empty((P,), dtype=torch.float32, device=self.device) if resident_kb else None
             self.pop = [torch.zeros((M, self.G), dtype=torch.float32, device=self.device) for _ in range(2)]
             self.fitness = torch.zeros((M,), dtype=torch.float32, device=self.device)
             self.ws_bytes = game_workspace_bytes(self.ctx)
             self.workspace = torch.empty((self.ws_bytes,), dtype=torch.uint8, device=self.device)
             game_set_stream(self.ctx, torch.cuda.current_stream(self.device).cuda_stream)
-        game_load_kb(self.ctx, self.X.data_ptr(), self.t.data_ptr())
+        if resident_kb:
+            game_load_kb(self.ctx, self.X.data_ptr(), self.t.data_ptr())
         game_bind_state(self.ctx, self.pop[0].data_ptr(), self.pop[1].data_ptr(), self.fitness.data_ptr(),
                         self.workspace.data_ptr(), self.ws_bytes)
         if scheme != SCHEME_AUTO:

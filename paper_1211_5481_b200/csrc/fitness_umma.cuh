@@ -1120,12 +1120,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             // x in blocks of 4 features.  Block b of a row; b and the feature indices are clamped into the row, so a
             // load never leaves it (features past N only exist in the zero-padded tail of the K axis, where phi is
             // multiplied by W image zeros: any finite value of the SAME row will do there, and a row that holds a
-            // non-finite value has a non-finite z anyway).  Rows of a pattern past P read row 0 (masked by the epilogue).
+            // non-finite value has a non-finite z anyway).  Rows of a pattern past P read the launch's first row (masked by the
+            // epilogue; with an out-of-core knowledge base only this launch's pattern range is in device memory).
             const float* xrow[kRPT];
 #pragma unroll
             for (int q = 0; q < kRPT; ++q) {
                 const long long p = static_cast<long long>(pt) * kBN + static_cast<long long>(crank) * kRows + r + q * (kRows / kRPT);
-                xrow[q] = prm.X + (p < prm.P ? p : 0) * prm.N;
+                xrow[q] = prm.X + (p < prm.P ? p : static_cast<long long>(prm.p_tile0) * kBN) * prm.N;
             }
             const bool vec4 = (prm.N & 3) == 0;       // rows are 16-byte aligned (X itself is: game_load_kb checks)
             const int last_blk = (prm.N - 1) >> 2, last_i = prm.N - 1;

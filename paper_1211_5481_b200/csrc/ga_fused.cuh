@@ -143,21 +143,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) ga_fused_kernel(const FusedP
 #pragma unroll
                 for (int g = 0; g < 8; ++g) s += s_grp[g][col];
                 const double mse = s / static_cast<double>(prm.P);
-                Fs[m] = static_cast<float>(prm.rmse ? sqrt(mse) : mse);
+                Fs[m] = static_cast<float>(prm.rmse == 1 ? sqrt(mse) : (prm.rmse == 2 ? 1.0 - mse : mse));
             }
             __syncthreads();
         }
         // ranks (chromosome per rank) and roulette prefix sums, in shared memory
         for (int m = tid; m < M; m += kFusedThreads) {
-            const float km = fit_key(Fs[m]);
+            const float km = fit_key(err_view(Fs[m], ga.maximize));
             int r = 0;
-            for (int j = 0; j < M; ++j) r += precedes(fit_key(Fs[j]), j, km, m) ? 1 : 0;
+            for (int j = 0; j < M; ++j) r += precedes(fit_key(err_view(Fs[j], ga.maximize)), j, km, m) ? 1 : 0;
             by_rank[r] = m;
         }
         if (ga.selection == 2 && tid == 0) {
             unsigned long long a = 0;
             for (int m = 0; m < M; ++m) {
-                a += roulette_weight(Fs[m]);
+                a += roulette_weight(err_view(Fs[m], ga.maximize));
                 prefix[m] = a;
             }
         }
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) ga_fused_kernel(const FusedP
                         if ((e & 3) == 0)
                             r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), ga.gen, kTagSelect, ga.key);
                         const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
-                        const float ki = fit_key(Fs[idx]);
+                        const float ki = fit_key(err_view(Fs[idx], ga.maximize));
                         const int side = e < ga.tournament ? 0 : 1;
                         if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
                             par[side] = idx;

@@ -18,6 +18,10 @@ constexpr int kGaThreads = 128;
 // ---- order on chromosomes (R7.1): a precedes b iff key(F[a]) < key(F[b]), ties -> lower index;
 // key(NaN) = +inf (NaN fitness is worst).  Lower fitness (MSE) is better (D4).
 __device__ __forceinline__ float fit_key(float f) { return (f != f) ? INFINITY : f; }
+// The error a fitness value stands for.  MSE / RMSE are errors themselves; under the paper's literal fitness 1 - error,
+// maximised (GAME_ERROR_ONE_MINUS_MSE) the operators work on e = 1 - fitness (one fp32 subtraction, exact for
+// fitness in [1/2, 1]), so that every operator is the SAME function of an error vector whatever is reported.
+__device__ __forceinline__ float err_view(float f, int maximize) { return maximize ? 1.0f - f : f; }
 
 __device__ __forceinline__ bool precedes(float ka, int a, float kb, int b) {
     return (ka < kb) || (ka == kb && a < b);
@@ -66,6 +70,7 @@ struct GaParams {
     PhiloxKey key;
     int immigrants;                       // last R child slots are replaced by fresh random chromosomes (R12)
     int selection;                        // 0 tournament, 1 ranking, 2 roulette (R10)
+    int maximize;                         // 1: fitness_dev holds 1 - error, see err_view
     const int* by_rank;                   // ranking: chromosome holding each rank (rank_kernel)
     const unsigned long long* prefix;     // roulette: inclusive prefix sums of the integer weights (roulette_prefix_kernel)
 };
@@ -110,12 +115,12 @@ __device__ __forceinline__ int roulette_from_word(uint32_t w, int M, const unsig
 }
 
 // by_rank[rank of chromosome c] = c; one block per chromosome (the same count as in ga_step_kernel).
-__global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* F, int M, int* by_rank) {
+__global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* F, int M, int* by_rank, int maximize) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
     const int c = blockIdx.x, tid = threadIdx.x;
-    const float kc = fit_key(__ldcg(F + c));
+    const float kc = fit_key(err_view(__ldcg(F + c), maximize));
     int cnt = 0;
-    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(__ldcg(F + j)), j, kc, c) ? 1 : 0;
+    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(err_view(__ldcg(F + j), maximize)), j, kc, c) ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if ((tid & 31) == 0) s_warp_cnt[tid >> 5] = cnt;
@@ -128,13 +133,13 @@ __global__ void __launch_bounds__(kGaThreads) rank_kernel(const float* F, int M,
 }
 
 // Inclusive prefix sums of the roulette weights; one block of 1024 threads, each owning a contiguous segment.
-__global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* F, int M, unsigned long long* prefix) {
+__global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* F, int M, unsigned long long* prefix, int maximize) {
     __shared__ unsigned long long s_tot[1024];
     const int tid = threadIdx.x;
     const int per = (M + 1023) / 1024;
     const int i0 = tid * per, i1 = min(M, i0 + per);
     unsigned long long acc = 0;
-    for (int i = i0; i < i1; ++i) acc += roulette_weight(__ldcg(F + i));
+    for (int i = i0; i < i1; ++i) acc += roulette_weight(err_view(__ldcg(F + i), maximize));
     s_tot[tid] = acc;
     __syncthreads();
     for (int o = 1; o < 1024; o <<= 1) {               // Hillis-Steele scan of the 1024 segment totals (integers: exact)
@@ -145,7 +150,7 @@ __global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* F, i
     }
     acc = tid > 0 ? s_tot[tid - 1] : 0ull;
     for (int i = i0; i < i1; ++i) {
-        acc += roulette_weight(__ldcg(F + i));
+        acc += roulette_weight(err_view(__ldcg(F + i), maximize));
         prefix[i] = acc;
     }
 }
@@ -205,9 +210,9 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
     }
 
     // (1) rank of chromosome c under the order
-    const float kc = fit_key(__ldcg(F + c));
+    const float kc = fit_key(err_view(__ldcg(F + c), p.maximize));
     int cnt = 0;
-    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(__ldcg(F + j)), j, kc, c) ? 1 : 0;
+    for (int j = tid; j < M; j += kGaThreads) cnt += precedes(fit_key(err_view(__ldcg(F + j), p.maximize)), j, kc, c) ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if ((tid & 31) == 0) s_warp_cnt[tid >> 5] = cnt;
@@ -256,7 +261,7 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
                 if ((e & 3) == 0)
                     r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
                 const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
-                const float ki = fit_key(__ldcg(F + idx));
+                const float ki = fit_key(err_view(__ldcg(F + idx), p.maximize));
                 const int side = e < k ? 0 : 1;
                 if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
                     par[side] = idx;
@@ -311,7 +316,7 @@ constexpr int kFinThreads = 1024, kFinCols = 32, kFinGroups = kFinThreads / kFin
 __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const double* part, int n_part, int m_stride, int M,
                                                                         double P_d, float* F, double* sse_out, float* best_out,
                                                                         float* blk_key, int* blk_idx, unsigned int* ticket,
-                                                                        int* stop, float threshold, int gen_index, int rmse,
+                                                                        int* stop, float threshold, int gen_index, int metric,
                                                                         RunState* run, int part_ff) {
     __shared__ float s_key[kFinThreads / 32];
     __shared__ int s_idx[kFinThreads / 32];
@@ -355,9 +360,10 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         if (sse_out != nullptr) {            // pattern-sharded evaluation: hand out the un-normalised sum instead
             sse_out[m] = s;
         } else {
-            const float f = static_cast<float>(rmse ? sqrt(s / P_d) : s / P_d);   // MSE or RMSE
+            // MSE or RMSE; or the fitness 1 - error (metric 2), whose order is taken on the error
+            const float f = static_cast<float>(metric == 1 ? sqrt(s / P_d) : (metric == 2 ? 1.0 - s / P_d : s / P_d));
             F[m] = f;
-            key = fit_key(f);
+            key = fit_key(err_view(f, metric == 2));
             idx = m;
         }
     }
@@ -419,7 +425,7 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
             *ticket = 0u;
             if (stop != nullptr) {
                 stop[1] = gen_index;                       // GA steps performed so far
-                if (best <= threshold) stop[0] = 1;        // learning-error threshold reached
+                if (err_view(best, metric == 2) <= threshold) stop[0] = 1;   // learning-error threshold reached
             }
         }
     }

@@ -2,6 +2,7 @@
 // orchestration (one stream, no per-generation host synchronisation).  Every step of the
 // hot path runs in the kernels of this directory; there is no CPU fallback.
 #include <cuda_runtime.h>
+#include <dlfcn.h>
 
 #include <cmath>
 #include <cstdarg>
@@ -39,7 +40,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_run = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_run = 0, off_sse = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -75,6 +76,8 @@ struct game_ctx {
     bool graph_ok = true;                            // false after a failed capture: plain launches from then on
     unsigned long long config_epoch = 0;             // bumped by every call that changes what a generation launches
     bool use_graph = true;                           // GAME_GRAPH=0 turns the graph path off (A/B measurements)
+    void* nccl_comm = nullptr;                       // ncclComm_t of the pattern-sharded loop (game_comm_init)
+    int comm_rank = 0, comm_world = 1;
     int* stop = nullptr;                             // device stop state, non-null only inside game_run_until
     float stop_threshold = 0.f;
     int stop_gen_index = 0;
@@ -85,6 +88,38 @@ struct game_ctx {
 };
 
 namespace {
+
+// ---- NCCL, loaded at run time (the library must load and work on one GPU without it): only the handful of entry points
+// the pattern-sharded loop needs, declared here from the public NCCL API.
+struct NcclUniqueId { char internal[128]; };
+struct NcclApi {
+    int (*GetUniqueId)(NcclUniqueId*) = nullptr;
+    int (*CommInitRank)(void**, int, NcclUniqueId, int) = nullptr;
+    int (*CommDestroy)(void*) = nullptr;
+    int (*AllReduce)(const void*, void*, size_t, int, int, void*, cudaStream_t) = nullptr;
+    const char* (*GetErrorString)(int) = nullptr;
+    bool ok = false;
+};
+constexpr int kNcclFloat64 = 8, kNcclSum = 0;      // ncclDataType_t / ncclRedOp_t values of the public header
+
+NcclApi& nccl() {
+    static NcclApi api;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* h = dlopen("libnccl.so.2", RTLD_NOW | RTLD_GLOBAL);      // the copy torch has loaded, if any; else the system's
+        if (!h) h = dlopen("libnccl.so", RTLD_NOW | RTLD_GLOBAL);
+        if (h) {
+            api.GetUniqueId = reinterpret_cast<decltype(api.GetUniqueId)>(dlsym(h, "ncclGetUniqueId"));
+            api.CommInitRank = reinterpret_cast<decltype(api.CommInitRank)>(dlsym(h, "ncclCommInitRank"));
+            api.CommDestroy = reinterpret_cast<decltype(api.CommDestroy)>(dlsym(h, "ncclCommDestroy"));
+            api.AllReduce = reinterpret_cast<decltype(api.AllReduce)>(dlsym(h, "ncclAllReduce"));
+            api.GetErrorString = reinterpret_cast<decltype(api.GetErrorString)>(dlsym(h, "ncclGetErrorString"));
+            api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllReduce;
+        }
+    }
+    return api;
+}
 
 int fail(const game_ctx* c, int code, const char* fmt, ...) {
     if (c) {
@@ -178,6 +213,144 @@ struct HostKb {
     const float* t;
 };
 
+// ---- the tensor-core path in pieces (shared by the resident, the host-range and the out-of-core evaluations)
+struct UmmaGeo {
+    int grid = 0, pair_cap = 0, m_pairs = 0, p_tiles_all = 0;
+};
+
+// fp16 hi / lo operand images (and row scales) of the current population, if the caller has written it since they were built
+int ensure_images(game_ctx* c) {
+    using namespace game;
+    if (c->img_valid) return GAME_OK;   // inside a generation loop the GA step keeps the images up to date (ga_step_kernel)
+    const float* W = c->pop[c->cur];
+    uint8_t* img = c->ws + c->off_img;
+    float* wscale = reinterpret_cast<float*>(c->ws + c->off_wscale);
+    const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
+    launch_chain(c->pdl, umma::row_scale_kernel, dim3(static_cast<unsigned>((c->m_stride * 32ll + 255) / 256)), dim3(256), 0,
+                 c->stream, W, wscale, c->M, c->G, c->m_stride);
+    int rc = check_launch(c, "row_scale_kernel");
+    if (rc) return rc;
+    launch_chain(c->pdl, umma::build_w_images_kernel, dim3(static_cast<unsigned>((n_thr + 255) / 256)), dim3(256), 0,
+                 c->stream, W, wscale, img, c->M, c->G, c->steps, c->m_tiles);
+    if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
+    c->img_valid = true;
+    return GAME_OK;
+}
+
+// Kernel parameters and grid for the whole knowledge base (pattern range fields are set per launch by the caller).
+void setup_umma(game_ctx* c, game::umma::Params& prm, UmmaGeo& geo) {
+    using namespace game;
+    prm.X = c->X; prm.t = c->t; prm.W = c->pop[c->cur]; prm.Wimg = c->ws + c->off_img;
+    prm.wscale = reinterpret_cast<float*>(c->ws + c->off_wscale); prm.zdump = nullptr;
+    prm.part = reinterpret_cast<double*>(c->ws + c->off_part);
+    prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
+    prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
+    geo.p_tiles_all = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
+    int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+    grid_cap &= ~1;                                              // CTA pairs (clusters of 2)
+    geo.pair_cap = grid_cap / 2;
+    geo.m_pairs = c->m_tiles / 2;
+    // work unit = (pattern tile, group of chromosome-tile pairs), dealt round-robin to the CTA pairs.  Splitting the
+    // chromosome tiles of a pattern tile into more groups evens out the last round but regenerates phi once per
+    // group (about one tile's time, exposed when a unit is short).  Cost model, in tile times:
+    // rounds x (tiles per unit + 1); measured on the c4 grid: M = 1024, P = 1e5 0.136 -> 0.098 ms against the former
+    // ">= 16 units per pair" rule, which cut that shape into units of one tile.
+    long long best_cost = -1;
+    int best_tpu = geo.m_pairs;
+    for (int g = 1; g <= geo.m_pairs; ++g) {
+        const int tpu = (geo.m_pairs + g - 1) / g;                 // chromosome-tile pairs per unit
+        if (g > 1 && tpu == (geo.m_pairs + g - 2) / (g - 1)) continue;   // same unit size as the previous g
+        const long long groups = (geo.m_pairs + tpu - 1) / tpu;
+        const long long rounds = (static_cast<long long>(geo.p_tiles_all) * groups + geo.pair_cap - 1) / geo.pair_cap;
+        const long long cost = rounds * (tpu + 1);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_tpu = tpu; }
+    }
+    prm.m_pairs_per_group = best_tpu;
+    prm.m_groups = (geo.m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
+    prm.dd = c->expansion == GAME_EXP_CHEBYSHEV ? c->d : 2 * c->d;
+    prm.shared = c->shared;
+    prm.steps = c->steps;
+    prm.stages = (c->steps + umma::kKS - 1) / umma::kKS;
+    prm.span = prm.stages > 1 ? umma::kKS : (c->steps + 1) / 2;      // one stage only: half of it per producer set
+    prm.resident = prm.stages <= umma::kMaxResidentStages ? 1 : 0;
+    // phi of a pattern tile stays in shared memory when it fits, twice over when that fits too (the producers
+    // then work one unit ahead of the MMAs)
+    prm.n_b = !prm.resident ? umma::kStreamBStages
+                            : (2 * prm.stages <= umma::kMaxResidentStages ? 2 * prm.stages : prm.stages);
+    prm.n_a = umma::kStagesTotal - prm.n_b;
+    prm.flush = prm.resident ? 0 : 1;
+    prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
+    prm.stop = c->stop;
+    prm.p_tile0 = 0; prm.p_tiles = geo.p_tiles_all; prm.zero_part = 1;
+    const long long units = static_cast<long long>(geo.p_tiles_all) * prm.m_groups;
+    geo.grid = 2 * static_cast<int>(units < geo.pair_cap ? units : geo.pair_cap);   // the same grid for every pattern range
+    c->last_umma_grid = geo.grid;
+}
+
+int launch_umma(game_ctx* c, const game::umma::Params& prm, int grid, bool pdl) {
+    using namespace game;
+#define GAME_LAUNCH(E, A) \
+    launch_chain(pdl, umma::fitness_umma_kernel<E, A>, dim3(grid), dim3(umma::kThreads), umma::kSmemBytes, c->stream, prm)
+    switch (c->expansion * 3 + c->act) {
+        case 0: GAME_LAUNCH(0, 0); break;
+        case 1: GAME_LAUNCH(0, 1); break;
+        case 2: GAME_LAUNCH(0, 2); break;
+        case 3: GAME_LAUNCH(1, 0); break;
+        case 4: GAME_LAUNCH(1, 1); break;
+        default: GAME_LAUNCH(1, 2); break;
+    }
+#undef GAME_LAUNCH
+    return check_launch(c, "fitness_umma_kernel");
+}
+
+bool wants_calibration(const game_ctx* c) {
+    return c->calibrate && c->act != GAME_ACT_SIGMOID &&
+           sizeof(double) * (static_cast<size_t>(c->G) + game::umma::kCalUnroll) <= kCalMaxSmem;
+}
+
+// Regression activations: measure every row's accumulation shrink on the first pattern tile (fitness_umma.cuh, "calibration")
+// and point prm.wscale at the corrected factors.  X0 / t0: where the first 256 patterns are (device).
+int launch_calibration(game_ctx* c, game::umma::Params& prm, const UmmaGeo& geo, bool pdl, const float* X0, const float* t0) {
+    using namespace game;
+    float* zdump = reinterpret_cast<float*>(c->ws + c->off_zdump);
+    float* zcorr = reinterpret_cast<float*>(c->ws + c->off_zcorr);
+    float* wscale = reinterpret_cast<float*>(c->ws + c->off_wscale);
+    umma::Params cal = prm;
+    cal.X = X0; cal.t = t0;
+    cal.p_tile0 = 0; cal.p_tiles = 1; cal.zero_part = 0; cal.zdump = zdump; cal.stall = nullptr;
+    cal.m_pairs_per_group = 1; cal.m_groups = geo.m_pairs;          // one chromosome-tile pair per CTA pair: shortest launch
+    const int cal_grid = 2 * (geo.m_pairs < geo.pair_cap ? geo.m_pairs : geo.pair_cap);
+    int rc = launch_umma(c, cal, cal_grid, pdl);
+    if (rc) return rc;
+    double* phi_s = reinterpret_cast<double*>(c->ws + c->off_calphi);
+    if (c->expansion == GAME_EXP_CHEBYSHEV)
+        launch_chain(pdl, umma::cal_phi_kernel<0>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, X0, phi_s,
+                     c->stop, c->P, c->N, c->d, c->shared);
+    else
+        launch_chain(pdl, umma::cal_phi_kernel<1>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, X0, phi_s,
+                     c->stop, c->P, c->N, c->d, c->shared);
+    if ((rc = check_launch(c, "cal_phi_kernel"))) return rc;
+    const size_t row_bytes = sizeof(double) * ((static_cast<size_t>(c->G - 1) + umma::kCalUnroll - 1) / umma::kCalUnroll * umma::kCalUnroll);
+    int rows = static_cast<int>(kCalMaxSmem / (row_bytes ? row_bytes : 1));
+    rows = rows > umma::kCalRows ? umma::kCalRows : (rows < 1 ? 1 : rows);
+    launch_chain(pdl, umma::calibrate_kernel, dim3((c->m_stride + rows - 1) / rows), dim3(umma::kCalThreads), rows * row_bytes,
+                 c->stream, prm.W, phi_s, zdump, wscale, zcorr, c->stop, c->P, c->M, c->G, c->m_stride, rows);
+    if ((rc = check_launch(c, "calibrate_kernel"))) return rc;
+    prm.wscale = zcorr;
+    return GAME_OK;
+}
+
+int launch_finalize(game_ctx* c, int n_part, float* best_out, double* sse_out, int part_ff) {
+    using namespace game;
+    const int fin_blocks = (c->M + kFinCols - 1) / kFinCols;
+    launch_chain(c->pdl, finalize_fitness_kernel, dim3(fin_blocks), dim3(kFinThreads), 0, c->stream,
+        reinterpret_cast<const double*>(c->ws + c->off_part), n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
+        reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
+        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index, c->rmse,
+        sse_out == nullptr ? c->run : static_cast<RunState*>(nullptr), part_ff);
+    return check_launch(c, "finalize_fitness_kernel");
+}
+
 // One fitness evaluation of the current population; best_out (device) may be NULL.  With `hk` the knowledge base is
 // copied from host memory in pattern ranges on a second stream, each range evaluated as soon as it has landed.
 int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, double* sse_out = nullptr) {
@@ -194,7 +367,6 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
         c->ticket_zeroed = true;
     }
-    double* part = reinterpret_cast<double*>(c->ws + c->off_part);
     const float* W = c->pop[c->cur];
     int n_part = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -204,61 +376,12 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         GAME_CUDA(cudaEventCreate(&ev1));
     }
     if (scheme == GAME_SCHEME_F16X3) {
-        uint8_t* img = c->ws + c->off_img;
-        const long long n_thr = static_cast<long long>(c->m_tiles) * c->steps * 2 * umma::kBM;
-        float* wscale = reinterpret_cast<float*>(c->ws + c->off_wscale);
-        if (!c->img_valid) {   // inside a generation loop the GA step keeps the images up to date (ga_step_kernel)
-            launch_chain(c->pdl, umma::row_scale_kernel, dim3(static_cast<unsigned>((c->m_stride * 32ll + 255) / 256)), dim3(256), 0,
-                         c->stream, W, wscale, c->M, c->G, c->m_stride);
-            if ((rc = check_launch(c, "row_scale_kernel"))) return rc;
-            launch_chain(c->pdl, umma::build_w_images_kernel, dim3(static_cast<unsigned>((n_thr + 255) / 256)), dim3(256), 0,
-                         c->stream, W, wscale, img, c->M, c->G, c->steps, c->m_tiles);
-            if ((rc = check_launch(c, "build_w_images_kernel"))) return rc;
-            c->img_valid = true;
-        }
+        if ((rc = ensure_images(c))) return rc;
         umma::Params prm;
-        prm.X = c->X; prm.t = c->t; prm.W = W; prm.Wimg = img; prm.wscale = wscale; prm.zdump = nullptr; prm.part = part;
-        prm.P = c->P; prm.N = c->N; prm.d = c->d; prm.M = c->M; prm.G = c->G;
-        prm.m_stride = c->m_stride; prm.m_tiles = c->m_tiles;
-        const int p_tiles_all = static_cast<int>((c->P + umma::kBN - 1) / umma::kBN);
-        int grid_cap = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
-        grid_cap &= ~1;                                              // CTA pairs (clusters of 2)
-        const int pair_cap = grid_cap / 2, m_pairs = c->m_tiles / 2;
-        // work unit = (pattern tile, group of chromosome-tile pairs), dealt round-robin to the CTA pairs.  Splitting the
-        // chromosome tiles of a pattern tile into more groups evens out the last round but regenerates phi once per
-        // group (about one tile's time, exposed when a unit is short).  Cost model, in tile times:
-        // rounds x (tiles per unit + 1); measured on the c4 grid: M = 1024, P = 1e5 0.136 -> 0.098 ms against the former
-        // ">= 16 units per pair" rule, which cut that shape into units of one tile.
-        long long best_cost = -1;
-        int best_tpu = m_pairs;
-        for (int g = 1; g <= m_pairs; ++g) {
-            const int tpu = (m_pairs + g - 1) / g;                 // chromosome-tile pairs per unit
-            if (g > 1 && tpu == (m_pairs + g - 2) / (g - 1)) continue;   // same unit size as the previous g
-            const long long groups = (m_pairs + tpu - 1) / tpu;
-            const long long rounds = (static_cast<long long>(p_tiles_all) * groups + pair_cap - 1) / pair_cap;
-            const long long cost = rounds * (tpu + 1);
-            if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_tpu = tpu; }
-        }
-        prm.m_pairs_per_group = best_tpu;
-        prm.m_groups = (m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
-        prm.dd = c->expansion == GAME_EXP_CHEBYSHEV ? c->d : 2 * c->d;
-        prm.shared = c->shared;
-        prm.steps = c->steps;
-        prm.stages = (c->steps + umma::kKS - 1) / umma::kKS;
-        prm.span = prm.stages > 1 ? umma::kKS : (c->steps + 1) / 2;      // one stage only: half of it per producer set
-        prm.resident = prm.stages <= umma::kMaxResidentStages ? 1 : 0;
-        // phi of a pattern tile stays in shared memory when it fits, twice over when that fits too (the producers
-        // then work one unit ahead of the MMAs)
-        prm.n_b = !prm.resident ? umma::kStreamBStages
-                                : (2 * prm.stages <= umma::kMaxResidentStages ? 2 * prm.stages : prm.stages);
-        prm.n_a = umma::kStagesTotal - prm.n_b;
-        prm.flush = prm.resident ? 0 : 1;
-        prm.stall = reinterpret_cast<long long*>(c->ws + c->off_stall);
-        prm.stop = c->stop;
-        const long long units = static_cast<long long>(p_tiles_all) * prm.m_groups;
-        const int grid = 2 * static_cast<int>(units < pair_cap ? units : pair_cap);   // the same grid for every range
+        UmmaGeo geo;
+        setup_umma(c, prm, geo);
+        const int p_tiles_all = geo.p_tiles_all, pair_cap = geo.pair_cap, grid = geo.grid;
         n_part = 2 * grid;
-        c->last_umma_grid = grid;
         // pattern ranges: one launch, or (host knowledge base >= 64 MB) 8 ranges pipelined against their H2D copies
         const size_t kb_bytes = sizeof(float) * static_cast<size_t>(c->P) * (c->N + 1);
         const int n_ranges = (hk != nullptr && kb_bytes >= (64u << 20) && p_tiles_all >= 64) ? 8 : 1;
@@ -304,59 +427,14 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
                 GAME_CUDA(cudaEventRecord(c->copy_events[k], c->copy_stream));
                 GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[k], 0));
             }
-            if (first_launch && c->calibrate && c->act != GAME_ACT_SIGMOID && sizeof(double) * (static_cast<size_t>(c->G) + umma::kCalUnroll) <= kCalMaxSmem) {
-                // regression activations: measure every row's accumulation shrink on the first pattern tile (calibrate_kernel)
-                float* zdump = reinterpret_cast<float*>(c->ws + c->off_zdump);
-                float* zcorr = reinterpret_cast<float*>(c->ws + c->off_zcorr);
-                umma::Params cal = prm;
-                cal.p_tile0 = 0; cal.p_tiles = 1; cal.zero_part = 0; cal.zdump = zdump; cal.stall = nullptr;
-                cal.m_pairs_per_group = 1; cal.m_groups = m_pairs;          // one chromosome-tile pair per CTA pair: shortest launch
-                const int cal_grid = 2 * (m_pairs < pair_cap ? m_pairs : pair_cap);
-                const int sel = c->expansion * 3 + c->act;
-#define GAME_LAUNCH_CAL(E, A) \
-    launch_chain(c->pdl && hk == nullptr, umma::fitness_umma_kernel<E, A>, dim3(cal_grid), dim3(umma::kThreads), umma::kSmemBytes, c->stream, cal)
-                switch (sel) {
-                    case 0: GAME_LAUNCH_CAL(0, 0); break;
-                    case 2: GAME_LAUNCH_CAL(0, 2); break;
-                    case 3: GAME_LAUNCH_CAL(1, 0); break;
-                    default: GAME_LAUNCH_CAL(1, 2); break;
-                }
-#undef GAME_LAUNCH_CAL
-                if ((rc = check_launch(c, "fitness_umma_kernel (calibration)"))) return rc;
-                double* phi_s = reinterpret_cast<double*>(c->ws + c->off_calphi);
-                if (c->expansion == GAME_EXP_CHEBYSHEV)
-                    launch_chain(c->pdl && hk == nullptr, umma::cal_phi_kernel<0>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, c->X,
-                                 phi_s, c->stop, c->P, c->N, c->d, c->shared);
-                else
-                    launch_chain(c->pdl && hk == nullptr, umma::cal_phi_kernel<1>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, c->X,
-                                 phi_s, c->stop, c->P, c->N, c->d, c->shared);
-                if ((rc = check_launch(c, "cal_phi_kernel"))) return rc;
-                const size_t row_bytes = sizeof(double) * ((static_cast<size_t>(c->G - 1) + umma::kCalUnroll - 1) / umma::kCalUnroll * umma::kCalUnroll);
-                int rows = static_cast<int>(kCalMaxSmem / (row_bytes ? row_bytes : 1));
-                rows = rows > umma::kCalRows ? umma::kCalRows : (rows < 1 ? 1 : rows);
-                launch_chain(c->pdl && hk == nullptr, umma::calibrate_kernel, dim3((c->m_stride + rows - 1) / rows), dim3(umma::kCalThreads),
-                             rows * row_bytes, c->stream, W, phi_s, zdump, wscale, zcorr, c->stop, c->P, c->M, c->G, c->m_stride, rows);
-                if ((rc = check_launch(c, "calibrate_kernel"))) return rc;
-                prm.wscale = zcorr;
+            if (first_launch && wants_calibration(c)) {
+                if ((rc = launch_calibration(c, prm, geo, c->pdl && hk == nullptr, c->X, c->t))) return rc;
                 if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));      // the roofline figure times the evaluation proper
             }
             prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = first_launch ? 1 : 0;
             first_launch = false;
-#define GAME_LAUNCH(E, A) \
-    launch_chain(c->pdl && hk == nullptr, umma::fitness_umma_kernel<E, A>, dim3(grid), dim3(umma::kThreads), umma::kSmemBytes, c->stream, prm)
-            const int sel = c->expansion * 3 + c->act;
-            switch (sel) {
-                case 0: GAME_LAUNCH(0, 0); break;
-                case 1: GAME_LAUNCH(0, 1); break;
-                case 2: GAME_LAUNCH(0, 2); break;
-                case 3: GAME_LAUNCH(1, 0); break;
-                case 4: GAME_LAUNCH(1, 1); break;
-                default: GAME_LAUNCH(1, 2); break;
-            }
-#undef GAME_LAUNCH
-            if (k + 1 < n_ranges && (rc = check_launch(c, "fitness_umma_kernel"))) return rc;
+            if ((rc = launch_umma(c, prm, grid, c->pdl && hk == nullptr))) return rc;
         }
-        if ((rc = check_launch(c, "fitness_umma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     } else {
         if (hk != nullptr) {
@@ -376,19 +454,95 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         n_part = grid;
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
         launch_chain(c->pdl && hk == nullptr, fitness_ffma_kernel, dim3(grid), dim3(kFfmaTile), smem, c->stream,
-                     c->X, c->t, W, part, c->P, c->N, c->d, c->M, c->G, c->expansion, c->act, c->m_stride, n_tiles, c->stop, c->shared);
+                     c->X, c->t, W, reinterpret_cast<double*>(c->ws + c->off_part), c->P, c->N, c->d, c->M, c->G, c->expansion, c->act,
+                     c->m_stride, n_tiles, c->stop, c->shared);
         if ((rc = check_launch(c, "fitness_ffma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
     }
     if (timed) c->events.emplace_back(ev0, ev1);
-    const int fin_blocks = (c->M + kFinCols - 1) / kFinCols;
-    launch_chain(c->pdl, finalize_fitness_kernel, dim3(fin_blocks), dim3(kFinThreads), 0, c->stream,
-        part, n_part, c->m_stride, c->M, static_cast<double>(c->P), c->fitness, sse_out, best_out,
-        reinterpret_cast<float*>(c->ws + c->off_blk_key), reinterpret_cast<int*>(c->ws + c->off_blk_idx),
-        reinterpret_cast<unsigned int*>(c->ws + c->off_ticket), c->stop, c->stop_threshold, c->stop_gen_index, c->rmse,
-        sse_out == nullptr ? c->run : static_cast<RunState*>(nullptr), scheme == GAME_SCHEME_F16X3 ? 1 : 0);
-    if ((rc = check_launch(c, "finalize_fitness_kernel"))) return rc;
+    if ((rc = launch_finalize(c, n_part, best_out, sse_out, scheme == GAME_SCHEME_F16X3 ? 1 : 0))) return rc;
     c->fitness_valid = sse_out == nullptr;
+    return GAME_OK;
+}
+
+// Out-of-core evaluation (a knowledge base too large for device memory): the patterns stay in HOST memory
+// and pass through a ring of `n_slots` device buffers of `slot_rows` patterns each; the copy of range r + 1 (and r + 2)
+// runs on the copy stream while the kernel works on range r, the partial sums are carried across the launches.  A slot
+// holds whole rounds of the persistent grid (its capacity is rounded down accordingly), so every pattern tile meets the
+// same CTA pair, in the same order, as in a resident evaluation: the fitness is bit-identical to it.
+int eval_streamed(game_ctx* c, const float* X_host, const float* t_host, float* X_ring, float* t_ring, long long slot_rows, int n_slots) {
+    using namespace game;
+    if (!c->pop[0] || !c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness_streamed before game_bind_state");
+    DeviceGuard guard(c->device >= 0 ? c->device : device_of(X_ring));
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    if (resolved_scheme(c) != GAME_SCHEME_F16X3 || !c->umma_ok)
+        return fail(c, GAME_ERR_UNSUPPORTED, "game_eval_fitness_streamed runs on the tensor-core scheme (F16X3) only");
+    if (c->stop != nullptr || c->run != nullptr) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness_streamed inside a generation loop");
+    if (!c->ticket_zeroed) {
+        GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
+        c->ticket_zeroed = true;
+    }
+    if ((rc = ensure_images(c))) return rc;
+    umma::Params prm;
+    UmmaGeo geo;
+    setup_umma(c, prm, geo);
+    // tiles per slot: a multiple of the number of pattern tiles after which the unit -> CTA pair assignment repeats
+    const int n_pairs = geo.grid / 2;
+    int a = n_pairs, b = prm.m_groups;
+    while (b) { const int r = a % b; a = b; b = r; }
+    const long long quantum = n_pairs / a;                                   // pattern tiles per whole number of rounds
+    long long slot_tiles = (slot_rows / umma::kBN) / quantum * quantum;
+    if (slot_tiles < 1) {
+        if (geo.p_tiles_all <= slot_rows / umma::kBN) slot_tiles = geo.p_tiles_all;      // everything fits one slot
+        else return fail(c, GAME_ERR_INVALID_ARG, "ring slots of %lld patterns are too small: this shape needs at least %lld per slot",
+                         slot_rows, quantum * umma::kBN);
+    }
+    if (!c->copy_stream) GAME_CUDA(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    while (static_cast<int>(c->copy_events.size()) < 2 * n_slots + 1) {
+        cudaEvent_t e;
+        GAME_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        c->copy_events.push_back(e);
+    }
+    // events [0, n_slots): slot filled; [n_slots, 2 n_slots): slot consumed; the copies follow everything enqueued so far
+    GAME_CUDA(cudaEventRecord(c->copy_events[2 * n_slots], c->stream));
+    GAME_CUDA(cudaStreamWaitEvent(c->copy_stream, c->copy_events[2 * n_slots], 0));
+    const long long n_ranges = (geo.p_tiles_all + slot_tiles - 1) / slot_tiles;
+    auto enqueue_copy = [&](long long r) -> int {
+        const int slot = static_cast<int>(r % n_slots);
+        const long long p0 = r * slot_tiles * umma::kBN;
+        long long p1 = p0 + slot_tiles * umma::kBN;
+        if (p1 > c->P) p1 = c->P;
+        if (r >= n_slots) GAME_CUDA(cudaStreamWaitEvent(c->copy_stream, c->copy_events[n_slots + slot], 0));   // its last reader is done
+        GAME_CUDA(cudaMemcpyAsync(X_ring + static_cast<size_t>(slot) * slot_rows * c->N, X_host + p0 * c->N,
+                                  sizeof(float) * static_cast<size_t>(p1 - p0) * c->N, cudaMemcpyHostToDevice, c->copy_stream));
+        GAME_CUDA(cudaMemcpyAsync(t_ring + static_cast<size_t>(slot) * slot_rows, t_host + p0, sizeof(float) * static_cast<size_t>(p1 - p0),
+                                  cudaMemcpyHostToDevice, c->copy_stream));
+        GAME_CUDA(cudaEventRecord(c->copy_events[slot], c->copy_stream));
+        return GAME_OK;
+    };
+    for (long long r = 0; r < n_ranges && r < n_slots - 1; ++r)
+        if ((rc = enqueue_copy(r))) return rc;                       // prime the ring
+    for (long long r = 0; r < n_ranges; ++r) {
+        const int slot = static_cast<int>(r % n_slots);
+        if (r + n_slots - 1 < n_ranges && (rc = enqueue_copy(r + n_slots - 1))) return rc;
+        GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[slot], 0));
+        const long long tile0 = r * slot_tiles;
+        const long long p0 = tile0 * umma::kBN;
+        // the kernel indexes patterns absolutely: hand it the slot's base moved back by the range's first pattern
+        const float* Xs = X_ring + static_cast<size_t>(slot) * slot_rows * c->N;
+        const float* ts = t_ring + static_cast<size_t>(slot) * slot_rows;
+        if (r == 0 && wants_calibration(c) && (rc = launch_calibration(c, prm, geo, false, Xs, ts))) return rc;
+        prm.X = reinterpret_cast<const float*>(reinterpret_cast<uintptr_t>(Xs) - sizeof(float) * static_cast<size_t>(p0) * c->N);
+        prm.t = reinterpret_cast<const float*>(reinterpret_cast<uintptr_t>(ts) - sizeof(float) * static_cast<size_t>(p0));
+        prm.p_tile0 = static_cast<int>(tile0);
+        prm.p_tiles = static_cast<int>(tile0 + slot_tiles <= geo.p_tiles_all ? slot_tiles : geo.p_tiles_all - tile0);
+        prm.zero_part = r == 0 ? 1 : 0;
+        if ((rc = launch_umma(c, prm, geo.grid, false))) return rc;
+        GAME_CUDA(cudaEventRecord(c->copy_events[n_slots + slot], c->stream));
+    }
+    if ((rc = launch_finalize(c, 2 * geo.grid, nullptr, nullptr, 1))) return rc;
+    c->fitness_valid = true;
     return GAME_OK;
 }
 
@@ -405,15 +559,16 @@ int step_internal(game_ctx* c, uint64_t seed, uint32_t gen) {
     p.t_mut = bernoulli_threshold(c->p_mut);
     p.sigma = c->sigma; p.gen = gen; p.key = make_key(seed);
     p.selection = c->selection;
+    p.maximize = c->rmse == 2 ? 1 : 0;
     p.immigrants = c->immigrants < c->M - c->elite ? c->immigrants : c->M - c->elite;
     p.by_rank = reinterpret_cast<const int*>(c->ws + c->off_by_rank);
     p.prefix = reinterpret_cast<const unsigned long long*>(c->ws + c->off_prefix);
     if (c->selection == GAME_SEL_RANKING) {
-        rank_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->fitness, c->M, reinterpret_cast<int*>(c->ws + c->off_by_rank));
+        rank_kernel<<<c->M, kGaThreads, 0, c->stream>>>(c->fitness, c->M, reinterpret_cast<int*>(c->ws + c->off_by_rank), p.maximize);
         if ((rc = check_launch(c, "rank_kernel"))) return rc;
     } else if (c->selection == GAME_SEL_ROULETTE) {
         roulette_prefix_kernel<<<1, 1024, 0, c->stream>>>(c->fitness, c->M,
-                                                           reinterpret_cast<unsigned long long*>(c->ws + c->off_prefix));
+                                                           reinterpret_cast<unsigned long long*>(c->ws + c->off_prefix), p.maximize);
         if ((rc = check_launch(c, "roulette_prefix_kernel"))) return rc;
     }
     launch_chain(c->pdl, ga_step_kernel, dim3(c->M), dim3(kGaThreads), 0, c->stream,
@@ -568,6 +723,7 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_prefix = off; off = align_up(off + sizeof(unsigned long long) * static_cast<size_t>(M));
     c->off_fused_bar = off; off = align_up(off + sizeof(unsigned int));
     c->off_run = off; off = align_up(off + sizeof(game::RunState));
+    c->off_sse = off; off = align_up(off + sizeof(double) * static_cast<size_t>(M));      // pattern-sharded loop: per-chromosome sums
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
@@ -580,6 +736,7 @@ int game_destroy(game_ctx* c) {
         cudaEventDestroy(ev.second);
     }
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->nccl_comm && nccl().ok) nccl().CommDestroy(c->nccl_comm);
     for (auto& e : c->copy_events) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
@@ -676,9 +833,9 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
 
 int game_set_error_metric(game_ctx* c, int32_t metric) {
     if (!c) return GAME_ERR_INVALID_ARG;
-    if (metric != GAME_ERROR_MSE && metric != GAME_ERROR_RMSE) return fail(c, GAME_ERR_INVALID_ARG, "unknown error metric %d", metric);
+    if (metric < GAME_ERROR_MSE || metric > GAME_ERROR_ONE_MINUS_MSE) return fail(c, GAME_ERR_INVALID_ARG, "unknown error metric %d", metric);
     c->config_epoch += 1;
-    c->rmse = metric == GAME_ERROR_RMSE ? 1 : 0;
+    c->rmse = metric;        // 0 MSE, 1 RMSE, 2 the paper's fitness 1 - MSE (maximised)
     c->fitness_valid = false;
     return GAME_OK;
 }
@@ -810,6 +967,7 @@ int game_evolve_fused(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens
     prm.ga.t_mut = bernoulli_threshold(c->p_mut);
     prm.ga.sigma = c->sigma; prm.ga.gen = gen0; prm.ga.key = make_key(seed);
     prm.ga.selection = c->selection;
+    prm.ga.maximize = c->rmse == 2 ? 1 : 0;
     prm.ga.immigrants = c->immigrants < c->M - c->elite ? c->immigrants : c->M - c->elite;
     prm.ga.by_rank = nullptr; prm.ga.prefix = nullptr;
     // The grid barrier counts arrivals in 32 bits (2 x grid per generation): at most 2^20 generations per launch, longer
@@ -869,10 +1027,74 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     return GAME_OK;
 }
 
+int game_eval_fitness_streamed(game_ctx* c, const float* X_host, const float* t_host, float* X_ring_dev, float* t_ring_dev,
+                               int64_t slot_rows, int32_t n_slots) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!X_host || !t_host || !X_ring_dev || !t_ring_dev) return fail(c, GAME_ERR_INVALID_ARG, "game_eval_fitness_streamed: null pointer");
+    if (slot_rows < game::umma::kBN || slot_rows % game::umma::kBN != 0)
+        return fail(c, GAME_ERR_INVALID_ARG, "slot_rows must be a positive multiple of %d", game::umma::kBN);
+    if (n_slots < 2 || n_slots > 8) return fail(c, GAME_ERR_INVALID_ARG, "n_slots must be in [2, 8]");
+    if (!aligned16(X_ring_dev) || !aligned16(t_ring_dev)) return fail(c, GAME_ERR_INVALID_ARG, "ring buffers must be 16-byte aligned");
+    return eval_streamed(c, X_host, t_host, X_ring_dev, t_ring_dev, slot_rows, n_slots);
+}
+
 int game_eval_sse(game_ctx* c, double* sse_dev) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!sse_dev) return fail(c, GAME_ERR_INVALID_ARG, "game_eval_sse: null sse_dev");
     return eval_internal(c, nullptr, nullptr, sse_dev);
+}
+
+int game_comm_unique_id(void* id128_host) {
+    if (!id128_host) return GAME_ERR_INVALID_ARG;
+    if (!nccl().ok) return GAME_ERR_UNSUPPORTED;
+    NcclUniqueId id;
+    if (nccl().GetUniqueId(&id) != 0) return GAME_ERR_CUDA;
+    std::memcpy(id128_host, id.internal, sizeof(id.internal));
+    return GAME_OK;
+}
+
+int game_comm_init(game_ctx* c, const void* id128_host, int32_t rank, int32_t world) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!id128_host || world < 1 || rank < 0 || rank >= world) return fail(c, GAME_ERR_INVALID_ARG, "game_comm_init: bad id, rank or world");
+    if (!nccl().ok) return fail(c, GAME_ERR_UNSUPPORTED, "libnccl.so.2 could not be loaded");
+    if (!c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_comm_init before game_bind_state (the communicator lives on the device of the bound buffers)");
+    DeviceGuard guard(c->device);
+    int rc = ensure_device(c);
+    if (rc) return rc;
+    if (c->nccl_comm) {
+        nccl().CommDestroy(c->nccl_comm);
+        c->nccl_comm = nullptr;
+    }
+    NcclUniqueId id;
+    std::memcpy(id.internal, id128_host, sizeof(id.internal));
+    const int e = nccl().CommInitRank(&c->nccl_comm, world, id, rank);
+    if (e != 0) {
+        c->nccl_comm = nullptr;
+        return fail(c, GAME_ERR_CUDA, "ncclCommInitRank: %s", nccl().GetErrorString ? nccl().GetErrorString(e) : "error");
+    }
+    c->comm_rank = rank;
+    c->comm_world = world;
+    return GAME_OK;
+}
+
+int game_evolve_sharded(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, int64_t P_total, float* best_fitness_dev) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->nccl_comm) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_sharded before game_comm_init");
+    if (P_total < c->P) return fail(c, GAME_ERR_INVALID_ARG, "P_total is the pattern count over ALL ranks (>= this rank's %lld)", c->P);
+    if (!c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_sharded before game_bind_state");
+    DeviceGuard guard(c->device);
+    double* sse = reinterpret_cast<double*>(c->ws + c->off_sse);
+    for (uint32_t i = 0; i < n_gens; ++i) {
+        int rc = eval_internal(c, nullptr, nullptr, sse);                 // this rank's un-normalised sums
+        if (rc) return rc;
+        const int e = nccl().AllReduce(sse, sse, static_cast<size_t>(c->M), kNcclFloat64, kNcclSum, c->nccl_comm, c->stream);
+        if (e != 0) return fail(c, GAME_ERR_CUDA, "ncclAllReduce: %s", nccl().GetErrorString ? nccl().GetErrorString(e) : "error");
+        rc = game_set_fitness_from_sse(c, sse, P_total, best_fitness_dev ? best_fitness_dev + i : nullptr);
+        if (rc) return rc;
+        rc = step_internal(c, seed, gen0 + i);                            // identical on every rank
+        if (rc) return rc;
+    }
+    return GAME_OK;
 }
 
 int game_set_fitness_from_sse(game_ctx* c, const double* sse_dev, int64_t P_total, float* best_fitness_dev) {

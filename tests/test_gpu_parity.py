@@ -459,6 +459,104 @@ def test_pattern_sharded_evaluation_single_device(game, world):
         G.close()
 
 
+def test_evolve_sharded_world_of_one_matches_evolve(game):
+    """game_evolve_sharded (the pattern-sharded generation loop inside the library: eval kernels, ncclAllReduce of M
+    doubles on the library's stream, finalisation, GA step) on a communicator of ONE rank -- the only world this box
+    has: NCCL is loaded, initialised and called in-stream, and the loop must reproduce game_run bit for bit."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=3000, M=200)
+    X, t, _ = wl.make_kb(cfg)
+    n = 5
+    A = make(game, cfg); A.load_kb(X, t); A.init_population(8)
+    ref_best = torch.zeros(n + 1, dtype=torch.float32, device="cuda")
+    A.run(8, 0, n, ref_best); A.sync()
+    B = make(game, cfg); B.load_kb(X, t); B.init_population(8)
+    try:
+        ident = game.game_comm_unique_id()
+    except game.GameError:
+        pytest.skip("NCCL cannot be loaded in this process")
+    game.game_comm_init(B.ctx, ident, 0, 1)
+    best = torch.zeros(n, dtype=torch.float32, device="cuda")
+    game.game_evolve_sharded(B.ctx, 8, 0, n, cfg.P, best.data_ptr()); B.sync()
+    assert np.array_equal(B.get_population().view(np.uint32), A.get_population().view(np.uint32))
+    assert np.array_equal(best.cpu().numpy(), ref_best.cpu().numpy()[:n])
+    A.close(); B.close()
+
+
+# ------------------------------------------------------------------------------------------------ out of core (N4)
+@pytest.mark.parametrize("base,over,slot_rows,n_slots", [
+    ("c3", dict(P=1_200_123, M=300), 50_176, 3),          # ring = 1/8 of the knowledge base; ragged last range and last tile
+    ("c2", dict(P=300_000, M=520), 19_200, 2),            # tanh: the calibration launch runs on the first slot
+    ("c1", dict(P=40_000, M=100), 65_536, 2),             # everything fits one slot
+])
+def test_streamed_out_of_core_evaluation_is_bit_identical(game, base, over, slot_rows, n_slots):
+    """game_eval_fitness_streamed: the knowledge base stays in pinned HOST memory and passes through a ring
+    of device buffers an eighth of its size; the fitness is bit-identical to the resident evaluation (same pattern tile ->
+    CTA pair assignment, same order of the partial sums), twice in a row (ring re-use across calls), and the GA step runs on it."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS[base], **over)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, 21)
+    R = make(game, cfg); R.load_kb(X, t); R.set_population(W); R.eval_fitness(); R.sync()
+    F_res = R.get_fitness()
+    R.close()
+    G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation, resident_kb=False)
+    G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+    assert G.X is None
+    G.set_population(W)
+    Xh, th = torch.from_numpy(X).pin_memory(), torch.from_numpy(t).pin_memory()
+    Xr = torch.full((n_slots * slot_rows, cfg.N), float("nan"), dtype=torch.float32, device="cuda")
+    tr = torch.full((n_slots * slot_rows,), float("nan"), dtype=torch.float32, device="cuda")
+    assert Xr.numel() * 4 <= max(X.nbytes // 8 + 4 * 256 * cfg.N * n_slots, 2 * 65_536 * cfg.N * 4)
+    for rep in range(2):
+        game.game_eval_fitness_streamed(G.ctx, Xh.data_ptr(), th.data_ptr(), Xr.data_ptr(), tr.data_ptr(), slot_rows, n_slots)
+        G.sync()
+        assert np.array_equal(G.get_fitness().view(np.uint32), F_res.view(np.uint32)), f"pass {rep}"
+    rows = sorted({0, min(127, cfg.M - 1), min(128, cfg.M - 1), cfg.M - 1})
+    assert_fitness_close(F_res[rows], oracle.eval_fitness(cfg.d, cfg.family, X, t, W[rows]), "streamed vs oracle")
+    G.step(5, 0); G.sync()
+    ref = oracle.step(W, F_res, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 5, 0)
+    assert np.array_equal(G.get_population().view(np.uint32), ref.view(np.uint32))
+    with pytest.raises(game.GameError) as e:          # a slot must hold one whole round of the persistent grid
+        game.game_eval_fitness_streamed(G.ctx, Xh.data_ptr(), th.data_ptr(), Xr.data_ptr(), tr.data_ptr(), 256, n_slots)
+    assert e.value.code == (game.ERR_INVALID_ARG if cfg.P > 256 * 74 else game.OK)
+    G.close()
+
+
+# ------------------------------------------------------------------------------------------------ the paper's fitness 1 - error
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("selection", [0, 1, 2])
+def test_one_minus_mse_fitness(game, selection, scheme):
+    """GAME_ERROR_ONE_MINUS_MSE (fitness = 1 - error, maximised): fitness_dev = 1 - MSE within 1e-5 of the
+    oracle's; the best-fitness trace holds the MAXIMUM; the GA operators are those of the oracle on the error vector
+    e = 1 - fitness (ONE fp32 subtraction, the same on both sides), bit for bit, for all three selection methods."""
+    import torch
+    cfg = wl.scaled(wl.CONFIGS["c1"], P=3000, M=150)
+    X, t, _ = wl.make_kb(cfg)
+    G = make(game, cfg, scheme); G.load_kb(X, t)
+    game.game_set_error_metric(G.ctx, game.ERROR_ONE_MINUS_MSE)
+    game.game_set_selection(G.ctx, selection)
+    G.init_population(3); G.sync()
+    W = G.get_population()
+    best = torch.full((3,), float("nan"), dtype=torch.float32, device="cuda")
+    G.run(3, 0, 0, best); G.sync()                      # one evaluation through the run loop: best[0]
+    F = G.get_fitness()
+    ref = 1.0 - oracle.eval_fitness(cfg.d, cfg.family, X, t, W)
+    assert np.max(np.abs(F - ref) / ref) <= 1e-5
+    assert best.cpu().numpy()[0] == F.max()
+    err = (np.float32(1.0) - F).astype(np.float32)
+    G.step(3, 0); G.sync()
+    W1 = oracle.step_sel(W, err, cfg.elite, cfg.tournament, selection, cfg.p_cross, cfg.p_mut, cfg.sigma, 3, 0)
+    assert np.array_equal(G.get_population().view(np.uint32), W1.view(np.uint32))
+    # the stop rule is a learning-ERROR threshold: 1 - best <= threshold
+    G.set_population(W)
+    done = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+    tr = torch.full((6,), float("nan"), dtype=torch.float32, device="cuda")
+    game.game_run_until(G.ctx, 3, 0, 5, float(1.0 - F.max()) * 1.0000001, tr.data_ptr(), done.data_ptr()); G.sync()
+    assert int(done.item()) == 0
+    G.close()
+
+
 # ------------------------------------------------------------------------------------------------ stop rule
 @pytest.mark.parametrize("scheme", SCHEMES)
 def test_run_until_stop_rule(game, scheme):

@@ -7,6 +7,7 @@ import subprocess
 import sys
 
 import numpy as np
+import pytest
 import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
@@ -95,3 +96,51 @@ def test_pattern_sharded_generation_gloo(tmp_path):
     mp.spawn(_shard_worker, args=(2, 29535, out), nprocs=2, join=True)
     r = json.load(open(out))
     assert r["same_pop"] and r["max_rel"] <= 1e-13
+
+
+def _lib_shard_worker(rank, world, port, out):
+    """Pattern-sharded generations driven through the LIBRARY's entry points (game_eval_sse -> all-reduce ->
+    game_set_fitness_from_sse -> game_step), two processes on the one GPU of the box; the all-reduce goes through gloo on
+    a CPU copy (two ranks cannot share one GPU under NCCL), so no kernel ever waits on another rank's kernel."""
+    import oracle
+    import paper_1211_5481_b200 as game
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cfg = wl.scaled(wl.CONFIGS["c3"], P=5003, M=200)
+    X, t, _ = wl.make_kb(cfg)                                     # same seed on every rank = one global knowledge base
+    p0, p1 = wl.shard_patterns(cfg.P, world, rank)
+    G = game.Game(p1 - p0, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation)
+    G.set_ga_params(cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma)
+    G.load_kb(X[p0:p1], t[p0:p1])
+    G.init_population(5)
+    W = oracle.init_population(cfg.M, cfg.G, 5)
+    sse = torch.zeros(cfg.M, dtype=torch.float64, device="cuda")
+    ok, worst = True, 0.0
+    for gen in range(3):
+        game.game_eval_sse(G.ctx, sse.data_ptr()); G.sync()
+        host = sse.cpu()
+        dist.all_reduce(host, op=dist.ReduceOp.SUM)
+        sse.copy_(host)
+        game.game_set_fitness_from_sse(G.ctx, sse.data_ptr(), cfg.P, None)
+        G.sync()
+        F = G.get_fitness()
+        F_ref = oracle.eval_fitness(cfg.d, cfg.family, X, t, W)
+        worst = max(worst, float(np.max(np.abs(F - F_ref) / F_ref)))
+        G.step(5, gen); G.sync()
+        W = oracle.step(W, F, cfg.elite, cfg.tournament, cfg.p_cross, cfg.p_mut, cfg.sigma, 5, gen)
+        ok = ok and np.array_equal(G.get_population().view(np.uint32), W.view(np.uint32))
+    pops = [torch.zeros(W.shape, dtype=torch.float32) for _ in range(world)]
+    dist.all_gather(pops, torch.from_numpy(G.get_population()))
+    if rank == 0:
+        json.dump({"lockstep": bool(ok), "same_pop": all(torch.equal(p_, pops[0]) for p_ in pops), "max_rel": worst}, open(out, "w"))
+    G.close()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_library_sharded_generations_two_processes_one_gpu(tmp_path):
+    out = str(tmp_path / "ls.json")
+    mp.spawn(_lib_shard_worker, args=(2, 29536, out), nprocs=2, join=True)
+    r = json.load(open(out))
+    assert r["lockstep"] and r["same_pop"] and r["max_rel"] <= 1e-5
