@@ -83,7 +83,7 @@ constexpr int kSmemBytes = kSmemBar + kBarBytes + kTsBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
 constexpr int kStallSlots = 16;                // diagnostic slots per CTA (Params::stall)
 #ifndef GAME_POLY_PAIRS
-#define GAME_POLY_PAIRS 1
+#define GAME_POLY_PAIRS 0
 #endif
 constexpr int kPolyPairs = GAME_POLY_PAIRS;    // of every four packed pairs of the epilogue, how many take 2^s from the FMA pipe
 static_assert(kSmemBytes <= 232448, "shared memory budget");
@@ -379,6 +379,10 @@ __device__ __forceinline__ int row_scale_exp(float amax) {
     const int k = kRowTargetExp - ilogbf(amax);
     return max(-100, min(100, k));
 }
+// The same from the largest |gene| taken as an unsigned integer maximum of the fp32 bit patterns (order-preserving for
+// non-negative floats; one redux.sync per warp): a NaN gene has the largest pattern of all and leaves the row unscaled.
+__device__ __forceinline__ uint32_t abs_bits(float v) { return __float_as_uint(v) & 0x7fffffffu; }
+__device__ __forceinline__ int row_scale_exp_bits(uint32_t amax_bits) { return row_scale_exp(__uint_as_float(amax_bits)); }
 // the factor the epilogue applies to the accumulated z of such a row: 2^-k / kPhiScale
 __device__ __forceinline__ float row_unscale(int k) { return ldexpf(1.0f, -k - kPhiScaleLog2); }
 __device__ __forceinline__ float row_scale_of_unscale(float f) { return 1.0f / (f * kPhiScale); }   // 2^k back from 2^-k / 16: exact
@@ -389,12 +393,11 @@ __global__ void row_scale_kernel(const float* W, float* wscale, int M, int G, in
     pdl_launch_dependents();
     const int m = static_cast<int>((static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (m >= m_stride) return;
-    float amax = 0.0f;
+    uint32_t amax = 0u;
     if (m < M)
-        for (int g = 1 + lane; g < G; g += 32) amax = fmaxf(amax, fabsf(__ldcg(W + static_cast<size_t>(m) * G + g)));
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-    if (lane == 0) wscale[m] = row_unscale(row_scale_exp(amax));
+        for (int g = 1 + lane; g < G; g += 32) amax = max(amax, abs_bits(__ldcg(W + static_cast<size_t>(m) * G + g)));
+    amax = __reduce_max_sync(0xffffffffu, amax);
+    if (lane == 0) wscale[m] = row_unscale(row_scale_exp_bits(amax));
 }
 
 // W [M][G] fp32 -> per (m_tile, step) 8 KB images: A_hi then A_lo, each [2 k-groups][128 rows][8 fp16].
@@ -1041,7 +1044,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(leader_acc_empty + 8);
                 }
-                mbar_wait_spin_then_sleep<32, 128>(bar_acc_full + 8 * buf, (buf ? uses1 : uses0) & 1);   // (complete already if chunks were merged)
+                // Short tiles (mid-size shapes): the epilogue is the slower side, the accumulator is usually there already and a
+                // nap would only add hand-off time.  Long tiles (tensor-bound shapes): the epilogue idles for most of a tile;
+                // sleep through part of that slack first and poll rarely, so that the wait executes next to nothing (polling
+                // at the short-tile rate was +1.0 G warp instructions and -4 % tensor-pipe activity at c3 under the power cap).
+                mbar_wait_spin_then_sleep<32, 128>(bar_acc_full + 8 * buf, (buf ? uses1 : uses0) & 1);
                 if (buf) ++uses1; else ++uses0;
                 tc_fence_after();
                 float sum = 0.0f, sum1 = 0.0f, sum2 = 0.0f, sum3 = 0.0f;
@@ -1131,6 +1138,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const bool vec4 = (prm.N & 3) == 0;       // rows are 16-byte aligned (X itself is: game_load_kb checks)
             const int last_blk = (prm.N - 1) >> 2, last_i = prm.N - 1;
             auto fetch4 = [&](const float* row, int b) {
+#ifdef GAME_X_NOLOAD   // measurement build only (wrong results): what the producers would cost if x cost nothing to fetch
+                return make_float4(0.1f * static_cast<float>(b & 7), 0.3f, -0.2f, 0.05f * static_cast<float>(reinterpret_cast<uintptr_t>(row) & 15));
+#endif
                 b = min(b, last_blk);
                 if (vec4) return __ldg(reinterpret_cast<const float4*>(row) + b);
                 const int i0 = 4 * b;

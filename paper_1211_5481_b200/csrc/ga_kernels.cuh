@@ -167,30 +167,35 @@ __global__ void __launch_bounds__(1024) roulette_prefix_kernel(const float* F, i
 // grid starts (pdl.cuh): they are read with ld.global.cg after griddepcontrol.wait, never through the non-coherent path
 // (no __ldg, no const __restrict__: ld.global.nc requires data that is read-only for the kernel's whole lifetime).
 // The images hold every row times its own power-of-two scale (fitness_umma.cuh: the largest gene of the row lands in
-// [2^13, 2^14)), so a row's images are written in a second pass, once the block knows the row's largest gene.
+// [2^13, 2^14)), so a row's images are written in a second pass, once the block knows the row's largest gene.  `amax` is
+// the thread's maximum of abs_bits over the genes >= 1 it wrote; a thread's first kGaRegGenes genes (g = tid + i * 128)
+// are handed over in registers, any further ones are re-read from `row` (the thread's own stores).  One barrier.
+constexpr int kGaRegGenes = 4;
 __device__ __forceinline__ void store_row_images(uint8_t* img, float* wscale, int img_steps, int m, const float* row, int G,
-                                                 float amax, float* s_red) {
+                                                 uint32_t amax, const float (&vreg)[kGaRegGenes], uint32_t* s_red) {
     const int tid = threadIdx.x;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-    __syncthreads();                                   // s_red may still be read from an earlier row of this block
+    amax = __reduce_max_sync(0xffffffffu, amax);
     if ((tid & 31) == 0) s_red[tid >> 5] = amax;
     __syncthreads();
     amax = s_red[0];
 #pragma unroll
-    for (int w = 1; w < kGaThreads / 32; ++w) amax = fmaxf(amax, s_red[w]);
-    const int k = umma::row_scale_exp(amax);
+    for (int w = 1; w < kGaThreads / 32; ++w) amax = max(amax, s_red[w]);
+    const int k = umma::row_scale_exp_bits(amax);
     const float scale = ldexpf(1.0f, k);
     if (tid == 0) wscale[m] = umma::row_unscale(k);
-    // every thread re-reads the genes it wrote itself (same thread, same address: no synchronisation needed)
-    for (int g = 1 + tid; g < G; g += kGaThreads) umma::store_w_image_gene(img, img_steps, m, g, row[g] * scale);
+#pragma unroll
+    for (int i = 0; i < kGaRegGenes; ++i) {
+        const int g = tid + i * kGaThreads;
+        if (g >= 1 && g < G) umma::store_w_image_gene(img, img_steps, m, g, vreg[i] * scale);
+    }
+    for (int g = tid + kGaRegGenes * kGaThreads; g < G; g += kGaThreads) umma::store_w_image_gene(img, img_steps, m, g, row[g] * scale);
 }
 
 __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, const float* F, float* Wn, GaParams p,
                                                               const int* stop, uint8_t* img, float* wscale, int img_steps,
                                                               const RunState* run) {
     __shared__ int s_warp_cnt[kGaThreads / 32];
-    __shared__ float s_red[kGaThreads / 32];
+    __shared__ uint32_t s_red_elite[kGaThreads / 32], s_red_child[kGaThreads / 32];   // one per use: no barrier between them
     __shared__ int s_rank;
     __shared__ int s_parent[2];
     __shared__ int s_cut;
@@ -227,26 +232,30 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
     if (rank < p.elite) {
         const float* src = W + static_cast<size_t>(c) * G;
         float* dst = Wn + static_cast<size_t>(rank) * G;
-        float amax = 0.0f;
-        for (int g = tid; g < G; g += kGaThreads) {
+        uint32_t amax = 0u;
+        float vreg[kGaRegGenes] = {0.f, 0.f, 0.f, 0.f};
+        for (int g = tid, i = 0; g < G; g += kGaThreads, ++i) {
             const float v = __ldcg(src + g);
             dst[g] = v;
-            if (g >= 1) amax = fmaxf(amax, fabsf(v));
+            if (i < kGaRegGenes) vreg[i] = v;
+            if (g >= 1) amax = max(amax, umma::abs_bits(v));
         }
-        if (img != nullptr) store_row_images(img, wscale, img_steps, rank, dst, G, amax, s_red);
+        if (img != nullptr) store_row_images(img, wscale, img_steps, rank, dst, G, amax, vreg, s_red_elite);
     }
     if (c < p.elite) return;  // slots 0..elite-1 are written by the elites themselves
     if (c >= M - p.immigrants) {
         // random replacement: genes uniform in [-1,1) as at initialisation, tag IMMIGRANT
         float* fresh = Wn + static_cast<size_t>(c) * G;
-        float amax = 0.0f;
-        for (int g = tid; g < G; g += kGaThreads) {
+        uint32_t amax = 0u;
+        float vreg[kGaRegGenes] = {0.f, 0.f, 0.f, 0.f};
+        for (int g = tid, i = 0; g < G; g += kGaThreads, ++i) {
             const uint4 r = philox4x32_10(static_cast<uint32_t>(g >> 2), static_cast<uint32_t>(c), p.gen, kTagImmigrant, p.key);
             const float v = gene_from_word(word_of(r, g & 3));
             fresh[g] = v;
-            if (g >= 1) amax = fmaxf(amax, fabsf(v));
+            if (i < kGaRegGenes) vreg[i] = v;
+            if (g >= 1) amax = max(amax, umma::abs_bits(v));
         }
-        if (img != nullptr) store_row_images(img, wscale, img_steps, c, fresh, G, amax, s_red);
+        if (img != nullptr) store_row_images(img, wscale, img_steps, c, fresh, G, amax, vreg, s_red_child);
         return;
     }
 
@@ -294,8 +303,9 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
     const int q = s_cut;
     float* child = Wn + static_cast<size_t>(c) * G;
     // per-gene Gaussian mutation, no clamping (D6)
-    float amax = 0.0f;
-    for (int g = tid; g < G; g += kGaThreads) {
+    uint32_t amax = 0u;
+    float vreg[kGaRegGenes] = {0.f, 0.f, 0.f, 0.f};
+    auto gene = [&](int g) {
         float v = __ldcg(g < q ? A + g : B + g);
         const uint4 rm = philox4x32_10(static_cast<uint32_t>(g), static_cast<uint32_t>(c), p.gen, kTagMutate, p.key);
         if (static_cast<unsigned long long>(rm.x) < p.t_mut) {
@@ -303,9 +313,16 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
             v = __fadd_rn(v, __fmul_rn(p.sigma, z));
         }
         child[g] = v;
-        if (g >= 1) amax = fmaxf(amax, fabsf(v));
+        if (g >= 1) amax = max(amax, umma::abs_bits(v));
+        return v;
+    };
+#pragma unroll
+    for (int i = 0; i < kGaRegGenes; ++i) {
+        const int g = tid + i * kGaThreads;
+        if (g < G) vreg[i] = gene(g);
     }
-    if (img != nullptr) store_row_images(img, wscale, img_steps, c, child, G, amax, s_red);
+    for (int g = tid + kGaRegGenes * kGaThreads; g < G; g += kGaThreads) gene(g);
+    if (img != nullptr) store_row_images(img, wscale, img_steps, c, child, G, amax, vreg, s_red_child);
 }
 
 // ---- fitness finalisation: F[m] = (sum over partial rows, in row order) / P in fp64, rounded to fp32

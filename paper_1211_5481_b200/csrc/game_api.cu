@@ -69,6 +69,7 @@ struct game_ctx {
     game::RunState* run = nullptr;                   // device run state, non-null only inside a graph-replayed generation loop
     // generation loop as a CUDA graph (run_generations): kGraphGens generations captured once, replayed
     cudaGraphExec_t graph_exec = nullptr;
+    cudaStream_t capture_stream = nullptr;           // capture needs a real stream: used when the context runs on the NULL stream
     unsigned long long graph_epoch = ~0ull;          // config_epoch the graph was captured under
     int graph_cur = -1;                              // population buffer that was current at capture
     unsigned long long graph_nodes = 0;              // kernel launches per replay
@@ -601,14 +602,27 @@ int ensure_graph(game_ctx* c) {
     }
     const unsigned long long launches0 = c->launches;
     cudaGraph_t graph = nullptr;
+    // The legacy default stream (what torch hands out as its current stream) cannot capture: record the chain on a stream of
+    // the library's own -- nothing executes during capture -- and replay the graph on the context's stream as usual.
+    cudaStream_t run_stream = c->stream;
+    if (run_stream == nullptr || run_stream == cudaStreamLegacy || run_stream == cudaStreamPerThread) {
+        if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            cudaGetLastError();
+            c->graph_ok = false;
+            return GAME_OK;
+        }
+        c->stream = c->capture_stream;
+    }
     if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
         cudaGetLastError();
+        c->stream = run_stream;
         c->graph_ok = false;
         return GAME_OK;
     }
     int rc = GAME_OK;
     for (uint32_t i = 0; i < kGraphGens && rc == GAME_OK; ++i) rc = plain_generation(c);
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    c->stream = run_stream;
     c->graph_nodes = c->launches - launches0;
     c->launches = launches0;                      // nothing has run yet
     if (rc != GAME_OK || e != cudaSuccess || graph == nullptr) {
@@ -736,6 +750,7 @@ int game_destroy(game_ctx* c) {
         cudaEventDestroy(ev.second);
     }
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     if (c->nccl_comm && nccl().ok) nccl().CommDestroy(c->nccl_comm);
     for (auto& e : c->copy_events) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
