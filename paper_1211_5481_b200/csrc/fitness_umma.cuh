@@ -458,11 +458,10 @@ __device__ __forceinline__ void store_w_image_gene(uint8_t* img, int steps, int 
 // So for the regression activations (identity, tanh) the shrink of every chromosome row is MEASURED before each
 // evaluation: one extra launch of the fitness kernel hands out the raw accumulators of the first pattern tile
 // (Params::zdump), cal_phi_kernel + calibrate_kernel recompute the same z for those <= 256 patterns on the CUDA cores (fp32
-// expansion as in the producers, products and sum in fp64) and fits z_exact = (1 + eps_m) z_tensor by least squares; the evaluation then runs
+// expansion as in the producers, products and sums in fp64) and fits z_exact = (1 + eps_m) z_tensor by least squares; the evaluation then runs
 // with the row's un-scaling factor times (1 + eps_m).
 constexpr int kCalThreads = kBN;         // one thread per sample pattern
-constexpr int kCalRows = 8;              // chromosome rows per block of calibrate_kernel (fewer when G is long)
-constexpr int kCalUnroll = 16;           // phi loads in flight per thread
+constexpr int kCalUnroll = 16;           // K padding of the staged rows
 
 // phi of the <= 256 sample patterns (the first pattern tile), as the producers generate it (fp32 recurrences), widened to
 // fp64 once: phi_s[(g - 1) * 256 + p] for genes g = 1..G-1.  One thread per pattern.
@@ -477,7 +476,8 @@ __global__ void __launch_bounds__(kCalThreads) cal_phi_kernel(const float* __res
     const float* xr = X + static_cast<size_t>(p < P ? p : 0) * N;
     if (shared)
         for (int jj = 0; jj < dd; ++jj) phi_s[static_cast<size_t>(jj) * kBN + p] = 0.0;
-    // per-feature coefficients: one block per feature; shared coefficients: one block adds up all features
+    // per-feature coefficients: one block per feature; shared coefficients: one block adds up all features (in the
+    // producers' order, so that the sums round alike)
     const int i_begin = shared ? 0 : blockIdx.x, i_end = shared ? N : blockIdx.x + 1;
     for (int i = i_begin; i < i_end; ++i) {
         const float x = __ldg(xr + i);
@@ -492,11 +492,11 @@ __global__ void __launch_bounds__(kCalThreads) cal_phi_kernel(const float* __res
         }
         for (int k = 0; k < d; ++k) {
             if (shared) {
-                out[static_cast<size_t>(k) * kBN] += static_cast<double>(cc);
-                if (EXPANSION == 1) out[static_cast<size_t>(d + k) * kBN] += static_cast<double>(sc);
+                out[static_cast<size_t>(k) * kBN] += cc;
+                if (EXPANSION == 1) out[static_cast<size_t>(d + k) * kBN] += sc;
             } else {
-                out[static_cast<size_t>(k) * kBN] = static_cast<double>(cc);
-                if (EXPANSION == 1) out[static_cast<size_t>(d + k) * kBN] = static_cast<double>(sc);
+                out[static_cast<size_t>(k) * kBN] = cc;
+                if (EXPANSION == 1) out[static_cast<size_t>(d + k) * kBN] = sc;
             }
             const float cn = fmaf(x2, cc, -cm);
             cm = cc; cc = cn;
@@ -509,67 +509,84 @@ __global__ void __launch_bounds__(kCalThreads) cal_phi_kernel(const float* __res
 }
 
 // zcorr[m] = wscale[m] (1 + eps_m), eps_m from the least-squares fit z_exact = (1 + eps_m) z_tensor over the sample
-// patterns.  A block takes `rows` consecutive chromosomes (their genes staged in shared memory as fp64) and all sample
-// patterns (one per thread): a small fp64 contraction, phi_s streamed once per block.
+// patterns.  z_exact = W phi_s is a small fp64 contraction, [M] x [G-1] x [256]: it runs on the fp64 TENSOR path
+// (mma.sync m8n8k4 f64), the one fast fp64 unit of this chip -- with scalar DFMA this kernel took 40 us at c2, in
+// float-float arithmetic on the FP32 pipe 64 us, against 655 us for the evaluation it calibrates.  A block takes 8
+// chromosome rows (genes staged in shared memory as fp64) and all 256 sample patterns, 32 per warp (four 8 x 8 tiles).
+constexpr int kCalRows = 8;              // chromosome rows per block = the M of the fp64 MMA
+__device__ __forceinline__ void dmma_m8n8k4(double (&acc)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(acc[0]), "+d"(acc[1])
+                 : "d"(a), "d"(b));
+}
 __global__ void __launch_bounds__(kCalThreads) calibrate_kernel(const float* W, const double* phi_s, const float* zdump,
                                                                 const float* wscale, float* zcorr, const int* stop, long long P,
-                                                                int M, int G, int m_stride, int rows) {
-    extern __shared__ double cal_w[];      // [rows][Kp]: the rows' genes 1..G-1 in fp64, zero-padded to a multiple of kCalUnroll
+                                                                int M, int G, int m_stride) {
+    extern __shared__ double cal_w[];      // [kCalRows][Kp]: the rows' genes 1..G-1 in fp64, zero-padded to a multiple of 16
     __shared__ double s_num[kCalRows][kCalThreads / 32], s_den[kCalRows][kCalThreads / 32];
     pdl_wait();                // the calibration launch's accumulators, phi_s, W and the row scales are complete
     pdl_launch_dependents();
     if (stop != nullptr && __ldcg(stop) != 0) return;
-    const int m0 = blockIdx.x * rows, p = threadIdx.x, K = G - 1;
-    const int Kp = (K + kCalUnroll - 1) / kCalUnroll * kCalUnroll;
-    for (int r = 0; r < rows; ++r) {
-        const int m = m0 + r;
-        for (int g = p; g < Kp; g += kCalThreads)
-            cal_w[static_cast<size_t>(r) * Kp + g] =
-                (m < M && g < K) ? static_cast<double>(__ldcg(W + static_cast<size_t>(m) * G + 1 + g)) : 0.0;
-    }
-    __syncthreads();
-    const int n = static_cast<int>(min(static_cast<long long>(kBN), P));
-    double z[kCalRows];
-#pragma unroll
-    for (int r = 0; r < kCalRows; ++r) z[r] = 0.0;
-    if (p < n) {
-        // kCalUnroll loads of phi in flight at a time: one block per SM cannot hide an L2 round trip per gene otherwise
-        for (int g0 = 0; g0 < Kp; g0 += kCalUnroll) {
-            double ph[kCalUnroll];
-#pragma unroll
-            for (int u = 0; u < kCalUnroll; ++u) ph[u] = g0 + u < K ? __ldcg(phi_s + static_cast<size_t>(g0 + u) * kBN + p) : 0.0;
-#pragma unroll
-            for (int u = 0; u < kCalUnroll; ++u)
-#pragma unroll
-                for (int r = 0; r < kCalRows; ++r)
-                    if (r < rows) z[r] = fma(cal_w[static_cast<size_t>(r) * Kp + g0 + u], ph[u], z[r]);
-        }
-    }
-#pragma unroll
+    const int m0 = blockIdx.x * kCalRows, tid = threadIdx.x, lane = tid & 31, wv = tid >> 5, K = G - 1;
+    const int Kp = (K + 15) / 16 * 16;
     for (int r = 0; r < kCalRows; ++r) {
-        if (r >= rows) break;
         const int m = m0 + r;
-        double num = 0.0, den = 0.0;
-        if (p < n && m < m_stride) {
-            const double zt = static_cast<double>(__ldcg(zdump + static_cast<size_t>(m) * kBN + p)) * static_cast<double>(__ldcg(wscale + m));
-            num = (z[r] - zt) * zt;
-            den = zt * zt;
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            num += __shfl_xor_sync(0xffffffffu, num, o);
-            den += __shfl_xor_sync(0xffffffffu, den, o);
-        }
-        if ((p & 31) == 0) { s_num[r][p >> 5] = num; s_den[r][p >> 5] = den; }
+        for (int g = tid; g < Kp; g += kCalThreads)
+            cal_w[static_cast<size_t>(r) * Kp + g] = (m < M && g < K) ? static_cast<double>(__ldcg(W + static_cast<size_t>(m) * G + 1 + g)) : 0.0;
     }
     __syncthreads();
-    if (p < rows && m0 + p < m_stride) {
-        const int m = m0 + p;
-        double num = 0.0, den = 0.0;
-        for (int wv = 0; wv < kCalThreads / 32; ++wv) { num += s_num[p][wv]; den += s_den[p][wv]; }   // fixed order: bit-stable
+    // fragments of mma.m8n8k4: A (8 x 4, row-major) thread -> (row lane / 4, k lane % 4); B (4 x 8) thread -> (k lane % 4,
+    // column lane / 4); C (8 x 8) thread -> row lane / 4, columns 2 (lane % 4) + {0, 1}
+    const int fr = lane >> 2, fk = lane & 3;
+    double acc[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    const double* bcol = phi_s + wv * 32 + fr;                     // + k * 256 + 8 j
+    const double* arow = cal_w + static_cast<size_t>(fr) * Kp + fk;
+    // every block reads the same phi_s: start each block at another K offset, so that they are not all after the same L2
+    // lines at the same time (the order of a row's sum still only depends on the row)
+    const int k_first = static_cast<int>((static_cast<unsigned>(blockIdx.x) * 16u) % static_cast<unsigned>(Kp));
+    for (int it = 0, k0 = k_first; it < Kp; it += 16, k0 = k0 + 16 < Kp ? k0 + 16 : 0) {
+        double a[4], b[4][4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {                               // 16 loads of phi in flight per thread
+            const int k = k0 + 4 * u + fk;
+            a[u] = arow[k0 + 4 * u];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[u][j] = k < K ? __ldcg(bcol + static_cast<size_t>(k) * kBN + 8 * j) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dmma_m8n8k4(acc[j], a[u], b[u][j]);
+    }
+    // least squares per row over this warp's 32 patterns, then over the warps (fixed order: bit-stable)
+    const int n = static_cast<int>(min(static_cast<long long>(kBN), P));
+    const int m = m0 + fr;
+    double num = 0.0, den = 0.0;
+    if (m < m_stride) {
+        const double f = static_cast<double>(__ldcg(wscale + m));
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int p = wv * 32 + 8 * j + 2 * fk + i;
+                if (p < n) {
+                    const double zt = static_cast<double>(__ldcg(zdump + static_cast<size_t>(m) * kBN + p)) * f;
+                    num += (acc[j][i] - zt) * zt;
+                    den += zt * zt;
+                }
+            }
+    }
+    num += __shfl_xor_sync(0xffffffffu, num, 1); den += __shfl_xor_sync(0xffffffffu, den, 1);
+    num += __shfl_xor_sync(0xffffffffu, num, 2); den += __shfl_xor_sync(0xffffffffu, den, 2);
+    if (fk == 0) { s_num[fr][wv] = num; s_den[fr][wv] = den; }
+    __syncthreads();
+    if (tid < kCalRows && m0 + tid < m_stride) {
+        const int mm = m0 + tid;
+        num = 0.0; den = 0.0;
+        for (int w = 0; w < kCalThreads / 32; ++w) { num += s_num[tid][w]; den += s_den[tid][w]; }
         double eps = den > 0.0 ? num / den : 0.0;
-        if (!(fabs(eps) <= 1e-4) || m >= M) eps = 0.0;   // non-finite rows, or a row the model does not describe: leave it alone
-        zcorr[m] = static_cast<float>(static_cast<double>(__ldcg(wscale + m)) * (1.0 + eps));
+        if (!(fabs(eps) <= 1e-4) || mm >= M) eps = 0.0;   // non-finite rows, or a row the model does not describe: leave it alone
+        zcorr[mm] = static_cast<float>(static_cast<double>(__ldcg(wscale + mm)) * (1.0 + eps));
     }
 }
 

@@ -259,43 +259,59 @@ __global__ void __launch_bounds__(kGaThreads) ga_step_kernel(const float* W, con
         return;
     }
 
-    // (2) tournaments: entrants 0..k-1 -> parent A, k..2k-1 -> parent B (with replacement)
-    if (tid == 0) {
+    // (2) tournaments: entrants 0..k-1 -> parent A, k..2k-1 -> parent B (with replacement).  The first warp draws the
+    // entrants in parallel (one per lane: a Philox block and a fitness load each, which one thread used to do one after
+    // the other) and takes the minimum of each side under the order -- a minimum, so the result is that of the sequential
+    // scan; lane 31 draws the crossover meanwhile.
+    if (tid < 32) {
         const int k = p.tournament;
-        int par[2] = {-1, -1};
+        float bkey[2] = {INFINITY, INFINITY};
+        int bidx[2] = {0x7fffffff, 0x7fffffff};
         if (p.selection == 0) {
-            float pkey[2] = {0.f, 0.f};
-            uint4 r = make_uint4(0, 0, 0, 0);
-            for (int e = 0; e < 2 * k; ++e) {
-                if ((e & 3) == 0)
-                    r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
+            for (int e = tid; e < 2 * k; e += 32) {
+                const uint4 r = philox4x32_10(static_cast<uint32_t>(e >> 2), static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
                 const int idx = static_cast<int>(index_below(word_of(r, e & 3), static_cast<uint32_t>(M)));
                 const float ki = fit_key(err_view(__ldcg(F + idx), p.maximize));
                 const int side = e < k ? 0 : 1;
-                if (par[side] < 0 || precedes(ki, idx, pkey[side], par[side])) {
-                    par[side] = idx;
-                    pkey[side] = ki;
+                if (precedes(ki, idx, bkey[side], bidx[side])) {
+                    bkey[side] = ki;
+                    bidx[side] = idx;
                 }
             }
-        } else {
+#pragma unroll
+            for (int side = 0; side < 2; ++side)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const float ok = __shfl_xor_sync(0xffffffffu, bkey[side], o);
+                    const int oi = __shfl_xor_sync(0xffffffffu, bidx[side], o);
+                    if (precedes(ok, oi, bkey[side], bidx[side])) {
+                        bkey[side] = ok;
+                        bidx[side] = oi;
+                    }
+                }
+        } else if (tid == 0) {
             // ranking / roulette: parents A and B from words 0 and 1 of one SELECT draw
             const uint4 r = philox4x32_10(0u, static_cast<uint32_t>(c), p.gen, kTagSelect, p.key);
             if (p.selection == 1) {
-                par[0] = p.by_rank[rank_from_word(r.x, M)];
-                par[1] = p.by_rank[rank_from_word(r.y, M)];
+                bidx[0] = p.by_rank[rank_from_word(r.x, M)];
+                bidx[1] = p.by_rank[rank_from_word(r.y, M)];
             } else {
-                par[0] = roulette_from_word(r.x, M, p.prefix);
-                par[1] = roulette_from_word(r.y, M, p.prefix);
+                bidx[0] = roulette_from_word(r.x, M, p.prefix);
+                bidx[1] = roulette_from_word(r.y, M, p.prefix);
             }
         }
-        s_parent[0] = par[0];
-        s_parent[1] = par[1];
-        // single-point crossover: child = A[0:q] ++ B[q:G], q in [1, G-1]; otherwise child = A
-        const uint4 rc = philox4x32_10(0u, static_cast<uint32_t>(c), p.gen, kTagCross, p.key);
-        int q = G;
-        if (static_cast<unsigned long long>(rc.x) < p.t_cross && G >= 2)
-            q = 1 + static_cast<int>(index_below(rc.y, static_cast<uint32_t>(G - 1)));
-        s_cut = q;
+        if (tid == 0) {
+            s_parent[0] = bidx[0];
+            s_parent[1] = bidx[1];
+        }
+        if (tid == 31) {
+            // single-point crossover: child = A[0:q] ++ B[q:G], q in [1, G-1]; otherwise child = A
+            const uint4 rc = philox4x32_10(0u, static_cast<uint32_t>(c), p.gen, kTagCross, p.key);
+            int q = G;
+            if (static_cast<unsigned long long>(rc.x) < p.t_cross && G >= 2)
+                q = 1 + static_cast<int>(index_below(rc.y, static_cast<uint32_t>(G - 1)));
+            s_cut = q;
+        }
     }
     __syncthreads();
     const float* A = W + static_cast<size_t>(s_parent[0]) * G;
@@ -351,22 +367,38 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
     float key = INFINITY;
     int idx = 0x7fffffff;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
-    // a partial row holds fp64 sums (FFMA kernel) or float-float pairs hi + lo in the same 8 bytes (tensor-core kernel)
-    auto slot = [&](int row) {
-        const double* a = part + static_cast<size_t>(row) * m_stride + m;
-        if (!part_ff) return __ldcg(a);
-        const float2 v = __ldcg(reinterpret_cast<const float2*>(a));
-        return static_cast<double>(v.x) + static_cast<double>(v.y);
-    };
-    if (m < M) {
+    if (m < M && !part_ff) {          // FFMA kernel: a partial row holds fp64 sums
         int r = grp;
         for (; r + 3 * kFinGroups < n_part; r += 4 * kFinGroups) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) acc[i] += slot(r + i * kFinGroups);
+            for (int i = 0; i < 4; ++i) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
         }
 #pragma unroll
         for (int i = 0; i < 3; ++i)      // the tail: at most three rows, same accumulator per position as above
-            if (r + i * kFinGroups < n_part) acc[i] += slot(r + i * kFinGroups);
+            if (r + i * kFinGroups < n_part) acc[i] += __ldcg(part + static_cast<size_t>(r + i * kFinGroups) * m_stride + m);
+    } else if (m < M) {
+        // tensor-core kernel: float-float pairs (hi, lo) in the same 8 bytes.  They are added in float-float arithmetic
+        // too (error-free TwoSum of the hi parts, the lo parts and the errors in a second fp32 sum) and widened to fp64
+        // once per accumulator: an fp64 add per row made this kernel 4 us slower (fp64 is a slow pipe on this chip).
+        float ah[4] = {0.f, 0.f, 0.f, 0.f}, al[4] = {0.f, 0.f, 0.f, 0.f};
+        auto add = [&](int i, int row) {
+            const float2 v = __ldcg(reinterpret_cast<const float2*>(part + static_cast<size_t>(row) * m_stride + m));
+            const float hi = __fadd_rn(ah[i], v.x);
+            const float bv = __fadd_rn(hi, -ah[i]);
+            const float er = __fadd_rn(__fadd_rn(ah[i], -__fadd_rn(hi, -bv)), __fadd_rn(v.x, -bv));
+            ah[i] = hi;
+            al[i] = __fadd_rn(al[i], __fadd_rn(v.y, er));
+        };
+        int r = grp;
+        for (; r + 3 * kFinGroups < n_part; r += 4 * kFinGroups) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) add(i, r + i * kFinGroups);
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+            if (r + i * kFinGroups < n_part) add(i, r + i * kFinGroups);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[i] = static_cast<double>(ah[i]) + static_cast<double>(al[i]);
     }
     s_grp[grp][col] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
     __syncthreads();
@@ -385,10 +417,6 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         }
     }
     if (sse_out != nullptr) return;
-    if (run != nullptr) {                          // graph replay: the trace slot comes from the device-side generation count
-        float* base = reinterpret_cast<float*>(__ldcg(reinterpret_cast<unsigned long long*>(&run->best)));
-        best_out = base != nullptr ? base + __ldcg(&run->evals) : nullptr;
-    }
     if (best_out == nullptr && run == nullptr) return;
     __threadfence();  // F[m] visible device-wide before this block takes its ticket
     auto warp_min = [](float& k, int& i) {
@@ -437,8 +465,13 @@ __global__ void __launch_bounds__(kFinThreads) finalize_fitness_kernel(const dou
         warp_min(key, idx);
         if (threadIdx.x == 0) {
             const float best = __ldcg(F + idx);  // the fitness itself (NaN if every chromosome is NaN: idx = 0)
+            if (run != nullptr) {                // graph replay: the trace slot comes from the device-side generation count
+                const int evals = __ldcg(&run->evals);
+                float* base = reinterpret_cast<float*>(__ldcg(reinterpret_cast<unsigned long long*>(&run->best)));
+                best_out = base != nullptr ? base + evals : nullptr;
+                run->evals = evals + 1;          // nobody reads it until the next kernel of the chain
+            }
             if (best_out != nullptr) *best_out = best;
-            if (run != nullptr) run->evals = __ldcg(&run->evals) + 1;     // nobody reads it until the next kernel of the chain
             *ticket = 0u;
             if (stop != nullptr) {
                 stop[1] = gen_index;                       // GA steps performed so far

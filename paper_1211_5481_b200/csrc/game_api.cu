@@ -267,6 +267,7 @@ void setup_umma(game_ctx* c, game::umma::Params& prm, UmmaGeo& geo) {
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_tpu = tpu; }
     }
     prm.m_pairs_per_group = best_tpu;
+    if (const char* e = std::getenv("GAME_TPU")) { const int v = std::atoi(e); if (v >= 1 && v <= geo.m_pairs) prm.m_pairs_per_group = v; }   // A/B override
     prm.m_groups = (geo.m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
     prm.dd = c->expansion == GAME_EXP_CHEBYSHEV ? c->d : 2 * c->d;
     prm.shared = c->shared;
@@ -306,7 +307,7 @@ int launch_umma(game_ctx* c, const game::umma::Params& prm, int grid, bool pdl) 
 
 bool wants_calibration(const game_ctx* c) {
     return c->calibrate && c->act != GAME_ACT_SIGMOID &&
-           sizeof(double) * (static_cast<size_t>(c->G) + game::umma::kCalUnroll) <= kCalMaxSmem;
+           sizeof(double) * game::umma::kCalRows * (static_cast<size_t>(c->G) + 16) <= kCalMaxSmem;
 }
 
 // Regression activations: measure every row's accumulation shrink on the first pattern tile (fitness_umma.cuh, "calibration")
@@ -331,11 +332,9 @@ int launch_calibration(game_ctx* c, game::umma::Params& prm, const UmmaGeo& geo,
         launch_chain(pdl, umma::cal_phi_kernel<1>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, X0, phi_s,
                      c->stop, c->P, c->N, c->d, c->shared);
     if ((rc = check_launch(c, "cal_phi_kernel"))) return rc;
-    const size_t row_bytes = sizeof(double) * ((static_cast<size_t>(c->G - 1) + umma::kCalUnroll - 1) / umma::kCalUnroll * umma::kCalUnroll);
-    int rows = static_cast<int>(kCalMaxSmem / (row_bytes ? row_bytes : 1));
-    rows = rows > umma::kCalRows ? umma::kCalRows : (rows < 1 ? 1 : rows);
-    launch_chain(pdl, umma::calibrate_kernel, dim3((c->m_stride + rows - 1) / rows), dim3(umma::kCalThreads), rows * row_bytes,
-                 c->stream, prm.W, phi_s, zdump, wscale, zcorr, c->stop, c->P, c->M, c->G, c->m_stride, rows);
+    const size_t row_bytes = sizeof(double) * ((static_cast<size_t>(c->G - 1) + 15) / 16 * 16);
+    launch_chain(pdl, umma::calibrate_kernel, dim3((c->m_stride + umma::kCalRows - 1) / umma::kCalRows), dim3(umma::kCalThreads),
+                 umma::kCalRows * row_bytes, c->stream, prm.W, phi_s, zdump, wscale, zcorr, c->stop, c->P, c->M, c->G, c->m_stride);
     if ((rc = check_launch(c, "calibrate_kernel"))) return rc;
     prm.wscale = zcorr;
     return GAME_OK;
