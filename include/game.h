@@ -67,10 +67,21 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *   F16X3    : tcgen05 tensor cores, fp32-recovering 2-term fp16 split of BOTH operands
  *              (v = hi + lo, hi = rn_f16(v), lo = rn_f16(v - hi)); three kind::f16 MMAs per K step
  *              (lo.hi, hi.lo, hi.hi; the lo.lo term, <= 2^-22 relative, is dropped), fp32 accumulation in TMEM.
- *              Precondition: |w| and |phi| < 65504 (fp16 range); phi is bounded by 1 for Chebyshev on
- *              |x| <= 1 and for trig; out-of-range values give Inf/NaN fitness, which the GA ranks worst.
- *              Accuracy: fitness within 1e-5 of fp64 (1e-7 .. 1e-6 measured for G <= 641); with IDENTITY activation
- *              and G > 2000 the fp32 accumulation over the long K extent reaches 1.0-1.4e-5.
+ *              Both operands are pre-scaled by exact powers of two, undone on the epilogue's FFMA: every chromosome row so
+ *              that its largest gene lands in [2^13, 2^14) (the split is then relative at ANY scale of the genes: 1e-8 and
+ *              300 behave alike), phi by 16.  Preconditions: finite genes (a row with an Inf / NaN gene gets a non-finite
+ *              fitness, which the GA ranks worst) and |phi| < 4094 (phi is bounded by 1 for Chebyshev on |x| <= 1 and for
+ *              trig).
+ *              Accuracy: fitness within 1e-5 of fp64 -- measured 6e-8 .. 1.4e-6 on the BASELINE shapes and on populations
+ *              around the optimum; see DESIGN.md section 2 for the table.  The tensor core adds into its accumulator with
+ *              truncation, which shrinks |z| by ~1.6e-8 per MMA; two measures keep that inside the bound where it would
+ *              not be: K extents beyond 320 genes are accumulated 20 K steps at a time and the chunks added in fp32
+ *              round-to-nearest (G = 2401, identity output: 2e-7), and for the regression activations (IDENTITY, TANH) the
+ *              shrink of every row is measured on the first 256 patterns against an fp64 contraction before each
+ *              evaluation and folded into the row's factor (one extra launch of the fused kernel + two small kernels per
+ *              evaluation; near-optimal regression with residual noise 0.01: 7.7e-6 / 8.7e-7 instead of 8.9e-5 / 8.9e-6;
+ *              GAME_CALIBRATE=0 in the environment at game_create turns it off; rows longer than 3184 genes are not
+ *              calibrated).
  *              Covers any N and d for Chebyshev, d <= 128 for the trigonometric family (the fp32 multiple-angle
  *              recurrence leaves the 1e-5 fitness bound beyond that: 2e-6 at d = 100, 2e-5 at d = 400).  The K axis
  *              is the gene order without the bias gene, 16 genes per K step; phi of a 256-pattern tile stays resident
@@ -78,8 +89,8 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *              d > 128 -> GAME_ERR_UNSUPPORTED when F16X3 is forced, FFMA under AUTO.  Shared coefficients
  *              (GAME_FAMILY_SHARED): covered for G - 1 <= 64 terms, FFMA beyond.
  *   FFMA covers G <= 448 (its shared-memory tile); forcing it on a larger G -> GAME_ERR_UNSUPPORTED.
- * Both schemes sum each tile's squared errors in fp32 and accumulate tile sums in fp64 in a fixed order
- * (run-to-run bit-stable; equal chromosomes get equal fitness in any slot). */
+ * Both schemes sum each tile's squared errors in fp32 and accumulate tile sums at ~48 bits or more (fp64, or float-float
+ * pairs) in a fixed order (run-to-run bit-stable; equal chromosomes get equal fitness in any slot). */
 enum { GAME_SCHEME_AUTO = 0, GAME_SCHEME_FFMA = 1, GAME_SCHEME_F16X3 = 2 };
 
 /* Create a context for a knowledge base of P patterns x N features, expansion degree d, population of
@@ -186,7 +197,9 @@ int game_step(game_ctx* ctx, uint64_t seed, uint32_t gen);
 
 /* n_gens x (eval, step with gen = gen0 + i) followed by a final eval, all on one stream with no host
  * synchronisation (PAPER.md:97, 170 future work (i)).  best_fitness_dev (device, [n_gens+1] float32, or
- * NULL) receives the best (lowest) fitness of each generation's population.  Async. */
+ * NULL) receives the best fitness of each generation's population (lowest; highest under GAME_ERROR_ONE_MINUS_MSE).  Seed,
+ * generation index and trace slot live in device memory, so runs of 16 or more generations are replayed from a CUDA graph
+ * captured once per configuration (GAME_GRAPH=0 in the environment at game_create: plain launches).  Async. */
 int game_run(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev);
 
 /* game_run with the paper's stop rule ("maximum number of iterations or the learning error threshold",
@@ -266,7 +279,9 @@ int game_evolve_sharded(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_
 
 /* Test / validation use case: outputs of ONE chromosome w_dev[G] (device; e.g. a row of the current
  * population) on Q patterns X_dev[Q][N] (device, any Q >= 1, independent of the bound knowledge base):
- * y_dev[q] = act(sum_g w[g] phi_g(x_q)), fp32.  Async. */
+ * y_dev[q] = act(sum_g w[g] phi_g(x_q)), computed in fp32 (recurrences and a G-term dot product): within 1e-5 of the fp64
+ * value relative to max(1, |y|).  Chromosomes of any accepted length (staged in shared memory up to 57 K genes, read through
+ * the caches beyond).  Async. */
 int game_predict(game_ctx* ctx, const float* w_dev, const float* X_dev, int64_t Q, float* y_dev);
 
 /* Confusion counts of thresholded outputs against 0/1 targets (PAPER.md:91, 140-146 classification quality):
