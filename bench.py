@@ -493,6 +493,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         W0 = oracle.init_population(cfg.M, cfg.G, seed)
         dt, _ = oracle_sample(cfg, X, t, W0, p_sample, seed, 0)
         cpu = {"value": p_sample * cfg.M / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "precision": "fp64, ONE thread, plain loops (the parity oracle as it stands; not a tuned or multi-core CPU baseline)",
                "host_cores_available": os.cpu_count(),
                "sample": f"one generation (oracle eval + GA step) on the first {p_sample} patterns x all {cfg.M} chromosomes of {cfg.name}"}
 

@@ -85,6 +85,10 @@ constexpr int kStallSlots = 16;                // diagnostic slots per CTA (Para
 #ifndef GAME_POLY_PAIRS
 #define GAME_POLY_PAIRS 0
 #endif
+#ifndef GAME_EARLY_PRODUCERS
+#define GAME_EARLY_PRODUCERS 1
+#endif
+constexpr bool kEarlyProducers = GAME_EARLY_PRODUCERS != 0;   // the phi producers start before griddepcontrol.wait (A/B switch)
 constexpr int kPolyPairs = GAME_POLY_PAIRS;    // of every four packed pairs of the epilogue, how many take 2^s from the FMA pipe
 static_assert(kSmemBytes <= 232448, "shared memory budget");
 // Operand pre-scaling (both powers of two, so exact, and undone by the epilogue's FFMA constant).  An fp16 hi/lo split is
@@ -129,6 +133,7 @@ struct Params {
     int resident;          // 1: phi generated once per unit and reused by all its chromosome tiles; n_b == stages, or
                            //    2 * stages (phi of the next unit is generated while this one is consumed)
     int n_a, n_b;          // A ring stages, B stages (n_a + n_b <= kStagesTotal)
+    int early;             // 1: the phi producers start their first work item before griddepcontrol.wait (small grids only, see below)
     int flush;             // 1 (streaming mode): accumulate kFlushStages stages at a time, chunk 0 into accumulator 0, the later
                            //    chunks into accumulator 1, which the epilogue adds to accumulator 0 (fp32, round to nearest)
 };
@@ -846,11 +851,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
 
     // Everything above (barriers, TMEM, the cluster handshake) touches no global memory and overlaps the tail of the
     // preceding kernel (pdl.cuh).  From here on the W images, W, the partial sums and the stop flag are complete.
-    pdl_wait();
-    pdl_launch_dependents();
-    GAME_PHASE(6);             // the preceding kernel has completed
-    const bool stopped = prm.stop != nullptr && __ldcg(prm.stop) != 0;   // uniform over the grid: written by an earlier kernel
-    if (stopped) units = 0;    // stop rule met: no work, no writes; fall through to the teardown (TMEM is allocated)
+    // The phi producers do not wait here: all they read is the knowledge base, which no kernel of the chain writes, and all
+    // they write is shared memory -- they generate their first work item while the preceding kernel is still running and
+    // wait afterwards (late_wait below; every thread of every kernel still passes griddepcontrol.wait before it exits).
+    // Only for grids that leave SMs free (Params::early): a grid that fills the chip squeezes the GA step it overlaps down to
+    // one block per SM, and its busy producers then cost that kernel more than they save here (c1: 48.7 -> 49.6 us per
+    // generation; c0, with 8 CTAs, 15.2 -> 13.6 us; the paper-shaped n1 22.5 -> 20.5 us).
+    const bool is_producer = kEarlyProducers && prm.early != 0 && warp >= 2 + kNumEpiWarps;
+    bool stopped = false;
+    if (!is_producer) {
+        pdl_wait();
+        pdl_launch_dependents();
+        GAME_PHASE(6);             // the preceding kernel has completed
+        stopped = prm.stop != nullptr && __ldcg(prm.stop) != 0;   // uniform over the grid: written by an earlier kernel
+        if (stopped) units = 0;    // stop rule met: no work, no writes; fall through to the teardown (TMEM is allocated)
+    }
 
     if (warp == 0) {
         // ============================================================== loader: W operand images -> A ring
@@ -1137,7 +1152,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
         const int n_items = (prm.steps + span - 1) / span;
         Ring rb;                                // ring position of the current fill's first stage
         uint32_t item = 0;                      // running item counter: item goes to set (item & 1)
+        // griddepcontrol.wait, late: after this thread's first work item, or before its second unit, or on the way out.
+        // Only then is the stop flag of game_run_until known: a stopped launch has filled at most one stage for nobody,
+        // which the teardown does not mind.
+        bool waited = false;
+        auto late_wait = [&]() {
+            if (waited) return;
+            waited = true;
+            pdl_wait();
+            pdl_launch_dependents();
+            if (prm.stop != nullptr && __ldcg(prm.stop) != 0) units = 0;
+        };
         for (int u = pair; u < units; u += n_pairs) {
+            if (u != pair) {
+                late_wait();
+                if (units == 0) break;
+            }
             const int pt = prm.p_tile0 + u / prm.m_groups, mg = u % prm.m_groups;
             const int mp0 = mg * prm.m_pairs_per_group;
             const int mp1 = min(mp0 + prm.m_pairs_per_group, m_pairs);
@@ -1343,10 +1373,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
                                 for (int e = prm.steps % kKS; e != 0 && e < kKS; ++e) mbar_arrive(bar_b_full + 8 * pos.i);
                         }
                     }
+                    late_wait();
+                    if (units == 0) break;
                 }
+                if (units == 0) break;
                 rb = rb.at(stages, n_b);
             }
         }
+        late_wait();
     }
 
     GAME_PHASE(7);             // the MMA warp has issued everything

@@ -286,6 +286,7 @@ void setup_umma(game_ctx* c, game::umma::Params& prm, UmmaGeo& geo) {
     prm.p_tile0 = 0; prm.p_tiles = geo.p_tiles_all; prm.zero_part = 1;
     const long long units = static_cast<long long>(geo.p_tiles_all) * prm.m_groups;
     geo.grid = 2 * static_cast<int>(units < geo.pair_cap ? units : geo.pair_cap);   // the same grid for every pattern range
+    prm.early = 2 * geo.grid <= c->num_sms ? 1 : 0;      // early-start producers only when at least half of the SMs stay free
     c->last_umma_grid = geo.grid;
 }
 

@@ -836,17 +836,18 @@ def test_random_shapes_fitness_and_step(game):
 def test_random_shapes_tensor_path_wide(game):
     """Seeded sweep of the tensor-core kernel over the corners the fixed cases do not reach together: shared and
     per-feature coefficients, degrees far beyond a K step, streaming K extents, M and P around the tile edges.  Fitness
-    within 1e-5 of the oracle (IDENTITY activation is kept to G <= 1200: DESIGN.md section 5, measured limit of the scheme)."""
+    within 1e-5 of the oracle for every activation up to G = 2401 (round 1 had to keep the identity output to G <= 1200: the
+    truncating TMEM accumulation; K-chunk flush + calibration close it)."""
     import torch
     rng = np.random.Generator(np.random.Philox(4096))
     done = 0
-    while done < 24:
+    while done < 32:
         expansion = int(rng.integers(0, 2)); act = int(rng.integers(0, 3)); shared = bool(rng.integers(0, 3) == 0)
         if shared:
             N = int(rng.integers(1, 20)); d = int(rng.integers(1, 33 if expansion else 65))
         else:
             N = int(rng.integers(1, 60)); d = int(rng.integers(1, 30 if expansion else 80))
-            while N * d * (2 if expansion else 1) > (1200 if act == 0 else 2000):
+            while N * d * (2 if expansion else 1) > 2400:
                 N = max(1, N // 2); d = max(1, d - 1)
         P = int(rng.choice([255, 256, 257, 700, 1500, 4000])) + int(rng.integers(0, 3))
         M = int(rng.choice([1, 2, 127, 128, 129, 255, 256, 257, 700, 1300])) + int(rng.integers(0, 2))
