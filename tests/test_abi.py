@@ -158,3 +158,37 @@ def test_shared_family_gene_counts(L):
     ctx = game.game_create(200, 11, 3, 23, game.family(game.EXP_CHEBYSHEV, game.ACT_SIGMOID, shared=True))
     assert game.game_num_genes(ctx) == 4
     game.game_destroy(ctx)
+
+
+def test_round2_entry_points_validate_arguments_without_a_device(L):
+    """The entry points added in round 2 (out-of-core evaluation, sharded loop, metric, diagnostics): argument and state
+    checks come before any device work, so they can be exercised here."""
+    ctx = game.game_create(100_000, 8, 4, 300, game.family(game.EXP_CHEBYSHEV, game.ACT_SIGMOID))
+    host = (C.c_float * 64)()
+    p = C.addressof(host)
+    p16 = (p + 15) & ~15
+    # streamed evaluation: null pointers, slot size not a multiple of 256, slot count out of range, unaligned ring
+    assert L.game_eval_fitness_streamed(ctx, None, p16, p16, p16, 512, 2) == game.ERR_INVALID_ARG
+    assert L.game_eval_fitness_streamed(ctx, p16, p16, p16, p16, 500, 2) == game.ERR_INVALID_ARG
+    assert L.game_eval_fitness_streamed(ctx, p16, p16, p16, p16, 512, 1) == game.ERR_INVALID_ARG
+    assert L.game_eval_fitness_streamed(ctx, p16, p16, p16, p16, 512, 9) == game.ERR_INVALID_ARG
+    assert L.game_eval_fitness_streamed(ctx, p16, p16, p16 + 4, p16, 512, 2) == game.ERR_INVALID_ARG
+    assert L.game_eval_fitness_streamed(ctx, p16, p16, p16, p16, 512, 2) == game.ERR_BAD_STATE          # before game_bind_state
+    # error metric: the paper's fitness 1 - MSE is accepted, anything else is not
+    for metric, rc in ((game.ERROR_MSE, game.OK), (game.ERROR_RMSE, game.OK), (game.ERROR_ONE_MINUS_MSE, game.OK), (3, game.ERR_INVALID_ARG),
+                       (-1, game.ERR_INVALID_ARG)):
+        assert L.game_set_error_metric(ctx, metric) == rc
+    # sharded loop: needs a communicator; the communicator needs bound buffers (their device)
+    assert L.game_evolve_sharded(ctx, 1, 0, 2, 100_000, None) == game.ERR_BAD_STATE
+    ident = (C.c_char * 128)()
+    assert L.game_comm_init(ctx, None, 0, 1) == game.ERR_INVALID_ARG
+    assert L.game_comm_init(ctx, ident, 2, 2) == game.ERR_INVALID_ARG
+    assert L.game_comm_init(ctx, ident, 0, 1) in (game.ERR_BAD_STATE, game.ERR_UNSUPPORTED)            # not bound / no NCCL here
+    assert L.game_comm_unique_id(None) == game.ERR_INVALID_ARG
+    # diagnostics
+    n = C.c_uint64(7)
+    assert L.game_graph_replays(ctx, C.byref(n)) == game.OK and n.value == 0
+    a, b, e = C.c_double(), C.c_double(), C.c_double()
+    assert L.game_mma_stall(ctx, C.byref(a), C.byref(b), C.byref(e), None, 0) == game.ERR_BAD_STATE
+    assert L.game_mma_stall(ctx, None, C.byref(b), C.byref(e), None, 0) == game.ERR_INVALID_ARG
+    game.game_destroy(ctx)
