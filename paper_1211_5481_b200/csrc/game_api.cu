@@ -40,7 +40,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_run = 0, off_sse = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_run = 0, off_sse = 0, off_wt = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -453,9 +453,13 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
         if (grid_ll > n_tiles) grid_ll = n_tiles;
         const int grid = static_cast<int>(grid_ll);
         n_part = grid;
+        float* Wt = reinterpret_cast<float*>(c->ws + c->off_wt);
+        launch_chain(c->pdl, ffma_transpose_kernel, dim3((c->G + 31) / 32, (c->m_stride + 31) / 32), dim3(256), 0, c->stream,
+                     W, Wt, c->M, c->G, c->m_stride);
+        if ((rc = check_launch(c, "ffma_transpose_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));
-        launch_chain(c->pdl && hk == nullptr, fitness_ffma_kernel, dim3(grid), dim3(kFfmaTile), smem, c->stream,
-                     c->X, c->t, W, reinterpret_cast<double*>(c->ws + c->off_part), c->P, c->N, c->d, c->M, c->G, c->expansion, c->act,
+        launch_chain(c->pdl && hk == nullptr, fitness_ffma_kernel, dim3(grid), dim3(kFfmaThreads), smem, c->stream,
+                     c->X, c->t, static_cast<const float*>(Wt), reinterpret_cast<double*>(c->ws + c->off_part), c->P, c->N, c->d, c->M, c->G, c->expansion, c->act,
                      c->m_stride, n_tiles, c->stop, c->shared);
         if ((rc = check_launch(c, "fitness_ffma_kernel"))) return rc;
         if (timed) GAME_CUDA(cudaEventRecord(ev1, c->stream));
@@ -738,6 +742,8 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->off_fused_bar = off; off = align_up(off + sizeof(unsigned int));
     c->off_run = off; off = align_up(off + sizeof(game::RunState));
     c->off_sse = off; off = align_up(off + sizeof(double) * static_cast<size_t>(M));      // pattern-sharded loop: per-chromosome sums
+    c->off_wt = off;          // FFMA scheme: W transposed, [G][m_stride]
+    if (G <= game::kFfmaMaxG) off = align_up(off + sizeof(float) * static_cast<size_t>(G) * c->m_stride);
     c->ws_bytes = off;
     *out = c;
     return GAME_OK;
