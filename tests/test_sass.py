@@ -60,7 +60,7 @@ def test_fitness_kernels_keep_noncoherent_loads_for_the_knowledge_base_only(sass
         for i, line in enumerate(open(os.path.join(CSRC, fn)), 1):
             code = line.split("//")[0]
             if "__ldg(" in code:
-                assert re.search(r"__ldg\((prm\.t|row|xr|reinterpret_cast<const float4\*>\(row\))", code), f"{fn}:{i}: {line.strip()}"
+                assert re.search(r"__ldg\((prm\.t|t \+|row|xr|reinterpret_cast<const float4\*>\(row\))", code), f"{fn}:{i}: {line.strip()}"
     # the kernels of the chain take their chain-written inputs as plain pointers
     src = open(os.path.join(CSRC, "ga_kernels.cuh")).read()
     sig = src[src.index("ga_step_kernel(const float* W"):][:200]
