@@ -43,9 +43,9 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 # bench values).  Each entry names the capture it comes from and the sha-256 prefix of csrc/fitness_umma.cuh at capture
 # time: when the kernel source has changed since, the figure is withheld (traffic = null) rather than repeated.
 NCU_TRAFFIC = {
-    "c1": {"bytes": 4664832, "source": "profiles/r02_README.md (4.66 MB read + 0 written; algorithmic 4.40 MB)", "kernel_sha": "ac9bbdd601dd"},
-    "c2": {"bytes": 72248064, "source": "profiles/r02_README.md (68.76 MB read + 3.49 MB written; algorithmic 68.0 MB)", "kernel_sha": "ac9bbdd601dd"},
-    "c3": {"bytes": 546117376, "source": "profiles/r02_README.md (535.74 MB read + 10.37 MB written; algorithmic 528.0 MB)", "kernel_sha": "ac9bbdd601dd"},
+    "c1": {"bytes": 4666880, "source": "profiles/r02_README.md (4.67 MB read + 0 written; algorithmic 4.40 MB)", "kernel_sha": "0fd22f973aa0"},
+    "c2": {"bytes": 70289408, "source": "profiles/r02_README.md (68.75 MB read + 1.54 MB written; algorithmic 68.0 MB)", "kernel_sha": "0fd22f973aa0"},
+    "c3": {"bytes": 544963584, "source": "profiles/r02_README.md (535.63 MB read + 9.33 MB written; algorithmic 528.0 MB)", "kernel_sha": "0fd22f973aa0"},
 }
 TENSOR_FLOP_PER_CLK_PER_SM = 8192          # dense fp16/bf16 tcgen05 rate (2.25 PFLOP/s nominal = 8192 x 148 SMs x 1.86 GHz)
 
