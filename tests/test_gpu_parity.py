@@ -279,10 +279,11 @@ def test_checkpoint_resume_bit_exact(game):
     G2.close()
 
 
-def test_generation_host_entry(game):
+@pytest.mark.parametrize("base", ["c1", "c2"])          # c2: tanh, i.e. with the calibration launches behind the upload
+def test_generation_host_entry(game, base):
     """The host-buffer entry point = load + eval + step + download."""
     import torch
-    cfg = wl.scaled(wl.CONFIGS["c1"], P=3000, M=150)
+    cfg = wl.scaled(wl.CONFIGS[base], P=3000, M=150)
     X, t, _ = wl.make_kb(cfg)
     W = wl.uniform_population(cfg.M, cfg.G, 11)
     G = make(game, cfg)
