@@ -167,6 +167,19 @@ def test_full_size_c4_largest_population(game):
     check(F[rows], oracle.eval_fitness(cfg.d, cfg.family, X, t, W[rows]), "c4 M=16384 P=1e6, sampled rows")
 
 
+@pytest.mark.slow
+def test_full_size_c4_largest_point(game):
+    """The largest point of BASELINE.json configs[4]: M = 16384, P = 1e7 (39 063 pattern tiles x 64 tile pairs, 100 ms of
+    kernel): eight sampled chromosomes, one by one on the oracle (~25 s)."""
+    cfg = wl.c4(16384, 10_000_000)
+    X, t, _ = wl.make_kb(cfg)
+    W = wl.uniform_population(cfg.M, cfg.G, seed=4)
+    F, used = run_fitness(game, cfg, X, t, W, game.SCHEME_AUTO)
+    assert used == game.SCHEME_F16X3 and np.all(np.isfinite(F))
+    rows = sorted({0, 127, 128, 8191, 16256, cfg.M - 1, int(np.argmin(F)), int(np.argmax(F))})
+    check(F[rows], oracle.eval_fitness(cfg.d, cfg.family, X, t, W[rows]), "c4 M=16384 P=1e7, sampled rows")
+
+
 # ------------------------------------------------------------------------------------------------ (c) small scales
 @pytest.mark.parametrize("scheme", [1, 2])
 @pytest.mark.parametrize("act", [wl.ACT_IDENTITY])
