@@ -318,6 +318,47 @@ int game_fitness_kernel_ms(game_ctx* ctx, double* total_ms, uint64_t* launches);
 /* ctx-owned string describing the last error on this context ("" if none); valid until the next call. */
 const char* game_last_error(const game_ctx* ctx);
 
+/* ONE fitness evaluation that allocates no device memory and needs no workspace -- for callers who have none to give.
+ *
+ * Who this is for.  Every other entry point borrows its scratch from the caller (the workspace of game_bind_state), so
+ * the caller must be able to obtain device memory.  Some cannot: a plug-in that runs inside a host application owning the
+ * whole GPU (it is handed input and output buffers from the host's pool and may not call cudaMalloc behind its back); a
+ * control or serving loop with a latency budget, where cudaMalloc / cudaFree would stall every stream of the device; a
+ * process whose device memory was fully assigned before this library was loaded.  Such a caller passes only inputs and
+ * the output; the scratch (the transposed population and the per-block partial sums of the FFMA scheme) sits in a fixed
+ * array of 4 456 448 bytes (4.25 MiB) that is part of libgame.so's device image.  Every GPU on which the process uses
+ * the library holds that array from module load until exit, called or not -- that is the cost of this entry point.
+ *
+ * What it computes.  fitness_dev[m] = (1/P) sum_p (act(sum_g W[m][g] phi_g(x_p)) - t_p)^2 (eq.(2),(3);
+ * MSE) for W_dev[M][G], X_dev[P][N], t_dev[P] (device, float32, row-major, 16-byte aligned, caller-owned, only read) into
+ * fitness_dev[M] (device, float32, written).  G and `family` are those of game_create.  The kernels, the grid and the
+ * order of summation are those of game_eval_fitness under GAME_SCHEME_FFMA (fp32 FFMA, fp64 partial sums in a fixed
+ * order), so the values agree with that path; the GA operators, the error-metric setting and the best-fitness output are
+ * not part of it.  Enqueued on cuda_stream (a cudaStream_t, NULL = default stream); asynchronous.
+ *
+ * Limits.  M <= GAME_NOALLOC_MAX_M (1024) and G <= GAME_NOALLOC_MAX_G (448, the FFMA kernel's own bound).  Anything
+ * larger returns GAME_ERR_UNSUPPORTED and says which limit was hit; use game_eval_fitness with a workspace instead.
+ * Bad pointers / shapes -> GAME_ERR_INVALID_ARG; no device, wrong architecture, launch failure -> GAME_ERR_CUDA.  There
+ * is no context, so the message goes to err_host (host buffer of err_len bytes, NUL-terminated, "" on success; may be NULL).
+ *
+ * No allocation: the call performs no cudaMalloc / cudaFree / cudaMallocAsync and calls no library routine that does; host
+ * side it uses a fixed table and a mutex.
+ *
+ * First call per device.  The first call that targets a given device (the device fitness_dev lives on, made current for
+ * the duration of the call) does a one-time set-up there: it asks the runtime where the array sits on that device and
+ * raises the fitness kernel's shared-memory limit.  Make that first call during initialisation, outside any stream
+ * capture; later calls go straight to the three kernel launches.
+ *
+ * Sharing.  There is ONE array per device and process.  Nothing is carried from call to call (each call rewrites the
+ * transposed population in full and every block clears its row of partial sums before adding to it, so stale contents
+ * of an earlier, differently shaped call are harmless), but two calls whose kernels can run at the same time on one
+ * device -- different streams, or different host threads without stream ordering between them -- overwrite each other's
+ * scratch and both results are garbage.  Keep all calls for a device on one stream, or order them with events. */
+enum { GAME_NOALLOC_MAX_M = 1024, GAME_NOALLOC_MAX_G = 448 };
+int game_eval_fitness_noalloc(const float* X_dev, const float* t_dev, const float* W_dev, float* fitness_dev,
+                              int64_t P, int32_t N, int32_t d, int32_t M, int32_t family, void* cuda_stream,
+                              char* err_host, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

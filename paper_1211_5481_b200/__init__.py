@@ -65,7 +65,10 @@ SIGNATURES = {
     "game_time_fitness_kernel": (C.c_int, [_VP, C.c_int32]),
     "game_fitness_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
     "game_last_error": (C.c_char_p, [_VP]),
+    "game_eval_fitness_noalloc": (C.c_int, [_F32P, _F32P, _F32P, _F32P, C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                            _VP, C.c_char_p, C.c_size_t]),
 }
+NOALLOC_MAX_M, NOALLOC_MAX_G = 1024, 448   # GAME_NOALLOC_MAX_M / _G of include/game.h
 
 _lib = None
 
@@ -287,6 +290,18 @@ def game_fitness_kernel_ms(ctx):
 def game_last_error(ctx) -> str:
     msg = lib().game_last_error(ctx)
     return msg.decode() if msg else ""
+
+
+def game_eval_fitness_noalloc(X_dev: int, t_dev: int, W_dev: int, fitness_dev: int, P: int, N: int, d: int, M: int, fam: int,
+                              cuda_stream: int | None = None) -> None:
+    """MSE fitness of W_dev[M][G] over X_dev[P][N], t_dev[P] into fitness_dev[M] without a context, a workspace or any
+    device allocation: the scratch is a fixed 4.25 MiB array inside libgame.so (M <= 1024, G <= 448; one per GPU, shared
+    by all calls, so keep the calls for a device on one stream).  Meant for callers who are handed their buffers and
+    cannot allocate -- see include/game.h.  Raises GameError with the library's message (limits included)."""
+    buf = C.create_string_buffer(256)
+    rc = lib().game_eval_fitness_noalloc(X_dev, t_dev, W_dev, fitness_dev, P, N, d, M, fam, cuda_stream, buf, len(buf))
+    if rc != OK:
+        raise GameError(rc, buf.value.decode())
 
 
 # ---- convenience: a context plus the torch tensors it borrows ---------------------------------------------

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1229,3 +1230,147 @@ int game_fitness_kernel_ms(game_ctx* c, double* total_ms, uint64_t* launches) {
 const char* game_last_error(const game_ctx* c) { return c ? c->err : "null context"; }
 
 }  // extern "C"
+
+// ---- game_eval_fitness_noalloc: one fitness evaluation for callers that have no device memory to spare ---------------
+//
+// Everything above borrows its scratch from the caller (game_bind_state's workspace), which presumes the caller can get
+// device memory from somewhere.  Some cannot: code that runs inside a host application which owns every byte of the GPU
+// (a plug-in handed its input and output tensors by an inference server or a simulation, with cudaMalloc off limits
+// because the host's pool is the only allocator), a latency-critical loop that must not hit cudaMalloc's implicit
+// device-wide synchronisation, or a process started with its memory budget already spent.  For them the scratch of the
+// FFMA evaluation -- the transposed population and the per-block partial sums -- lives in the fixed array below, which is
+// part of the library image: the driver places it on every GPU that loads libgame.so and keeps it there until the process
+// exits, whether or not this entry point is ever called.  The price is a hard size limit and one shared copy per GPU.
+//
+// The kernels are the ones game_eval_fitness launches under GAME_SCHEME_FFMA, on the same grid, so the result is the one
+// that path gives; only the place the scratch lives in differs.
+namespace {
+
+constexpr size_t kNoAllocPartBytes = sizeof(double) * kMaxPartRows * GAME_NOALLOC_MAX_M;   // [320][m_stride] fp64 partial sums
+constexpr size_t kNoAllocWtBytes = sizeof(float) * GAME_NOALLOC_MAX_G * GAME_NOALLOC_MAX_M; // [G][m_stride] transposed W
+constexpr size_t kNoAllocBytes = kNoAllocPartBytes + kNoAllocWtBytes;                       // 4 456 448 B = 4.25 MiB per GPU
+static_assert(GAME_NOALLOC_MAX_G <= game::kFfmaMaxG, "the FFMA kernel's shared-memory tile bounds G");
+static_assert(GAME_NOALLOC_MAX_M % 256 == 0 && kNoAllocPartBytes % kAlign == 0, "the row stride is M rounded up to 256");
+
+// HOST code must never hand this name to a kernel: on the host side it is only a handle for the runtime's symbol table,
+// not a device address.  noalloc_setup() asks the runtime for the real address, once per device.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+constexpr int kNoAllocMaxDevices = 64;
+struct NoAllocDevice {
+    bool ready = false;
+    unsigned char* scratch = nullptr;   // device address of g_noalloc_scratch ON THIS DEVICE (every device has its own copy)
+    int num_sms = 0;
+};
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mutex;
+
+int noalloc_fail(char* err, size_t err_len, int code, const char* fmt, ...) {
+    if (err != nullptr && err_len > 0) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(err, err_len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+// First call on a device, with that device current: look up where the array sits on it, read what the grid sizing needs,
+// raise the fitness kernel's dynamic shared-memory limit.  None of this allocates device memory.
+int noalloc_setup(int dev, const NoAllocDevice** out, char* err, size_t err_len) {
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return noalloc_fail(err, err_len, GAME_ERR_UNSUPPORTED, "device ordinal %d is beyond the %d this entry point keeps state for", dev, kNoAllocMaxDevices);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoAllocDevice& s = g_noalloc_dev[dev];
+    if (!s.ready) {
+        int major = 0, sms = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return noalloc_fail(err, err_len, GAME_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+        if (major != 10) return noalloc_fail(err, err_len, GAME_ERR_CUDA, "device %d is sm_%dx; this library is built for sm_100a only", dev, major);
+        unsigned char* ptr = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_noalloc_scratch);
+        if (e != cudaSuccess || ptr == nullptr) {
+            cudaGetLastError();
+            return noalloc_fail(err, err_len, GAME_ERR_CUDA, "cudaGetSymbolAddress(static scratch) on device %d: %s", dev, cudaGetErrorString(e));
+        }
+        e = cudaFuncSetAttribute(game::fitness_ffma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, game::kFfmaMaxG * game::kFfmaTile * 4);
+        if (e != cudaSuccess) return noalloc_fail(err, err_len, GAME_ERR_CUDA, "cudaFuncSetAttribute(fitness_ffma_kernel): %s", cudaGetErrorString(e));
+        s.scratch = ptr;
+        s.num_sms = sms;
+        s.ready = true;
+    }
+    *out = &s;
+    return GAME_OK;
+}
+
+}  // namespace
+
+extern "C" int game_eval_fitness_noalloc(const float* X_dev, const float* t_dev, const float* W_dev, float* fitness_dev,
+                                         int64_t P, int32_t N, int32_t d, int32_t M, int32_t family, void* cuda_stream,
+                                         char* err_host, size_t err_len) {
+    using namespace game;
+    if (err_host != nullptr && err_len > 0) err_host[0] = '\0';
+    // ---- arguments first (host only, so a bad call fails the same way with or without a GPU)
+    if (!X_dev || !t_dev || !W_dev || !fitness_dev) return noalloc_fail(err_host, err_len, GAME_ERR_INVALID_ARG, "null device pointer");
+    if (!aligned16(X_dev) || !aligned16(t_dev) || !aligned16(W_dev) || !aligned16(fitness_dev))
+        return noalloc_fail(err_host, err_len, GAME_ERR_INVALID_ARG, "device pointers must be 16-byte aligned");
+    const int expansion = family & 0xff, act = (family >> 8) & 0xff, shared = (family >> 16) & 1;
+    if (P < 1 || N < 1 || d < 1 || M < 1 || (family >> 17) != 0 || expansion > GAME_EXP_TRIG || act > GAME_ACT_TANH)
+        return noalloc_fail(err_host, err_len, GAME_ERR_INVALID_ARG, "bad shape or family (P, N, d, M >= 1; family as in game_create)");
+    if (P > (1ll << 40) || N > 4096 || d > 4096) return noalloc_fail(err_host, err_len, GAME_ERR_INVALID_ARG, "P, N or d beyond what game_create accepts");
+    const long long G = static_cast<long long>(shared ? 1 : N) * d * (expansion == GAME_EXP_TRIG ? 2 : 1) + 1;
+    if (M > GAME_NOALLOC_MAX_M)
+        return noalloc_fail(err_host, err_len, GAME_ERR_UNSUPPORTED,
+                            "M = %d chromosomes exceed the static scratch of game_eval_fitness_noalloc (at most %d); use game_eval_fitness with a workspace",
+                            M, GAME_NOALLOC_MAX_M);
+    if (G > GAME_NOALLOC_MAX_G)
+        return noalloc_fail(err_host, err_len, GAME_ERR_UNSUPPORTED,
+                            "G = %lld genes exceed the static scratch of game_eval_fitness_noalloc (at most %d); use game_eval_fitness with a workspace",
+                            G, GAME_NOALLOC_MAX_G);
+    // ---- the device the buffers live on becomes current for the set-up and the launches
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        return noalloc_fail(err_host, err_len, GAME_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    int dev = device_of(fitness_dev);
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return noalloc_fail(err_host, err_len, GAME_ERR_CUDA, "cudaGetDevice failed");
+    DeviceGuard guard(dev);
+    const NoAllocDevice* s = nullptr;
+    if (int rc = noalloc_setup(dev, &s, err_host, err_len)) return rc;
+
+    // ---- same geometry as the FFMA branch of eval_internal (same grid => same summation order => same bits)
+    const int m_stride = (M + 255) / 256 * 256;
+    const int Gi = static_cast<int>(G);
+    double* part = reinterpret_cast<double*>(s->scratch);                         // rows [0, grid): each block clears its own row
+    float* Wt = reinterpret_cast<float*>(s->scratch + kNoAllocPartBytes);         // [G][m_stride]: rewritten in full, pad columns zero
+    const long long n_tiles = (P + kFfmaTile - 1) / kFfmaTile;
+    const size_t smem = static_cast<size_t>(Gi) * kFfmaTile * sizeof(float);
+    int per_sm = static_cast<int>((220u * 1024u) / (smem + 1024));
+    if (per_sm < 1) per_sm = 1;
+    long long grid_ll = static_cast<long long>(s->num_sms) * per_sm;
+    if (grid_ll > kMaxPartRows) grid_ll = kMaxPartRows;
+    if (grid_ll > n_tiles) grid_ll = n_tiles;
+    const int grid = static_cast<int>(grid_ll);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = launch_chain(false, ffma_transpose_kernel, dim3((Gi + 31) / 32, (m_stride + 31) / 32), dim3(256), 0, stream,
+                                 W_dev, Wt, M, Gi, m_stride);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(err_host, err_len, GAME_ERR_CUDA, "ffma_transpose_kernel: %s", cudaGetErrorString(e));
+    e = launch_chain(false, fitness_ffma_kernel, dim3(grid), dim3(kFfmaThreads), smem, stream, X_dev, t_dev,
+                     static_cast<const float*>(Wt), part, static_cast<long long>(P), N, d, M, Gi, expansion, act, m_stride, n_tiles,
+                     static_cast<const int*>(nullptr), shared);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(err_host, err_len, GAME_ERR_CUDA, "fitness_ffma_kernel: %s", cudaGetErrorString(e));
+    // fixed-order fp64 sum of the partial rows, / P, one rounding to fp32; with no best-fitness output the kernel touches
+    // none of the bookkeeping buffers its context-bound launches use (it returns before them)
+    const int fin_blocks = (M + kFinCols - 1) / kFinCols;
+    e = launch_chain(false, finalize_fitness_kernel, dim3(fin_blocks), dim3(kFinThreads), 0, stream,
+                     static_cast<const double*>(part), grid, m_stride, M, static_cast<double>(P), fitness_dev,
+                     static_cast<double*>(nullptr), static_cast<float*>(nullptr), static_cast<float*>(nullptr),
+                     static_cast<int*>(nullptr), static_cast<unsigned int*>(nullptr), static_cast<int*>(nullptr), 0.0f, 0,
+                     static_cast<int>(GAME_ERROR_MSE), static_cast<RunState*>(nullptr), 0);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(err_host, err_len, GAME_ERR_CUDA, "finalize_fitness_kernel: %s", cudaGetErrorString(e));
+    return GAME_OK;
+}
