@@ -4,25 +4,15 @@ Random123 known-answer file is not in the container, so the three vectors of tes
 computed from the SC'11 definition; this is the cross-check against code neither side wrote."""
 import ctypes as C
 import os
-import subprocess
 
 import numpy as np
 import pytest
 
 import oracle
+from curand_helper import build_helper
 
 pytestmark = pytest.mark.gpu
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "curand_philox_check.cu")
-LIB = os.path.join(HERE, "libcurand_philox_check.so")
-
-
-def build_helper() -> str:
-    if not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
-        nvcc = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "nvcc")
-        subprocess.run([nvcc, "-O2", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fPIC",
-                        "-shared", "-cudart", "static", "-o", LIB, SRC], check=True)
-    return LIB
 
 
 def curand_blocks(rows: np.ndarray) -> np.ndarray:
