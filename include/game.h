@@ -118,7 +118,11 @@ int game_set_scheme(game_ctx* ctx, int32_t scheme);
 int game_get_scheme(const game_ctx* ctx, int32_t* scheme);
 
 /* Bind the knowledge base ("the dataset is never altered"): X_dev[P][N] float32
- * row-major, t_dev[P] float32 targets.  Borrowed; read by every game_eval_fitness. */
+ * row-major, t_dev[P] float32 targets.  Borrowed; read by every game_eval_fitness.
+ * The caller may rewrite X_dev / t_dev between calls with work enqueued on the context's stream (a kernel, a copy); plain
+ * stream order is all that is needed.  (The library's kernels are chained by programmatic dependent launch and, on small
+ * grids, start reading the knowledge base before their predecessor has finished -- but only behind a kernel the library
+ * itself enqueued within the same call; the first kernel of every public call waits for everything enqueued before it.) */
 int game_load_kb(game_ctx* ctx, const float* X_dev, const float* t_dev);
 
 /* Bind the mutable state: two population buffers popA_dev/popB_dev [M][G] float32 (the current

@@ -854,6 +854,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
     // The phi producers do not wait here: all they read is the knowledge base, which no kernel of the chain writes, and all
     // they write is shared memory -- they generate their first work item while the preceding kernel is still running and
     // wait afterwards (late_wait below; every thread of every kernel still passes griddepcontrol.wait before it exits).
+    // The host sets Params::early only when the kernel ahead on the stream is one of the library's own (game_api.cu,
+    // chain_launches): a caller's kernel that has just rewritten the borrowed X is then at least two launches back and,
+    // because every library kernel waits before it releases its dependents, complete.
     // Only for grids that leave SMs free (Params::early): a grid that fills the chip squeezes the GA step it overlaps down to
     // one block per SM, and its busy producers then cost that kernel more than they save here (c1: 48.7 -> 49.6 us per
     // generation; c0, with 8 CTAs, 15.2 -> 13.6 us; the paper-shaped n1 22.5 -> 20.5 us).

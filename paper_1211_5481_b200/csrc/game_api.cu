@@ -65,6 +65,12 @@ struct game_ctx {
     int num_sms = 0;
     int device = -1;                                 // ordinal of the device the bound buffers live on (-1: unknown, use the current one)
     unsigned long long launches = 0;
+    // Kernels this context has enqueued since the current public call began (begin_call).  The tensor-core fitness kernel may
+    // let its phi producers read X and t BEFORE griddepcontrol.wait (Params::early) only when its predecessor on the stream
+    // is one of the library's own kernels -- all of which wait before they signal their dependents, so everything the caller
+    // enqueued earlier (a kernel that fills the borrowed X, say) has completed by then.  The first launch of a public call
+    // has an unknown predecessor and always waits first.
+    unsigned long long chain_launches = 0;
     int last_umma_grid = 0;                          // CTAs of the last tensor-core fitness launch (game_mma_stall)
     bool timing = false;
     game::RunState* run = nullptr;                   // device run state, non-null only inside a graph-replayed generation loop
@@ -206,8 +212,12 @@ int check_launch(game_ctx* c, const char* what) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, what);
     c->launches += 1;
+    c->chain_launches += 1;
     return GAME_OK;
 }
+
+// Start of a public call that evaluates: whatever precedes its first kernel on the stream is the caller's business.
+void begin_call(game_ctx* c) { c->chain_launches = 0; }
 
 // Host knowledge base to be uploaded range by range while earlier ranges are being evaluated (game_generation_host).
 struct HostKb {
@@ -287,7 +297,9 @@ void setup_umma(game_ctx* c, game::umma::Params& prm, UmmaGeo& geo) {
     prm.p_tile0 = 0; prm.p_tiles = geo.p_tiles_all; prm.zero_part = 1;
     const long long units = static_cast<long long>(geo.p_tiles_all) * prm.m_groups;
     geo.grid = 2 * static_cast<int>(units < geo.pair_cap ? units : geo.pair_cap);   // the same grid for every pattern range
-    prm.early = 2 * geo.grid <= c->num_sms ? 1 : 0;      // early-start producers only when at least half of the SMs stay free
+    // early-start producers only when at least half of the SMs stay free, and only behind one of the library's own kernels
+    // (game_ctx::chain_launches; include/game.h, game_load_kb)
+    prm.early = (2 * geo.grid <= c->num_sms && c->chain_launches > 0) ? 1 : 0;
     c->last_umma_grid = geo.grid;
 }
 
@@ -485,6 +497,7 @@ int eval_streamed(game_ctx* c, const float* X_host, const float* t_host, float* 
     if (resolved_scheme(c) != GAME_SCHEME_F16X3 || !c->umma_ok)
         return fail(c, GAME_ERR_UNSUPPORTED, "game_eval_fitness_streamed runs on the tensor-core scheme (F16X3) only");
     if (c->stop != nullptr || c->run != nullptr) return fail(c, GAME_ERR_BAD_STATE, "game_eval_fitness_streamed inside a generation loop");
+    begin_call(c);
     if (!c->ticket_zeroed) {
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
         c->ticket_zeroed = true;
@@ -624,12 +637,20 @@ int ensure_graph(game_ctx* c) {
         c->graph_ok = false;
         return GAME_OK;
     }
+    // A capture executes nothing: whatever the recorded calls did to the host-side mirror of the device state (which buffer
+    // is current, whether fitness and W images are valid) is put back, so that a capture that fails half-way leaves the
+    // context exactly as it found it and the plain launches that follow start from the truth.
+    const int cur0 = c->cur;
+    const bool fitness_valid0 = c->fitness_valid, img_valid0 = c->img_valid;
     int rc = GAME_OK;
     for (uint32_t i = 0; i < kGraphGens && rc == GAME_OK; ++i) rc = plain_generation(c);
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
     c->stream = run_stream;
     c->graph_nodes = c->launches - launches0;
     c->launches = launches0;                      // nothing has run yet
+    c->cur = cur0;
+    c->fitness_valid = fitness_valid0;
+    c->img_valid = img_valid0;
     if (rc != GAME_OK || e != cudaSuccess || graph == nullptr) {
         cudaGetLastError();
         if (graph) cudaGraphDestroy(graph);
@@ -656,9 +677,17 @@ int run_generations(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, 
     DeviceGuard guard(c->device);
     int rc = ensure_device(c);
     if (rc) return rc;
+    begin_call(c);
     RunState* run = reinterpret_cast<RunState*>(c->ws + c->off_run);
     set_run_state_kernel<<<1, 1, 0, c->stream>>>(run, make_key(seed), gen0, best_dev);
     if ((rc = check_launch(c, "set_run_state_kernel"))) return rc;
+    // c->run is non-null only while this function is on the stack: with it set, eval and step take seed, generation index
+    // and trace slot from the device run state instead of their arguments, which must never leak into a later public call
+    // (every exit below, early error returns included, goes through the guard).
+    struct RunScope {
+        game_ctx* c;
+        ~RunScope() { c->run = nullptr; }
+    } run_scope{c};
     c->run = run;
     if (!c->ticket_zeroed) {
         GAME_CUDA(cudaMemsetAsync(c->ws + c->off_ticket, 0, sizeof(unsigned int), c->stream));
@@ -687,7 +716,6 @@ int run_generations(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, 
     }
     for (; rc == GAME_OK && done < n_gens; ++done) rc = plain_generation(c);
     if (rc == GAME_OK && final_eval) rc = eval_internal(c, nullptr);
-    c->run = nullptr;
     return rc;
 }
 
@@ -917,6 +945,7 @@ int game_assume_fitness(game_ctx* c) {
 
 int game_eval_fitness(game_ctx* c) {
     if (!c) return GAME_ERR_INVALID_ARG;
+    begin_call(c);
     return eval_internal(c, nullptr);
 }
 
@@ -937,6 +966,7 @@ int game_run_until(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t max_gens,
     if (!c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_run_until before game_bind_state");
     DeviceGuard guard(c->device);
     int* stop = reinterpret_cast<int*>(c->ws + c->off_stop);
+    begin_call(c);
     GAME_CUDA(cudaMemsetAsync(stop, 0, 2 * sizeof(int), c->stream));
     c->stop = stop;
     c->stop_threshold = threshold;
@@ -1039,6 +1069,7 @@ int game_generation_host(game_ctx* c, const float* X_host, const float* t_host, 
     const HostKb hk{X_host, t_host};
     int rc = ensure_device(c);
     if (rc) return rc;
+    begin_call(c);
     rc = eval_internal(c, nullptr, &hk);
     if (rc) return rc;
     rc = step_internal(c, seed, gen);
@@ -1063,6 +1094,7 @@ int game_eval_fitness_streamed(game_ctx* c, const float* X_host, const float* t_
 int game_eval_sse(game_ctx* c, double* sse_dev) {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!sse_dev) return fail(c, GAME_ERR_INVALID_ARG, "game_eval_sse: null sse_dev");
+    begin_call(c);
     return eval_internal(c, nullptr, nullptr, sse_dev);
 }
 
@@ -1106,6 +1138,7 @@ int game_evolve_sharded(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_ge
     if (!c->ws) return fail(c, GAME_ERR_BAD_STATE, "game_evolve_sharded before game_bind_state");
     DeviceGuard guard(c->device);
     double* sse = reinterpret_cast<double*>(c->ws + c->off_sse);
+    begin_call(c);
     for (uint32_t i = 0; i < n_gens; ++i) {
         int rc = eval_internal(c, nullptr, nullptr, sse);                 // this rank's un-normalised sums
         if (rc) return rc;

@@ -722,6 +722,33 @@ def test_dependent_launch_chain_is_race_free(game, base, over, scheme, selection
             assert np.array_equal(a, b)
 
 
+def test_caller_rewrites_knowledge_base_on_the_stream(game):
+    """include/game.h, game_load_kb: the caller may rewrite the borrowed X / t with work on the context's stream and evaluate
+    again, with nothing but stream order in between.  On small grids (c0: 8 CTAs) the fitness kernel's phi producers start
+    reading X before griddepcontrol.wait, which is only sound behind one of the library's own kernels -- so the first kernel
+    of a public call must not do it.  Here the W images are already valid (no image pass ahead of the fitness kernel) and a
+    device-side copy kernel fills X right before game_eval_fitness, on every activation (identity / tanh put the calibration
+    launch first instead)."""
+    import torch
+    for act in (wl.ACT_SIGMOID, wl.ACT_TANH):
+        cfg = wl.scaled(wl.CONFIGS["c0"], activation=act)
+        X1, t1, _ = wl.make_kb(cfg)
+        X2, t2, _ = wl.make_kb(cfg, seed=99)
+        G = make(game, cfg, 2); G.load_kb(X1, t1)
+        G.init_population(5); G.eval_fitness()                      # builds the W images; fitness over (X1, t1)
+        X2d = torch.as_tensor(X2, device="cuda"); t2d = torch.as_tensor(t2, device="cuda")
+        big = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+        for rep in range(3):
+            src = (X2d, t2d) if rep % 2 == 0 else (torch.as_tensor(X1, device="cuda"), torch.as_tensor(t1, device="cuda"))
+            big.zero_()                                             # keeps the stream busy: the copies below are still queued
+            G.X.copy_(src[0]); G.t.copy_(src[1])                    # device-side kernels on the context's stream
+            G.eval_fitness()                                        # population unchanged: the fitness kernel goes first
+            G.sync()
+            F_ref = oracle.eval_fitness(cfg.d, cfg.family, X2 if rep % 2 == 0 else X1, t2 if rep % 2 == 0 else t1, G.get_population())
+            assert_fitness_close(G.get_fitness(), F_ref, f"act {act} rep {rep}")
+        G.close()
+
+
 # ------------------------------------------------------------------------------------------------ fused persistent loop
 @pytest.mark.parametrize("base,over,selection,immigrants", [
     ("c0", {}, 0, 0), ("c0", dict(P=777, M=37), 1, 3), ("n1", {}, 1, 0), ("n1", dict(P=500, M=23), 2, 2),
