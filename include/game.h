@@ -73,12 +73,23 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *              fitness, which the GA ranks worst) and |phi| < 4094 (phi is bounded by 1 for Chebyshev on |x| <= 1 and for
  *              trig).
  *              Accuracy: fitness within 1e-5 of fp64 -- measured 6e-8 .. 1.4e-6 on the BASELINE shapes and on populations
- *              around the optimum; see DESIGN.md section 2 for the table.  The tensor core adds into its accumulator with
+ *              around the optimum; see DESIGN.md section 2 for the table.  The one regime with a weaker statement is a
+ *              REGRESSION fit (IDENTITY, TANH) that is nearly perfect: with residual noise sigma and outputs of size
+ *              rms(z), a relative error eps of z moves the fitness of a near-optimal chromosome by ~eps rms(z) / sigma.
+ *              The scheme's outputs carry ~4e-7 rms(z) of unsystematic error each (it averages out as 1 / sqrt(P)) and,
+ *              after calibration (below), up to ~1e-7 of systematic error (the noise of the calibration fit itself), so
+ *              the 1e-5 bound holds for rms(z) / sigma <= 100, i.e. fitness >= 1e-4 of the mean square output; beyond
+ *              that the bound is 2e-7 rms(z) / sigma (measured at P = 9000, identity output: 2.1e-5 at rms(z) / sigma =
+ *              230, 2.7e-5 at 760, 4.8e-5 at 2300, 1.0e-4 at 7600, where plain fp32 arithmetic -- GAME_SCHEME_FFMA,
+ *              unbiased rounding -- gives 6.9e-7, 5.5e-6, 8.5e-6, 1.1e-5: force FFMA if a fit that good must be ranked
+ *              to 1e-5; tanh outputs stay below 2.5e-5 throughout).  Classification outputs
+ *              (SIGMOID against 0/1 targets) never get there.  The tensor core adds into its accumulator with
  *              truncation, which shrinks |z| by ~1.6e-8 per MMA; two measures keep that inside the bound where it would
  *              not be: K extents beyond 320 genes are accumulated 20 K steps at a time and the chunks added in fp32
  *              round-to-nearest (G = 2401, identity output: 2e-7), and for the regression activations (IDENTITY, TANH) the
- *              shrink of every row is measured on the first 256 patterns against an fp64 contraction before each
- *              evaluation and folded into the row's factor (one extra launch of the fused kernel + two small kernels per
+ *              shrink of every row is measured on 256 patterns spread evenly over the knowledge base (rows 0, s, 2s, ..
+ *              with s = P / 256: the order of the patterns does not matter) against an fp64 contraction before each
+ *              evaluation and folded into the row's factor (one extra launch of the fused kernel + three small kernels per
  *              evaluation; near-optimal regression with residual noise 0.01: 7.7e-6 / 8.7e-7 instead of 8.9e-5 / 8.9e-6;
  *              GAME_CALIBRATE=0 in the environment at game_create turns it off; rows longer than 3184 genes are not
  *              calibrated).
@@ -311,6 +322,23 @@ int game_mma_stall(game_ctx* ctx, double* frac_a_full, double* frac_b_full, doub
  * argument) and replay it; every replay adds its kernel count to game_launch_count.  0 when the graph path is off
  * (GAME_GRAPH=0 in the environment at game_create), unavailable, or the run was shorter than 16 generations. */
 int game_graph_replays(const game_ctx* ctx, uint64_t* replays);
+
+/* Whether the per-row calibration of the tensor-core scheme is doing its job (scheme F16X3 above: for the regression
+ * activations IDENTITY and TANH the 1e-5 accuracy statement rests on it).
+ *   active        : 1 if an evaluation under the current settings calibrates (scheme resolves to F16X3, activation IDENTITY
+ *                   or TANH, rows of at most 3184 genes, GAME_CALIBRATE not 0 at game_create), else 0 -- sigmoid outputs need
+ *                   none, the FFMA scheme has nothing to calibrate.
+ *   rows_rejected : in the LAST calibrated evaluation, the number of chromosomes whose measured shrink was not applied because
+ *                   the fit came out non-finite or beyond 1e-4 in magnitude (a row with an Inf / NaN gene; a row whose outputs
+ *                   on the sample patterns are all ~0, so that rounding noise dominates the fit).  Such a row is evaluated
+ *                   with the uncalibrated scheme (error up to ~1e-4 relative on a near-optimal regression fit instead of
+ *                   1e-5).  0 before the first calibrated evaluation.
+ * The sample is 256 patterns spread evenly over the knowledge base this context is bound to (the host-buffer and
+ * out-of-core entries pick the same rows from host memory, so they stay bit-identical to the resident evaluation).  Under
+ * pattern sharding (game_eval_sse / game_evolve_sharded) every rank samples its OWN shard: the correction, of relative size
+ * ~1e-6, therefore depends on how the patterns are partitioned -- well inside the accuracy bound, but sharded sums are not
+ * bit-identical to a one-GPU evaluation for these activations.  Synchronises the stream. */
+int game_calibration_status(game_ctx* ctx, int32_t* active, int32_t* rows_rejected);
 
 /* Timing hook for the roofline line: when enabled, game_eval_fitness brackets the fused fitness kernel
  * with CUDA events on the context's stream; game_fitness_kernel_ms returns the sum of the recorded

@@ -64,6 +64,7 @@ SIGNATURES = {
     "game_mma_stall": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), _VP, C.c_int32]),
     "game_time_fitness_kernel": (C.c_int, [_VP, C.c_int32]),
     "game_fitness_kernel_ms": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
+    "game_calibration_status": (C.c_int, [_VP, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
     "game_last_error": (C.c_char_p, [_VP]),
     "game_eval_fitness_noalloc": (C.c_int, [_F32P, _F32P, _F32P, _F32P, C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                             _VP, C.c_char_p, C.c_size_t]),
@@ -285,6 +286,13 @@ def game_fitness_kernel_ms(ctx):
     ms, n = C.c_double(), C.c_uint64()
     _check(ctx, lib().game_fitness_kernel_ms(ctx, C.byref(ms), C.byref(n)))
     return ms.value, n.value
+
+
+def game_calibration_status(ctx):
+    """(active, rows_rejected) of the tensor-core scheme's per-row calibration; see include/game.h."""
+    a, r = C.c_int32(), C.c_int32()
+    _check(ctx, lib().game_calibration_status(ctx, C.byref(a), C.byref(r)))
+    return bool(a.value), r.value
 
 
 def game_last_error(ctx) -> str:

@@ -461,14 +461,33 @@ __device__ __forceinline__ void store_w_image_gene(uint8_t* img, int steps, int 
 // whose residual r = y - t is small against z it does not average out over the patterns, dF/F = -2 eps <z r> / <r r>,
 // up to eps sqrt<z z> / sigma for residual noise sigma (measured 8.9e-5 at sigma = 0.01, identity output).
 // So for the regression activations (identity, tanh) the shrink of every chromosome row is MEASURED before each
-// evaluation: one extra launch of the fitness kernel hands out the raw accumulators of the first pattern tile
+// evaluation: one extra launch of the fitness kernel hands out the raw accumulators of a sample of <= 256 patterns
 // (Params::zdump), cal_phi_kernel + calibrate_kernel recompute the same z for those <= 256 patterns on the CUDA cores (fp32
 // expansion as in the producers, products and sums in fp64) and fits z_exact = (1 + eps_m) z_tensor by least squares; the evaluation then runs
 // with the row's un-scaling factor times (1 + eps_m).
 constexpr int kCalThreads = kBN;         // one thread per sample pattern
 constexpr int kCalUnroll = 16;           // K padding of the staged rows
 
-// phi of the <= 256 sample patterns (the first pattern tile), as the producers generate it (fp32 recurrences), widened to
+// The sample: n = min(256, rows) patterns spread EVENLY over the knowledge base (rows 0, s, 2 s, ... with s = rows / n),
+// copied into a small buffer of the workspace, so that the order of the patterns -- a catalogue sorted by a feature, by
+// the target, by anything that correlates with |z| -- does not decide what the fit sees.  (The first 256 patterns as they
+// came were the sample until round 3; on a knowledge base sorted by |w* . phi| that left 5e-4 of error on a near-optimal
+// identity fit.)  Host-resident knowledge bases are sampled with one strided copy instead (game_api.cu).
+__global__ void __launch_bounds__(256) cal_gather_kernel(const float* X, const float* t, float* Xs, float* ts, const int* stop,
+                                                         long long n, long long stride, int N) {
+    pdl_wait();                // X and t may have been written by whatever ran before on the stream
+    pdl_launch_dependents();
+    if (stop != nullptr && __ldcg(stop) != 0) return;
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < n * N;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long i = idx / N, f = idx - i * N;
+        Xs[idx] = __ldcg(X + i * stride * N + f);
+    }
+    for (long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; i < n; i += static_cast<long long>(gridDim.x) * blockDim.x)
+        ts[i] = __ldcg(t + i * stride);
+}
+
+// phi of the <= 256 sample patterns, as the producers generate it (fp32 recurrences), widened to
 // fp64 once: phi_s[(g - 1) * 256 + p] for genes g = 1..G-1.  One thread per pattern.
 template <int EXPANSION>
 __global__ void __launch_bounds__(kCalThreads) cal_phi_kernel(const float* __restrict__ X, double* phi_s, const int* stop, long long P,
@@ -525,8 +544,8 @@ __device__ __forceinline__ void dmma_m8n8k4(double (&acc)[2], double a, double b
                  : "d"(a), "d"(b));
 }
 __global__ void __launch_bounds__(kCalThreads) calibrate_kernel(const float* W, const double* phi_s, const float* zdump,
-                                                                const float* wscale, float* zcorr, const int* stop, long long P,
-                                                                int M, int G, int m_stride) {
+                                                                const float* wscale, float* zcorr, int* rejected,
+                                                                const int* stop, long long P, int M, int G, int m_stride) {
     extern __shared__ double cal_w[];      // [kCalRows][Kp]: the rows' genes 1..G-1 in fp64, zero-padded to a multiple of 16
     __shared__ double s_num[kCalRows][kCalThreads / 32], s_den[kCalRows][kCalThreads / 32];
     pdl_wait();                // the calibration launch's accumulators, phi_s, W and the row scales are complete
@@ -589,8 +608,12 @@ __global__ void __launch_bounds__(kCalThreads) calibrate_kernel(const float* W, 
         const int mm = m0 + tid;
         num = 0.0; den = 0.0;
         for (int w = 0; w < kCalThreads / 32; ++w) { num += s_num[tid][w]; den += s_den[tid][w]; }
-        double eps = den > 0.0 ? num / den : 0.0;
-        if (!(fabs(eps) <= 1e-4) || mm >= M) eps = 0.0;   // non-finite rows, or a row the model does not describe: leave it alone
+        double eps = den == 0.0 ? 0.0 : num / den;      // all-zero outputs: nothing to fit; a NaN / Inf row gives a NaN eps
+        // non-finite rows, or a row the model does not describe (the shrink it corrects is ~1e-6): leave it alone, and say so
+        // (game_calibration_status counts these rows; one flag per row, written by the row's own thread: no atomics)
+        const bool reject = mm < M && !(fabs(eps) <= 1e-4);
+        if (rejected != nullptr) rejected[mm] = reject ? 1 : 0;
+        if (reject || mm >= M) eps = 0.0;
         zcorr[mm] = static_cast<float>(static_cast<double>(__ldcg(wscale + mm)) * (1.0 + eps));
     }
 }

@@ -41,7 +41,7 @@ struct game_ctx {
     bool umma_ok = false;
     int m_tiles = 0, m_stride = 0, steps = 0;
     // workspace layout (byte offsets)
-    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_run = 0, off_sse = 0, off_wt = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
+    size_t off_part = 0, off_img = 0, off_wscale = 0, off_zcorr = 0, off_zdump = 0, off_calphi = 0, off_calrej = 0, off_calx = 0, off_run = 0, off_sse = 0, off_wt = 0, off_blk_key = 0, off_blk_idx = 0, off_ticket = 0, off_stall = 0, off_stop = 0, off_by_rank = 0, off_prefix = 0, off_fused_bar = 0, ws_bytes = 0;
     // bound buffers (borrowed)
     const float* X = nullptr;
     const float* t = nullptr;
@@ -54,6 +54,8 @@ struct game_ctx {
     bool ticket_zeroed = false;
     // GA parameters
     int elite = 2, tournament = 3, selection = GAME_SEL_TOURNAMENT, immigrants = 0, rmse = 0;
+    bool sample_staged = false;     // the calibration sample in the workspace is that of the current public call (stage_sample)
+    bool calibrated_once = false;   // a calibration has been enqueued since game_bind_state: off_calrej holds its row flags
     bool calibrate = true;   // regression activations on the tensor-core scheme: measure each row's accumulation shrink (calibrate_kernel)
     bool pdl = true;   // programmatic dependent launch along the generation's kernel chain (pdl.cuh); GAME_PDL=0 turns it off
     double p_cross = 0.9, p_mut = 0.05;
@@ -217,7 +219,10 @@ int check_launch(game_ctx* c, const char* what) {
 }
 
 // Start of a public call that evaluates: whatever precedes its first kernel on the stream is the caller's business.
-void begin_call(game_ctx* c) { c->chain_launches = 0; }
+void begin_call(game_ctx* c) {
+    c->chain_launches = 0;
+    c->sample_staged = false;      // the caller may have rewritten the knowledge base: the calibration sample is taken afresh
+}
 
 // Host knowledge base to be uploaded range by range while earlier ranges are being evaluated (game_generation_host).
 struct HostKb {
@@ -324,20 +329,57 @@ bool wants_calibration(const game_ctx* c) {
            sizeof(double) * game::umma::kCalRows * (static_cast<size_t>(c->G) + 16) <= kCalMaxSmem;
 }
 
-// Regression activations: measure every row's accumulation shrink on the first pattern tile (fitness_umma.cuh, "calibration")
-// and point prm.wscale at the corrected factors.  X0 / t0: where the first 256 patterns are (device).
-int launch_calibration(game_ctx* c, game::umma::Params& prm, const UmmaGeo& geo, bool pdl, const float* X0, const float* t0) {
+// Regression activations: measure every row's accumulation shrink on a sample of min(256, P) patterns spread evenly over
+// the knowledge base (fitness_umma.cuh, "calibration") and point prm.wscale at the corrected factors.  Xsrc / tsrc: the
+// knowledge base of P patterns, on the device (gathered by a kernel) or, with src_is_host, in host memory (one strided copy
+// each for X and t -- the host-buffer and out-of-core entries, where only part of the patterns is on the device yet).
+// Both ways pick the same rows, so a streamed evaluation stays bit-identical to the resident one.
+// The sample patterns into the workspace (off_calx).  Done once per public call: inside a generation loop nobody but the
+// library's own kernels runs between two evaluations, so the knowledge base -- and with it the sample -- cannot change.
+int stage_sample(game_ctx* c, bool pdl, const float* Xsrc, const float* tsrc, bool src_is_host) {
+    using namespace game;
+    float* Xs = reinterpret_cast<float*>(c->ws + c->off_calx);
+    float* ts = Xs + static_cast<size_t>(umma::kBN) * c->N;
+    const long long n = c->P < umma::kBN ? c->P : umma::kBN;
+    long long stride = c->P / n;
+    const long long max_stride = (1ll << 30) / (static_cast<long long>(sizeof(float)) * c->N);   // pitch limit of a 2-D copy
+    if (stride > max_stride) stride = max_stride > 1 ? max_stride : 1;
+    if (src_is_host) {
+        GAME_CUDA(cudaMemcpy2DAsync(Xs, sizeof(float) * c->N, Xsrc, sizeof(float) * static_cast<size_t>(stride) * c->N,
+                                    sizeof(float) * c->N, static_cast<size_t>(n), cudaMemcpyHostToDevice, c->stream));
+        GAME_CUDA(cudaMemcpy2DAsync(ts, sizeof(float), tsrc, sizeof(float) * static_cast<size_t>(stride), sizeof(float),
+                                    static_cast<size_t>(n), cudaMemcpyHostToDevice, c->stream));
+    } else {
+        const long long work = n * c->N;
+        launch_chain(pdl, umma::cal_gather_kernel, dim3(static_cast<unsigned>((work + 255) / 256)), dim3(256), 0, c->stream, Xsrc, tsrc,
+                     Xs, ts, static_cast<const int*>(c->stop), n, stride, c->N);
+        if (int rc = check_launch(c, "cal_gather_kernel")) return rc;
+    }
+    c->sample_staged = true;
+    return GAME_OK;
+}
+
+int launch_calibration(game_ctx* c, game::umma::Params& prm, const UmmaGeo& geo, bool pdl, const float* Xsrc, const float* tsrc,
+                       bool src_is_host) {
     using namespace game;
     float* zdump = reinterpret_cast<float*>(c->ws + c->off_zdump);
     float* zcorr = reinterpret_cast<float*>(c->ws + c->off_zcorr);
     float* wscale = reinterpret_cast<float*>(c->ws + c->off_wscale);
+    float* Xs = reinterpret_cast<float*>(c->ws + c->off_calx);
+    float* ts = Xs + static_cast<size_t>(umma::kBN) * c->N;
+    int rc = GAME_OK;
+    const bool fresh = !c->sample_staged;
+    if (fresh && (rc = stage_sample(c, pdl, Xsrc, tsrc, src_is_host))) return rc;
     umma::Params cal = prm;
-    cal.X = X0; cal.t = t0;
+    cal.X = Xs; cal.t = ts;
     cal.p_tile0 = 0; cal.p_tiles = 1; cal.zero_part = 0; cal.zdump = zdump; cal.stall = nullptr;
     cal.m_pairs_per_group = 1; cal.m_groups = geo.m_pairs;          // one chromosome-tile pair per CTA pair: shortest launch
+    // The fitness kernel reads its patterns with non-coherent loads (fine for a knowledge base nobody writes while it runs).
+    // When the sample buffer has just been written on this stream the launch is a plain one, i.e. a full kernel boundary.
     const int cal_grid = 2 * (geo.m_pairs < geo.pair_cap ? geo.m_pairs : geo.pair_cap);
-    int rc = launch_umma(c, cal, cal_grid, pdl);
+    rc = launch_umma(c, cal, cal_grid, fresh ? false : pdl);
     if (rc) return rc;
+    const float* X0 = Xs;
     double* phi_s = reinterpret_cast<double*>(c->ws + c->off_calphi);
     if (c->expansion == GAME_EXP_CHEBYSHEV)
         launch_chain(pdl, umma::cal_phi_kernel<0>, dim3(c->shared ? 1 : c->N), dim3(umma::kCalThreads), 0, c->stream, X0, phi_s,
@@ -348,9 +390,11 @@ int launch_calibration(game_ctx* c, game::umma::Params& prm, const UmmaGeo& geo,
     if ((rc = check_launch(c, "cal_phi_kernel"))) return rc;
     const size_t row_bytes = sizeof(double) * ((static_cast<size_t>(c->G - 1) + 15) / 16 * 16);
     launch_chain(pdl, umma::calibrate_kernel, dim3((c->m_stride + umma::kCalRows - 1) / umma::kCalRows), dim3(umma::kCalThreads),
-                 umma::kCalRows * row_bytes, c->stream, prm.W, phi_s, zdump, wscale, zcorr, c->stop, c->P, c->M, c->G, c->m_stride);
+                 umma::kCalRows * row_bytes, c->stream, prm.W, phi_s, zdump, wscale, zcorr, reinterpret_cast<int*>(c->ws + c->off_calrej),
+                 c->stop, c->P, c->M, c->G, c->m_stride);
     if ((rc = check_launch(c, "calibrate_kernel"))) return rc;
     prm.wscale = zcorr;
+    c->calibrated_once = true;
     return GAME_OK;
 }
 
@@ -442,7 +486,8 @@ int eval_internal(game_ctx* c, float* best_out, const HostKb* hk = nullptr, doub
                 GAME_CUDA(cudaStreamWaitEvent(c->stream, c->copy_events[k], 0));
             }
             if (first_launch && wants_calibration(c)) {
-                if ((rc = launch_calibration(c, prm, geo, c->pdl && hk == nullptr, c->X, c->t))) return rc;
+                if ((rc = launch_calibration(c, prm, geo, c->pdl && hk == nullptr, hk != nullptr ? hk->X : c->X,
+                                             hk != nullptr ? hk->t : c->t, hk != nullptr))) return rc;
                 if (timed) GAME_CUDA(cudaEventRecord(ev0, c->stream));      // the roofline figure times the evaluation proper
             }
             prm.p_tile0 = tile0; prm.p_tiles = tile1 - tile0; prm.zero_part = first_launch ? 1 : 0;
@@ -551,7 +596,7 @@ int eval_streamed(game_ctx* c, const float* X_host, const float* t_host, float* 
         // the kernel indexes patterns absolutely: hand it the slot's base moved back by the range's first pattern
         const float* Xs = X_ring + static_cast<size_t>(slot) * slot_rows * c->N;
         const float* ts = t_ring + static_cast<size_t>(slot) * slot_rows;
-        if (r == 0 && wants_calibration(c) && (rc = launch_calibration(c, prm, geo, false, Xs, ts))) return rc;
+        if (r == 0 && wants_calibration(c) && (rc = launch_calibration(c, prm, geo, false, X_host, t_host, true))) return rc;
         prm.X = reinterpret_cast<const float*>(reinterpret_cast<uintptr_t>(Xs) - sizeof(float) * static_cast<size_t>(p0) * c->N);
         prm.t = reinterpret_cast<const float*>(reinterpret_cast<uintptr_t>(ts) - sizeof(float) * static_cast<size_t>(p0));
         prm.p_tile0 = static_cast<int>(tile0);
@@ -678,6 +723,10 @@ int run_generations(game_ctx* c, uint64_t seed, uint32_t gen0, uint32_t n_gens, 
     int rc = ensure_device(c);
     if (rc) return rc;
     begin_call(c);
+    // the calibration sample, before anything that may be captured into a graph (the graph then holds no gather)
+    if (resolved_scheme(c) == GAME_SCHEME_F16X3 && c->umma_ok && wants_calibration(c) &&
+        (rc = stage_sample(c, false, c->X, c->t, false)))
+        return rc;
     RunState* run = reinterpret_cast<RunState*>(c->ws + c->off_run);
     set_run_state_kernel<<<1, 1, 0, c->stream>>>(run, make_key(seed), gen0, best_dev);
     if ((rc = check_launch(c, "set_run_state_kernel"))) return rc;
@@ -760,6 +809,10 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(float) * static_cast<size_t>(c->m_stride) * game::umma::kBN);
     c->off_calphi = off;      // fp64 phi of the sample patterns
     if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(double) * static_cast<size_t>(G) * game::umma::kBN);
+    c->off_calx = off;        // the sample patterns themselves: X [256][N] and t [256]
+    if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(float) * game::umma::kBN * (static_cast<size_t>(N) + 1));
+    c->off_calrej = off;      // one flag per row: the calibration left the row uncorrected (game_calibration_status)
+    if (c->umma_ok && act != GAME_ACT_SIGMOID) off = align_up(off + sizeof(int) * static_cast<size_t>(c->m_stride));
     const size_t fin_blocks = (static_cast<size_t>(M) + game::kFinCols - 1) / game::kFinCols;
     c->off_blk_key = off; off = align_up(off + fin_blocks * sizeof(float));
     c->off_blk_idx = off; off = align_up(off + fin_blocks * sizeof(int));
@@ -857,6 +910,7 @@ int game_bind_state(game_ctx* c, float* popA_dev, float* popB_dev, float* fitnes
     c->pop[1] = popB_dev;
     c->fitness = fitness_dev;
     c->ws = static_cast<unsigned char*>(workspace_dev);
+    c->calibrated_once = false;
     {
         const int dev = device_of(workspace_dev);
         if (dev >= 0 && dev != c->device) { c->device = dev; c->device_checked = false; }
@@ -1257,6 +1311,21 @@ int game_fitness_kernel_ms(game_ctx* c, double* total_ms, uint64_t* launches) {
     }
     *total_ms = sum;
     *launches = c->events.size();
+    return GAME_OK;
+}
+
+int game_calibration_status(game_ctx* c, int32_t* active, int32_t* rows_rejected) {
+    if (!c || !active || !rows_rejected) return GAME_ERR_INVALID_ARG;
+    *active = (resolved_scheme(c) == GAME_SCHEME_F16X3 && c->umma_ok && wants_calibration(c)) ? 1 : 0;
+    *rows_rejected = 0;
+    if (!c->calibrated_once || !c->ws) return GAME_OK;
+    DeviceGuard guard(c->device);
+    std::vector<int> h(static_cast<size_t>(c->m_stride));
+    GAME_CUDA(cudaMemcpyAsync(h.data(), c->ws + c->off_calrej, sizeof(int) * h.size(), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(cudaStreamSynchronize(c->stream));
+    int n = 0;
+    for (int m = 0; m < c->M; ++m) n += h[static_cast<size_t>(m)] != 0 ? 1 : 0;
+    *rows_rejected = n;
     return GAME_OK;
 }
 

@@ -683,7 +683,7 @@ def test_step_keeps_w_images(game, base, over, selection, immigrants):
     for gen in range(4):
         n0 = G.launch_count()
         G.eval_fitness(); G.sync()
-        cal = 3 if cfg.activation != wl.ACT_SIGMOID else 0        # regression activations: calibration launch, cal_phi_kernel, calibrate_kernel
+        cal = 4 if cfg.activation != wl.ACT_SIGMOID else 0        # regression activations: sample gather, calibration launch, cal_phi_kernel, calibrate_kernel
         assert G.launch_count() - n0 == (4 if gen == 0 else 2) + cal   # row scales + image pass only before the first generation
         F = G.get_fitness()
         W = G.get_population()
