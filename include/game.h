@@ -167,6 +167,13 @@ int game_set_selection(game_ctx* ctx, int32_t selection);
  * GA operators then work on the error e = 1 - fitness_dev (one fp32 subtraction): elitism, tournaments, ranking and the
  * roulette weights (which are floor(clamp(1 - e, 0, 1) 2^32), i.e. the fitness itself) are the functions of an error vector
  * documented above, and the threshold of game_run_until is still a learning-ERROR threshold (stop when 1 - best <= it).
+ * RESOLUTION under GAME_ERROR_ONE_MINUS_MSE: the operators are a function of fitness_dev alone (that is what makes them
+ * reproducible from a fitness vector, game_assume_fitness included), and float(1 - MSE) has a spacing of 6e-8 just below 1.
+ * Two chromosomes whose MSE differ by less than that get the same fitness and tie (the lower index wins); the subtraction
+ * 1 - fitness_dev is exact, the rounding of 1 - MSE before it is not.  At the paper's own error levels (MSE threshold
+ * 1e-3) this is 4-5 digits below what is compared; on a regression fit with MSE below ~1e-6 most of the
+ * population ties, the true best can drop out of the elite and the search stalls: run the search on GAME_ERROR_MSE or
+ * GAME_ERROR_RMSE there (full fp32 relative resolution at any error level) and report 1 - MSE at the end if wanted.
  * Invalidates the fitness. */
 enum { GAME_ERROR_MSE = 0, GAME_ERROR_RMSE = 1, GAME_ERROR_ONE_MINUS_MSE = 2 };
 int game_set_error_metric(game_ctx* ctx, int32_t metric);

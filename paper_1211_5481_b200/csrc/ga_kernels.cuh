@@ -20,7 +20,9 @@ constexpr int kGaThreads = 128;
 __device__ __forceinline__ float fit_key(float f) { return (f != f) ? INFINITY : f; }
 // The error a fitness value stands for.  MSE / RMSE are errors themselves; under the paper's literal fitness 1 - error,
 // maximised (GAME_ERROR_ONE_MINUS_MSE) the operators work on e = 1 - fitness (one fp32 subtraction, exact for
-// fitness in [1/2, 1]), so that every operator is the SAME function of an error vector whatever is reported.
+// fitness in [1/2, 1]), so that every operator is the SAME function of an error vector whatever is reported.  What is NOT
+// exact is the rounding of 1 - MSE to fp32 when the fitness was written (spacing 6e-8 below 1): errors closer than that tie.
+// include/game.h (game_set_error_metric, "RESOLUTION") says when to search on the MSE itself instead.
 __device__ __forceinline__ float err_view(float f, int maximize) { return maximize ? 1.0f - f : f; }
 
 __device__ __forceinline__ bool precedes(float ka, int a, float kb, int b) {
