@@ -44,8 +44,8 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 # time: when the kernel source has changed since, the figure is withheld (traffic = null) rather than repeated.
 NCU_TRAFFIC = {
     "c1": {"bytes": 4666880, "source": "profiles/r02_README.md (4.67 MB read + 0 written; algorithmic 4.40 MB)", "kernel_sha": "0fd22f973aa0"},
-    "c2": {"bytes": 70289408, "source": "profiles/r02_README.md (68.75 MB read + 1.54 MB written; algorithmic 68.0 MB)", "kernel_sha": "0fd22f973aa0"},
-    "c3": {"bytes": 544963584, "source": "profiles/r02_README.md (535.63 MB read + 9.33 MB written; algorithmic 528.0 MB)", "kernel_sha": "0fd22f973aa0"},
+    "c2": {"bytes": 70417408, "source": "profiles/r03_README.md (68.75 MB read + 1.67 MB written; algorithmic 68.0 MB)", "kernel_sha": "b20770215ef3"},
+    "c3": {"bytes": 545894400, "source": "profiles/r03_README.md (536.24 MB read + 9.66 MB written; algorithmic 528.0 MB)", "kernel_sha": "b20770215ef3"},
 }
 TENSOR_FLOP_PER_CLK_PER_SM = 8192          # dense fp16/bf16 tcgen05 rate (2.25 PFLOP/s nominal = 8192 x 148 SMs x 1.86 GHz)
 
@@ -282,6 +282,10 @@ def sweep_points(args, game, torch, peaks, peaks_src):
         pts.append({"workload": f"{name}: BASELINE.json configs[{name[1:]}]", "P": cfg.P, "G": cfg.G, "M": cfg.M, "steps": steps,
                     "evals_per_s": cfg.P * cfg.M * steps / (ms * 1e-3), "generations_per_s": steps / (ms * 1e-3),
                     "ms_per_step": ms / steps, "gpu_launches": int(launches), "kernel_ms": rf["kernel_ms_avg"],
+                    # everything of a generation that is not the fused fitness kernel: finalisation, GA step, launch gaps and,
+                    # for regression outputs (c2), the calibration launches, which kernel_ms does not include
+                    "other_ms_per_step": ms / steps - rf["kernel_ms_avg"],
+                    "calibration": "3 launches per evaluation, outside kernel_ms" if cfg.activation != wl.ACT_SIGMOID else "none",
                     "tensor_tflops": rf["achieved"], "tensor_frac_of_sustained": rf["frac"], "tensor_frac_of_burst": rf.get("frac_of_burst"),
                     "mufu_frac_at_max_clock": rf["mufu_frac_at_max_clock"], "hbm_frac": rf["hbm_frac_of_measured"],
                     "binding_unit": "launch latency" if name in ("c0", "c1") else rf["binding_unit"], "clocks": clocks,

@@ -91,7 +91,7 @@ enum { GAME_ACT_IDENTITY = 0, GAME_ACT_SIGMOID = 1, GAME_ACT_TANH = 2 };
  *              with s = P / 256: the order of the patterns does not matter) against an fp64 contraction before each
  *              evaluation and folded into the row's factor (one extra launch of the fused kernel + three small kernels per
  *              evaluation; near-optimal regression with residual noise 0.01: 7.7e-6 / 8.7e-7 instead of 8.9e-5 / 8.9e-6;
- *              GAME_CALIBRATE=0 in the environment at game_create turns it off; rows longer than 3184 genes are not
+ *              game_set_option(GAME_OPT_CALIBRATE, 0) turns it off; rows longer than 3184 genes are not
  *              calibrated).
  *              Covers any N and d for Chebyshev, d <= 128 for the trigonometric family (the fp32 multiple-angle
  *              recurrence leaves the 1e-5 fitness bound beyond that: 2e-6 at d = 100, 2e-5 at d = 400).  The K axis
@@ -147,6 +147,21 @@ int game_bind_state(game_ctx* ctx, float* popA_dev, float* popB_dev, float* fitn
  * Defaults: elite 2, tournament 3, p_cross 0.9, p_mut 0.05, sigma 0.1. */
 int game_set_ga_params(game_ctx* ctx, int32_t elite, int32_t tournament, double p_cross, double p_mut,
                        float sigma);
+
+/* Execution switches, for measurements and for callers with special needs; none of them is read from the environment.
+ * Defaults give the fastest correct path.  Changing one makes the next generation loop re-capture its CUDA graph.
+ *   GAME_OPT_PDL        1 (default): the kernels of a generation are chained by programmatic dependent launch; 0: plain
+ *                       stream-ordered launches.  Results are bit-identical either way.
+ *   GAME_OPT_GRAPH      1 (default): game_run / game_evolve replay 16 generations at a time from a CUDA graph; 0: plain
+ *                       launches.  Bit-identical either way.
+ *   GAME_OPT_CALIBRATE  1 (default): the per-row calibration of the tensor-core scheme for IDENTITY / TANH outputs (see
+ *                       GAME_SCHEME_F16X3).  0 CHANGES RESULTS: the accuracy statement of F16X3 for regression outputs no
+ *                       longer holds (near-optimal fits: ~1e-4 instead of 1e-5); it marks the fitness stale.
+ *   GAME_OPT_UNIT_PAIRS 0 (default): the library sizes the tensor-core kernel's work units by its cost model; n >= 1: n
+ *                       chromosome-tile pairs per unit (clamped to what the population has).  Bit-identical either way.
+ * Unknown option or bad value -> GAME_ERR_INVALID_ARG. */
+enum { GAME_OPT_PDL = 0, GAME_OPT_GRAPH = 1, GAME_OPT_CALIBRATE = 2, GAME_OPT_UNIT_PAIRS = 3 };
+int game_set_option(game_ctx* ctx, int32_t option, int32_t value);
 
 /* Selection method of game_step.  TOURNAMENT (default, BASELINE.json) uses the `tournament` size of game_set_ga_params.
  * RANKING and ROULETTE are the paper's own methods, defined here with integer arithmetic only
@@ -221,7 +236,7 @@ int game_step(game_ctx* ctx, uint64_t seed, uint32_t gen);
  * synchronisation (PAPER.md:97, 170 future work (i)).  best_fitness_dev (device, [n_gens+1] float32, or
  * NULL) receives the best fitness of each generation's population (lowest; highest under GAME_ERROR_ONE_MINUS_MSE).  Seed,
  * generation index and trace slot live in device memory, so runs of 16 or more generations are replayed from a CUDA graph
- * captured once per configuration (GAME_GRAPH=0 in the environment at game_create: plain launches).  Async. */
+ * captured once per configuration (game_set_option(GAME_OPT_GRAPH, 0): plain launches).  Async. */
 int game_run(game_ctx* ctx, uint64_t seed, uint32_t gen0, uint32_t n_gens, float* best_fitness_dev);
 
 /* game_run with the paper's stop rule ("maximum number of iterations or the learning error threshold",
@@ -327,13 +342,13 @@ int game_mma_stall(game_ctx* ctx, double* frac_a_full, double* frac_b_full, doub
 /* Number of CUDA-graph replays this context has issued so far: game_run / game_evolve capture the launch chain of 16
  * generations once (seed, generation index and best-fitness slot live in device memory, so the graph needs no per-generation
  * argument) and replay it; every replay adds its kernel count to game_launch_count.  0 when the graph path is off
- * (GAME_GRAPH=0 in the environment at game_create), unavailable, or the run was shorter than 16 generations. */
+ * (game_set_option(GAME_OPT_GRAPH, 0)), unavailable, or the run was shorter than 16 generations. */
 int game_graph_replays(const game_ctx* ctx, uint64_t* replays);
 
 /* Whether the per-row calibration of the tensor-core scheme is doing its job (scheme F16X3 above: for the regression
  * activations IDENTITY and TANH the 1e-5 accuracy statement rests on it).
  *   active        : 1 if an evaluation under the current settings calibrates (scheme resolves to F16X3, activation IDENTITY
- *                   or TANH, rows of at most 3184 genes, GAME_CALIBRATE not 0 at game_create), else 0 -- sigmoid outputs need
+ *                   or TANH, rows of at most 3184 genes, GAME_OPT_CALIBRATE left on), else 0 -- sigmoid outputs need
  *                   none, the FFMA scheme has nothing to calibrate.
  *   rows_rejected : in the LAST calibrated evaluation, the number of chromosomes whose measured shrink was not applied because
  *                   the fit came out non-finite or beyond 1e-4 in magnitude (a row with an Inf / NaN gene; a row whose outputs

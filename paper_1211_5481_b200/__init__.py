@@ -18,6 +18,7 @@ ACT_IDENTITY, ACT_SIGMOID, ACT_TANH = 0, 1, 2
 SCHEME_AUTO, SCHEME_FFMA, SCHEME_F16X3 = 0, 1, 2
 SEL_TOURNAMENT, SEL_RANKING, SEL_ROULETTE = 0, 1, 2
 ERROR_MSE, ERROR_RMSE, ERROR_ONE_MINUS_MSE = 0, 1, 2
+OPT_PDL, OPT_GRAPH, OPT_CALIBRATE, OPT_UNIT_PAIRS = 0, 1, 2, 3
 OK, ERR_INVALID_ARG, ERR_BAD_STATE, ERR_CUDA, ERR_WORKSPACE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -36,6 +37,7 @@ SIGNATURES = {
     "game_load_kb": (C.c_int, [_VP, _F32P, _F32P]),
     "game_bind_state": (C.c_int, [_VP, _F32P, _F32P, _F32P, _VP, C.c_size_t]),
     "game_set_ga_params": (C.c_int, [_VP, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_float]),
+    "game_set_option": (C.c_int, [_VP, C.c_int32, C.c_int32]),
     "game_set_selection": (C.c_int, [_VP, C.c_int32]),
     "game_set_immigrants": (C.c_int, [_VP, C.c_int32]),
     "game_set_error_metric": (C.c_int, [_VP, C.c_int32]),
@@ -162,6 +164,10 @@ def game_set_error_metric(ctx, metric: int) -> None:
 
 def game_set_immigrants(ctx, immigrants: int) -> None:
     _check(ctx, lib().game_set_immigrants(ctx, immigrants))
+
+
+def game_set_option(ctx, option: int, value: int) -> None:
+    _check(ctx, lib().game_set_option(ctx, option, value))
 
 
 def game_set_selection(ctx, selection: int) -> None:

@@ -82,14 +82,10 @@ constexpr int kTsBytes = kBN * 4;                 // targets of the current patt
 constexpr int kSmemBytes = kSmemBar + kBarBytes + kTsBytes;
 constexpr int kTmemCols = 512;                 // two 128 x 256 fp32 accumulators per CTA
 constexpr int kStallSlots = 16;                // diagnostic slots per CTA (Params::stall)
-#ifndef GAME_POLY_PAIRS
-#define GAME_POLY_PAIRS 0
-#endif
 #ifndef GAME_EARLY_PRODUCERS
 #define GAME_EARLY_PRODUCERS 1
 #endif
 constexpr bool kEarlyProducers = GAME_EARLY_PRODUCERS != 0;   // the phi producers start before griddepcontrol.wait (A/B switch)
-constexpr int kPolyPairs = GAME_POLY_PAIRS;    // of every four packed pairs of the epilogue, how many take 2^s from the FMA pipe
 static_assert(kSmemBytes <= 232448, "shared memory budget");
 // Operand pre-scaling (both powers of two, so exact, and undone by the epilogue's FFMA constant).  An fp16 hi/lo split is
 // only RELATIVE down to 2^-14: below that the lo half is an fp16 subnormal (quantum 2^-24) and an operand of magnitude
@@ -331,15 +327,10 @@ __device__ __forceinline__ float rcp_approx(float x) {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// NaN-propagating clamps (fminf / fmaxf return the other operand for a NaN, which would turn a NaN z into a finite error).
+// NaN-propagating clamp (fminf returns the other operand for a NaN, which would turn a NaN z into a finite error).
 __device__ __forceinline__ float min_nan(float a, float b) {
     float r;
     asm("min.NaN.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
-    return r;
-}
-__device__ __forceinline__ float max_nan(float a, float b) {
-    float r;
-    asm("max.NaN.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
     return r;
 }
 
@@ -725,30 +716,6 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
-// 2^s for a pair of arguments on the FMA pipe (packed FP32) instead of the 16-lane MUFU pipe, which is what bounds the
-// epilogue of the mid-size shapes (ncu: XU pipe 80 % busy inside the epilogue's arithmetic).  s in [-126, 30] (clamped by
-// the caller): n = round(s) through the 1.5 * 2^23 trick, r = s - n in [-1/2, 1/2], 2^r by a degree-6 minimax polynomial
-// (Remez fit on [-1/2, 1/2]; in fp32 Horner form max relative error 9.3e-8, mean 1e-10 -- ex2.approx is 1.7e-7), times
-// 2^n built in the exponent field; returns 1 + 2^s (the caller's next step) on the last FMA.  A NaN stays a NaN.
-__device__ __forceinline__ f32x2 one_plus_exp2_poly2(f32x2 s2) {
-    const float magic = 12582912.0f;                                   // 1.5 * 2^23
-    const f32x2 t2 = add2(s2, pack2(magic, magic));
-    const f32x2 n2 = add2(t2, pack2(-magic, -magic));
-    const f32x2 r2 = add2(s2, mul2(n2, pack2(-1.0f, -1.0f)));
-    f32x2 p = fma2(pack2(0x1.41d334p-13f, 0x1.41d334p-13f), r2, pack2(0x1.5f456ap-10f, 0x1.5f456ap-10f));
-    p = fma2(p, r2, pack2(0x1.3b2dbcp-7f, 0x1.3b2dbcp-7f));
-    p = fma2(p, r2, pack2(0x1.c6aed4p-5f, 0x1.c6aed4p-5f));
-    p = fma2(p, r2, pack2(0x1.ebfbdap-3f, 0x1.ebfbdap-3f));
-    p = fma2(p, r2, pack2(0x1.62e430p-1f, 0x1.62e430p-1f));
-    p = fma2(p, r2, pack2(1.0f, 1.0f));
-    float t0, t1;
-    unpack2(t2, t0, t1);
-    // the low mantissa bits of t hold n (two's complement): 2^n = bits((n + 127) << 23)
-    const float sc0 = __uint_as_float((__float_as_uint(t0) << 23) + 0x3f800000u);
-    const float sc1 = __uint_as_float((__float_as_uint(t1) << 23) + 0x3f800000u);
-    return fma2(p, pack2(sc0, sc1), pack2(1.0f, 1.0f));
-}
-
 // Eight outputs: two interleaved quads (columns 0,2,4,6 and 1,3,5,7), one in each half of the packed operations, each with
 // ONE reciprocal per four outputs as in act_err2_quad.  tA, tB: staged targets of columns 0..3 and 4..7.  acc: two packed
 // running sums (four scalar sums).
@@ -762,10 +729,9 @@ __device__ __forceinline__ void act_err2_oct(const uint32_t* v, float c, float b
         const f32x2 s = fma2(pack2(__uint_as_float(v[2 * k]), __uint_as_float(v[2 * k + 1])), c2, b2);
         float s0, s1;
         unpack2(s, s0, s1);
-        if (k < kPolyPairs)      // this many of the four pairs take their 2^s from the FMA pipe, the others from the MUFU pipe
-            a[k] = one_plus_exp2_poly2(pack2(max_nan(min_nan(s0, 30.0f), -126.0f), max_nan(min_nan(s1, 30.0f), -126.0f)));
-        else
-            a[k] = add2(pack2(ex2_approx(min_nan(s0, 30.0f)), ex2_approx(min_nan(s1, 30.0f))), one2);
+        // (2^s of part of the pairs from a degree-6 polynomial on the FMA pipe instead of MUFU was measured in rounds 2 and 3
+        // and removed: profiles/r03_README.md)
+        a[k] = add2(pack2(ex2_approx(min_nan(s0, 30.0f)), ex2_approx(min_nan(s1, 30.0f))), one2);
     }
     const f32x2 p01 = mul2(a[0], a[1]), p23 = mul2(a[2], a[3]);
     float q0, q1;
@@ -1211,9 +1177,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1) fitness
             const bool vec4 = (prm.N & 3) == 0;       // rows are 16-byte aligned (X itself is: game_load_kb checks)
             const int last_blk = (prm.N - 1) >> 2, last_i = prm.N - 1;
             auto fetch4 = [&](const float* row, int b) {
-#ifdef GAME_X_NOLOAD   // measurement build only (wrong results): what the producers would cost if x cost nothing to fetch
-                return make_float4(0.1f * static_cast<float>(b & 7), 0.3f, -0.2f, 0.05f * static_cast<float>(reinterpret_cast<uintptr_t>(row) & 15));
-#endif
                 b = min(b, last_blk);
                 if (vec4) return __ldg(reinterpret_cast<const float4*>(row) + b);
                 const int i0 = 4 * b;

@@ -57,7 +57,8 @@ struct game_ctx {
     bool sample_staged = false;     // the calibration sample in the workspace is that of the current public call (stage_sample)
     bool calibrated_once = false;   // a calibration has been enqueued since game_bind_state: off_calrej holds its row flags
     bool calibrate = true;   // regression activations on the tensor-core scheme: measure each row's accumulation shrink (calibrate_kernel)
-    bool pdl = true;   // programmatic dependent launch along the generation's kernel chain (pdl.cuh); GAME_PDL=0 turns it off
+    bool pdl = true;   // programmatic dependent launch along the generation's kernel chain (pdl.cuh); game_set_option(GAME_OPT_PDL)
+    int unit_pairs = 0;   // chromosome-tile pairs per work unit of the tensor-core kernel; 0: the cost model of setup_umma decides
     double p_cross = 0.9, p_mut = 0.05;
     float sigma = 0.1f;
     // execution
@@ -85,7 +86,7 @@ struct game_ctx {
     unsigned long long graph_replays = 0;            // graph launches so far (game_graph_replays)
     bool graph_ok = true;                            // false after a failed capture: plain launches from then on
     unsigned long long config_epoch = 0;             // bumped by every call that changes what a generation launches
-    bool use_graph = true;                           // GAME_GRAPH=0 turns the graph path off (A/B measurements)
+    bool use_graph = true;                           // game_set_option(GAME_OPT_GRAPH, 0) turns the graph path off
     void* nccl_comm = nullptr;                       // ncclComm_t of the pattern-sharded loop (game_comm_init)
     int comm_rank = 0, comm_world = 1;
     int* stop = nullptr;                             // device stop state, non-null only inside game_run_until
@@ -283,7 +284,7 @@ void setup_umma(game_ctx* c, game::umma::Params& prm, UmmaGeo& geo) {
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_tpu = tpu; }
     }
     prm.m_pairs_per_group = best_tpu;
-    if (const char* e = std::getenv("GAME_TPU")) { const int v = std::atoi(e); if (v >= 1 && v <= geo.m_pairs) prm.m_pairs_per_group = v; }   // A/B override
+    if (c->unit_pairs >= 1 && c->unit_pairs <= geo.m_pairs) prm.m_pairs_per_group = c->unit_pairs;   // game_set_option override
     prm.m_groups = (geo.m_pairs + prm.m_pairs_per_group - 1) / prm.m_pairs_per_group;
     prm.dd = c->expansion == GAME_EXP_CHEBYSHEV ? c->d : 2 * c->d;
     prm.shared = c->shared;
@@ -795,9 +796,6 @@ int game_create(game_ctx** out, int64_t P, int32_t N, int32_t d, int32_t M, int3
     c->m_tiles = 2 * ((M + 2 * game::umma::kBM - 1) / (2 * game::umma::kBM));   // one chromosome tile per CTA of a pair
     c->m_stride = c->m_tiles * game::umma::kBM;
     c->umma_ok = umma_ok;
-    if (const char* e = std::getenv("GAME_PDL")) c->pdl = e[0] != '0';   // A/B switch for measurements; default on
-    if (const char* e = std::getenv("GAME_CALIBRATE")) c->calibrate = e[0] != '0';   // A/B switch; default on
-    if (const char* e = std::getenv("GAME_GRAPH")) c->use_graph = e[0] != '0';       // A/B switch; default on
     c->steps = static_cast<int>((G - 1 + 15) / 16);   // K steps of 16 genes; the bias gene is not part of the contraction
     size_t off = 0;
     c->off_part = off; off = align_up(off + sizeof(double) * kMaxPartRows * static_cast<size_t>(c->m_stride));
@@ -932,6 +930,25 @@ int game_set_ga_params(game_ctx* c, int32_t elite, int32_t tournament, double p_
     c->config_epoch += 1;
     c->elite = elite; c->tournament = tournament;
     c->p_cross = p_cross; c->p_mut = p_mut; c->sigma = sigma;
+    return GAME_OK;
+}
+
+int game_set_option(game_ctx* c, int32_t option, int32_t value) {
+    if (!c) return GAME_ERR_INVALID_ARG;
+    switch (option) {
+        case GAME_OPT_PDL: c->pdl = value != 0; break;
+        case GAME_OPT_GRAPH: c->use_graph = value != 0; break;
+        case GAME_OPT_CALIBRATE:
+            c->calibrate = value != 0;
+            c->fitness_valid = false;          // the next evaluation gives (slightly) different numbers
+            break;
+        case GAME_OPT_UNIT_PAIRS:
+            if (value < 0) return fail(c, GAME_ERR_INVALID_ARG, "GAME_OPT_UNIT_PAIRS takes 0 (automatic) or a positive count");
+            c->unit_pairs = value;
+            break;
+        default: return fail(c, GAME_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+    c->config_epoch += 1;                      // a captured generation graph is rebuilt under the new setting
     return GAME_OK;
 }
 

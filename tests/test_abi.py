@@ -192,3 +192,19 @@ def test_round2_entry_points_validate_arguments_without_a_device(L):
     assert L.game_mma_stall(ctx, C.byref(a), C.byref(b), C.byref(e), None, 0) == game.ERR_BAD_STATE
     assert L.game_mma_stall(ctx, None, C.byref(b), C.byref(e), None, 0) == game.ERR_INVALID_ARG
     game.game_destroy(ctx)
+
+
+def test_set_option_validation(L):
+    """game_set_option: the documented switches (no environment variables are read), unknown options and bad values rejected."""
+    ctx = game.game_create(1000, 10, 6, 64, game.family(game.EXP_CHEBYSHEV, game.ACT_TANH))
+    for opt in (game.OPT_PDL, game.OPT_GRAPH, game.OPT_CALIBRATE):
+        for v in (0, 1):
+            assert L.game_set_option(ctx, opt, v) == game.OK
+    assert L.game_set_option(ctx, game.OPT_UNIT_PAIRS, 2) == game.OK
+    assert L.game_set_option(ctx, game.OPT_UNIT_PAIRS, 0) == game.OK
+    assert L.game_set_option(ctx, game.OPT_UNIT_PAIRS, -1) == game.ERR_INVALID_ARG
+    assert L.game_set_option(ctx, 99, 1) == game.ERR_INVALID_ARG and b"99" in L.game_last_error(ctx)
+    assert L.game_set_option(None, game.OPT_PDL, 1) == game.ERR_INVALID_ARG
+    game.game_destroy(ctx)
+    src = open(os.path.join(ROOT, "paper_1211_5481_b200", "csrc", "game_api.cu")).read()
+    assert "getenv" not in src

@@ -696,12 +696,12 @@ def test_step_keeps_w_images(game, base, over, selection, immigrants):
 
 @pytest.mark.parametrize("base,over,scheme,selection", [
     ("c0", {}, 2, 0), ("c1", dict(P=6000, M=300), 2, 1), ("c2", dict(P=2500, M=131), 2, 2), ("c1", dict(P=3000, M=64), 1, 0)])
-def test_dependent_launch_chain_is_race_free(game, base, over, scheme, selection, monkeypatch):
+def test_dependent_launch_chain_is_race_free(game, base, over, scheme, selection):
     """The generation's kernels run under programmatic dependent launch (csrc/pdl.cuh): each one is launched while its
     predecessor still runs and parks in griddepcontrol.wait.  A missing or misplaced wait would let a kernel read what its
     predecessor has not written yet, so 40 generations enqueued back to back must give the same populations, fitness
-    vectors and best-fitness trace, bit for bit, as the same run with plain stream-ordered launches (GAME_PDL=0).  The same
-    holds for the loop replayed from a CUDA graph of 16 generations (GAME_GRAPH, the default; seed and generation index in
+    vectors and best-fitness trace, bit for bit, as the same run with plain stream-ordered launches (game_set_option(GAME_OPT_PDL, 0)).  The same
+    holds for the loop replayed from a CUDA graph of 16 generations (GAME_OPT_GRAPH, the default; seed and generation index in
     device memory): 40 = 2 replays + 8 plain generations + the final evaluation."""
     import torch
     cfg = wl.scaled(wl.CONFIGS[base], **over)
@@ -709,9 +709,8 @@ def test_dependent_launch_chain_is_race_free(game, base, over, scheme, selection
     n = 40
     out = []
     for pdl, graph in (("0", "0"), ("1", "0"), ("1", "1"), ("0", "1")):      # plain launches / PDL chain / both replayed from a CUDA graph
-        monkeypatch.setenv("GAME_PDL", pdl)                 # read by game_create
-        monkeypatch.setenv("GAME_GRAPH", graph)
         G = make(game, cfg, scheme); G.load_kb(X, t)
+        game.game_set_option(G.ctx, game.OPT_PDL, int(pdl)); game.game_set_option(G.ctx, game.OPT_GRAPH, int(graph))
         game.game_set_selection(G.ctx, selection); game.game_set_immigrants(G.ctx, 2)
         best = torch.zeros(n + 1, dtype=torch.float32, device="cuda")
         G.init_population(17); G.run(17, 0, n, best); G.sync()
