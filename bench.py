@@ -253,7 +253,9 @@ def sweep_points(args, game, torch, peaks, peaks_src):
     """The other BASELINE.json configurations in the same process: c0, c1, c2 as generation loops (device-resident,
     uninstrumented loop + an instrumented pass for the kernel time) and the configs[4] fitness-kernel grid."""
     pts = []
-    for name, steps, warmup in (("c0", 400, 40), ("c1", 400, 40), ("c2", 100, 10)):
+    # timed windows of 50-150 ms: with 400 steps c0 was timed over 5 ms and c1 over 20 ms, right after the host-side
+    # generation of their knowledge bases, and c1 came out at 50 or 60 us per generation from run to run
+    for name, steps, warmup in (("c0", 4000, 400), ("c1", 2000, 200), ("c2", 200, 20)):
         cfg = wl.CONFIGS[name]
         X, t, _ = wl.make_kb(cfg)
         G = game.Game(cfg.P, cfg.N, cfg.d, cfg.M, cfg.expansion, cfg.activation)
@@ -516,7 +518,8 @@ def run_ours(args, cfg, rank, world, local_rank):
         line["sweep"] = sweep_points(args, game, torch, peaks, peaks_src)
         line["sweep_note"] = ("c0/c1/c2: generation loops (game_evolve, device-resident, no instrumentation in the timed loop; kernel_ms "
                               "from a separate instrumented pass); c4: game_eval_fitness only, every point timed alone against the burst peak; "
-                              "peaks: " + peaks_src + " MEASURED_PEAKS.json")
+                              "peaks: " + peaks_src + " MEASURED_PEAKS.json; c0 / c1 / c2 are timed over 50-150 ms right after the power-capped c3 leg: "
+                              "their `clocks` say at which SM clock (c0 alone on a cool GPU: 72-74 k generations/s at 1965 MHz)")
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
